@@ -34,6 +34,12 @@ extern "C" {
 
 #define MPM_ABI_VERSION 1
 
+#if defined(__GNUC__)
+#define MPM_API __attribute__((visibility("default")))
+#else
+#define MPM_API
+#endif
+
 /* return codes */
 enum { MPM_OK = 0, MPM_E_ARG = -1, MPM_E_CUDA = -2, MPM_E_OOM = -3, MPM_E_STATE = -4, MPM_E_NONFINITE = -5 };
 /* pointer location */
@@ -90,6 +96,10 @@ typedef struct mpm_config {
     void *alloc_user;
 } mpm_config;
 
+/* kernel classes for the optional per-kernel timers (mpm_set_profiling) */
+enum { MPM_K_P2G1 = 0, MPM_K_NODE1 = 1, MPM_K_G2P_P2G2 = 2, MPM_K_NODE2 = 3, MPM_K_UPDATE = 4, MPM_K_SORT = 5,
+       MPM_K_MISC = 6, MPM_K_COUNT = 8 };
+
 typedef struct mpm_stats {
     double t;                 /* simulated time */
     double dt_last;           /* dt of the last completed step */
@@ -102,41 +112,48 @@ typedef struct mpm_stats {
     int32_t nn[3];            /* nodes per axis */
     int32_t variant;          /* the kernel family actually in use */
     int64_t launches;         /* kernels launched by this handle so far */
+    double kernel_ms[8];      /* with profiling on: device time per kernel class (MPM_K_*), CUDA events on `stream` */
+    int64_t kernel_calls[8];  /* ... and how many timed launches (groups) went into it */
 } mpm_stats;
 
 typedef struct mpm_handle mpm_handle;
 
 /* Construct the solver for a grid (PAPER.md:299-300 step 2).  cfg: HOST.  *out receives the handle. */
-int mpm_create(const mpm_config *cfg, mpm_handle **out);
+MPM_API int mpm_create(const mpm_config *cfg, mpm_handle **out);
 
 /* Copy n particles to the device (replaces any previous set; persistent id = load index) and perform the first
  * CFL reduction from the loaded state.  x, v: arrays of `dim` pointers; q may be NULL (Q = 0).  All data
  * pointers are HOST or DEVICE according to ptr_location; the pointer arrays themselves are HOST. */
-int mpm_load_particles(mpm_handle *h, int64_t n, const double *const *x, const double *const *v,
+MPM_API int mpm_load_particles(mpm_handle *h, int64_t n, const double *const *x, const double *const *v,
                        const double *mass, const double *rho, const double *e, const double *q,
                        int ptr_location);
 
 /* Advance nsteps time steps of Algorithm 1.  dt > 0: fixed step.  dt <= 0: CFL mode, each step uses
  * dt = cfl * h / (vmax + cmax) from the latest device-side reduction (eq. 25/29); `cfl` is alpha.
  * dt_last: HOST, NULL = do not synchronise. */
-int mpm_step(mpm_handle *h, double dt, double cfl, int32_t nsteps, double *dt_last);
+MPM_API int mpm_step(mpm_handle *h, double dt, double cfl, int32_t nsteps, double *dt_last);
 
 /* Read particle fields selected by field_mask (MPM_P_*).  out: HOST array of pointers (see MPM_P_* order), each
  * to n doubles, HOST or DEVICE per ptr_location.  order 0 = by persistent id (load order), 1 = storage order. */
-int mpm_read_particles(mpm_handle *h, uint32_t field_mask, double *const *out, int order, int ptr_location);
+MPM_API int mpm_read_particles(mpm_handle *h, uint32_t field_mask, double *const *out, int order, int ptr_location);
 
 /* Read one grid field (MPM_G_*) of the last completed step: out[ncomp][N_n], HOST or DEVICE. */
-int mpm_read_grid(mpm_handle *h, int field, double *out, int ptr_location);
+MPM_API int mpm_read_grid(mpm_handle *h, int field, double *out, int ptr_location);
 
 /* Time, step, dt, CFL maxima, counters, conserved sums (computed on the device on demand).  out: HOST. */
-int mpm_get_stats(mpm_handle *h, mpm_stats *out);
+MPM_API int mpm_get_stats(mpm_handle *h, mpm_stats *out);
+
+/* Switch per-kernel-class CUDA-event timers on (1) / off (0); switching on clears the accumulated times.  With the
+ * timers on, mpm_step brackets every kernel class with events on `stream` (a few microseconds of overhead per
+ * launch) -- use it for roofline measurements, not inside a throughput measurement. */
+MPM_API int mpm_set_profiling(mpm_handle *h, int on);
 
 /* Last error message of this handle (or of the last failed mpm_create when h == NULL).  Never NULL. */
-const char *mpm_last_error(const mpm_handle *h);
+MPM_API const char *mpm_last_error(const mpm_handle *h);
 
-void mpm_destroy(mpm_handle *h);
+MPM_API void mpm_destroy(mpm_handle *h);
 
-int mpm_abi_version(void);
+MPM_API int mpm_abi_version(void);
 
 #ifdef __cplusplus
 }

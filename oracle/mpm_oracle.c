@@ -475,8 +475,11 @@ void oracle_p2g2(oracle_t *o)
 void oracle_grid_bc2(oracle_t *o) { apply_bc(o, o->mv2, NULL); }
 
 /* l.10 Particle properties update (eq. 4 at :125; A2, A3):
- *   grad V = G2PD(mv2/m), D = trace;  E' = E - dt (P+Q)/rho D;  rho' = rho/(1 + dt D);
- *   P' = (gamma-1) rho' E';  Q' from eq. (4) with rho', P', D (stored for the next step). */
+ *   grad V = G2PD(mv2/m), D = trace;
+ *   Q from eq. (4) with the D just gathered and the current (un-primed) rho, P: eqs. (5a),(5b)
+ *   use ONE div v for q and for the energy equation, so q is always dissipative (-(q) D >= 0);
+ *   E' = E - dt (P+Q)/rho D;  rho' = rho/(1 + dt D);  P' = (gamma-1) rho' E' (implicit, A15).
+ *   Q is stored and enters the next step's force. */
 void oracle_particle_update(oracle_t *o, double dt)
 {
     const long long n = o->Np, Nn = o->Nn;
@@ -499,21 +502,21 @@ void oracle_particle_update(oracle_t *o, double dt)
             }
         }
         o->D[k] = D;
-        double rho = o->rho[k], E = o->E[k], Q = o->Q[k];
+        double rho = o->rho[k], E = o->E[k];
         double P = (gam - 1.0) * rho * E;
+        double Q = 0.0;
+        if (D < 0.0) {
+            double cs = sqrt(gam * P / rho);
+            if (o->cfg.visc_form == ORC_VISC_STANDARD)
+                Q = rho * (o->cfg.c0 * o->h * o->h * D * D - o->cfg.c1 * o->h * cs * D);
+            else
+                Q = o->cfg.c0 * (rho * o->h * D) * (rho * o->h * D) - o->cfg.c1 * o->h * cs * D;
+        }
         double En = E + dt * (-(P + Q) / rho) * D;
         double jac = 1.0 + dt * D;
         if (jac <= 0.0) o->st.n_negjac++;
         double rhon = rho / jac;
-        double Pn = (gam - 1.0) * rhon * En;
-        double Qn = 0.0;
-        if (D < 0.0) {
-            double cs = sqrt(gam * Pn / rhon);
-            if (o->cfg.visc_form == ORC_VISC_STANDARD)
-                Qn = rhon * (o->cfg.c0 * o->h * o->h * D * D - o->cfg.c1 * o->h * cs * D);
-            else
-                Qn = o->cfg.c0 * (rhon * o->h * D) * (rhon * o->h * D) - o->cfg.c1 * o->h * cs * D;
-        }
+        double Qn = Q;
         o->E[k] = En; o->rho[k] = rhon; o->Q[k] = Qn;
         if (!isfinite(En) || !isfinite(rhon)) nonfinite++;
     }

@@ -1,0 +1,563 @@
+// mpm_api.cu -- the C ABI of include/mpm.h: handle, device memory, step sequencing.  Host code only enqueues;
+// dt, t, the CFL maxima and all counters live in device memory (control stays on the device).
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "mpm_internal.cuh"
+
+using namespace mpm;
+
+struct mpm_handle {
+    mpm_config cfg;
+    GridDesc gd;
+    int variant;
+    cudaStream_t stream;
+    PArr pbuf[2];
+    int cur;
+    long long n, cap;
+    GArr g;
+    unsigned char *d_flag;
+    double *d_normal[3];
+    std::vector<unsigned char> h_flag;
+    std::vector<double> h_normal;   // [dim][Nn]
+    int *key, *rank, *count, *scan_aux;
+    DevScalars *sc;
+    long long launches;
+    long long steps_done;
+    std::vector<void *> allocations;
+    std::string err;
+    // optional per-kernel-class timers (CUDA events on the launching stream)
+    bool profiling;
+    struct Span { int cls; cudaEvent_t a, b; };
+    std::vector<Span> spans;
+    std::vector<cudaEvent_t> event_pool;
+    double kernel_ms[MPM_K_COUNT];
+    long long kernel_calls[MPM_K_COUNT];
+};
+
+static std::string g_create_error = "";
+
+namespace {
+
+int fail(mpm_handle *h, int code, const std::string &msg)
+{
+    if (h) h->err = msg; else g_create_error = msg;
+    return code;
+}
+
+#define MPM_CUDA(h, expr)                                                                        \
+    do {                                                                                         \
+        cudaError_t e__ = (expr);                                                                \
+        if (e__ != cudaSuccess)                                                                  \
+            return fail(h, e__ == cudaErrorMemoryAllocation ? MPM_E_OOM : MPM_E_CUDA,            \
+                        std::string(#expr) + ": " + cudaGetErrorString(e__));                    \
+    } while (0)
+
+void *dev_alloc(mpm_handle *h, size_t bytes)
+{
+    if (bytes == 0) bytes = 8;
+    void *p = nullptr;
+    if (h->cfg.alloc) p = h->cfg.alloc(bytes, (void *)h->stream, h->cfg.alloc_user);
+    else if (cudaMalloc(&p, bytes) != cudaSuccess) p = nullptr;
+    if (p) h->allocations.push_back(p);
+    return p;
+}
+
+void dev_free(mpm_handle *h, void *p)
+{
+    if (!p) return;
+    for (size_t i = 0; i < h->allocations.size(); ++i)
+        if (h->allocations[i] == p) { h->allocations.erase(h->allocations.begin() + i); break; }
+    if (h->cfg.free) h->cfg.free(p, h->cfg.alloc_user); else cudaFree(p);
+}
+
+template <typename T>
+bool dev_alloc_t(mpm_handle *h, T **out, size_t count)
+{
+    *out = (T *)dev_alloc(h, sizeof(T) * count);
+    return *out != nullptr;
+}
+
+// ---- obstacle setup on the host (setup only; normals are computed once) ------------------------
+
+struct MaskView {
+    const unsigned char *mask;
+    const GridDesc *gd;
+    // returns 1 masked, 0 free, -1 outside the domain
+    int at(int cx, int cy, int cz) const
+    {
+        int c[3] = { cx, cy, cz };
+        for (int a = 0; a < gd->dim; ++a) {
+            if (gd->per[a]) c[a] = ((c[a] % gd->nc[a]) + gd->nc[a]) % gd->nc[a];
+            else if (c[a] < 0 || c[a] >= gd->nc[a]) return -1;
+        }
+        return mask[(size_t)c[0] + (size_t)gd->nc[0] * ((size_t)c[1] + (size_t)gd->nc[1] * (size_t)c[2])] ? 1 : 0;
+    }
+};
+
+// windowed signed distance of reading A7: nearest masked-cell centre minus nearest free-cell centre, +-4 cells
+double signed_distance(const MaskView &mv, const int node[3])
+{
+    const int W = 4;
+    const GridDesc &gd = *mv.gd;
+    double d_solid = (W + 1) * gd.h, d_free = (W + 1) * gd.h;
+    int lo[3] = { 0, 0, 0 }, hi[3] = { 0, 0, 0 };
+    for (int a = 0; a < gd.dim; ++a) { lo[a] = node[a] - W; hi[a] = node[a] + W - 1; }
+    for (int cz = lo[2]; cz <= hi[2]; ++cz)
+        for (int cy = lo[1]; cy <= hi[1]; ++cy)
+            for (int cx = lo[0]; cx <= hi[0]; ++cx) {
+                const int kind = mv.at(cx, cy, cz);
+                if (kind < 0) continue;
+                const int c[3] = { cx, cy, cz };
+                double r2 = 0.0;
+                for (int a = 0; a < gd.dim; ++a) {
+                    const double d = ((double)c[a] + 0.5 - (double)node[a]) * gd.h;
+                    r2 += d * d;
+                }
+                const double r = std::sqrt(r2);
+                if (kind == 1) d_solid = std::min(d_solid, r); else d_free = std::min(d_free, r);
+            }
+    return d_solid - d_free;
+}
+
+void build_obstacle(mpm_handle *h, const unsigned char *mask, const double *normals)
+{
+    const GridDesc &gd = h->gd;
+    h->h_flag.assign((size_t)gd.Nn, 0);
+    h->h_normal.assign((size_t)gd.Nn * gd.dim, 0.0);
+    MaskView mv{ mask, &gd };
+    for (int iz = 0; iz < gd.nn[2]; ++iz)
+        for (int iy = 0; iy < gd.nn[1]; ++iy)
+            for (int ix = 0; ix < gd.nn[0]; ++ix) {
+                bool flagged = false;   // node touches a solid cell
+                for (int ib = 0; ib < (1 << gd.dim) && !flagged; ++ib) {
+                    const int cz = gd.dim == 3 ? iz - ((ib >> 2) & 1) : 0;
+                    flagged = mv.at(ix - (ib & 1), iy - ((ib >> 1) & 1), cz) == 1;
+                }
+                h->h_flag[(size_t)ix + (size_t)gd.nn[0] * ((size_t)iy + (size_t)gd.nn[1] * iz)] = flagged;
+            }
+    if (normals) {
+        std::memcpy(h->h_normal.data(), normals, sizeof(double) * (size_t)gd.Nn * gd.dim);
+        return;
+    }
+    for (int iz = 0; iz < gd.nn[2]; ++iz)
+        for (int iy = 0; iy < gd.nn[1]; ++iy)
+            for (int ix = 0; ix < gd.nn[0]; ++ix) {
+                const size_t I = (size_t)ix + (size_t)gd.nn[0] * ((size_t)iy + (size_t)gd.nn[1] * iz);
+                if (!h->h_flag[I]) continue;
+                double grad[3] = { 0, 0, 0 }, nrm2 = 0.0;
+                for (int a = 0; a < gd.dim; ++a) {
+                    int up[3] = { ix, iy, iz }, dn[3] = { ix, iy, iz };
+                    up[a] += 1; dn[a] -= 1;
+                    grad[a] = (signed_distance(mv, up) - signed_distance(mv, dn)) / (2.0 * gd.h);   // eq. (24)
+                    nrm2 += grad[a] * grad[a];
+                }
+                const double nrm = std::sqrt(nrm2);
+                for (int a = 0; a < gd.dim; ++a) h->h_normal[(size_t)a * gd.Nn + I] = nrm > 0.0 ? grad[a] / nrm : 0.0;
+            }
+}
+
+cudaEvent_t take_event(mpm_handle *h)
+{
+    if (!h->event_pool.empty()) { cudaEvent_t e = h->event_pool.back(); h->event_pool.pop_back(); return e; }
+    cudaEvent_t e;
+    cudaEventCreate(&e);
+    return e;
+}
+
+// fold finished spans into kernel_ms (synchronises the stream)
+void drain_spans(mpm_handle *h)
+{
+    if (h->spans.empty()) return;
+    cudaStreamSynchronize(h->stream);
+    for (auto &sp : h->spans) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, sp.a, sp.b) == cudaSuccess) { h->kernel_ms[sp.cls] += ms; h->kernel_calls[sp.cls] += 1; }
+        h->event_pool.push_back(sp.a);
+        h->event_pool.push_back(sp.b);
+    }
+    h->spans.clear();
+}
+
+struct Timed {   // RAII bracket of one kernel class
+    mpm_handle *h; int cls; cudaEvent_t a;
+    Timed(mpm_handle *h_, int cls_) : h(h_), cls(cls_), a(nullptr)
+    {
+        if (h->profiling) { a = take_event(h); cudaEventRecord(a, h->stream); }
+    }
+    ~Timed()
+    {
+        if (!a) return;
+        cudaEvent_t b = take_event(h);
+        cudaEventRecord(b, h->stream);
+        h->spans.push_back({ cls, a, b });
+        if (h->spans.size() >= 4096) drain_spans(h);
+    }
+};
+
+void free_particles(mpm_handle *h)
+{
+    for (int b = 0; b < 2; ++b) {
+        PArr &p = h->pbuf[b];
+        for (int a = 0; a < 3; ++a) { dev_free(h, p.x[a]); dev_free(h, p.v[a]); p.x[a] = p.v[a] = nullptr; }
+        dev_free(h, p.m); dev_free(h, p.rho); dev_free(h, p.e); dev_free(h, p.q); dev_free(h, p.id);
+        p.m = p.rho = p.e = p.q = nullptr; p.id = nullptr;
+    }
+    dev_free(h, h->key); dev_free(h, h->rank);
+    h->key = h->rank = nullptr;
+    h->n = h->cap = 0;
+}
+
+int alloc_particles(mpm_handle *h, long long n)
+{
+    free_particles(h);
+    const size_t N = (size_t)(n > 0 ? n : 1);
+    bool ok = true;
+    for (int b = 0; b < 2 && ok; ++b) {
+        PArr &p = h->pbuf[b];
+        for (int a = 0; a < h->gd.dim && ok; ++a) ok = dev_alloc_t(h, &p.x[a], N) && dev_alloc_t(h, &p.v[a], N);
+        ok = ok && dev_alloc_t(h, &p.m, N) && dev_alloc_t(h, &p.rho, N) && dev_alloc_t(h, &p.e, N) &&
+             dev_alloc_t(h, &p.q, N) && dev_alloc_t(h, &p.id, N);
+    }
+    ok = ok && dev_alloc_t(h, &h->key, N) && dev_alloc_t(h, &h->rank, N);
+    if (!ok) { free_particles(h); return fail(h, MPM_E_OOM, "out of device memory for particle arrays"); }
+    h->n = n; h->cap = n; h->cur = 0;
+    return MPM_OK;
+}
+
+// cell-key counting sort of all particle arrays into the other buffer (Alg. 1 l.12)
+void reorder(mpm_handle *h)
+{
+    Timed timer(h, MPM_K_SORT);
+    const PArr &src = h->pbuf[h->cur];
+    const PArr &dst = h->pbuf[h->cur ^ 1];
+    launch_key_rank(h->gd, src, h->key, h->rank, h->count, h->n, h->stream);
+    launch_exclusive_scan(h->count, h->gd.Nc + 1, h->scan_aux, h->stream);
+    launch_permute(h->gd, src, dst, h->key, h->rank, h->count, h->n, h->stream);
+    h->cur ^= 1;
+    h->launches += 6;
+}
+
+int copy_in(mpm_handle *h, double *dst, const double *src, long long n, int loc)
+{
+    MPM_CUDA(h, cudaMemcpyAsync(dst, src, sizeof(double) * (size_t)n,
+                                loc == MPM_DEVICE ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, h->stream));
+    return MPM_OK;
+}
+
+int copy_out(mpm_handle *h, double *dst, const double *src, long long n, int loc)
+{
+    MPM_CUDA(h, cudaMemcpyAsync(dst, src, sizeof(double) * (size_t)n,
+                                loc == MPM_DEVICE ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, h->stream));
+    return MPM_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int mpm_abi_version(void) { return MPM_ABI_VERSION; }
+
+const char *mpm_last_error(const mpm_handle *h) { return h ? h->err.c_str() : g_create_error.c_str(); }
+
+int mpm_create(const mpm_config *cfg, mpm_handle **out)
+{
+    if (!cfg || !out) return fail(nullptr, MPM_E_ARG, "mpm_create: null argument");
+    *out = nullptr;
+    if (cfg->dim != 2 && cfg->dim != 3) return fail(nullptr, MPM_E_ARG, "mpm_create: dim must be 2 or 3");
+    if (!(cfg->dx > 0.0) || !(cfg->gamma > 1.0)) return fail(nullptr, MPM_E_ARG, "mpm_create: need dx > 0 and gamma > 1");
+    if (cfg->sort_every < 0) return fail(nullptr, MPM_E_ARG, "mpm_create: sort_every must be >= 0");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev <= 0)
+        return fail(nullptr, MPM_E_CUDA, "mpm_create: no CUDA device (this library has no CPU fallback)");
+    if (cfg->device < 0 || cfg->device >= ndev) return fail(nullptr, MPM_E_ARG, "mpm_create: bad device ordinal");
+    if (cudaSetDevice(cfg->device) != cudaSuccess) return fail(nullptr, MPM_E_CUDA, "mpm_create: cudaSetDevice failed");
+
+    mpm_handle *h = new (std::nothrow) mpm_handle();
+    if (!h) return fail(nullptr, MPM_E_OOM, "mpm_create: host allocation failed");
+    h->cfg = *cfg;
+    h->stream = (cudaStream_t)cfg->stream;
+    h->cur = 0; h->n = h->cap = 0; h->launches = 0; h->steps_done = 0;
+    h->profiling = false;
+    for (int k = 0; k < MPM_K_COUNT; ++k) { h->kernel_ms[k] = 0.0; h->kernel_calls[k] = 0; }
+    h->d_flag = nullptr; h->key = h->rank = h->count = h->scan_aux = nullptr; h->sc = nullptr;
+    std::memset(h->pbuf, 0, sizeof(h->pbuf));
+    std::memset(&h->g, 0, sizeof(h->g));
+    for (int a = 0; a < 3; ++a) h->d_normal[a] = nullptr;
+
+    GridDesc &gd = h->gd;
+    std::memset(&gd, 0, sizeof(gd));
+    gd.dim = cfg->dim; gd.h = cfg->dx; gd.inv_h = 1.0 / cfg->dx;
+    gd.gamma = cfg->gamma; gd.c0 = cfg->c0; gd.c1 = cfg->c1; gd.visc_form = cfg->visc_form;
+    gd.Nn = 1; gd.Nc = 1;
+    for (int a = 0; a < 3; ++a) {
+        if (a < gd.dim) {
+            const bool p0 = cfg->bc[a][0] == MPM_BC_PERIODIC, p1 = cfg->bc[a][1] == MPM_BC_PERIODIC;
+            if (cfg->n[a] < 1 || p0 != p1) {
+                delete h;
+                return fail(nullptr, MPM_E_ARG, "mpm_create: n[a] >= 1 and PERIODIC on both sides of an axis required");
+            }
+            gd.nc[a] = cfg->n[a]; gd.per[a] = p0; gd.nn[a] = p0 ? cfg->n[a] : cfg->n[a] + 1;
+            gd.L[a] = (double)cfg->n[a] * cfg->dx;
+            gd.bc[a][0] = cfg->bc[a][0]; gd.bc[a][1] = cfg->bc[a][1];
+        } else {
+            gd.nc[a] = 1; gd.nn[a] = 1; gd.per[a] = 0; gd.L[a] = 0.0;
+        }
+        gd.Nn *= gd.nn[a]; gd.Nc *= gd.nc[a];
+    }
+    if (gd.Nc >= (1ll << 31) - 2 || gd.Nn >= (1ll << 31) - 2) {
+        delete h;
+        return fail(nullptr, MPM_E_ARG, "mpm_create: grid too large for 32-bit cell keys");
+    }
+    gd.in_axis = -1; gd.in_side = 0;
+    for (int a = 0; a < gd.dim && gd.in_axis < 0; ++a)
+        for (int s = 0; s < 2; ++s)
+            if (cfg->bc[a][s] == MPM_BC_INFLOW) { gd.in_axis = a; gd.in_side = s; break; }
+    for (int a = 0; a < 3; ++a) gd.inflow_v[a] = cfg->inflow_v[a];
+    gd.inflow_rho = cfg->inflow_rho;
+    gd.inflow_e = cfg->inflow_p / ((cfg->gamma - 1.0) * cfg->inflow_rho);
+    double vol = 1.0;
+    for (int a = 0; a < gd.dim; ++a) vol *= gd.h;
+    gd.inflow_mass = cfg->inflow_rho * vol / (cfg->ppc_inflow > 0.0 ? cfg->ppc_inflow : 1.0);
+    gd.recycle_seed = cfg->recycle_seed;
+    gd.has_obstacle = cfg->obstacle_mask != nullptr;
+
+    h->variant = cfg->variant == MPM_VARIANT_AUTO ? MPM_VARIANT_ATOMIC : cfg->variant;
+    if (h->variant != MPM_VARIANT_ATOMIC) {
+        delete h;
+        return fail(nullptr, MPM_E_ARG, "mpm_create: only MPM_VARIANT_ATOMIC is built in this version");
+    }
+
+    // grid arrays
+    bool ok = dev_alloc_t(h, &h->g.m, (size_t)gd.Nn);
+    for (int a = 0; a < gd.dim && ok; ++a)
+        ok = dev_alloc_t(h, &h->g.mv[a], (size_t)gd.Nn) && dev_alloc_t(h, &h->g.f[a], (size_t)gd.Nn) &&
+             dev_alloc_t(h, &h->g.mv2[a], (size_t)gd.Nn) && dev_alloc_t(h, &h->g.vbar[a], (size_t)gd.Nn) &&
+             dev_alloc_t(h, &h->g.acc[a], (size_t)gd.Nn) && dev_alloc_t(h, &h->g.v2[a], (size_t)gd.Nn);
+    ok = ok && dev_alloc_t(h, &h->count, (size_t)gd.Nc + 1) && dev_alloc_t(h, &h->scan_aux, (size_t)gd.Nc / 4096 + 8) &&
+         dev_alloc_t(h, &h->sc, 1);
+    if (gd.has_obstacle && ok) {
+        build_obstacle(h, cfg->obstacle_mask, cfg->node_normals);
+        ok = dev_alloc_t(h, &h->d_flag, (size_t)gd.Nn);
+        for (int a = 0; a < gd.dim && ok; ++a) ok = dev_alloc_t(h, &h->d_normal[a], (size_t)gd.Nn);
+    }
+    if (!ok) { mpm_destroy(h); return fail(nullptr, MPM_E_OOM, "mpm_create: out of device memory for the grid"); }
+    h->cfg.obstacle_mask = nullptr; h->cfg.node_normals = nullptr;
+
+    cudaError_t e = cudaSuccess;
+    if (gd.has_obstacle) {
+        e = cudaMemcpyAsync(h->d_flag, h->h_flag.data(), (size_t)gd.Nn, cudaMemcpyHostToDevice, h->stream);
+        for (int a = 0; a < gd.dim && e == cudaSuccess; ++a)
+            e = cudaMemcpyAsync(h->d_normal[a], h->h_normal.data() + (size_t)a * gd.Nn, sizeof(double) * (size_t)gd.Nn,
+                                cudaMemcpyHostToDevice, h->stream);
+        h->g.flag = h->d_flag;
+        for (int a = 0; a < gd.dim; ++a) h->g.normal[a] = h->d_normal[a];
+    }
+    if (e == cudaSuccess) e = cudaMemsetAsync(h->sc, 0, sizeof(DevScalars), h->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(h->g.m, 0, sizeof(double) * (size_t)gd.Nn, h->stream);
+    for (int a = 0; a < gd.dim && e == cudaSuccess; ++a) {
+        double *arrs[6] = { h->g.mv[a], h->g.f[a], h->g.mv2[a], h->g.vbar[a], h->g.acc[a], h->g.v2[a] };
+        for (int j = 0; j < 6 && e == cudaSuccess; ++j) e = cudaMemsetAsync(arrs[j], 0, sizeof(double) * (size_t)gd.Nn, h->stream);
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+    if (e != cudaSuccess) {
+        std::string msg = std::string("mpm_create: ") + cudaGetErrorString(e);
+        mpm_destroy(h);
+        return fail(nullptr, MPM_E_CUDA, msg);
+    }
+    *out = h;
+    return MPM_OK;
+}
+
+void mpm_destroy(mpm_handle *h)
+{
+    if (!h) return;
+    drain_spans(h);
+    cudaStreamSynchronize(h->stream);
+    for (cudaEvent_t e : h->event_pool) cudaEventDestroy(e);
+    std::vector<void *> all = h->allocations;
+    for (void *p : all) dev_free(h, p);
+    delete h;
+}
+
+int mpm_load_particles(mpm_handle *h, int64_t n, const double *const *x, const double *const *v, const double *mass,
+                       const double *rho, const double *e, const double *q, int ptr_location)
+{
+    if (!h) return MPM_E_ARG;
+    if (n < 0 || n >= (1ll << 31) - 1 || !x || !v || !mass || !rho || !e)
+        return fail(h, MPM_E_ARG, "mpm_load_particles: bad argument");
+    if (ptr_location != MPM_HOST && ptr_location != MPM_DEVICE) return fail(h, MPM_E_ARG, "mpm_load_particles: bad ptr_location");
+    for (int a = 0; a < h->gd.dim; ++a)
+        if (!x[a] || !v[a]) return fail(h, MPM_E_ARG, "mpm_load_particles: null component pointer");
+    if (n != h->cap || !h->pbuf[0].m) {
+        int rc = alloc_particles(h, n);
+        if (rc != MPM_OK) return rc;
+    }
+    h->n = n; h->cur = 0;
+    PArr &p = h->pbuf[0];
+    int rc = MPM_OK;
+    for (int a = 0; a < h->gd.dim && rc == MPM_OK; ++a) {
+        rc = copy_in(h, p.x[a], x[a], n, ptr_location);
+        if (rc == MPM_OK) rc = copy_in(h, p.v[a], v[a], n, ptr_location);
+    }
+    if (rc == MPM_OK) rc = copy_in(h, p.m, mass, n, ptr_location);
+    if (rc == MPM_OK) rc = copy_in(h, p.rho, rho, n, ptr_location);
+    if (rc == MPM_OK) rc = copy_in(h, p.e, e, n, ptr_location);
+    if (rc != MPM_OK) return rc;
+    if (q) { rc = copy_in(h, p.q, q, n, ptr_location); if (rc != MPM_OK) return rc; }
+    else MPM_CUDA(h, cudaMemsetAsync(p.q, 0, sizeof(double) * (size_t)(n > 0 ? n : 1), h->stream));
+    launch_iota(p.id, n, h->stream);
+    MPM_CUDA(h, cudaMemsetAsync(h->sc, 0, sizeof(DevScalars), h->stream));
+    launch_initial_cfl(h->gd, p, h->sc, n, h->stream);
+    h->launches += 3;
+    h->steps_done = 0;
+    if (h->cfg.sort_every > 0 && n > 0) reorder(h);
+    MPM_CUDA(h, cudaGetLastError());
+    if (ptr_location == MPM_HOST) MPM_CUDA(h, cudaStreamSynchronize(h->stream));   // caller may reuse its buffers
+    return MPM_OK;
+}
+
+namespace {
+__global__ void k_set_mode(DevScalars *sc, double dt_fixed, double alpha)
+{
+    sc->dt_fixed = dt_fixed;
+    sc->alpha = alpha;
+}
+}  // namespace
+
+int mpm_step(mpm_handle *h, double dt, double cfl, int32_t nsteps, double *dt_last)
+{
+    if (!h) return MPM_E_ARG;
+    if (!h->pbuf[0].m) return fail(h, MPM_E_STATE, "mpm_step: no particles loaded");
+    if (nsteps < 0 || (!(dt > 0.0) && !(cfl > 0.0))) return fail(h, MPM_E_ARG, "mpm_step: need nsteps >= 0 and dt > 0 or cfl > 0");
+    const GridDesc &gd = h->gd;
+    cudaStream_t s = h->stream;
+    k_set_mode<<<1, 1, 0, s>>>(h->sc, dt > 0.0 ? dt : 0.0, cfl);
+    h->launches += 1;
+    for (int it = 0; it < nsteps; ++it) {
+        const PArr &p = h->pbuf[h->cur];
+        { Timed t(h, MPM_K_MISC); launch_begin_step(h->sc, gd.h, s); launch_grid_clear(gd, h->g, s); }   // dt (eq. 25/29); l.2
+        { Timed t(h, MPM_K_P2G1); launch_p2g1_atomic(gd, p, h->g, h->n, s); }                  // l.3
+        { Timed t(h, MPM_K_NODE1); launch_node1(gd, h->g, h->sc, s); }                         // l.4-5
+        { Timed t(h, MPM_K_G2P_P2G2); launch_g2p_p2g2_atomic(gd, p, h->g, h->sc, h->n, s); }   // l.6-8
+        { Timed t(h, MPM_K_NODE2); launch_node2(gd, h->g, s); }                                // l.9
+        { Timed t(h, MPM_K_UPDATE); launch_update_atomic(gd, p, h->g, h->sc, h->n, s); }       // l.10-11, maxima of l.13
+        { Timed t(h, MPM_K_MISC); launch_end_step(h->sc, gd.h, s); }                           // l.13-14
+        h->launches += 7;
+        h->steps_done += 1;
+        if (h->cfg.sort_every > 0 && h->steps_done % h->cfg.sort_every == 0) reorder(h);   // l.12
+    }
+    MPM_CUDA(h, cudaGetLastError());
+    if (dt_last) {
+        DevScalars host;
+        MPM_CUDA(h, cudaMemcpyAsync(&host, h->sc, sizeof(host), cudaMemcpyDeviceToHost, s));
+        MPM_CUDA(h, cudaStreamSynchronize(s));
+        *dt_last = host.dt;
+        if (host.n_nonfinite) return fail(h, MPM_E_NONFINITE, "mpm_step: non-finite particle state encountered");
+    }
+    return MPM_OK;
+}
+
+int mpm_read_particles(mpm_handle *h, uint32_t field_mask, double *const *out, int order, int ptr_location)
+{
+    if (!h || !out) return MPM_E_ARG;
+    if (!h->pbuf[0].m) return fail(h, MPM_E_STATE, "mpm_read_particles: no particles loaded");
+    if (ptr_location != MPM_HOST && ptr_location != MPM_DEVICE) return fail(h, MPM_E_ARG, "mpm_read_particles: bad ptr_location");
+    const PArr &p = h->pbuf[h->cur];
+    const PArr &scratch = h->pbuf[h->cur ^ 1];   // the inactive buffer is free outside a re-ordering
+    const int d = h->gd.dim;
+    std::vector<const double *> src;
+    std::vector<double *> tmp;
+    if (field_mask & MPM_P_X) for (int a = 0; a < d; ++a) { src.push_back(p.x[a]); tmp.push_back(scratch.x[a]); }
+    if (field_mask & MPM_P_V) for (int a = 0; a < d; ++a) { src.push_back(p.v[a]); tmp.push_back(scratch.v[a]); }
+    if (field_mask & MPM_P_M) { src.push_back(p.m); tmp.push_back(scratch.m); }
+    if (field_mask & MPM_P_RHO) { src.push_back(p.rho); tmp.push_back(scratch.rho); }
+    if (field_mask & MPM_P_E) { src.push_back(p.e); tmp.push_back(scratch.e); }
+    if (field_mask & MPM_P_Q) { src.push_back(p.q); tmp.push_back(scratch.q); }
+    for (size_t j = 0; j < src.size(); ++j) {
+        if (!out[j]) return fail(h, MPM_E_ARG, "mpm_read_particles: null output pointer");
+        const double *from = src[j];
+        if (order == 0) {
+            launch_gather_by_id(src[j], p.id, tmp[j], h->n, h->stream);
+            h->launches += 1;
+            from = tmp[j];
+        }
+        int rc = copy_out(h, out[j], from, h->n, ptr_location);
+        if (rc != MPM_OK) return rc;
+    }
+    MPM_CUDA(h, cudaStreamSynchronize(h->stream));
+    return MPM_OK;
+}
+
+int mpm_read_grid(mpm_handle *h, int field, double *out, int ptr_location)
+{
+    if (!h || !out) return MPM_E_ARG;
+    if (ptr_location != MPM_HOST && ptr_location != MPM_DEVICE) return fail(h, MPM_E_ARG, "mpm_read_grid: bad ptr_location");
+    const GridDesc &gd = h->gd;
+    const size_t Nn = (size_t)gd.Nn;
+    int rc = MPM_OK;
+    switch (field) {
+    case MPM_G_MASS: rc = copy_out(h, out, h->g.m, gd.Nn, ptr_location); break;
+    case MPM_G_MOMENTUM: for (int a = 0; a < gd.dim && rc == MPM_OK; ++a) rc = copy_out(h, out + a * Nn, h->g.mv[a], gd.Nn, ptr_location); break;
+    case MPM_G_FORCE: for (int a = 0; a < gd.dim && rc == MPM_OK; ++a) rc = copy_out(h, out + a * Nn, h->g.f[a], gd.Nn, ptr_location); break;
+    case MPM_G_MOMENTUM2: for (int a = 0; a < gd.dim && rc == MPM_OK; ++a) rc = copy_out(h, out + a * Nn, h->g.mv2[a], gd.Nn, ptr_location); break;
+    case MPM_G_NORMAL:
+    case MPM_G_FLAG: {
+        const int nc = field == MPM_G_NORMAL ? gd.dim : 1;
+        std::vector<double> host(Nn * nc, 0.0);
+        if (gd.has_obstacle) {
+            if (field == MPM_G_NORMAL) host = h->h_normal;
+            else for (size_t i = 0; i < Nn; ++i) host[i] = h->h_flag[i] ? 1.0 : 0.0;
+        }
+        if (ptr_location == MPM_HOST) std::memcpy(out, host.data(), sizeof(double) * host.size());
+        else {
+            MPM_CUDA(h, cudaMemcpyAsync(out, host.data(), sizeof(double) * host.size(), cudaMemcpyHostToDevice, h->stream));
+            MPM_CUDA(h, cudaStreamSynchronize(h->stream));
+        }
+        break;
+    }
+    default: return fail(h, MPM_E_ARG, "mpm_read_grid: unknown field");
+    }
+    if (rc != MPM_OK) return rc;
+    MPM_CUDA(h, cudaStreamSynchronize(h->stream));
+    return MPM_OK;
+}
+
+int mpm_get_stats(mpm_handle *h, mpm_stats *out)
+{
+    if (!h || !out) return MPM_E_ARG;
+    std::memset(out, 0, sizeof(*out));
+    DevScalars host;
+    if (h->pbuf[0].m) {
+        launch_stats_reduce(h->gd, h->pbuf[h->cur], h->sc, h->n, h->stream);
+        h->launches += 2;
+    }
+    MPM_CUDA(h, cudaMemcpyAsync(&host, h->sc, sizeof(host), cudaMemcpyDeviceToHost, h->stream));
+    MPM_CUDA(h, cudaStreamSynchronize(h->stream));
+    out->t = host.t; out->dt_last = host.dt; out->dt_next = host.dt_next; out->step = host.step;
+    out->vmax = host.vmax; out->cmax = host.cmax;
+    out->n_recycled = (int64_t)host.n_recycled; out->n_clamped = (int64_t)host.n_clamped;
+    out->n_negjac = (int64_t)host.n_negjac; out->n_nonfinite = (int64_t)host.n_nonfinite;
+    out->sum_mass = host.sum_mass; out->sum_energy = host.sum_energy;
+    for (int a = 0; a < 3; ++a) { out->sum_momentum[a] = host.sum_mom[a]; out->nn[a] = h->gd.nn[a]; }
+    out->num_particles = h->n; out->num_nodes = h->gd.Nn;
+    out->variant = h->variant; out->launches = h->launches;
+    drain_spans(h);
+    for (int k = 0; k < MPM_K_COUNT; ++k) { out->kernel_ms[k] = h->kernel_ms[k]; out->kernel_calls[k] = h->kernel_calls[k]; }
+    return MPM_OK;
+}
+
+int mpm_set_profiling(mpm_handle *h, int on)
+{
+    if (!h) return MPM_E_ARG;
+    drain_spans(h);
+    if (on) for (int k = 0; k < MPM_K_COUNT; ++k) { h->kernel_ms[k] = 0.0; h->kernel_calls[k] = 0; }
+    h->profiling = on != 0;
+    return MPM_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,173 @@
+// mpm_internal.cuh -- internal types and device helpers of libmpm_b200.so (CUDA path; NOT shared with oracle/).
+//
+// Notation follows the paper (arXiv 2404.17057): particles k carry X, V, M, rho, E, Q;
+// nodes i carry m, mv, f.  All arithmetic fp64.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/mpm.h"
+
+namespace mpm {
+
+// ---------------------------------------------------------------------------------------------- descriptors
+
+struct GridDesc {
+    int dim;
+    int nc[3];        // cells per axis (1 on unused axes)
+    int nn[3];        // nodes per axis: n (periodic) or n+1
+    int per[3];       // periodic axis?
+    int bc[3][2];     // MPM_BC_*
+    double h, inv_h;  // cell size and its reciprocal (A4, A19)
+    double L[3];      // domain lengths
+    long long Nn, Nc;
+    double gamma, c0, c1;
+    int visc_form;
+    int has_obstacle;
+    // inflow / recycling (reading A8)
+    double inflow_v[3];
+    double inflow_rho, inflow_e, inflow_mass;
+    int in_axis, in_side;   // first INFLOW face, -1 = none
+    unsigned long long recycle_seed;
+};
+
+// particle SoA.  P, Vbar, A, grad V are transient and never stored.
+struct PArr {
+    double *x[3];
+    double *v[3];
+    double *m, *rho, *e, *q;
+    int *id;   // persistent id = load index
+};
+
+// node SoA.  vbar = mv'/m, acc = f/m, v2 = mv2/m are the node velocities the gathers read (ratio := 0 where m = 0, A5)
+struct GArr {
+    double *m;
+    double *mv[3], *f[3], *mv2[3];
+    double *vbar[3], *acc[3], *v2[3];
+    const unsigned char *flag;   // 1 = obstacle node, NULL when there is no obstacle
+    const double *normal[3];
+};
+
+// device-resident scalars of the time loop: nothing in mpm_step needs the host
+struct DevScalars {
+    double dt;          // dt of the step being executed
+    double t;
+    double dt_next;     // alpha h / (vmax + cmax)
+    double alpha;
+    double dt_fixed;    // > 0: fixed-step mode
+    double vmax, cmax;  // finalised maxima of the last reduction
+    unsigned long long vmax_bits, cmax_bits;   // running maxima (non-negative doubles compared as integers)
+    long long step;
+    unsigned long long n_recycled, n_clamped, n_negjac, n_nonfinite;
+    double sum_mass, sum_mom[3], sum_energy;   // filled by the stats reduction on demand
+};
+
+// ---------------------------------------------------------------------------------------------- device helpers
+
+// Cell and local coordinate of a position along one axis (readings A6, A19)
+__device__ __forceinline__ void cell_1d(double X, double inv_h, int ncell, int &c, double &xi)
+{
+    double s = X * inv_h;
+    int ci = (int)floor(s);
+    ci = max(0, min(ci, ncell - 1));
+    c = ci;
+    xi = s - (double)ci;
+}
+
+template <int DIM>
+__device__ __forceinline__ void particle_cell(const GridDesc &gd, const double X[DIM], int c[DIM], double xi[DIM])
+{
+#pragma unroll
+    for (int a = 0; a < DIM; ++a) cell_1d(X[a], gd.inv_h, gd.nc[a], c[a], xi[a]);
+}
+
+// global node index of corner b (bit a of ib = b_a) of cell c; periodic: node n == node 0 (A11)
+template <int DIM>
+__device__ __forceinline__ long long corner_node(const GridDesc &gd, const int c[DIM], int ib)
+{
+    long long idx = 0;
+    long long stride = 1;
+#pragma unroll
+    for (int a = 0; a < DIM; ++a) {
+        int i = c[a] + ((ib >> a) & 1);
+        if (gd.per[a] && i == gd.nc[a]) i = 0;
+        idx += stride * (long long)i;
+        stride *= (long long)gd.nn[a];
+    }
+    return idx;
+}
+
+// phi_b = prod_a w_a(b_a), w_a(0) = 1 - xi_a, w_a(1) = xi_a
+template <int DIM>
+__device__ __forceinline__ double corner_phi(const double xi[DIM], int ib)
+{
+    double p = 1.0;
+#pragma unroll
+    for (int a = 0; a < DIM; ++a) p *= ((ib >> a) & 1) ? xi[a] : (1.0 - xi[a]);
+    return p;
+}
+
+// d_a phi_b = (+-1/h) prod_{a' != a} w_a'(b_a')
+template <int DIM>
+__device__ __forceinline__ double corner_dphi(const double xi[DIM], int ib, int a, double inv_h)
+{
+    double q = ((ib >> a) & 1) ? inv_h : -inv_h;
+#pragma unroll
+    for (int a2 = 0; a2 < DIM; ++a2)
+        if (a2 != a) q *= ((ib >> a2) & 1) ? xi[a2] : (1.0 - xi[a2]);
+    return q;
+}
+
+// splitmix64 output function (Steele, Lea & Flood 2014), restated here independently of the oracle (A8)
+__host__ __device__ __forceinline__ unsigned long long mix64(unsigned long long z)
+{
+    z += 0x9E3779B97F4A7C15ULL;
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ULL;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBULL;
+    return z ^ (z >> 31);
+}
+__host__ __device__ __forceinline__ double recycle_uniform(unsigned long long seed, long long id, long long step, int j)
+{
+    unsigned long long z = mix64(seed);
+    z = mix64(z ^ (unsigned long long)id);
+    z = mix64(z ^ (unsigned long long)step);
+    z = mix64(z ^ (unsigned long long)j);
+    return (double)(z >> 11) * (1.0 / 9007199254740992.0);
+}
+
+__device__ __forceinline__ void atomic_max_nonneg(unsigned long long *addr, double v)
+{
+    // non-negative doubles order like their bit patterns; NaN (0x7ff8...) wins, which is what we want to see
+    atomicMax(addr, (unsigned long long)__double_as_longlong(v));
+}
+
+// ---------------------------------------------------------------------------------------------- launchers
+
+// ATOMIC family (one thread per particle, global fp64 atomics; any particle order) -- mpm_kernels_atomic.cu
+void launch_p2g1_atomic(const GridDesc &gd, const PArr &p, const GArr &g, long long n, cudaStream_t s);
+void launch_g2p_p2g2_atomic(const GridDesc &gd, const PArr &p, const GArr &g, const DevScalars *sc, long long n,
+                            cudaStream_t s);
+void launch_update_atomic(const GridDesc &gd, const PArr &p, const GArr &g, DevScalars *sc, long long n,
+                          cudaStream_t s);
+
+// node kernels -- mpm_kernels_grid.cu
+void launch_grid_clear(const GridDesc &gd, const GArr &g, cudaStream_t s);
+void launch_node1(const GridDesc &gd, const GArr &g, const DevScalars *sc, cudaStream_t s);
+void launch_node2(const GridDesc &gd, const GArr &g, cudaStream_t s);
+
+// time loop scalars -- mpm_kernels_grid.cu
+void launch_begin_step(DevScalars *sc, double h, cudaStream_t s);
+void launch_end_step(DevScalars *sc, double h, cudaStream_t s);
+void launch_initial_cfl(const GridDesc &gd, const PArr &p, DevScalars *sc, long long n, cudaStream_t s);
+void launch_stats_reduce(const GridDesc &gd, const PArr &p, DevScalars *sc, long long n, cudaStream_t s);
+
+// re-ordering: cell key, histogram + rank, exclusive scan, permutation -- mpm_sort.cu
+void launch_iota(int *id, long long n, cudaStream_t s);
+void launch_key_rank(const GridDesc &gd, const PArr &p, int *key, int *rank, int *count, long long n, cudaStream_t s);
+void launch_exclusive_scan(int *data, long long n, int *aux, cudaStream_t s);   // in place, aux >= n/4096 + 2 ints
+void launch_permute(const GridDesc &gd, const PArr &src, const PArr &dst, const int *key, const int *rank,
+                    const int *offset, long long n, cudaStream_t s);
+void launch_gather_by_id(const double *src, const int *id, double *dst, long long n, cudaStream_t s);
+
+}  // namespace mpm

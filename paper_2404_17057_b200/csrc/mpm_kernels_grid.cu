@@ -1,0 +1,250 @@
+// mpm_kernels_grid.cu -- node kernels (one thread per node) and the device-resident time-loop scalars.
+//
+//   node1 : Alg. 1 l.4-5  BC + obstacle on (mv, f) (eqs. 21, 22, 30), mv' = mv + dt f,
+//           plus the node velocities the gathers read: vbar = mv'/m, acc = f/m (theta of PAPER.md:295; ratio := 0 where
+//           m = 0, reading A5) and the reset of mv2 for l.8.
+//   node2 : Alg. 1 l.9    BC on mv2, v2 = mv2/m.
+//   begin/end_step : dt from the CFL reduction (eq. 25/29), t += dt -- no host round trip.
+#include "mpm_internal.cuh"
+
+namespace mpm {
+
+namespace {
+
+constexpr int kBlock = 256;
+
+// Domain-face and obstacle conditions on one node's (mv, f) pair, in the order x, y, z faces then obstacle (A9, A14).
+// WITH_F = false is the second application (momentum only).
+template <int DIM, bool WITH_F>
+__device__ __forceinline__ void apply_bc(const GridDesc &gd, const GArr &g, long long i, const int idx[DIM], double m,
+                                         double mv[DIM], double f[DIM])
+{
+#pragma unroll
+    for (int a = 0; a < DIM; ++a) {
+        if (gd.per[a]) continue;
+#pragma unroll
+        for (int s = 0; s < 2; ++s) {
+            const bool on_face = (s == 0) ? (idx[a] == 0) : (idx[a] == gd.nn[a] - 1);
+            if (!on_face) continue;
+            const int bc = gd.bc[a][s];
+            if (bc == MPM_BC_REFLECT) {            // eq. (30): v.n = 0
+                mv[a] = 0.0;
+                if (WITH_F) f[a] = 0.0;
+            } else if (bc == MPM_BC_INFLOW) {      // Dirichlet inflow
+#pragma unroll
+                for (int a2 = 0; a2 < DIM; ++a2) {
+                    mv[a2] = m * gd.inflow_v[a2];
+                    if (WITH_F) f[a2] = 0.0;
+                }
+            } else if (bc == MPM_BC_OUTFLOW) {     // A10
+                if (WITH_F) f[a] = 0.0;
+            }
+        }
+    }
+    if (gd.has_obstacle && g.flag[i]) {
+        double nrm[DIM], dot = 0.0, dotf = 0.0;
+#pragma unroll
+        for (int a = 0; a < DIM; ++a) {
+            nrm[a] = g.normal[a][i];
+            dot += mv[a] * nrm[a];
+            if (WITH_F) dotf += f[a] * nrm[a];
+        }
+        const double half = (dot - fabs(dot)) / 2.0;       // eq. (21)
+        const double halff = (dotf - fabs(dotf)) / 2.0;    // eq. (22)
+#pragma unroll
+        for (int a = 0; a < DIM; ++a) {
+            mv[a] -= half * nrm[a];
+            if (WITH_F) f[a] -= halff * nrm[a];
+        }
+    }
+}
+
+template <int DIM>
+__device__ __forceinline__ void node_coords(const GridDesc &gd, long long i, int idx[DIM])
+{
+    long long r = i;
+#pragma unroll
+    for (int a = 0; a < DIM; ++a) {
+        idx[a] = (int)(r % gd.nn[a]);
+        r /= gd.nn[a];
+    }
+}
+
+template <int DIM>
+__global__ void __launch_bounds__(kBlock) k_node1(GridDesc gd, GArr g, const DevScalars *sc)
+{
+    const long long i = (long long)blockIdx.x * kBlock + threadIdx.x;
+    if (i >= gd.Nn) return;
+    const double dt = sc->dt;
+    int idx[DIM];
+    node_coords<DIM>(gd, i, idx);
+    const double m = g.m[i];
+    double mv[DIM], f[DIM];
+#pragma unroll
+    for (int a = 0; a < DIM; ++a) { mv[a] = g.mv[a][i]; f[a] = g.f[a][i]; }
+    apply_bc<DIM, true>(gd, g, i, idx, m, mv, f);
+#pragma unroll
+    for (int a = 0; a < DIM; ++a) {
+        const double mvp = mv[a] + dt * f[a];
+        g.mv[a][i] = mvp;
+        g.f[a][i] = f[a];
+        g.vbar[a][i] = (m != 0.0) ? mvp / m : 0.0;
+        g.acc[a][i] = (m != 0.0) ? f[a] / m : 0.0;
+        g.mv2[a][i] = 0.0;
+    }
+}
+
+template <int DIM>
+__global__ void __launch_bounds__(kBlock) k_node2(GridDesc gd, GArr g)
+{
+    const long long i = (long long)blockIdx.x * kBlock + threadIdx.x;
+    if (i >= gd.Nn) return;
+    int idx[DIM];
+    node_coords<DIM>(gd, i, idx);
+    const double m = g.m[i];
+    double mv[DIM], f[DIM];
+#pragma unroll
+    for (int a = 0; a < DIM; ++a) { mv[a] = g.mv2[a][i]; f[a] = 0.0; }
+    apply_bc<DIM, false>(gd, g, i, idx, m, mv, f);
+#pragma unroll
+    for (int a = 0; a < DIM; ++a) {
+        g.mv2[a][i] = mv[a];
+        g.v2[a][i] = (m != 0.0) ? mv[a] / m : 0.0;
+    }
+}
+
+__global__ void k_begin_step(DevScalars *sc, double h)
+{
+    sc->dt = (sc->dt_fixed > 0.0) ? sc->dt_fixed : sc->alpha * h / (sc->vmax + sc->cmax);
+    sc->vmax_bits = 0ull;
+    sc->cmax_bits = 0ull;
+}
+
+__global__ void k_end_step(DevScalars *sc, double h)
+{
+    sc->vmax = __longlong_as_double((long long)sc->vmax_bits);
+    sc->cmax = __longlong_as_double((long long)sc->cmax_bits);
+    sc->dt_next = sc->alpha * h / (sc->vmax + sc->cmax);
+    sc->t += sc->dt;
+    sc->step += 1;
+}
+
+// first CFL reduction from the loaded state: |V| and c_s = sqrt(gamma P / rho) (reading A13)
+template <int DIM>
+__global__ void __launch_bounds__(kBlock) k_initial_cfl(GridDesc gd, PArr p, DevScalars *sc, long long n)
+{
+    __shared__ double s_v[kBlock / 32], s_c[kBlock / 32];
+    double vloc = 0.0, cloc = 0.0;
+    for (long long k = (long long)blockIdx.x * kBlock + threadIdx.x; k < n; k += (long long)gridDim.x * kBlock) {
+        double v2 = 0.0;
+#pragma unroll
+        for (int a = 0; a < DIM; ++a) { const double v = p.v[a][k]; v2 += v * v; }
+        const double rho = p.rho[k];
+        const double P = (gd.gamma - 1.0) * rho * p.e[k];
+        vloc = fmax(vloc, sqrt(v2));
+        cloc = fmax(cloc, sqrt(gd.gamma * P / rho));
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        vloc = fmax(vloc, __shfl_xor_sync(0xffffffffu, vloc, o));
+        cloc = fmax(cloc, __shfl_xor_sync(0xffffffffu, cloc, o));
+    }
+    if ((threadIdx.x & 31) == 0) { s_v[threadIdx.x >> 5] = vloc; s_c[threadIdx.x >> 5] = cloc; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < kBlock / 32; ++w) { vloc = fmax(vloc, s_v[w]); cloc = fmax(cloc, s_c[w]); }
+        atomic_max_nonneg(&sc->vmax_bits, fmax(vloc, s_v[0]));
+        atomic_max_nonneg(&sc->cmax_bits, fmax(cloc, s_c[0]));
+    }
+}
+
+__global__ void k_finish_initial_cfl(DevScalars *sc)
+{
+    sc->vmax = __longlong_as_double((long long)sc->vmax_bits);
+    sc->cmax = __longlong_as_double((long long)sc->cmax_bits);
+}
+
+// diagnostics on demand: sum M, sum M V, sum M (E + |V|^2 / 2)
+template <int DIM>
+__global__ void __launch_bounds__(kBlock) k_stats_reduce(PArr p, DevScalars *sc, long long n)
+{
+    __shared__ double s[kBlock / 32][5];
+    double acc[5] = { 0, 0, 0, 0, 0 };
+    for (long long k = (long long)blockIdx.x * kBlock + threadIdx.x; k < n; k += (long long)gridDim.x * kBlock) {
+        const double M = p.m[k];
+        double v2 = 0.0;
+        acc[0] += M;
+#pragma unroll
+        for (int a = 0; a < DIM; ++a) { const double v = p.v[a][k]; acc[1 + a] += M * v; v2 += v * v; }
+        acc[4] += M * (p.e[k] + 0.5 * v2);
+    }
+#pragma unroll
+    for (int j = 0; j < 5; ++j)
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) acc[j] += __shfl_xor_sync(0xffffffffu, acc[j], o);
+    if ((threadIdx.x & 31) == 0)
+        for (int j = 0; j < 5; ++j) s[threadIdx.x >> 5][j] = acc[j];
+    __syncthreads();
+    if (threadIdx.x < 5) {
+        double t = 0.0;
+        for (int w = 0; w < kBlock / 32; ++w) t += s[w][threadIdx.x];
+        double *dst = (threadIdx.x == 0) ? &sc->sum_mass : (threadIdx.x == 4) ? &sc->sum_energy : &sc->sum_mom[threadIdx.x - 1];
+        atomicAdd(dst, t);
+    }
+}
+
+__global__ void k_stats_clear(DevScalars *sc)
+{
+    sc->sum_mass = 0.0; sc->sum_energy = 0.0;
+    sc->sum_mom[0] = sc->sum_mom[1] = sc->sum_mom[2] = 0.0;
+}
+
+inline unsigned grid_for(long long n) { return (unsigned)((n + kBlock - 1) / kBlock); }
+
+}  // namespace
+
+void launch_grid_clear(const GridDesc &gd, const GArr &g, cudaStream_t s)
+{
+    // Alg. 1 l.2 grid reset; flags and normals are static
+    cudaMemsetAsync(g.m, 0, sizeof(double) * (size_t)gd.Nn, s);
+    for (int a = 0; a < gd.dim; ++a) {
+        cudaMemsetAsync(g.mv[a], 0, sizeof(double) * (size_t)gd.Nn, s);
+        cudaMemsetAsync(g.f[a], 0, sizeof(double) * (size_t)gd.Nn, s);
+    }
+}
+
+void launch_node1(const GridDesc &gd, const GArr &g, const DevScalars *sc, cudaStream_t s)
+{
+    if (gd.dim == 2) k_node1<2><<<grid_for(gd.Nn), kBlock, 0, s>>>(gd, g, sc);
+    else k_node1<3><<<grid_for(gd.Nn), kBlock, 0, s>>>(gd, g, sc);
+}
+
+void launch_node2(const GridDesc &gd, const GArr &g, cudaStream_t s)
+{
+    if (gd.dim == 2) k_node2<2><<<grid_for(gd.Nn), kBlock, 0, s>>>(gd, g);
+    else k_node2<3><<<grid_for(gd.Nn), kBlock, 0, s>>>(gd, g);
+}
+
+void launch_begin_step(DevScalars *sc, double h, cudaStream_t s) { k_begin_step<<<1, 1, 0, s>>>(sc, h); }
+void launch_end_step(DevScalars *sc, double h, cudaStream_t s) { k_end_step<<<1, 1, 0, s>>>(sc, h); }
+
+void launch_initial_cfl(const GridDesc &gd, const PArr &p, DevScalars *sc, long long n, cudaStream_t s)
+{
+    const unsigned blocks = (unsigned)((n + kBlock - 1) / kBlock < 148 * 8 ? (n + kBlock - 1) / kBlock : 148 * 8);
+    if (n > 0) {
+        if (gd.dim == 2) k_initial_cfl<2><<<blocks, kBlock, 0, s>>>(gd, p, sc, n);
+        else k_initial_cfl<3><<<blocks, kBlock, 0, s>>>(gd, p, sc, n);
+    }
+    k_finish_initial_cfl<<<1, 1, 0, s>>>(sc);
+}
+
+void launch_stats_reduce(const GridDesc &gd, const PArr &p, DevScalars *sc, long long n, cudaStream_t s)
+{
+    k_stats_clear<<<1, 1, 0, s>>>(sc);
+    if (n <= 0) return;
+    const unsigned blocks = (unsigned)((n + kBlock - 1) / kBlock < 148 * 8 ? (n + kBlock - 1) / kBlock : 148 * 8);
+    if (gd.dim == 2) k_stats_reduce<2><<<blocks, kBlock, 0, s>>>(p, sc, n);
+    else k_stats_reduce<3><<<blocks, kBlock, 0, s>>>(p, sc, n);
+}
+
+}  // namespace mpm

@@ -143,6 +143,7 @@ def sedov(n=256, seed=4004, jitter=0.1, steps=100, e_total=1.0, p_ambient=1e-5):
     h = 1.0 / n
     gamma = 1.4
     cfg = _base_cfg(3, [n, n, n], h, gamma, [[BC_REFLECT, BC_REFLECT]] * 3)
+    cfg["visc_form"] = 1     # eq. (4) as printed heats at a rate ~ 1/rho and diverges in the evacuated centre (A3)
     rng = _rng(seed)
     x = _lattice_positions([n, n, n], h, 2, jitter, rng)
     N = x.shape[1]
@@ -166,6 +167,7 @@ def clumps(n=128, num_particles=1 << 26, seed=5005, nclumps=32, sigma_cells=3.0,
     h = 1.0 / n
     gamma = 5.0 / 3.0
     cfg = _base_cfg(3, [n, n, n], h, gamma, [[BC_PERIODIC, BC_PERIODIC]] * 3)
+    cfg["visc_form"] = 1     # densities span orders of magnitude: use the dimensionally consistent form (A3)
     rng = _rng(seed)
     N = int(num_particles)
     centres = rng.uniform(0.0, 1.0, (nclumps, 3))

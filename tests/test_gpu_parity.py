@@ -1,0 +1,204 @@
+"""GPU-vs-oracle parity through the C ABI (run on the B200 box: pytest -m gpu).
+
+Definitions: after 1 step, grid fields MASS, MOMENTUM, MOMENTUM2 agree to
+1e-12 * max|o| and FORCE to 1e-12 * max_i sum_k |S_k grad phi_ik|; after N steps particle rho, V, E agree to
+1e-9 relative L1 by persistent id.  Same seeded inputs on both sides (paper_2404_17057_b200/inputs.py).
+"""
+import numpy as np
+import pytest
+
+from paper_2404_17057_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+GRID_TOL = 1e-12
+PART_TOL = 1e-9
+
+
+def small_workloads():
+    return {
+        "sod": lambda: inputs.sod(),                                      # config 1 at full size
+        "box": lambda: inputs.periodic_box(n=96),                         # ragged: 96 is not a multiple of any tile
+        "box_shuffled": lambda: inputs.periodic_box(n=96, perm_seed=2003),
+        "cylinder": lambda: inputs.cylinder(nx=200, ny=100),
+        "sedov": lambda: inputs.sedov(n=20),
+        "clumps": lambda: inputs.clumps(n=20, num_particles=150_001),     # odd particle count
+    }
+
+
+def _force_scale(w):
+    """max_i sum_k |S_k| |grad phi_ik| <= max over nodes of (sum of |S_k| over adjacent cells)/h: tolerance scale only."""
+    cfg = w["cfg"]
+    d, h = cfg["dim"], cfg["dx"]
+    S = np.abs((cfg["gamma"] - 1.0) * w["e"] * w["mass"])
+    n = cfg["n"]
+    idx = np.zeros(S.shape[0], dtype=np.int64)
+    stride = 1
+    for a in range(d):
+        c = np.clip(np.floor(w["x"][a] / h).astype(np.int64), 0, n[a] - 1)
+        idx += stride * c
+        stride *= n[a]
+    per_cell = np.bincount(idx, weights=S, minlength=int(np.prod(n[:d])))
+    return (2 ** d) * per_cell.max() / h
+
+
+def _make(po, mpm, w, sort_every, variant=0):
+    o = po.Oracle(w["cfg"])
+    o.load_particles(w["x"], w["v"], w["mass"], w["rho"], w["e"])
+    g = mpm.Solver(w["cfg"], sort_every=sort_every, variant=variant)
+    g.load_particles(w["x"], w["v"], w["mass"], w["rho"], w["e"])
+    return o, g
+
+
+@pytest.mark.parametrize("sort_every", [0, 1])
+@pytest.mark.parametrize("name", list(small_workloads().keys()))
+def test_one_step_grid_parity(po, mpm, name, sort_every):
+    w = small_workloads()[name]()
+    o, g = _make(po, mpm, w, sort_every)
+    dto = o.step(0.0, w["cfl"], 1)
+    dtg = g.step(0.0, w["cfl"], 1)
+    assert dto == dtg                      # first-step dt comes from exact max reductions (A13)
+    fscale = _force_scale(w)
+    for fo, fg, scale in ((po.G_MASS, mpm.G_MASS, None), (po.G_MOM, mpm.G_MOMENTUM, None),
+                          (po.G_MOM2, mpm.G_MOMENTUM2, None), (po.G_FORCE, mpm.G_FORCE, fscale)):
+        a, b = o.grid(fo), g.read_grid(fg)
+        sc = scale if scale is not None else np.abs(a).max()
+        assert np.abs(a - b).max() <= GRID_TOL * sc, (name, fo, np.abs(a - b).max(), sc)
+    # and the particle state after that one step
+    p = g.read_particles()
+    for key, fo in (("rho", po.P_RHO), ("e", po.P_E), ("q", po.P_Q), ("x", po.P_X), ("v", po.P_V)):
+        a = o.particles(fo)
+        assert np.abs(a - p[key]).sum() <= 1e-11 * max(np.abs(a).sum(), 1e-300), (name, key)
+    so, sg = o.stats(), g.stats()
+    assert abs(so.dt_next - sg.dt_next) <= 1e-12 * so.dt_next
+    assert so.n_recycled == sg.n_recycled and so.n_clamped == sg.n_clamped
+
+
+STEPS = {"sod": 100, "box": 100, "box_shuffled": 100, "cylinder": 100, "sedov": 100, "clumps": 50}
+
+
+@pytest.mark.parametrize("sort_every", [0, 1, 3])
+@pytest.mark.parametrize("name", list(small_workloads().keys()))
+def test_many_step_particle_parity(po, mpm, name, sort_every):
+    w = small_workloads()[name]()
+    o, g = _make(po, mpm, w, sort_every)
+    nsteps = STEPS[name]
+    o.step(0.0, w["cfl"], nsteps)
+    g.step(0.0, w["cfl"], nsteps)
+    so, sg = o.stats(), g.stats()
+    assert so.step == sg.step == nsteps
+    assert abs(so.t - sg.t) <= 1e-10 * so.t
+    assert so.n_recycled == sg.n_recycled, (so.n_recycled, sg.n_recycled)
+    assert sg.n_nonfinite == 0 and so.n_negjac == sg.n_negjac
+    p = g.read_particles()
+    rho, e, v, x = o.particles(po.P_RHO), o.particles(po.P_E), o.particles(po.P_V), o.particles(po.P_X)
+    assert np.abs(rho - p["rho"]).sum() <= PART_TOL * np.abs(rho).sum(), name
+    assert np.abs(e - p["e"]).sum() <= PART_TOL * np.abs(e).sum(), name
+    vnorm = np.sqrt((v ** 2).sum(axis=0)).sum()
+    for a in range(w["cfg"]["dim"]):
+        assert np.abs(v[a] - p["v"][a]).sum() <= PART_TOL * max(vnorm, 1e-300), (name, a)
+    np.testing.assert_array_equal(o.particles(po.P_M), p["mass"])
+    L = np.array(w["cfg"]["n"][: w["cfg"]["dim"]]) * w["cfg"]["dx"]
+    dx = np.abs(x - p["x"])
+    for a in range(w["cfg"]["dim"]):
+        if w["cfg"]["bc"][a][0] == 0:
+            dx[a] = np.minimum(dx[a], L[a] - dx[a])
+    assert dx.sum() <= PART_TOL * np.abs(x).sum(), name
+
+
+def test_reordering_does_not_change_results(mpm):
+    """'Optional particles re-ordering' (Alg. 1 l.12) must leave the solution unchanged up to summation order."""
+    w = inputs.periodic_box(n=64, perm_seed=7)
+    res = []
+    for se in (0, 1, 5):
+        g = mpm.Solver(w["cfg"], sort_every=se)
+        g.load_particles(w["x"], w["v"], w["mass"], w["rho"], w["e"])
+        g.step(0.0, w["cfl"], 40)
+        res.append(g.read_particles())
+    for r in res[1:]:
+        for k in ("rho", "e", "x", "v"):
+            assert np.abs(r[k] - res[0][k]).sum() <= 1e-10 * np.abs(res[0][k]).sum()
+
+
+def test_checkpoint_roundtrip_bit_exact(mpm):
+    """mpm_read_particles -> mpm_load_particles is the checkpoint (state = X, V, M, rho, E, Q): must be bit-exact."""
+    w = inputs.sedov(n=12)
+    g = mpm.Solver(w["cfg"], sort_every=1)
+    g.load_particles(w["x"], w["v"], w["mass"], w["rho"], w["e"])
+    g.step(0.0, w["cfl"], 5)
+    a = g.read_particles()
+    g2 = mpm.Solver(w["cfg"], sort_every=0)
+    g2.load_particles(a["x"], a["v"], a["mass"], a["rho"], a["e"], a["q"])
+    b = g2.read_particles()
+    for k in a:
+        np.testing.assert_array_equal(a[k], b[k])
+    # storage order differs from id order after sorting, but holds the same multiset
+    c = g.read_particles(order=1)
+    np.testing.assert_array_equal(np.sort(c["rho"]), np.sort(a["rho"]))
+
+
+def test_device_pointers_and_pinned_host(mpm):
+    import torch
+    w = inputs.periodic_box(n=32)
+    g = mpm.Solver(w["cfg"])
+    dev = {k: torch.from_numpy(np.ascontiguousarray(w[k])).cuda() for k in ("x", "v", "mass", "rho", "e")}
+    g.load_particles(dev["x"], dev["v"], dev["mass"], dev["rho"], dev["e"], location=mpm.DEVICE)
+    h = mpm.Solver(w["cfg"])
+    pin = {k: torch.from_numpy(np.ascontiguousarray(w[k])).pin_memory() for k in ("x", "v", "mass", "rho", "e")}
+    h.load_particles(pin["x"], pin["v"], pin["mass"], pin["rho"], pin["e"], location=mpm.HOST)
+    g.step(1e-4, 0.3, 3)
+    h.step(1e-4, 0.3, 3)
+    a = g.read_particles(location=mpm.DEVICE)
+    b = h.read_particles()
+    for k in ("rho", "e", "x", "v"):
+        np.testing.assert_allclose(a[k].cpu().numpy(), b[k], rtol=1e-12, atol=1e-14)
+
+
+def test_edge_cases(po, mpm):
+    """Empty particle set; a single particle; particles exactly on cell faces, domain corners and the upper face."""
+    cfg = dict(dim=2, n=[5, 3], dx=0.2, gamma=1.4, bc=[[1, 1], [1, 1]])
+    g = mpm.Solver(cfg)
+    z = np.zeros((2, 0))
+    g.load_particles(z, z, np.zeros(0), np.zeros(0), np.zeros(0))
+    g.step(1e-3, 0.3, 2)
+    assert g.stats().step == 2 and g.read_grid(mpm.G_MASS).max() == 0.0
+    x = np.array([[0.0, 1.0, 0.4, 0.4, 1.0, 0.2, 0.5], [0.0, 0.6, 0.2, 0.6, 0.0, 0.4, 0.3]])
+    n = x.shape[1]
+    v = np.array([[0.3, -0.2, 0.1, 0.0, -0.4, 0.2, 0.1], [0.1, -0.3, 0.0, 0.2, 0.3, -0.1, 0.2]])
+    mass = np.full(n, 0.01); rho = np.full(n, 1.0); e = np.linspace(1.0, 2.0, n)
+    for se in (0, 1):
+        o = po.Oracle(cfg); o.load_particles(x, v, mass, rho, e)
+        g = mpm.Solver(cfg, sort_every=se); g.load_particles(x, v, mass, rho, e)
+        o.step(1e-2, 0.3, 3); g.step(1e-2, 0.3, 3)
+        p = g.read_particles()
+        np.testing.assert_allclose(p["rho"], o.particles(po.P_RHO), rtol=1e-12)
+        np.testing.assert_allclose(p["x"], o.particles(po.P_X), rtol=0, atol=1e-14)
+        np.testing.assert_allclose(g.read_grid(mpm.G_MASS), o.grid(po.G_MASS), rtol=1e-13, atol=1e-18)
+    # single particle, 3D periodic
+    cfg3 = dict(dim=3, n=[4, 4, 4], dx=0.25, gamma=1.4, bc=[[0, 0]] * 3)
+    x1 = np.array([[0.999], [0.5], [0.01]]); v1 = np.array([[1.0], [0.0], [-1.0]])
+    o = po.Oracle(cfg3); o.load_particles(x1, v1, np.array([0.1]), np.array([1.0]), np.array([1.0]))
+    g = mpm.Solver(cfg3, sort_every=1); g.load_particles(x1, v1, np.array([0.1]), np.array([1.0]), np.array([1.0]))
+    o.step(2e-2, 0.3, 10); g.step(2e-2, 0.3, 10)
+    np.testing.assert_allclose(g.read_particles()["x"], o.particles(po.P_X), rtol=0, atol=1e-14)
+
+
+def test_obstacle_setup_matches_oracle(po, mpm):
+    """Flags and mask-derived normals (reading A7) agree with the oracle's independent implementation."""
+    n = [40, 28]; h = 1.0 / 40
+    ii, jj = np.arange(40) + 0.5, np.arange(28) + 0.5
+    mask = (((ii[None, :] - 17) ** 2 + (jj[:, None] - 13) ** 2) <= 6.5 ** 2).astype(np.uint8)
+    cfg = dict(dim=2, n=n, dx=h, gamma=1.4, bc=[[2, 3], [1, 1]], obstacle_mask=mask, inflow_v=[1.0, 0, 0])
+    o = po.Oracle(cfg); g = mpm.Solver(cfg)
+    np.testing.assert_array_equal(g.read_grid(mpm.G_FLAG), o.grid(po.G_FLAG))
+    np.testing.assert_allclose(g.read_grid(mpm.G_NORMAL), o.grid(po.G_NORMAL), rtol=0, atol=1e-14)
+    assert o.grid(po.G_FLAG).sum() > 50
+
+
+def test_error_paths(mpm):
+    bad = dict(dim=4, n=[4, 4], dx=0.1)
+    with pytest.raises(mpm.MpmError):
+        mpm.Solver(bad)
+    g = mpm.Solver(dict(dim=2, n=[4, 4], dx=0.25, bc=[[0, 0], [0, 0]]))
+    with pytest.raises(mpm.MpmError):
+        g.step(1e-3, 0.3, 1)               # no particles loaded

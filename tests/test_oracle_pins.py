@@ -160,10 +160,9 @@ def test_p2g_p2gd_g2p_g2pd_brute_force(po, dim, periodic):
     scale = np.abs(np.where(m != 0, mv2 / safe, 0.0)).max() / h
     np.testing.assert_allclose(o.particles(po.P_DIV), D, rtol=0, atol=1e-13 * scale)
     # particle thermodynamics exactly as printed (eq. 4)
-    En = e - dt * (P + q) / rho * D
+    Qn = np.where(D < 0, 1.0 * (rho * h * D) ** 2 - 1.0 * h * np.sqrt(1.4 * P / rho) * D, 0.0)   # eq. (4), same D
+    En = e - dt * (P + Qn) / rho * D
     rhon = rho / (1.0 + dt * D)
-    Pn = 0.4 * rhon * En
-    Qn = np.where(D < 0, 1.0 * (rhon * h * D) ** 2 - 1.0 * h * np.sqrt(1.4 * Pn / rhon) * D, 0.0)
     np.testing.assert_allclose(o.particles(po.P_E), En, rtol=1e-12)
     np.testing.assert_allclose(o.particles(po.P_RHO), rhon, rtol=1e-12)
     np.testing.assert_allclose(o.particles(po.P_Q), Qn, rtol=1e-10, atol=1e-14)
@@ -225,7 +224,10 @@ def test_uniform_compression_closed_form(po):
     np.testing.assert_allclose(D[interior], -a * dim, rtol=1e-12)
     P = 0.4 * 1.3 * 2.0
     np.testing.assert_allclose(o.particles(po.P_RHO)[interior], 1.3 / (1 - a * dim * dt), rtol=1e-12)
-    np.testing.assert_allclose(o.particles(po.P_E)[interior], 2.0 + dt * a * dim * P / 1.3, rtol=1e-12)
+    Dc = -a * dim
+    Qc = (1.3 * h * Dc) ** 2 - h * np.sqrt(1.4 * P / 1.3) * Dc          # eq. (4), compression
+    np.testing.assert_allclose(o.particles(po.P_E)[interior], 2.0 + dt * a * dim * (P + Qc) / 1.3, rtol=1e-12)
+    np.testing.assert_allclose(o.particles(po.P_Q)[interior], Qc, rtol=1e-12)
 
 
 # --------------------------------------------------------------------------- conservation
@@ -269,8 +271,12 @@ def test_energy_work_identity_and_dt2_drift(po, dim):
     one-step total-energy defect is O(dt^2): halving dt cuts it ~4x."""
     defects = []
     for dt in (4e-3, 2e-3):
-        o, cfg, (x, v, mass, rho, e, q) = _periodic_box(po, dim, seed=9)
-        # Q = 0 initially so that the force is the pure pressure force and the identity has no stale-Q term
+        # pressure work only: c0 = c1 = 0 and no initial Q, so that f is the pure pressure force
+        rng = np.random.default_rng(9)
+        n = [8, 8, 8][:dim]; h = 1.0 / 8
+        cfg = _cfg(dim, n, h, [[0, 0]] * dim, c0=0.0, c1=0.0)
+        o = po.Oracle(cfg)
+        x, v, mass, rho, e, q = _random_particles(rng, dim, n, h, 600)
         o.load_particles(x, v, mass, rho, e, None)
         ke0 = 0.5 * (mass * (v ** 2).sum(axis=0)).sum(); ie0 = (mass * e).sum()
         o.grid_reset(); o.p2g1(); o.grid_bc(); o.grid_advance(dt); o.g2p_velocity(dt); o.p2g2(); o.grid_bc2()
@@ -284,6 +290,17 @@ def test_energy_work_identity_and_dt2_drift(po, dim):
         assert abs(lhs - work) <= 1e-12 * scale
         ke1 = 0.5 * (mass * (v1 ** 2).sum(axis=0)).sum()
         defects.append((ke1 + (mass * e1).sum()) - (ke0 + ie0))
+        # with the viscosity on, the extra heating is -dt sum_k M_k Q_k D_k / rho_k >= 0 with Q from THIS step's D
+        # (eqs. 4, 5a, 5b: one div v for q and for the energy equation -- reading A2)
+        o2 = po.Oracle(_cfg(dim, n, h, [[0, 0]] * dim))
+        o2.load_particles(x, v, mass, rho, e, None)
+        o2.grid_reset(); o2.p2g1(); o2.grid_bc(); o2.grid_advance(dt); o2.g2p_velocity(dt); o2.p2g2(); o2.grid_bc2()
+        o2.particle_update(dt)
+        D = o2.particles(po.P_DIV); Q = o2.particles(po.P_Q)
+        assert (Q[D >= 0] == 0).all() and (Q[D < 0] > 0).all()
+        extra = (mass * (o2.particles(po.P_E) - e1)).sum()
+        expect = -dt * (mass * Q * D / rho).sum()
+        assert expect > 0 and abs(extra - expect) <= 1e-12 * expect
     ratio = defects[0] / defects[1]
     assert 3.5 <= ratio <= 4.5, ratio
 
@@ -539,8 +556,8 @@ def _sod_l1(po, o, t):
 
 def test_sod_against_exact_solution_paper_setup(po):
     """The paper's own Sod run: 1 x 100 cells, regular particle lattice, t = 0.143, compared with the
-    exact solution (PAPER.md:537).  Bound B = 1.25 x the value the oracle gave when it was frozen (0.02722);
-    the L1 error falls under refinement 25 -> 50 -> 100 cells.  Also pins the wave structure: plateau pressure
+    exact solution (PAPER.md:537).  Bound B = 1.25 x the value the oracle gave when it was frozen (0.02868);
+    the L1 error falls under refinement 25 -> 50 cells (0.0398 -> 0.0284) and has levelled off by 100.  Also pins the wave structure: plateau pressure
     and velocity near (p*, u*) and the shock position near 0.5 + S t.
     (Beyond ~100 cells the Q1 + FLIP scheme's cell-crossing noise makes the particle density error GROW with
     refinement -- a property of the method as published, recorded in DESIGN.md, not a defect to pin.)"""
@@ -548,8 +565,8 @@ def test_sod_against_exact_solution_paper_setup(po):
     for nx in (25, 50, 100):
         o, w = _run_sod_to(po, nx, 1, 0.143)
         errs.append(_sod_l1(po, o, 0.143))
-    assert errs[0] > errs[1] > errs[2], errs
-    assert errs[2] <= 1.25 * 0.02722, errs
+    assert errs[0] > 1.3 * errs[1] and errs[2] < 1.05 * errs[1], errs
+    assert errs[2] <= 1.25 * 0.02868, errs
     x = o.particles(po.P_X)[0]; v = o.particles(po.P_V)[0]
     rho = o.particles(po.P_RHO); e = o.particles(po.P_E)
     ps, us, _, _ = riemann.star_state(1.0, 0.0, 1.0, 0.125, 0.0, 0.1)
@@ -575,12 +592,12 @@ def test_sod_against_exact_solution_paper_setup(po):
 
 def test_sod_config1_jittered_bound(po):
     """BASELINE config 1 itself (256 x 4, jitter 0.1 dx, CFL 0.3, 100 steps): L1 density error vs the exact solution
-    at the reached time stays under B = 1.25 x the frozen oracle value (0.1366)."""
+    at the reached time stays under B = 1.25 x the frozen oracle value (0.1091)."""
     w = inputs.sod()
     o = po.Oracle(w["cfg"])
     o.load_particles(w["x"], w["v"], w["mass"], w["rho"], w["e"])
     o.step(0.0, w["cfl"], 100)
     s = o.stats()
     err = _sod_l1(po, o, s.t)
-    assert err <= 1.25 * 0.1366, err
+    assert err <= 1.25 * 0.1091, err
     assert s.n_negjac == 0 and s.n_nonfinite == 0
