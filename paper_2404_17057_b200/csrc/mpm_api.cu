@@ -25,6 +25,14 @@ struct mpm_handle {
     std::vector<unsigned char> h_flag;
     std::vector<double> h_normal;   // [dim][Nn]
     int *key, *rank, *count, *scan_aux;
+    // SORTED family: cell offsets (double-buffered; the inactive one doubles as the per-cell counter of the fused
+    // re-ordering), group map, force payload S (double-buffered with the particles), destination records
+    int *off[2];
+    int ocur;
+    int *goff, *grp_cell, *grp_first, *n_groups;
+    double *S[2];
+    unsigned long long *dest;
+    long long max_groups;
     DevScalars *sc;
     long long launches;
     long long steps_done;
@@ -209,6 +217,8 @@ void free_particles(mpm_handle *h)
     }
     dev_free(h, h->key); dev_free(h, h->rank);
     h->key = h->rank = nullptr;
+    dev_free(h, h->S[0]); dev_free(h, h->S[1]); dev_free(h, h->dest); dev_free(h, h->grp_cell); dev_free(h, h->grp_first);
+    h->S[0] = h->S[1] = nullptr; h->dest = nullptr; h->grp_cell = h->grp_first = nullptr;
     h->n = h->cap = 0;
 }
 
@@ -224,22 +234,66 @@ int alloc_particles(mpm_handle *h, long long n)
              dev_alloc_t(h, &p.q, N) && dev_alloc_t(h, &p.id, N);
     }
     ok = ok && dev_alloc_t(h, &h->key, N) && dev_alloc_t(h, &h->rank, N);
+    if (ok && h->variant == MPM_VARIANT_SORTED) {
+        const long long gs = 1ll << h->gd.dim;
+        h->max_groups = n / gs + (n < h->gd.Nc ? n : h->gd.Nc) + 1;
+        ok = dev_alloc_t(h, &h->S[0], N) && dev_alloc_t(h, &h->S[1], N) && dev_alloc_t(h, &h->dest, N) &&
+             dev_alloc_t(h, &h->grp_cell, (size_t)h->max_groups) && dev_alloc_t(h, &h->grp_first, (size_t)h->max_groups);
+    }
     if (!ok) { free_particles(h); return fail(h, MPM_E_OOM, "out of device memory for particle arrays"); }
     h->n = n; h->cap = n; h->cur = 0;
     return MPM_OK;
 }
 
-// cell-key counting sort of all particle arrays into the other buffer (Alg. 1 l.12)
+// cell-key counting sort of all particle arrays into the other buffer (Alg. 1 l.12).  SORTED family: only after a
+// load (every later step re-orders inside its own sweeps); it also builds the group map and the force payload.
 void reorder(mpm_handle *h)
 {
     Timed timer(h, MPM_K_SORT);
     const PArr &src = h->pbuf[h->cur];
     const PArr &dst = h->pbuf[h->cur ^ 1];
-    launch_key_rank(h->gd, src, h->key, h->rank, h->count, h->n, h->stream);
-    launch_exclusive_scan(h->count, h->gd.Nc + 1, h->scan_aux, h->stream);
-    launch_permute(h->gd, src, dst, h->key, h->rank, h->count, h->n, h->stream);
+    int *count = h->variant == MPM_VARIANT_SORTED ? h->off[h->ocur] : h->count;
+    launch_key_rank(h->gd, src, h->key, h->rank, count, h->n, h->stream);
+    launch_exclusive_scan(count, h->gd.Nc + 1, h->scan_aux, h->stream);
+    launch_permute(h->gd, src, dst, h->key, h->rank, count, h->n, h->stream);
     h->cur ^= 1;
     h->launches += 6;
+    if (h->variant == MPM_VARIANT_SORTED) {
+        launch_force_payload(h->gd, dst, h->S[h->cur], h->n, h->stream);
+        launch_build_groups(h->gd, count, h->goff, h->scan_aux, h->grp_cell, h->grp_first, h->n_groups, h->stream);
+        h->launches += 6;
+    }
+}
+
+// one step of Algorithm 1 with the SORTED kernel family (see mpm_kernels_sorted.cu)
+void step_sorted(mpm_handle *h)
+{
+    const GridDesc &gd = h->gd;
+    cudaStream_t s = h->stream;
+    const PArr &p = h->pbuf[h->cur];
+    const PArr &q = h->pbuf[h->cur ^ 1];
+    int *off_old = h->off[h->ocur], *off_new = h->off[h->ocur ^ 1];
+    const SortedMap map{ h->grp_cell, h->grp_first, off_old, h->n_groups };
+    {
+        Timed t(h, MPM_K_MISC);
+        launch_begin_step(h->sc, gd.h, s);                                                // dt (eq. 25/29)
+        launch_grid_clear(gd, h->g, s);                                                   // l.2
+        cudaMemsetAsync(off_new, 0, sizeof(int) * (size_t)(gd.Nc + 1), s);                // per-cell counters of l.12
+    }
+    { Timed t(h, MPM_K_P2G1); launch_p2g1_sorted(gd, p, h->S[h->cur], h->g, map, h->max_groups, s); }              // l.3
+    { Timed t(h, MPM_K_NODE1); launch_node1(gd, h->g, h->sc, s); }                                                 // l.4-5
+    { Timed t(h, MPM_K_G2P_P2G2);
+      launch_g2p_p2g2_sorted(gd, p, h->g, h->g.na, h->sc, map, off_new, h->dest, h->max_groups, s); }              // l.6-8
+    { Timed t(h, MPM_K_NODE2); launch_node2(gd, h->g, s); }                                                        // l.9
+    { Timed t(h, MPM_K_SORT); launch_exclusive_scan(off_new, gd.Nc + 1, h->scan_aux, s); }                         // l.12 offsets
+    { Timed t(h, MPM_K_UPDATE);
+      launch_update_sorted(gd, p, q, h->g.na, h->g.nb, h->sc, map, off_new, h->dest, h->S[h->cur ^ 1], h->max_groups, s); }  // l.10-12
+    { Timed t(h, MPM_K_MISC); launch_end_step(h->sc, gd.h, s); }                                                   // l.13-14
+    { Timed t(h, MPM_K_SORT);
+      launch_build_groups(gd, off_new, h->goff, h->scan_aux, h->grp_cell, h->grp_first, h->n_groups, s); }         // next step's groups
+    h->cur ^= 1;
+    h->ocur ^= 1;
+    h->launches += 16;
 }
 
 int copy_in(mpm_handle *h, double *dst, const double *src, long long n, int loc)
@@ -285,6 +339,8 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
     h->profiling = false;
     for (int k = 0; k < MPM_K_COUNT; ++k) { h->kernel_ms[k] = 0.0; h->kernel_calls[k] = 0; }
     h->d_flag = nullptr; h->key = h->rank = h->count = h->scan_aux = nullptr; h->sc = nullptr;
+    h->off[0] = h->off[1] = nullptr; h->ocur = 0; h->goff = h->grp_cell = h->grp_first = h->n_groups = nullptr;
+    h->S[0] = h->S[1] = nullptr; h->dest = nullptr; h->max_groups = 0;
     std::memset(h->pbuf, 0, sizeof(h->pbuf));
     std::memset(&h->g, 0, sizeof(h->g));
     for (int a = 0; a < 3; ++a) h->d_normal[a] = nullptr;
@@ -326,18 +382,28 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
     gd.recycle_seed = cfg->recycle_seed;
     gd.has_obstacle = cfg->obstacle_mask != nullptr;
 
-    h->variant = cfg->variant == MPM_VARIANT_AUTO ? MPM_VARIANT_ATOMIC : cfg->variant;
-    if (h->variant != MPM_VARIANT_ATOMIC) {
+    h->variant = cfg->variant == MPM_VARIANT_AUTO ? (cfg->sort_every == 1 ? MPM_VARIANT_SORTED : MPM_VARIANT_ATOMIC)
+                                                   : cfg->variant;
+    if (h->variant != MPM_VARIANT_ATOMIC && h->variant != MPM_VARIANT_SORTED) {
         delete h;
-        return fail(nullptr, MPM_E_ARG, "mpm_create: only MPM_VARIANT_ATOMIC is built in this version");
+        return fail(nullptr, MPM_E_ARG, "mpm_create: unknown kernel variant");
     }
+    const bool sorted = h->variant == MPM_VARIANT_SORTED;
 
     // grid arrays
     bool ok = dev_alloc_t(h, &h->g.m, (size_t)gd.Nn);
-    for (int a = 0; a < gd.dim && ok; ++a)
+    for (int a = 0; a < gd.dim && ok; ++a) {
         ok = dev_alloc_t(h, &h->g.mv[a], (size_t)gd.Nn) && dev_alloc_t(h, &h->g.f[a], (size_t)gd.Nn) &&
-             dev_alloc_t(h, &h->g.mv2[a], (size_t)gd.Nn) && dev_alloc_t(h, &h->g.vbar[a], (size_t)gd.Nn) &&
-             dev_alloc_t(h, &h->g.acc[a], (size_t)gd.Nn) && dev_alloc_t(h, &h->g.v2[a], (size_t)gd.Nn);
+             dev_alloc_t(h, &h->g.mv2[a], (size_t)gd.Nn);
+        if (ok && !sorted)
+            ok = dev_alloc_t(h, &h->g.vbar[a], (size_t)gd.Nn) && dev_alloc_t(h, &h->g.acc[a], (size_t)gd.Nn) &&
+                 dev_alloc_t(h, &h->g.v2[a], (size_t)gd.Nn);
+    }
+    if (ok && sorted)
+        ok = dev_alloc_t(h, &h->g.na, (size_t)gd.Nn * 2 * gd.dim) && dev_alloc_t(h, &h->g.nb, (size_t)gd.Nn * gd.dim) &&
+             dev_alloc_t(h, &h->off[0], (size_t)gd.Nc + 1) && dev_alloc_t(h, &h->off[1], (size_t)gd.Nc + 1) &&
+             dev_alloc_t(h, &h->goff, (size_t)gd.Nc + 1) && dev_alloc_t(h, &h->n_groups, 1);
+    // the scan's block sums: one int per 4096 scanned elements
     ok = ok && dev_alloc_t(h, &h->count, (size_t)gd.Nc + 1) && dev_alloc_t(h, &h->scan_aux, (size_t)gd.Nc / 4096 + 8) &&
          dev_alloc_t(h, &h->sc, 1);
     if (gd.has_obstacle && ok) {
@@ -361,8 +427,12 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
     if (e == cudaSuccess) e = cudaMemsetAsync(h->g.m, 0, sizeof(double) * (size_t)gd.Nn, h->stream);
     for (int a = 0; a < gd.dim && e == cudaSuccess; ++a) {
         double *arrs[6] = { h->g.mv[a], h->g.f[a], h->g.mv2[a], h->g.vbar[a], h->g.acc[a], h->g.v2[a] };
-        for (int j = 0; j < 6 && e == cudaSuccess; ++j) e = cudaMemsetAsync(arrs[j], 0, sizeof(double) * (size_t)gd.Nn, h->stream);
+        for (int j = 0; j < 6 && e == cudaSuccess; ++j)
+            if (arrs[j]) e = cudaMemsetAsync(arrs[j], 0, sizeof(double) * (size_t)gd.Nn, h->stream);
     }
+    if (sorted && e == cudaSuccess) e = cudaMemsetAsync(h->g.na, 0, sizeof(double) * (size_t)gd.Nn * 2 * gd.dim, h->stream);
+    if (sorted && e == cudaSuccess) e = cudaMemsetAsync(h->g.nb, 0, sizeof(double) * (size_t)gd.Nn * gd.dim, h->stream);
+    if (sorted && e == cudaSuccess) e = cudaMemsetAsync(h->n_groups, 0, sizeof(int), h->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
     if (e != cudaSuccess) {
         std::string msg = std::string("mpm_create: ") + cudaGetErrorString(e);
@@ -415,7 +485,7 @@ int mpm_load_particles(mpm_handle *h, int64_t n, const double *const *x, const d
     launch_initial_cfl(h->gd, p, h->sc, n, h->stream);
     h->launches += 3;
     h->steps_done = 0;
-    if (h->cfg.sort_every > 0 && n > 0) reorder(h);
+    if ((h->cfg.sort_every > 0 || h->variant == MPM_VARIANT_SORTED) && n > 0) reorder(h);
     MPM_CUDA(h, cudaGetLastError());
     if (ptr_location == MPM_HOST) MPM_CUDA(h, cudaStreamSynchronize(h->stream));   // caller may reuse its buffers
     return MPM_OK;
@@ -439,6 +509,12 @@ int mpm_step(mpm_handle *h, double dt, double cfl, int32_t nsteps, double *dt_la
     k_set_mode<<<1, 1, 0, s>>>(h->sc, dt > 0.0 ? dt : 0.0, cfl);
     h->launches += 1;
     for (int it = 0; it < nsteps; ++it) {
+        if (h->variant == MPM_VARIANT_SORTED) {
+            if (h->n > 0) step_sorted(h);
+            else { launch_begin_step(h->sc, gd.h, s); launch_grid_clear(gd, h->g, s); launch_end_step(h->sc, gd.h, s); h->launches += 2; }
+            h->steps_done += 1;
+            continue;
+        }
         const PArr &p = h->pbuf[h->cur];
         { Timed t(h, MPM_K_MISC); launch_begin_step(h->sc, gd.h, s); launch_grid_clear(gd, h->g, s); }   // dt (eq. 25/29); l.2
         { Timed t(h, MPM_K_P2G1); launch_p2g1_atomic(gd, p, h->g, h->n, s); }                  // l.3

@@ -40,11 +40,14 @@ struct PArr {
     int *id;   // persistent id = load index
 };
 
-// node SoA.  vbar = mv'/m, acc = f/m, v2 = mv2/m are the node velocities the gathers read (ratio := 0 where m = 0, A5)
+// node SoA.  vbar = mv'/m, acc = f/m, v2 = mv2/m are the node velocities the gathers read (ratio := 0 where m = 0, A5):
+// component-major (vbar, acc, v2; ATOMIC family) or node-major (na[node][2 dim] = vbar, acc; nb[node][dim] = v2; SORTED
+// family, so that one corner's channels come in with 16-byte loads).  The unused set is NULL.
 struct GArr {
     double *m;
     double *mv[3], *f[3], *mv2[3];
     double *vbar[3], *acc[3], *v2[3];
+    double *na, *nb;
     const unsigned char *flag;   // 1 = obstacle node, NULL when there is no obstacle
     const double *normal[3];
 };
@@ -142,6 +145,14 @@ __device__ __forceinline__ void atomic_max_nonneg(unsigned long long *addr, doub
     atomicMax(addr, (unsigned long long)__double_as_longlong(v));
 }
 
+// cell-sorted order: off[c] .. off[c+1] are the particles of cell c; every cell is cut into groups of <= 2^dim particles
+struct SortedMap {
+    const int *grp_cell;    // [n_groups] cell of the group
+    const int *grp_first;   // [n_groups] first particle of the group
+    const int *off;         // [Nc + 1] cell offsets
+    const int *n_groups;    // device scalar
+};
+
 // ---------------------------------------------------------------------------------------------- launchers
 
 // ATOMIC family (one thread per particle, global fp64 atomics; any particle order) -- mpm_kernels_atomic.cu
@@ -150,6 +161,18 @@ void launch_g2p_p2g2_atomic(const GridDesc &gd, const PArr &p, const GArr &g, co
                             cudaStream_t s);
 void launch_update_atomic(const GridDesc &gd, const PArr &p, const GArr &g, DevScalars *sc, long long n,
                           cudaStream_t s);
+
+// SORTED family (cell-sorted particles, lane groups, butterfly reductions, fused re-ordering) -- mpm_kernels_sorted.cu
+void launch_force_payload(const GridDesc &gd, const PArr &p, double *S, long long n, cudaStream_t s);
+void launch_build_groups(const GridDesc &gd, const int *off, int *gcount_goff, int *scan_aux, int *grp_cell, int *grp_first,
+                         int *n_groups, cudaStream_t s);
+void launch_p2g1_sorted(const GridDesc &gd, const PArr &p, const double *S, const GArr &g, const SortedMap &map,
+                        long long max_groups, cudaStream_t s);
+void launch_g2p_p2g2_sorted(const GridDesc &gd, const PArr &p, const GArr &g, const double *na, const DevScalars *sc,
+                            const SortedMap &map, int *count, unsigned long long *dest, long long max_groups, cudaStream_t s);
+void launch_update_sorted(const GridDesc &gd, const PArr &p, const PArr &q, const double *na, const double *nb, DevScalars *sc,
+                          const SortedMap &map, const int *off_new, const unsigned long long *dest, double *S_out,
+                          long long max_groups, cudaStream_t s);
 
 // node kernels -- mpm_kernels_grid.cu
 void launch_grid_clear(const GridDesc &gd, const GArr &g, cudaStream_t s);

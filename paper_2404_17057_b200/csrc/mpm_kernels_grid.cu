@@ -88,8 +88,15 @@ __global__ void __launch_bounds__(kBlock) k_node1(GridDesc gd, GArr g, const Dev
         const double mvp = mv[a] + dt * f[a];
         g.mv[a][i] = mvp;
         g.f[a][i] = f[a];
-        g.vbar[a][i] = (m != 0.0) ? mvp / m : 0.0;
-        g.acc[a][i] = (m != 0.0) ? f[a] / m : 0.0;
+        const double vb = (m != 0.0) ? mvp / m : 0.0;
+        const double ac = (m != 0.0) ? f[a] / m : 0.0;
+        if (g.na) {
+            g.na[i * (2 * DIM) + a] = vb;
+            g.na[i * (2 * DIM) + DIM + a] = ac;
+        } else {
+            g.vbar[a][i] = vb;
+            g.acc[a][i] = ac;
+        }
         g.mv2[a][i] = 0.0;
     }
 }
@@ -109,7 +116,8 @@ __global__ void __launch_bounds__(kBlock) k_node2(GridDesc gd, GArr g)
 #pragma unroll
     for (int a = 0; a < DIM; ++a) {
         g.mv2[a][i] = mv[a];
-        g.v2[a][i] = (m != 0.0) ? mv[a] / m : 0.0;
+        const double v2 = (m != 0.0) ? mv[a] / m : 0.0;
+        if (g.nb) g.nb[i * DIM + a] = v2; else g.v2[a][i] = v2;
     }
 }
 

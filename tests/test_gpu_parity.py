@@ -50,11 +50,16 @@ def _make(po, mpm, w, sort_every, variant=0):
     return o, g
 
 
-@pytest.mark.parametrize("sort_every", [0, 1])
+# (sort_every, variant): ATOMIC unsorted / ATOMIC with a separate sort / SORTED family (binding.VARIANT_* = 1, 2)
+MODES = [(0, 1), (1, 1), (1, 2)]
+
+
+@pytest.mark.parametrize("mode", MODES)
 @pytest.mark.parametrize("name", list(small_workloads().keys()))
-def test_one_step_grid_parity(po, mpm, name, sort_every):
+def test_one_step_grid_parity(po, mpm, name, mode):
     w = small_workloads()[name]()
-    o, g = _make(po, mpm, w, sort_every)
+    o, g = _make(po, mpm, w, mode[0], mode[1])
+    assert g.stats().variant == mode[1]
     dto = o.step(0.0, w["cfl"], 1)
     dtg = g.step(0.0, w["cfl"], 1)
     assert dto == dtg                      # first-step dt comes from exact max reductions (A13)
@@ -77,11 +82,11 @@ def test_one_step_grid_parity(po, mpm, name, sort_every):
 STEPS = {"sod": 100, "box": 100, "box_shuffled": 100, "cylinder": 100, "sedov": 100, "clumps": 50}
 
 
-@pytest.mark.parametrize("sort_every", [0, 1, 3])
+@pytest.mark.parametrize("mode", MODES + [(3, 1)])
 @pytest.mark.parametrize("name", list(small_workloads().keys()))
-def test_many_step_particle_parity(po, mpm, name, sort_every):
+def test_many_step_particle_parity(po, mpm, name, mode):
     w = small_workloads()[name]()
-    o, g = _make(po, mpm, w, sort_every)
+    o, g = _make(po, mpm, w, mode[0], mode[1])
     nsteps = STEPS[name]
     o.step(0.0, w["cfl"], nsteps)
     g.step(0.0, w["cfl"], nsteps)
@@ -110,8 +115,8 @@ def test_reordering_does_not_change_results(mpm):
     """'Optional particles re-ordering' (Alg. 1 l.12) must leave the solution unchanged up to summation order."""
     w = inputs.periodic_box(n=64, perm_seed=7)
     res = []
-    for se in (0, 1, 5):
-        g = mpm.Solver(w["cfg"], sort_every=se)
+    for se, variant in ((0, 1), (1, 1), (5, 1), (1, 2)):
+        g = mpm.Solver(w["cfg"], sort_every=se, variant=variant)
         g.load_particles(w["x"], w["v"], w["mass"], w["rho"], w["e"])
         g.step(0.0, w["cfl"], 40)
         res.append(g.read_particles())
@@ -166,9 +171,9 @@ def test_edge_cases(po, mpm):
     n = x.shape[1]
     v = np.array([[0.3, -0.2, 0.1, 0.0, -0.4, 0.2, 0.1], [0.1, -0.3, 0.0, 0.2, 0.3, -0.1, 0.2]])
     mass = np.full(n, 0.01); rho = np.full(n, 1.0); e = np.linspace(1.0, 2.0, n)
-    for se in (0, 1):
+    for se, variant in ((0, 1), (1, 1), (1, 2)):
         o = po.Oracle(cfg); o.load_particles(x, v, mass, rho, e)
-        g = mpm.Solver(cfg, sort_every=se); g.load_particles(x, v, mass, rho, e)
+        g = mpm.Solver(cfg, sort_every=se, variant=variant); g.load_particles(x, v, mass, rho, e)
         o.step(1e-2, 0.3, 3); g.step(1e-2, 0.3, 3)
         p = g.read_particles()
         np.testing.assert_allclose(p["rho"], o.particles(po.P_RHO), rtol=1e-12)
