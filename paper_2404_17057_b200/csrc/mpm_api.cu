@@ -29,7 +29,8 @@ struct mpm_handle {
     // re-ordering), group map, force payload S (double-buffered with the particles), destination records
     int *off[2];
     int ocur;
-    int *goff, *grp_cell, *grp_first, *n_groups;
+    int *goff, *n_groups;
+    int4 *groups;
     double *S[2];
     unsigned long long *dest;
     long long max_groups;
@@ -217,8 +218,8 @@ void free_particles(mpm_handle *h)
     }
     dev_free(h, h->key); dev_free(h, h->rank);
     h->key = h->rank = nullptr;
-    dev_free(h, h->S[0]); dev_free(h, h->S[1]); dev_free(h, h->dest); dev_free(h, h->grp_cell); dev_free(h, h->grp_first);
-    h->S[0] = h->S[1] = nullptr; h->dest = nullptr; h->grp_cell = h->grp_first = nullptr;
+    dev_free(h, h->S[0]); dev_free(h, h->S[1]); dev_free(h, h->dest); dev_free(h, h->groups);
+    h->S[0] = h->S[1] = nullptr; h->dest = nullptr; h->groups = nullptr;
     h->n = h->cap = 0;
 }
 
@@ -238,7 +239,7 @@ int alloc_particles(mpm_handle *h, long long n)
         const long long gs = 1ll << h->gd.dim;
         h->max_groups = n / gs + (n < h->gd.Nc ? n : h->gd.Nc) + 1;
         ok = dev_alloc_t(h, &h->S[0], N) && dev_alloc_t(h, &h->S[1], N) && dev_alloc_t(h, &h->dest, N) &&
-             dev_alloc_t(h, &h->grp_cell, (size_t)h->max_groups) && dev_alloc_t(h, &h->grp_first, (size_t)h->max_groups);
+             dev_alloc_t(h, &h->groups, (size_t)h->max_groups);
     }
     if (!ok) { free_particles(h); return fail(h, MPM_E_OOM, "out of device memory for particle arrays"); }
     h->n = n; h->cap = n; h->cur = 0;
@@ -260,7 +261,7 @@ void reorder(mpm_handle *h)
     h->launches += 6;
     if (h->variant == MPM_VARIANT_SORTED) {
         launch_force_payload(h->gd, dst, h->S[h->cur], h->n, h->stream);
-        launch_build_groups(h->gd, count, h->goff, h->scan_aux, h->grp_cell, h->grp_first, h->n_groups, h->stream);
+        launch_build_groups(h->gd, count, h->goff, h->scan_aux, h->groups, h->n_groups, h->stream);
         h->launches += 6;
     }
 }
@@ -273,7 +274,8 @@ void step_sorted(mpm_handle *h)
     const PArr &p = h->pbuf[h->cur];
     const PArr &q = h->pbuf[h->cur ^ 1];
     int *off_old = h->off[h->ocur], *off_new = h->off[h->ocur ^ 1];
-    const SortedMap map{ h->grp_cell, h->grp_first, off_old, h->n_groups };
+    const SortedMap map{ h->groups, h->n_groups };
+    (void)off_old;
     {
         Timed t(h, MPM_K_MISC);
         launch_begin_step(h->sc, gd.h, s);                                                // dt (eq. 25/29)
@@ -290,7 +292,7 @@ void step_sorted(mpm_handle *h)
       launch_update_sorted(gd, p, q, h->g.na, h->g.nb, h->sc, map, off_new, h->dest, h->S[h->cur ^ 1], h->max_groups, s); }  // l.10-12
     { Timed t(h, MPM_K_MISC); launch_end_step(h->sc, gd.h, s); }                                                   // l.13-14
     { Timed t(h, MPM_K_SORT);
-      launch_build_groups(gd, off_new, h->goff, h->scan_aux, h->grp_cell, h->grp_first, h->n_groups, s); }         // next step's groups
+      launch_build_groups(gd, off_new, h->goff, h->scan_aux, h->groups, h->n_groups, s); }                         // next step's groups
     h->cur ^= 1;
     h->ocur ^= 1;
     h->launches += 16;
@@ -339,7 +341,7 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
     h->profiling = false;
     for (int k = 0; k < MPM_K_COUNT; ++k) { h->kernel_ms[k] = 0.0; h->kernel_calls[k] = 0; }
     h->d_flag = nullptr; h->key = h->rank = h->count = h->scan_aux = nullptr; h->sc = nullptr;
-    h->off[0] = h->off[1] = nullptr; h->ocur = 0; h->goff = h->grp_cell = h->grp_first = h->n_groups = nullptr;
+    h->off[0] = h->off[1] = nullptr; h->ocur = 0; h->goff = h->n_groups = nullptr; h->groups = nullptr;
     h->S[0] = h->S[1] = nullptr; h->dest = nullptr; h->max_groups = 0;
     std::memset(h->pbuf, 0, sizeof(h->pbuf));
     std::memset(&h->g, 0, sizeof(h->g));
@@ -389,6 +391,11 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
         return fail(nullptr, MPM_E_ARG, "mpm_create: unknown kernel variant");
     }
     const bool sorted = h->variant == MPM_VARIANT_SORTED;
+    if (sorted) {   // the group records pack the cell coordinates into one int
+        const int lim = gd.dim == 3 ? 1024 : 65535;
+        for (int a = 0; a < gd.dim; ++a)
+            if (gd.nc[a] > lim) { delete h; return fail(nullptr, MPM_E_ARG, "mpm_create: SORTED family needs n[a] <= 1024 (3D) / 65535 (2D)"); }
+    }
 
     // grid arrays
     bool ok = dev_alloc_t(h, &h->g.m, (size_t)gd.Nn);

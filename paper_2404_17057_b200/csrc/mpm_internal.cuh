@@ -145,11 +145,10 @@ __device__ __forceinline__ void atomic_max_nonneg(unsigned long long *addr, doub
     atomicMax(addr, (unsigned long long)__double_as_longlong(v));
 }
 
-// cell-sorted order: off[c] .. off[c+1] are the particles of cell c; every cell is cut into groups of <= 2^dim particles
+// cell-sorted order: off[c] .. off[c+1] are the particles of cell c; every cell is cut into groups of <= 2^dim particles.
+// One 16-byte record per group: {first particle, count, linear cell, packed cell coordinates}.
 struct SortedMap {
-    const int *grp_cell;    // [n_groups] cell of the group
-    const int *grp_first;   // [n_groups] first particle of the group
-    const int *off;         // [Nc + 1] cell offsets
+    const int4 *groups;     // [n_groups]
     const int *n_groups;    // device scalar
 };
 
@@ -164,8 +163,8 @@ void launch_update_atomic(const GridDesc &gd, const PArr &p, const GArr &g, DevS
 
 // SORTED family (cell-sorted particles, lane groups, butterfly reductions, fused re-ordering) -- mpm_kernels_sorted.cu
 void launch_force_payload(const GridDesc &gd, const PArr &p, double *S, long long n, cudaStream_t s);
-void launch_build_groups(const GridDesc &gd, const int *off, int *gcount_goff, int *scan_aux, int *grp_cell, int *grp_first,
-                         int *n_groups, cudaStream_t s);
+void launch_build_groups(const GridDesc &gd, const int *off, int *gcount_goff, int *scan_aux, int4 *groups, int *n_groups,
+                         cudaStream_t s);
 void launch_p2g1_sorted(const GridDesc &gd, const PArr &p, const double *S, const GArr &g, const SortedMap &map,
                         long long max_groups, cudaStream_t s);
 void launch_g2p_p2g2_sorted(const GridDesc &gd, const PArr &p, const GArr &g, const double *na, const DevScalars *sc,

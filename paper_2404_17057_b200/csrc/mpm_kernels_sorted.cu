@@ -1,13 +1,15 @@
 // mpm_kernels_sorted.cu -- SORTED kernel family: particles are kept EXACTLY cell-sorted every step and processed in
-// aligned lane groups, one cell per group, one particle per lane (GS = 2^d lanes: 8 in 3D, 4 in 2D).
+// aligned lane groups, one cell per group.  A group has LG = 2^d / 2 lanes (4 in 3D, 2 in 2D) and holds up to 2^d
+// particles of one cell, two per lane (lane l takes particles first + l and first + LG + l).
 //
 // What this buys over the paper's one-thread-per-particle + atomicAdd design:
-//   * scatters (Alg. 1 l.3 and l.8): every lane computes its particle's contribution to the 2^d corners of the cell,
-//     the group sums them with a transposed XOR butterfly (2^d - 1 shuffles per channel) after which lane j owns the
-//     total of corner j, and issues ONE global fp64 reduction per channel: 2^d x fewer REDs, spread over 2^d nodes.
+//   * scatters (Alg. 1 l.3 and l.8): a lane adds up the contributions of its two particles to the 2^d corners of the
+//     cell in registers, the group sums them with a transposed XOR butterfly (2^d - 2 shuffles per channel) after which
+//     lane l owns the totals of corners l and l + LG, and issues ONE global fp64 reduction per corner and channel:
+//     2^d x fewer REDs than one atomicAdd per particle, corner and channel.
 //     (Shared-memory fp64 atomicAdd is a CAS loop on sm_100a -- ATOMS.CAST.SPIN.64 -- so it is never used.)
-//   * gathers (l.6, l.10, l.11): lane j fetches the node values of corner j once per group (16-byte loads from
-//     node-major arrays), parks them in shared memory, and every lane reads all corners back as conflict-free
+//   * gathers (l.6, l.10, l.11): lane l fetches the node values of corners l and l + LG once per group (16-byte loads
+//     from node-major arrays), parks them in shared memory, and every lane reads all corners back as conflict-free
 //     128-bit broadcasts: 2^d x fewer global gathers.
 //   * gradient channels are folded into phi-weighted channels using sum_{b_a} w_a(b_a) = 1:
 //       f_a(b) = +-(1/h) sum_{b_a} T_S(b),  T_S(b) = sum_k S_k phi_b(X_k)             (P2G#1: 1+d+1 channels, not 1+2d)
@@ -16,6 +18,9 @@
 //     and its rank in it (one returning integer atomic), a scan of the per-cell counts gives the new cell offsets, and
 //     the update kernel of l.10-11 writes every particle straight to its sorted slot in the other buffer: no
 //     separate permutation pass.
+//   * kernels are persistent (grid = a multiple of the SM count, grid-stride loop over 16-byte group records, the
+//     next record prefetched while the current group is processed), so the dependent chain in front of the particle
+//     loads is one load deep.
 // A particle whose true cell differs from its group's cell (never the case when the invariant holds; cheap to test)
 // takes a slow path with direct global reductions / gathers, so correctness never depends on the ordering.
 #include "mpm_internal.cuh"
@@ -29,62 +34,70 @@ constexpr unsigned kFull = 0xffffffffu;
 
 template <int DIM>
 struct Geo {
-    static constexpr int GS = 1 << DIM;            // lanes per group = corners per cell
-    static constexpr int NG = 32 / GS;             // groups per warp
-    static constexpr int GPB = kBlock / GS;        // groups per block
-    // shared staging of corner node values: [group][corner][channel]; strides chosen so that the 16-byte broadcast
-    // reads of the NG groups of a warp fall into distinct banks
+    static constexpr int NB = 1 << DIM;            // corners per cell = particles per group
+    static constexpr int LG = NB / 2;              // lanes per group
+    static constexpr int NG = 32 / LG;             // groups per warp
+    static constexpr int GPB = kBlock / LG;        // groups per block and iteration
+    // shared staging of corner node values: [group][corner][channel]; the group stride is == 4 (mod 32) words so that
+    // the 16-byte broadcast reads of the groups of a warp fall into distinct banks
     static constexpr int CH = (DIM == 3) ? 8 : 6;                       // doubles per corner (vbar, acc, dsum, pad)
-    static constexpr int CORNER_STRIDE = CH;                            // doubles
-    static constexpr int GROUP_STRIDE = (DIM == 3) ? 68 : 26;           // doubles: 544 B / 208 B
+    static constexpr int GROUP_STRIDE = (DIM == 3) ? 66 : 34;           // doubles
     static constexpr int WARP_DOUBLES = NG * GROUP_STRIDE;
 };
 
 __device__ __forceinline__ double shfl_xor_d(double v, int m) { return __shfl_xor_sync(kFull, v, m); }
 
-// after the call v[0] holds the group-wide sum for corner j = lane-in-group (see header comment)
+// Transposed butterfly over the LG lanes of a group.  Before: register r of lane l holds the lane's contribution to
+// corner r ^ l.  After: registers r = q * LG (q = 0, 1) hold the group totals of corners l + q * LG.
 template <int DIM>
 __device__ __forceinline__ void butterfly(double v[1 << DIM])
 {
-    if (DIM == 3) {
+    constexpr int NB = 1 << DIM, LG = Geo<DIM>::LG;
 #pragma unroll
-        for (int r = 0; r < 4; ++r) v[r] += shfl_xor_d(v[r + 4], 4);
+    for (int m = LG / 2; m >= 1; m >>= 1) {
+#pragma unroll
+        for (int r = 0; r < NB; ++r)
+            if ((r & m) == 0 && (r & (LG - 1) & ~(2 * m - 1)) == 0) v[r] += shfl_xor_d(v[r | m], m);
     }
-#pragma unroll
-    for (int r = 0; r < 2; ++r) v[r] += shfl_xor_d(v[r + 2], 2);
-    v[0] += shfl_xor_d(v[1], 1);
 }
 
 struct Group {
-    int cell;      // linear cell index of the group
     int first;     // first particle of the group
-    int cnt;       // particles in the group (<= GS), 0 = idle group
+    int cnt;       // particles in the group (<= 2^d), 0 = idle
+    int cell;      // linear cell index
+    int cpack;     // packed cell coordinates (3D: 10 bits each, 2D: 16 bits each)
 };
 
-template <int DIM>
-__device__ __forceinline__ Group load_group(const int *grp_cell, const int *grp_first, const int *off, const int *n_groups,
-                                            int &j)
+__device__ __forceinline__ Group fetch_group(const int4 *__restrict__ groups, long long gidx, int n_groups)
 {
-    constexpr int GS = Geo<DIM>::GS;
-    const long long gidx = (long long)blockIdx.x * Geo<DIM>::GPB + threadIdx.x / GS;
-    j = threadIdx.x % GS;
-    Group g{ 0, 0, 0 };
-    if (gidx < (long long)*n_groups) {
-        g.cell = grp_cell[gidx];
-        g.first = grp_first[gidx];
-        g.cnt = min(GS, off[g.cell + 1] - g.first);
+    Group g{ 0, 0, 0, 0 };
+    if (gidx < (long long)n_groups) {
+        const int4 r = __ldg(groups + gidx);
+        g.first = r.x; g.cnt = r.y; g.cell = r.z; g.cpack = r.w;
     }
     return g;
 }
 
 template <int DIM>
-__device__ __forceinline__ void cell_coords(const GridDesc &gd, int cell, int c[DIM])
+__device__ __forceinline__ void unpack_coords(int cpack, int c[DIM])
 {
+    if (DIM == 3) { c[0] = cpack & 1023; c[1] = (cpack >> 10) & 1023; c[DIM - 1] = (cpack >> 20) & 1023; }
+    else { c[0] = cpack & 65535; c[1] = (cpack >> 16) & 65535; }
+}
+
+// node index of corner b of cell c (periodic wrap: node n == node 0, A11)
+template <int DIM>
+__device__ __forceinline__ int corner_node_i(const GridDesc &gd, const int c[DIM], int b)
+{
+    int idx = 0, stride = 1;
 #pragma unroll
     for (int a = 0; a < DIM; ++a) {
-        c[a] = cell % gd.nc[a];
-        cell /= gd.nc[a];
+        int i = c[a] + ((b >> a) & 1);
+        if (gd.per[a] && i == gd.nc[a]) i = 0;
+        idx += stride * i;
+        stride *= gd.nn[a];
     }
+    return idx;
 }
 
 // local coordinates w.r.t. the GROUP's cell; returns false if the particle's own cell (A6, A19) is a different one
@@ -108,14 +121,14 @@ __device__ __forceinline__ void natural_weights(const double xi[DIM], double w[1
 #pragma unroll
     for (int b = 0; b < (1 << DIM); ++b) w[b] = corner_phi<DIM>(xi, b);
 }
-// ... and in butterfly order (scatters): register r of lane j holds the weight of corner r ^ j
+// ... and in butterfly order (scatters): register r of lane l holds the weight of corner r ^ l (l < LG)
 template <int DIM>
-__device__ __forceinline__ void swizzled_weights(const double xi[DIM], int j, double w[1 << DIM])
+__device__ __forceinline__ void swizzled_weights(const double xi[DIM], int l, double w[1 << DIM])
 {
     double p[DIM][2];
 #pragma unroll
     for (int a = 0; a < DIM; ++a) {
-        const bool hi = (j >> a) & 1;
+        const bool hi = (l >> a) & 1;       // l < LG: only the low axes are ever swapped
         p[a][0] = hi ? xi[a] : 1.0 - xi[a];
         p[a][1] = hi ? 1.0 - xi[a] : xi[a];
     }
@@ -128,10 +141,19 @@ __device__ __forceinline__ void swizzled_weights(const double xi[DIM], int j, do
     }
 }
 
+// max over the warp of a NON-NEGATIVE double with two integer REDUX ops (bit patterns order like the values)
+__device__ __forceinline__ double warp_max_nonneg(double v)
+{
+    const unsigned hi = (unsigned)__double2hiint(v), lo = (unsigned)__double2loint(v);
+    const unsigned mhi = __reduce_max_sync(kFull, hi);
+    const unsigned mlo = __reduce_max_sync(kFull, hi == mhi ? lo : 0u);
+    return __hiloint2double((int)mhi, (int)mlo);
+}
+
 // ---------------------------------------------------------------------------------------------- slow paths
 template <int DIM>
 __device__ __forceinline__ void slow_p2g1(const GridDesc &gd, const GArr &g, const double X[DIM], const double V[DIM],
-                                       double M, double S)
+                                          double M, double S)
 {
     int c[DIM];
     double xi[DIM];
@@ -151,7 +173,7 @@ __device__ __forceinline__ void slow_p2g1(const GridDesc &gd, const GArr &g, con
 
 template <int DIM>
 __device__ __forceinline__ void slow_gather(const GridDesc &gd, const double *na, const double *nb, const double X[DIM],
-                                         double Vb[DIM], double A[DIM], double *D)
+                                            double Vb[DIM], double A[DIM], double *D)
 {
     int c[DIM];
     double xi[DIM];
@@ -191,7 +213,8 @@ __device__ __forceinline__ void slow_p2g2(const GridDesc &gd, const GArr &g, con
 // ---------------------------------------------------------------------------------------------- shared pieces
 
 // Alg. 1 l.11 for one particle: X' = X + dt Vbar, periodic wrap (A11), outflow detection, recycling position (A8),
-// clamp.  Used by BOTH the gather kernel (to find the new cell) and the update kernel (to write X'), so the two agree.
+// clamp.  Used by BOTH the gather kernel (to find the new cell) and the update kernel (to write X'); the update kernel
+// places the particle by the key the gather kernel stored, so a last-bit disagreement could only cost a slow path.
 template <int DIM>
 __device__ __forceinline__ void move_particle(const GridDesc &gd, const double X[DIM], const double Vb[DIM], double dt,
                                               long long id, long long step, double Xn[DIM], bool &recycled, int &nclamp)
@@ -201,8 +224,10 @@ __device__ __forceinline__ void move_particle(const GridDesc &gd, const double X
     for (int a = 0; a < DIM; ++a) {
         double x = fma(dt, Vb[a], X[a]);
         if (gd.per[a]) {
-            x = x - gd.L[a] * floor(x / gd.L[a]);
-            if (x >= gd.L[a]) x = 0.0;
+            if (x < 0.0 || x >= gd.L[a]) {
+                x = x - gd.L[a] * floor(x / gd.L[a]);
+                if (x >= gd.L[a]) x = 0.0;
+            }
         } else {
             if (x < 0.0 && gd.bc[a][0] == MPM_BC_OUTFLOW) recycle = true;
             if (x > gd.L[a] && gd.bc[a][1] == MPM_BC_OUTFLOW) recycle = true;
@@ -251,14 +276,7 @@ __device__ __forceinline__ int cell_key(const GridDesc &gd, const double X[DIM])
     return key;
 }
 
-// node index of corner j of cell c (periodic wrap: node n == node 0)
-template <int DIM>
-__device__ __forceinline__ int group_node(const GridDesc &gd, const int c[DIM], int j)
-{
-    return (int)corner_node<DIM>(gd, c, j);
-}
-
-// lane j stages vbar, acc of corner j (node-major array na[node][2 DIM]) into shared memory; returns nothing
+// lane l stages vbar, acc of one corner (node-major array na[node][2 DIM]) into shared memory
 template <int DIM>
 __device__ __forceinline__ void stage_na(const double *__restrict__ na, int node, double *s_corner)
 {
@@ -268,7 +286,7 @@ __device__ __forceinline__ void stage_na(const double *__restrict__ na, int node
     for (int q = 0; q < DIM; ++q) dst[q] = __ldg(src + q);
 }
 
-// phi-weighted gather of the staged channels: out[c] = sum_b w[b] vals[b][c], c < 2*NP2 (pairs of doubles)
+// phi-weighted gather of the staged channels: out[c] = sum_b w[b] vals[b][c], c < 2*NPAIR
 template <int DIM, int NPAIR>
 __device__ __forceinline__ void gather_pairs(const double *s_group, const double w[1 << DIM], double out[2 * NPAIR])
 {
@@ -276,7 +294,7 @@ __device__ __forceinline__ void gather_pairs(const double *s_group, const double
     for (int c = 0; c < 2 * NPAIR; ++c) out[c] = 0.0;
 #pragma unroll
     for (int b = 0; b < (1 << DIM); ++b) {
-        const double2 *row = reinterpret_cast<const double2 *>(s_group + b * Geo<DIM>::CORNER_STRIDE);
+        const double2 *row = reinterpret_cast<const double2 *>(s_group + b * Geo<DIM>::CH);
 #pragma unroll
         for (int q = 0; q < NPAIR; ++q) {
             const double2 t = row[q];
@@ -290,61 +308,82 @@ __device__ __forceinline__ void gather_pairs(const double *s_group, const double
 // m, mv from phi-weighted channels (M, M V); f from the phi-weighted channel S = (P+Q) M / rho
 template <int DIM>
 __global__ void __launch_bounds__(kBlock) k_p2g1_sorted(GridDesc gd, PArr p, const double *__restrict__ Sarr, GArr g,
-                                                        const int *__restrict__ grp_cell, const int *__restrict__ grp_first,
-                                                        const int *__restrict__ off, const int *__restrict__ n_groups)
+                                                        const int4 *__restrict__ groups, const int *__restrict__ n_groups_p)
 {
-    constexpr int NB = 1 << DIM;
-    int j;
-    const Group grp = load_group<DIM>(grp_cell, grp_first, off, n_groups, j);
-    int c[DIM];
-    cell_coords<DIM>(gd, grp.cell, c);
-    double w[NB];
+    constexpr int NB = 1 << DIM, LG = Geo<DIM>::LG, GPB = Geo<DIM>::GPB;
+    const int n_groups = *n_groups_p;
+    const int l = threadIdx.x % LG;
+    const long long stride = (long long)gridDim.x * GPB;
+    long long gidx = (long long)blockIdx.x * GPB + threadIdx.x / LG;
+    Group next = fetch_group(groups, gidx, n_groups);
+    for (long long g0 = (long long)blockIdx.x * GPB; g0 < n_groups; g0 += stride, gidx += stride) {
+        const Group grp = next;
+        next = fetch_group(groups, gidx + stride, n_groups);
+        int c[DIM];
+        unpack_coords<DIM>(grp.cpack, c);
+        // issue all particle loads first
+        double X[2][DIM], V[2][DIM], M[2], S[2];
+        bool valid[2];
 #pragma unroll
-    for (int r = 0; r < NB; ++r) w[r] = 0.0;
-    double M = 0.0, S = 0.0, MV[DIM];
+        for (int i = 0; i < 2; ++i) {
+            valid[i] = (l + LG * i) < grp.cnt;
+            const long long k = valid[i] ? (long long)grp.first + l + LG * i : 0;
 #pragma unroll
-    for (int a = 0; a < DIM; ++a) MV[a] = 0.0;
-    if (j < grp.cnt) {
-        const long long k = grp.first + j;
-        double X[DIM], V[DIM], xi[DIM];
-#pragma unroll
-        for (int a = 0; a < DIM; ++a) { X[a] = p.x[a][k]; V[a] = p.v[a][k]; }
-        M = p.m[k];
-        S = Sarr[k];
-        if (local_coords<DIM>(gd, X, c, xi)) {
-            swizzled_weights<DIM>(xi, j, w);
-#pragma unroll
-            for (int a = 0; a < DIM; ++a) MV[a] = M * V[a];
-        } else {
-            slow_p2g1<DIM>(gd, g, X, V, M, S);
-            M = 0.0; S = 0.0;
+            for (int a = 0; a < DIM; ++a) { X[i][a] = valid[i] ? p.x[a][k] : 0.0; V[i][a] = valid[i] ? p.v[a][k] : 0.0; }
+            M[i] = valid[i] ? p.m[k] : 0.0;
+            S[i] = valid[i] ? Sarr[k] : 0.0;
         }
-    }
-    // group sums per corner: channels M, M V_a, S
-    double v[NB];
-    double tot[DIM + 2];
+        double w[2][NB];
 #pragma unroll
-    for (int ch = 0; ch < DIM + 2; ++ch) {
-        const double pay = (ch == 0) ? M : (ch == DIM + 1) ? S : MV[ch - 1];
+        for (int i = 0; i < 2; ++i) {
+            double xi[DIM];
+            const bool fast = valid[i] && local_coords<DIM>(gd, X[i], c, xi);
+            if (valid[i] && !fast) { slow_p2g1<DIM>(gd, g, X[i], V[i], M[i], S[i]); M[i] = 0.0; S[i] = 0.0; }
+            if (fast) swizzled_weights<DIM>(xi, l, w[i]);
+            else {
 #pragma unroll
-        for (int r = 0; r < NB; ++r) v[r] = pay * w[r];
-        butterfly<DIM>(v);
-        tot[ch] = v[0];
-    }
-    // force of corner j: f_a = +-(1/h) (T_S(j) + T_S(j ^ bit_a)), sign + where the corner is on the high side of axis a
-    double F[DIM];
+                for (int r = 0; r < NB; ++r) w[i][r] = 0.0;
+            }
+        }
+        // lane totals per corner, then group totals: channels M, M V_a, S
+        double tot[DIM + 2][2];
 #pragma unroll
-    for (int a = 0; a < DIM; ++a) {
-        const double pair = tot[DIM + 1] + shfl_xor_d(tot[DIM + 1], 1 << a);
-        F[a] = ((j >> a) & 1) ? pair * gd.inv_h : -(pair * gd.inv_h);
-    }
-    if (grp.cnt > 0) {
-        const int node = group_node<DIM>(gd, c, j);
-        atomicAdd(&g.m[node], tot[0]);
+        for (int ch = 0; ch < DIM + 2; ++ch) {
+            double pay[2];
+#pragma unroll
+            for (int i = 0; i < 2; ++i) pay[i] = (ch == 0) ? M[i] : (ch == DIM + 1) ? S[i] : M[i] * V[i][ch - 1];
+            double v[NB];
+#pragma unroll
+            for (int r = 0; r < NB; ++r) v[r] = fma(pay[1], w[1][r], pay[0] * w[0][r]);
+            butterfly<DIM>(v);
+            tot[ch][0] = v[0];
+            tot[ch][1] = v[LG];
+        }
+        // forces of corners b_q = l + q LG: f_a = +-(1/h) (T_S(b) + T_S(b ^ bit_a)), + on the high side of axis a
+        double F[DIM][2];
 #pragma unroll
         for (int a = 0; a < DIM; ++a) {
-            atomicAdd(&g.mv[a][node], tot[1 + a]);
-            atomicAdd(&g.f[a][node], F[a]);
+#pragma unroll
+            for (int q = 0; q < 2; ++q) {
+                double other;
+                if ((1 << a) < LG) other = shfl_xor_d(tot[DIM + 1][q], 1 << a);
+                else other = tot[DIM + 1][q ^ 1];
+                const int b = l + q * LG;
+                const double pair = (tot[DIM + 1][q] + other) * gd.inv_h;
+                F[a][q] = ((b >> a) & 1) ? pair : -pair;
+            }
+        }
+        if (grp.cnt > 0) {
+#pragma unroll
+            for (int q = 0; q < 2; ++q) {
+                const int node = corner_node_i<DIM>(gd, c, l + q * LG);
+                atomicAdd(&g.m[node], tot[0][q]);
+#pragma unroll
+                for (int a = 0; a < DIM; ++a) {
+                    atomicAdd(&g.mv[a][node], tot[1 + a][q]);
+                    atomicAdd(&g.f[a][node], F[a][q]);
+                }
+            }
         }
     }
 }
@@ -355,73 +394,100 @@ __global__ void __launch_bounds__(kBlock) k_p2g1_sorted(GridDesc gd, PArr p, con
 template <int DIM>
 __global__ void __launch_bounds__(kBlock) k_g2p_p2g2_sorted(GridDesc gd, PArr p, GArr g, const double *__restrict__ na,
                                                             const DevScalars *__restrict__ sc,
-                                                            const int *__restrict__ grp_cell, const int *__restrict__ grp_first,
-                                                            const int *__restrict__ off, const int *__restrict__ n_groups,
+                                                            const int4 *__restrict__ groups, const int *__restrict__ n_groups_p,
                                                             int *__restrict__ count, unsigned long long *__restrict__ dest)
 {
-    constexpr int NB = 1 << DIM;
+    constexpr int NB = 1 << DIM, LG = Geo<DIM>::LG, GPB = Geo<DIM>::GPB;
     __shared__ __align__(16) double s_vals[(kBlock / 32) * Geo<DIM>::WARP_DOUBLES];
-    int j;
-    const Group grp = load_group<DIM>(grp_cell, grp_first, off, n_groups, j);
-    int c[DIM];
-    cell_coords<DIM>(gd, grp.cell, c);
-    const int warp = threadIdx.x >> 5, gi = (threadIdx.x & 31) / Geo<DIM>::GS;
-    double *s_group = s_vals + warp * Geo<DIM>::WARP_DOUBLES + gi * Geo<DIM>::GROUP_STRIDE;
-    const int node = group_node<DIM>(gd, c, j);
-    if (grp.cnt > 0) stage_na<DIM>(na, node, s_group + j * Geo<DIM>::CORNER_STRIDE);
-    __syncwarp();
+    const int n_groups = *n_groups_p;
     const double dt = sc->dt;
-    double ws[NB];
+    const long long step = sc->step;
+    const int l = threadIdx.x % LG;
+    const int warp = threadIdx.x >> 5, gi = (threadIdx.x & 31) / LG;
+    double *s_group = s_vals + warp * Geo<DIM>::WARP_DOUBLES + gi * Geo<DIM>::GROUP_STRIDE;
+    const long long stride = (long long)gridDim.x * GPB;
+    long long gidx = (long long)blockIdx.x * GPB + threadIdx.x / LG;
+    Group next = fetch_group(groups, gidx, n_groups);
+    for (long long g0 = (long long)blockIdx.x * GPB; g0 < n_groups; g0 += stride, gidx += stride) {
+        const Group grp = next;
+        next = fetch_group(groups, gidx + stride, n_groups);
+        int c[DIM];
+        unpack_coords<DIM>(grp.cpack, c);
+        double X[2][DIM], V[2][DIM], M[2];
+        int id[2];
+        bool valid[2];
 #pragma unroll
-    for (int r = 0; r < NB; ++r) ws[r] = 0.0;
-    double MV[DIM];
+        for (int i = 0; i < 2; ++i) {
+            valid[i] = (l + LG * i) < grp.cnt;
+            const long long k = valid[i] ? (long long)grp.first + l + LG * i : 0;
 #pragma unroll
-    for (int a = 0; a < DIM; ++a) MV[a] = 0.0;
-    if (j < grp.cnt) {
-        const long long k = grp.first + j;
-        double X[DIM], V[DIM], xi[DIM], Vb[DIM], A[DIM];
-#pragma unroll
-        for (int a = 0; a < DIM; ++a) { X[a] = p.x[a][k]; V[a] = p.v[a][k]; }
-        const double M = p.m[k];
-        const bool fast = local_coords<DIM>(gd, X, c, xi);
-        if (fast) {
-            double w[NB], out[2 * DIM];
-            natural_weights<DIM>(xi, w);
-            gather_pairs<DIM, DIM>(s_group, w, out);
-#pragma unroll
-            for (int a = 0; a < DIM; ++a) { Vb[a] = out[a]; A[a] = out[DIM + a]; }
-            swizzled_weights<DIM>(xi, j, ws);
-        } else {
-            slow_gather<DIM>(gd, na, nullptr, X, Vb, A, nullptr);
+            for (int a = 0; a < DIM; ++a) { X[i][a] = valid[i] ? p.x[a][k] : 0.0; V[i][a] = valid[i] ? p.v[a][k] : 0.0; }
+            M[i] = valid[i] ? p.m[k] : 0.0;
+            id[i] = valid[i] ? p.id[k] : 0;
         }
+        int node[2];
 #pragma unroll
-        for (int a = 0; a < DIM; ++a) MV[a] = M * fma(dt, A[a], V[a]);   // M V'
-        if (!fast) {
-            slow_p2g2<DIM>(gd, g, X, MV);
+        for (int q = 0; q < 2; ++q) node[q] = corner_node_i<DIM>(gd, c, l + q * LG);
+        if (grp.cnt > 0) {
 #pragma unroll
-            for (int a = 0; a < DIM; ++a) MV[a] = 0.0;
+            for (int q = 0; q < 2; ++q) stage_na<DIM>(na, node[q], s_group + (l + q * LG) * Geo<DIM>::CH);
         }
-        // where the particle will be after l.11, and its rank among the particles that end up in that cell
-        double Xn[DIM];
-        bool recycled;
-        int nclamp;
-        move_particle<DIM>(gd, X, Vb, dt, (long long)p.id[k], sc->step, Xn, recycled, nclamp);
-        const int key = cell_key<DIM>(gd, Xn);
-        const int rank = atomicAdd(&count[key], 1);
-        dest[k] = ((unsigned long long)(unsigned)key << 32) | (unsigned)rank;
-    }
-    double v[NB];
-    double tot[DIM];
+        __syncwarp();
+        double ws[2][NB], MV[2][DIM];
 #pragma unroll
-    for (int a = 0; a < DIM; ++a) {
+        for (int i = 0; i < 2; ++i) {
 #pragma unroll
-        for (int r = 0; r < NB; ++r) v[r] = MV[a] * ws[r];
-        butterfly<DIM>(v);
-        tot[a] = v[0];
-    }
-    if (grp.cnt > 0) {
+            for (int r = 0; r < NB; ++r) ws[i][r] = 0.0;
 #pragma unroll
-        for (int a = 0; a < DIM; ++a) atomicAdd(&g.mv2[a][node], tot[a]);
+            for (int a = 0; a < DIM; ++a) MV[i][a] = 0.0;
+            if (valid[i]) {
+                const long long k = (long long)grp.first + l + LG * i;
+                double xi[DIM], Vb[DIM], A[DIM];
+                const bool fast = local_coords<DIM>(gd, X[i], c, xi);
+                if (fast) {
+                    double w[NB], out[2 * DIM];
+                    natural_weights<DIM>(xi, w);
+                    gather_pairs<DIM, DIM>(s_group, w, out);
+#pragma unroll
+                    for (int a = 0; a < DIM; ++a) { Vb[a] = out[a]; A[a] = out[DIM + a]; }
+                    swizzled_weights<DIM>(xi, l, ws[i]);
+                } else {
+                    slow_gather<DIM>(gd, na, nullptr, X[i], Vb, A, nullptr);
+                }
+#pragma unroll
+                for (int a = 0; a < DIM; ++a) MV[i][a] = M[i] * fma(dt, A[a], V[i][a]);   // M V'
+                if (!fast) {
+                    slow_p2g2<DIM>(gd, g, X[i], MV[i]);
+#pragma unroll
+                    for (int a = 0; a < DIM; ++a) MV[i][a] = 0.0;
+                }
+                // where the particle will be after l.11, and its rank among the particles that end up in that cell
+                double Xn[DIM];
+                bool recycled;
+                int nclamp;
+                move_particle<DIM>(gd, X[i], Vb, dt, (long long)id[i], step, Xn, recycled, nclamp);
+                const int key = cell_key<DIM>(gd, Xn);
+                const int rank = atomicAdd(&count[key], 1);
+                dest[k] = ((unsigned long long)(unsigned)key << 32) | (unsigned)rank;
+            }
+        }
+        double tot[DIM][2];
+#pragma unroll
+        for (int a = 0; a < DIM; ++a) {
+            double v[NB];
+#pragma unroll
+            for (int r = 0; r < NB; ++r) v[r] = fma(MV[1][a], ws[1][r], MV[0][a] * ws[0][r]);
+            butterfly<DIM>(v);
+            tot[a][0] = v[0];
+            tot[a][1] = v[LG];
+        }
+        if (grp.cnt > 0) {
+#pragma unroll
+            for (int q = 0; q < 2; ++q)
+#pragma unroll
+                for (int a = 0; a < DIM; ++a) atomicAdd(&g.mv2[a][node[q]], tot[a][q]);
+        }
+        __syncwarp();      // the staging area is rewritten by the next iteration
     }
 }
 
@@ -432,117 +498,154 @@ __global__ void __launch_bounds__(kBlock) k_g2p_p2g2_sorted(GridDesc gd, PArr p,
 template <int DIM>
 __global__ void __launch_bounds__(kBlock) k_update_sorted(GridDesc gd, PArr p, PArr q, const double *__restrict__ na,
                                                           const double *__restrict__ nb, DevScalars *sc,
-                                                          const int *__restrict__ grp_cell, const int *__restrict__ grp_first,
-                                                          const int *__restrict__ off, const int *__restrict__ n_groups,
+                                                          const int4 *__restrict__ groups, const int *__restrict__ n_groups_p,
                                                           const int *__restrict__ off_new,
                                                           const unsigned long long *__restrict__ dest, double *__restrict__ S_out)
 {
-    constexpr int NB = 1 << DIM;
+    constexpr int NB = 1 << DIM, LG = Geo<DIM>::LG, GPB = Geo<DIM>::GPB;
     constexpr int NPAIR = (DIM == 3) ? 4 : 3;
     __shared__ __align__(16) double s_vals[(kBlock / 32) * Geo<DIM>::WARP_DOUBLES];
     __shared__ double s_v[kBlock / 32], s_c[kBlock / 32];
-    int j;
-    const Group grp = load_group<DIM>(grp_cell, grp_first, off, n_groups, j);
-    int c[DIM];
-    cell_coords<DIM>(gd, grp.cell, c);
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, gi = lane / Geo<DIM>::GS;
+    const int n_groups = *n_groups_p;
+    const double dt = sc->dt;
+    const long long step = sc->step;
+    const int l = threadIdx.x % LG;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, gi = lane / LG;
     double *s_group = s_vals + warp * Geo<DIM>::WARP_DOUBLES + gi * Geo<DIM>::GROUP_STRIDE;
-    const int node = group_node<DIM>(gd, c, j);
-    // stage vbar, acc of corner j, and dsum_j = sum_a (v2_a(high corner) - v2_a(low corner)) / h
-    double v2[DIM];
-#pragma unroll
-    for (int a = 0; a < DIM; ++a) v2[a] = (grp.cnt > 0) ? __ldg(nb + (long long)node * DIM + a) : 0.0;
-    double dsum = 0.0;
-#pragma unroll
-    for (int a = 0; a < DIM; ++a) {
-        const double other = shfl_xor_d(v2[a], 1 << a);
-        dsum += ((j >> a) & 1) ? (v2[a] - other) : (other - v2[a]);
-    }
-    if (grp.cnt > 0) {
-        stage_na<DIM>(na, node, s_group + j * Geo<DIM>::CORNER_STRIDE);
-        s_group[j * Geo<DIM>::CORNER_STRIDE + 2 * DIM] = dsum * gd.inv_h;
-        if (DIM == 3) s_group[j * Geo<DIM>::CORNER_STRIDE + 7] = 0.0; else s_group[j * Geo<DIM>::CORNER_STRIDE + 5] = 0.0;
-    }
-    __syncwarp();
+    const long long stride = (long long)gridDim.x * GPB;
+    long long gidx = (long long)blockIdx.x * GPB + threadIdx.x / LG;
+    Group next = fetch_group(groups, gidx, n_groups);
     double vloc = 0.0, cloc = 0.0;
     int n_rec = 0, n_clamp = 0, n_neg = 0, n_nonfin = 0;
-    if (j < grp.cnt) {
-        const long long k = grp.first + j;
-        const double dt = sc->dt;
-        double X[DIM], V[DIM], xi[DIM], Vb[DIM], A[DIM], D;
+    const double gm1 = gd.gamma - 1.0;
+    for (long long g0 = (long long)blockIdx.x * GPB; g0 < n_groups; g0 += stride, gidx += stride) {
+        const Group grp = next;
+        next = fetch_group(groups, gidx + stride, n_groups);
+        int c[DIM];
+        unpack_coords<DIM>(grp.cpack, c);
+        double X[2][DIM], V[2][DIM], M[2], rho[2], E[2];
+        int id[2];
+        unsigned long long dk[2];
+        bool valid[2];
 #pragma unroll
-        for (int a = 0; a < DIM; ++a) { X[a] = p.x[a][k]; V[a] = p.v[a][k]; }
-        double M = p.m[k], rho = p.rho[k], E = p.e[k];
-        const int id = p.id[k];
-        const unsigned long long dk = dest[k];
-        if (local_coords<DIM>(gd, X, c, xi)) {
-            double w[NB], out[2 * NPAIR];
-            natural_weights<DIM>(xi, w);
-            gather_pairs<DIM, NPAIR>(s_group, w, out);
+        for (int i = 0; i < 2; ++i) {
+            valid[i] = (l + LG * i) < grp.cnt;
+            const long long k = valid[i] ? (long long)grp.first + l + LG * i : 0;
 #pragma unroll
-            for (int a = 0; a < DIM; ++a) { Vb[a] = out[a]; A[a] = out[DIM + a]; }
-            D = out[2 * DIM];
-        } else {
-            slow_gather<DIM>(gd, na, nb, X, Vb, A, &D);
+            for (int a = 0; a < DIM; ++a) { X[i][a] = valid[i] ? p.x[a][k] : 0.0; V[i][a] = valid[i] ? p.v[a][k] : 0.0; }
+            M[i] = valid[i] ? p.m[k] : 0.0;
+            rho[i] = valid[i] ? p.rho[k] : 1.0;
+            E[i] = valid[i] ? p.e[k] : 0.0;
+            id[i] = valid[i] ? p.id[k] : 0;
+            dk[i] = valid[i] ? dest[k] : 0ull;
         }
+        // stage vbar, acc of corners l, l + LG, and dsum_b = sum_a (v2_a(high corner) - v2_a(low corner)) / h
+        double v2[2][DIM];
+        int node[2];
 #pragma unroll
-        for (int a = 0; a < DIM; ++a) V[a] = fma(dt, A[a], V[a]);   // V'
-        // particle thermodynamics (eq. 4 with this step's D: reading A2)
-        const double P = (gd.gamma - 1.0) * rho * E;
-        double Q = 0.0;
-        if (D < 0.0) {
-            const double cs0 = sqrt(gd.gamma * P / rho);
-            if (gd.visc_form == MPM_VISC_STANDARD)
-                Q = rho * (gd.c0 * gd.h * gd.h * D * D - gd.c1 * gd.h * cs0 * D);
-            else
-                Q = gd.c0 * (rho * gd.h * D) * (rho * gd.h * D) - gd.c1 * gd.h * cs0 * D;
+        for (int qq = 0; qq < 2; ++qq) {
+            node[qq] = corner_node_i<DIM>(gd, c, l + qq * LG);
+#pragma unroll
+            for (int a = 0; a < DIM; ++a) v2[qq][a] = (grp.cnt > 0) ? __ldg(nb + (long long)node[qq] * DIM + a) : 0.0;
         }
-        double En = E + dt * (-(P + Q) / rho) * D;
-        const double jac = 1.0 + dt * D;
-        if (jac <= 0.0) n_neg = 1;
-        double rhon = rho / jac;
-        const double Pn = (gd.gamma - 1.0) * rhon * En;
-        const double cs = sqrt(gd.gamma * Pn / rhon);
-        if (!isfinite(En) || !isfinite(rhon)) n_nonfin = 1;
-        double vv = 0.0, vb2 = 0.0;
+        double dsum[2] = { 0.0, 0.0 };
 #pragma unroll
-        for (int a = 0; a < DIM; ++a) { vv += V[a] * V[a]; vb2 += Vb[a] * Vb[a]; }
-        vloc = fmax(sqrt(vv), sqrt(vb2));
-        cloc = cs;
-        double Xn[DIM];
-        bool recycled;
-        move_particle<DIM>(gd, X, Vb, dt, (long long)id, sc->step, Xn, recycled, n_clamp);
-        if (recycled) {
+        for (int a = 0; a < DIM; ++a) {
 #pragma unroll
-            for (int a = 0; a < DIM; ++a) V[a] = gd.inflow_v[a];
-            rhon = gd.inflow_rho; En = gd.inflow_e; Q = 0.0; M = gd.inflow_mass;
-            n_rec = 1;
+            for (int qq = 0; qq < 2; ++qq) {
+                double other;
+                if ((1 << a) < LG) other = shfl_xor_d(v2[qq][a], 1 << a);
+                else other = v2[qq ^ 1][a];
+                const int b = l + qq * LG;
+                dsum[qq] += ((b >> a) & 1) ? (v2[qq][a] - other) : (other - v2[qq][a]);
+            }
         }
-        const long long dst = (long long)off_new[(int)(dk >> 32)] + (long long)(unsigned)(dk & 0xffffffffull);
+        if (grp.cnt > 0) {
 #pragma unroll
-        for (int a = 0; a < DIM; ++a) { q.x[a][dst] = Xn[a]; q.v[a][dst] = V[a]; }
-        q.m[dst] = M;
-        q.rho[dst] = rhon;
-        q.e[dst] = En;
-        q.q[dst] = Q;
-        q.id[dst] = id;
-        S_out[dst] = ((gd.gamma - 1.0) * rhon * En + Q) * M / rhon;     // eq. (13) payload of the next step
+            for (int qq = 0; qq < 2; ++qq) {
+                double *s_corner = s_group + (l + qq * LG) * Geo<DIM>::CH;
+                stage_na<DIM>(na, node[qq], s_corner);
+                *reinterpret_cast<double2 *>(s_corner + 2 * DIM) = make_double2(dsum[qq] * gd.inv_h, 0.0);
+            }
+        }
+        __syncwarp();
+#pragma unroll
+        for (int i = 0; i < 2; ++i) {
+            if (valid[i]) {
+                double xi[DIM], Vb[DIM], A[DIM], D;
+                if (local_coords<DIM>(gd, X[i], c, xi)) {
+                    double w[NB], out[2 * NPAIR];
+                    natural_weights<DIM>(xi, w);
+                    gather_pairs<DIM, NPAIR>(s_group, w, out);
+#pragma unroll
+                    for (int a = 0; a < DIM; ++a) { Vb[a] = out[a]; A[a] = out[DIM + a]; }
+                    D = out[2 * DIM];
+                } else {
+                    slow_gather<DIM>(gd, na, nb, X[i], Vb, A, &D);
+                }
+                double Vn[DIM];
+#pragma unroll
+                for (int a = 0; a < DIM; ++a) Vn[a] = fma(dt, A[a], V[i][a]);   // V'
+                // particle thermodynamics (eq. 4 with this step's D: reading A2).  P/rho = (gamma-1) E
+                // and gamma P/rho = gamma (gamma-1) E are used in place of the quotients (one rounding apart).
+                const double r = rho[i], e0 = E[i];
+                double Q = 0.0, Q_over_rho = 0.0;
+                if (D < 0.0) {
+                    const double cs0 = sqrt(gd.gamma * gm1 * e0);
+                    if (gd.visc_form == MPM_VISC_STANDARD) {
+                        Q_over_rho = gd.c0 * gd.h * gd.h * D * D - gd.c1 * gd.h * cs0 * D;
+                        Q = r * Q_over_rho;
+                    } else {
+                        Q = gd.c0 * (r * gd.h * D) * (r * gd.h * D) - gd.c1 * gd.h * cs0 * D;
+                        Q_over_rho = Q / r;
+                    }
+                }
+                double En = e0 - dt * (gm1 * e0 + Q_over_rho) * D;
+                const double jac = fma(dt, D, 1.0);
+                if (jac <= 0.0) n_neg++;
+                double rhon = r / jac;
+                const double cs = sqrt(gd.gamma * gm1 * En);
+                if (!isfinite(En) || !isfinite(rhon)) n_nonfin++;
+                double vv = 0.0, vb2 = 0.0;
+#pragma unroll
+                for (int a = 0; a < DIM; ++a) { vv = fma(Vn[a], Vn[a], vv); vb2 = fma(Vb[a], Vb[a], vb2); }
+                vloc = fmax(vloc, fmax(vv, vb2));      // squared; the root is taken once at the end
+                cloc = fmax(cloc, cs);
+                double Xn[DIM];
+                bool recycled;
+                int nclamp;
+                move_particle<DIM>(gd, X[i], Vb, dt, (long long)id[i], step, Xn, recycled, nclamp);
+                n_clamp += nclamp;
+                double Mn = M[i];
+                if (recycled) {
+#pragma unroll
+                    for (int a = 0; a < DIM; ++a) Vn[a] = gd.inflow_v[a];
+                    rhon = gd.inflow_rho; En = gd.inflow_e; Q = 0.0; Mn = gd.inflow_mass;
+                    n_rec++;
+                }
+                const long long dst = (long long)off_new[(int)(dk[i] >> 32)] + (long long)(unsigned)(dk[i] & 0xffffffffull);
+#pragma unroll
+                for (int a = 0; a < DIM; ++a) { q.x[a][dst] = Xn[a]; q.v[a][dst] = Vn[a]; }
+                q.m[dst] = Mn;
+                q.rho[dst] = rhon;
+                q.e[dst] = En;
+                q.q[dst] = Q;
+                q.id[dst] = id[i];
+                S_out[dst] = (gm1 * rhon * En + Q) * Mn / rhon;     // eq. (13) payload of the next step
+            }
+        }
+        __syncwarp();      // the staging area is rewritten by the next iteration
     }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        vloc = fmax(vloc, __shfl_xor_sync(kFull, vloc, o));
-        cloc = fmax(cloc, __shfl_xor_sync(kFull, cloc, o));
-    }
+    // block maxima -> one atomicMax per block (max is order-free, so this is exact)
+    vloc = warp_max_nonneg(sqrt(vloc));
+    cloc = warp_max_nonneg(cloc >= 0.0 ? cloc : 0.0);
     if (lane == 0) { s_v[warp] = vloc; s_c[warp] = cloc; }
-    const unsigned any_rec = __ballot_sync(kFull, n_rec), any_neg = __ballot_sync(kFull, n_neg),
-                   any_nf = __ballot_sync(kFull, n_nonfin);
-    int clamp_sum = n_clamp;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) clamp_sum += __shfl_xor_sync(kFull, clamp_sum, o);
+    const int rec_sum = __reduce_add_sync(kFull, n_rec), neg_sum = __reduce_add_sync(kFull, n_neg),
+              nf_sum = __reduce_add_sync(kFull, n_nonfin), clamp_sum = __reduce_add_sync(kFull, n_clamp);
     if (lane == 0) {
-        if (any_rec) atomicAdd(&sc->n_recycled, (unsigned long long)__popc(any_rec));
-        if (any_neg) atomicAdd(&sc->n_negjac, (unsigned long long)__popc(any_neg));
-        if (any_nf) atomicAdd(&sc->n_nonfinite, (unsigned long long)__popc(any_nf));
+        if (rec_sum) atomicAdd(&sc->n_recycled, (unsigned long long)rec_sum);
+        if (neg_sum) atomicAdd(&sc->n_negjac, (unsigned long long)neg_sum);
+        if (nf_sum) atomicAdd(&sc->n_nonfinite, (unsigned long long)nf_sum);
         if (clamp_sum) atomicAdd(&sc->n_clamped, (unsigned long long)clamp_sum);
     }
     __syncthreads();
@@ -565,27 +668,49 @@ __global__ void __launch_bounds__(kBlock) k_force_payload(double gamma, const do
     if (k < n) S[k] = ((gamma - 1.0) * rho[k] * e[k] + q[k]) * m[k] / rho[k];
 }
 
-// groups per cell = ceil(count / GS), from the cell offsets
-__global__ void __launch_bounds__(kBlock) k_group_counts(const int *off, int *gcount, int ncell, int gs)
+// groups per cell = ceil(count / capacity), from the cell offsets
+__global__ void __launch_bounds__(kBlock) k_group_counts(const int *off, int *gcount, int ncell, int cap)
 {
     const int c = blockIdx.x * kBlock + threadIdx.x;
-    if (c < ncell) gcount[c] = (off[c + 1] - off[c] + gs - 1) / gs;
+    if (c < ncell) gcount[c] = (off[c + 1] - off[c] + cap - 1) / cap;
     else if (c == ncell) gcount[c] = 0;
 }
 
-// fill the group map from the scanned group offsets; goff[ncell] = total number of groups
-__global__ void __launch_bounds__(kBlock) k_group_fill(const int *off, const int *goff, int *grp_cell, int *grp_first,
-                                                       int *n_groups, int ncell, int gs)
+// fill the group records from the scanned group offsets; goff[ncell] = total number of groups
+template <int DIM>
+__global__ void __launch_bounds__(kBlock) k_group_fill(GridDesc gd, const int *off, const int *goff, int4 *groups,
+                                                       int *n_groups, int ncell)
 {
+    constexpr int CAP = 1 << DIM;
     const int c = blockIdx.x * kBlock + threadIdx.x;
     if (c == 0) *n_groups = goff[ncell];
     if (c >= ncell) return;
     const int g0 = goff[c], g1 = goff[c + 1];
+    if (g0 == g1) return;
+    int cpack;
+    if (DIM == 3) {
+        const int cx = c % gd.nc[0], cy = (c / gd.nc[0]) % gd.nc[1], cz = c / (gd.nc[0] * gd.nc[1]);
+        cpack = cx | (cy << 10) | (cz << 20);
+    } else {
+        cpack = (c % gd.nc[0]) | ((c / gd.nc[0]) << 16);
+    }
     int first = off[c];
-    for (int g = g0; g < g1; ++g, first += gs) { grp_cell[g] = c; grp_first[g] = first; }
+    const int end = off[c + 1];
+    for (int gq = g0; gq < g1; ++gq, first += CAP) groups[gq] = make_int4(first, min(CAP, end - first), c, cpack);
 }
 
 inline unsigned blocks_for(long long n, int per) { return (unsigned)((n + per - 1) / per); }
+
+// persistent launch: enough blocks to fill the 148 SMs a few times over, never more than the work needs
+inline unsigned persistent_blocks(long long max_groups, int gpb, int per_sm)
+{
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const long long want = (long long)sms * per_sm;
+    const long long need = (max_groups + gpb - 1) / gpb;
+    return (unsigned)(need < want ? (need > 0 ? need : 1) : want);
+}
 
 }  // namespace
 
@@ -594,14 +719,15 @@ void launch_force_payload(const GridDesc &gd, const PArr &p, double *S, long lon
     if (n > 0) k_force_payload<<<blocks_for(n, kBlock), kBlock, 0, s>>>(gd.gamma, p.m, p.rho, p.e, p.q, S, n);
 }
 
-void launch_build_groups(const GridDesc &gd, const int *off, int *gcount_goff, int *scan_aux, int *grp_cell, int *grp_first,
-                         int *n_groups, cudaStream_t s)
+void launch_build_groups(const GridDesc &gd, const int *off, int *gcount_goff, int *scan_aux, int4 *groups, int *n_groups,
+                         cudaStream_t s)
 {
-    const int gs = 1 << gd.dim;
+    const int cap = 1 << gd.dim;
     const int ncell = (int)gd.Nc;
-    k_group_counts<<<blocks_for(ncell + 1, kBlock), kBlock, 0, s>>>(off, gcount_goff, ncell, gs);
+    k_group_counts<<<blocks_for(ncell + 1, kBlock), kBlock, 0, s>>>(off, gcount_goff, ncell, cap);
     launch_exclusive_scan(gcount_goff, ncell + 1, scan_aux, s);
-    k_group_fill<<<blocks_for(ncell, kBlock), kBlock, 0, s>>>(off, gcount_goff, grp_cell, grp_first, n_groups, ncell, gs);
+    if (gd.dim == 2) k_group_fill<2><<<blocks_for(ncell, kBlock), kBlock, 0, s>>>(gd, off, gcount_goff, groups, n_groups, ncell);
+    else k_group_fill<3><<<blocks_for(ncell, kBlock), kBlock, 0, s>>>(gd, off, gcount_goff, groups, n_groups, ncell);
 }
 
 void launch_p2g1_sorted(const GridDesc &gd, const PArr &p, const double *S, const GArr &g, const SortedMap &map,
@@ -609,9 +735,9 @@ void launch_p2g1_sorted(const GridDesc &gd, const PArr &p, const double *S, cons
 {
     if (max_groups <= 0) return;
     if (gd.dim == 2)
-        k_p2g1_sorted<2><<<blocks_for(max_groups, Geo<2>::GPB), kBlock, 0, s>>>(gd, p, S, g, map.grp_cell, map.grp_first, map.off, map.n_groups);
+        k_p2g1_sorted<2><<<persistent_blocks(max_groups, Geo<2>::GPB, 8), kBlock, 0, s>>>(gd, p, S, g, map.groups, map.n_groups);
     else
-        k_p2g1_sorted<3><<<blocks_for(max_groups, Geo<3>::GPB), kBlock, 0, s>>>(gd, p, S, g, map.grp_cell, map.grp_first, map.off, map.n_groups);
+        k_p2g1_sorted<3><<<persistent_blocks(max_groups, Geo<3>::GPB, 8), kBlock, 0, s>>>(gd, p, S, g, map.groups, map.n_groups);
 }
 
 void launch_g2p_p2g2_sorted(const GridDesc &gd, const PArr &p, const GArr &g, const double *na, const DevScalars *sc,
@@ -619,9 +745,9 @@ void launch_g2p_p2g2_sorted(const GridDesc &gd, const PArr &p, const GArr &g, co
 {
     if (max_groups <= 0) return;
     if (gd.dim == 2)
-        k_g2p_p2g2_sorted<2><<<blocks_for(max_groups, Geo<2>::GPB), kBlock, 0, s>>>(gd, p, g, na, sc, map.grp_cell, map.grp_first, map.off, map.n_groups, count, dest);
+        k_g2p_p2g2_sorted<2><<<persistent_blocks(max_groups, Geo<2>::GPB, 8), kBlock, 0, s>>>(gd, p, g, na, sc, map.groups, map.n_groups, count, dest);
     else
-        k_g2p_p2g2_sorted<3><<<blocks_for(max_groups, Geo<3>::GPB), kBlock, 0, s>>>(gd, p, g, na, sc, map.grp_cell, map.grp_first, map.off, map.n_groups, count, dest);
+        k_g2p_p2g2_sorted<3><<<persistent_blocks(max_groups, Geo<3>::GPB, 8), kBlock, 0, s>>>(gd, p, g, na, sc, map.groups, map.n_groups, count, dest);
 }
 
 void launch_update_sorted(const GridDesc &gd, const PArr &p, const PArr &q, const double *na, const double *nb, DevScalars *sc,
@@ -630,9 +756,9 @@ void launch_update_sorted(const GridDesc &gd, const PArr &p, const PArr &q, cons
 {
     if (max_groups <= 0) return;
     if (gd.dim == 2)
-        k_update_sorted<2><<<blocks_for(max_groups, Geo<2>::GPB), kBlock, 0, s>>>(gd, p, q, na, nb, sc, map.grp_cell, map.grp_first, map.off, map.n_groups, off_new, dest, S_out);
+        k_update_sorted<2><<<persistent_blocks(max_groups, Geo<2>::GPB, 8), kBlock, 0, s>>>(gd, p, q, na, nb, sc, map.groups, map.n_groups, off_new, dest, S_out);
     else
-        k_update_sorted<3><<<blocks_for(max_groups, Geo<3>::GPB), kBlock, 0, s>>>(gd, p, q, na, nb, sc, map.grp_cell, map.grp_first, map.off, map.n_groups, off_new, dest, S_out);
+        k_update_sorted<3><<<persistent_blocks(max_groups, Geo<3>::GPB, 8), kBlock, 0, s>>>(gd, p, q, na, nb, sc, map.groups, map.n_groups, off_new, dest, S_out);
 }
 
 }  // namespace mpm
