@@ -157,6 +157,22 @@ def oracle_rate(workload, size, steps, warmup=0):
     return n * steps / dt, dt, n, w["name"]
 
 
+def max_over_ranks(value, world, device="cpu"):
+    """max of a host float over all ranks (the contract's max-over-ranks timing); works for nccl (cuda) and gloo (cpu)."""
+    if world <= 1:
+        return float(value)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_rate(n_per_rank, steps, ms_max, world):
+    """particle-steps/s of the WHOLE job: every rank advances n_per_rank particles (weak scaling, replicas)."""
+    return world * n_per_rank * steps / (ms_max * 1e-3)
+
+
 def run_reference(args):
     """--impl reference: the oracle as it stands on the host cores; each step is one oracle step on a bounded sample."""
     rank = int(os.environ.get("RANK", "0"))
@@ -219,11 +235,8 @@ def run_ours(args):
     ms = ev0.elapsed_time(ev1)
     st = g.stats()
     launches = int(st.launches - launches0) - 2          # minus the stats reduction itself
-    if world > 1:
-        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = world * n_p * args.steps / (ms * 1e-3)
+    ms = max_over_ranks(ms, world, "cuda")
+    value = whole_job_rate(n_p, args.steps, ms, world)
 
     # ---- per-kernel durations (CUDA events on the launching stream, separate pass so the timers do not perturb `value`)
     prof_steps = min(args.steps, 10)
@@ -274,11 +287,8 @@ def run_ours(args):
             g.read_particles(out=out, location=mpm.HOST)
         barrier()
         e2e_s = time.perf_counter() - t0
-        if world > 1:
-            t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            e2e_s = float(t.item())
-        line["e2e"] = {"value": world * n_p * esteps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d,
+        e2e_s = max_over_ranks(e2e_s, world, "cuda")
+        line["e2e"] = {"value": whole_job_rate(n_p, esteps, e2e_s * 1e3, world), "unit": UNIT, "h2d_bytes_per_step": h2d,
                        "d2h_bytes_per_step": d2h, "steps": esteps,
                        "note": "each step: mpm_load_particles(pinned host) + mpm_step(1) + mpm_read_particles(pinned host)"}
         del pinned, out
