@@ -214,8 +214,8 @@ def run_ours(args):
     w = make_workload(args.workload, args.size, rank)
     cfg, dim = w["cfg"], w["cfg"]["dim"]
     n_p = int(w["mass"].shape[0])
-    g = mpm.Solver(cfg, sort_every=1, variant=mpm.VARIANT_SORTED if args.variant == "sorted" else mpm.VARIANT_ATOMIC,
-                   device=local)
+    variant = {"tiled": mpm.VARIANT_TILED, "sorted": mpm.VARIANT_SORTED, "atomic": mpm.VARIANT_ATOMIC}[args.variant]
+    g = mpm.Solver(cfg, sort_every=1, variant=variant, device=local)
     n_n = g.num_nodes
     g.load_particles(w["x"], w["v"], w["mass"], w["rho"], w["e"])          # inputs resident in HBM before timing
     stream = g.stream
@@ -315,7 +315,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="sedov", choices=["sedov", "clumps", "cylinder", "box", "sod"])
     ap.add_argument("--size", type=int, default=0, help="grid resolution override (0 = BASELINE.json size)")
-    ap.add_argument("--variant", default="sorted", choices=["sorted", "atomic"])
+    ap.add_argument("--variant", default="tiled", choices=["tiled", "sorted", "atomic"])
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -52,13 +52,16 @@ enum { MPM_HOST = 0, MPM_DEVICE = 1 };
 enum { MPM_BC_PERIODIC = 0, MPM_BC_REFLECT = 1, MPM_BC_INFLOW = 2, MPM_BC_OUTFLOW = 3 };
 /* artificial viscosity q of eq. (4): as printed, or the textbook rho (c0 h^2 D^2 - c1 h c_s D) */
 enum { MPM_VISC_PRINTED = 0, MPM_VISC_STANDARD = 1 };
-/* kernel family.  AUTO = SORTED when sort_every == 1, else ATOMIC.
+/* kernel family.  AUTO = TILED when sort_every == 1, else ATOMIC.
  * ATOMIC: one thread per particle, global fp64 atomics (the paper's design); any particle order;
  *         sort_every = k > 0 adds a separate cell-key counting sort every k steps.
  * SORTED: particles are kept exactly cell-sorted every step (the re-ordering is fused into the sweeps); one cell per
  *         group of 2^dim lanes, contributions summed inside the group before one global reduction per corner and
- *         channel, corner node values staged once per group.  Ignores sort_every (always 1). */
-enum { MPM_VARIANT_AUTO = 0, MPM_VARIANT_ATOMIC = 1, MPM_VARIANT_SORTED = 2 };
+ *         channel, corner node values staged once per group.  Ignores sort_every (always 1).
+ * TILED:  SORTED's lane groups with tile-major cell order, even-aligned cell slots (128-bit particle loads) and
+ *         shared-memory grid tiles: node values of a tile are loaded once per block, scatters accumulate in shared
+ *         memory and reach global memory as one reduction per tile node.  Ignores sort_every (always 1). */
+enum { MPM_VARIANT_AUTO = 0, MPM_VARIANT_ATOMIC = 1, MPM_VARIANT_SORTED = 2, MPM_VARIANT_TILED = 3 };
 /* particle fields (bit mask for mpm_read_particles; output pointers are consumed in this order, a vector field
  * takes `dim` pointers) */
 enum { MPM_P_X = 1, MPM_P_V = 2, MPM_P_M = 4, MPM_P_RHO = 8, MPM_P_E = 16, MPM_P_Q = 32 };

@@ -16,7 +16,7 @@ OK, E_ARG, E_CUDA, E_OOM, E_STATE, E_NONFINITE = 0, -1, -2, -3, -4, -5
 HOST, DEVICE = 0, 1
 BC_PERIODIC, BC_REFLECT, BC_INFLOW, BC_OUTFLOW = 0, 1, 2, 3
 VISC_PRINTED, VISC_STANDARD = 0, 1
-VARIANT_AUTO, VARIANT_ATOMIC, VARIANT_SORTED = 0, 1, 2
+VARIANT_AUTO, VARIANT_ATOMIC, VARIANT_SORTED, VARIANT_TILED = 0, 1, 2, 3
 P_X, P_V, P_M, P_RHO, P_E, P_Q = 1, 2, 4, 8, 16, 32
 G_MASS, G_MOMENTUM, G_FORCE, G_MOMENTUM2, G_NORMAL, G_FLAG = 0, 1, 2, 3, 4, 5
 

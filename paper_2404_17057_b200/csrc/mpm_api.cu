@@ -29,6 +29,8 @@ struct mpm_handle {
     // re-ordering), group map, force payload S (double-buffered with the particles), destination records
     int *off[2];
     int ocur;
+    int *coff;            // TILED: compact storage offsets, allocated on the first storage-order read
+    long long slots;      // TILED: allocated slots per particle array (particles + one spare slot per odd cell)
     int *goff, *n_groups;
     int4 *groups;
     double *S[2];
@@ -226,7 +228,10 @@ void free_particles(mpm_handle *h)
 int alloc_particles(mpm_handle *h, long long n)
 {
     free_particles(h);
-    const size_t N = (size_t)(n > 0 ? n : 1);
+    // TILED: every cell's slot range starts at an even slot -> at most one unused slot per occupied cell
+    const bool tiled = h->variant == MPM_VARIANT_TILED;
+    h->slots = tiled ? n + (n < h->gd.Nc ? n : h->gd.Nc) + 8 : n;
+    const size_t N = (size_t)(h->slots > 0 ? h->slots : 1);
     bool ok = true;
     for (int b = 0; b < 2 && ok; ++b) {
         PArr &p = h->pbuf[b];
@@ -235,13 +240,24 @@ int alloc_particles(mpm_handle *h, long long n)
              dev_alloc_t(h, &p.q, N) && dev_alloc_t(h, &p.id, N);
     }
     ok = ok && dev_alloc_t(h, &h->key, N) && dev_alloc_t(h, &h->rank, N);
-    if (ok && h->variant == MPM_VARIANT_SORTED) {
+    if (ok && (h->variant == MPM_VARIANT_SORTED || tiled)) {
         const long long gs = 1ll << h->gd.dim;
         h->max_groups = n / gs + (n < h->gd.Nc ? n : h->gd.Nc) + 1;
         ok = dev_alloc_t(h, &h->S[0], N) && dev_alloc_t(h, &h->S[1], N) && dev_alloc_t(h, &h->dest, N) &&
              dev_alloc_t(h, &h->groups, (size_t)h->max_groups);
     }
     if (!ok) { free_particles(h); return fail(h, MPM_E_OOM, "out of device memory for particle arrays"); }
+    if (tiled) {   // unused slots are read (and masked) by the 128-bit loads: keep them finite
+        for (int b = 0; b < 2; ++b) {
+            PArr &p = h->pbuf[b];
+            for (int a = 0; a < h->gd.dim; ++a) { cudaMemsetAsync(p.x[a], 0, 8 * N, h->stream); cudaMemsetAsync(p.v[a], 0, 8 * N, h->stream); }
+            cudaMemsetAsync(p.m, 0, 8 * N, h->stream); cudaMemsetAsync(p.rho, 0, 8 * N, h->stream);
+            cudaMemsetAsync(p.e, 0, 8 * N, h->stream); cudaMemsetAsync(p.q, 0, 8 * N, h->stream);
+            cudaMemsetAsync(p.id, 0, 4 * N, h->stream);
+            cudaMemsetAsync(h->S[b], 0, 8 * N, h->stream);
+        }
+        cudaMemsetAsync(h->dest, 0, 8 * N, h->stream);
+    }
     h->n = n; h->cap = n; h->cur = 0;
     return MPM_OK;
 }
@@ -253,6 +269,17 @@ void reorder(mpm_handle *h)
     Timed timer(h, MPM_K_SORT);
     const PArr &src = h->pbuf[h->cur];
     const PArr &dst = h->pbuf[h->cur ^ 1];
+    if (h->variant == MPM_VARIANT_TILED) {
+        // counts per tile-major key -> even-rounded slot offsets -> permutation; then groups and the force payload
+        launch_key_rank(h->gd, src, h->key, h->rank, h->count, h->n, h->stream);
+        launch_exclusive_scan_from(h->count, h->off[0], h->gd.Nkeys + 1, h->scan_aux, true, h->stream);
+        launch_permute(h->gd, src, dst, h->key, h->rank, h->off[0], h->n, h->stream);
+        h->cur ^= 1;
+        launch_force_payload_slots(h->gd, dst, h->S[h->cur], h->slots, h->stream);
+        launch_build_groups_tiled(h->gd, h->count, h->off[0], h->goff, h->scan_aux, h->groups, h->n_groups, h->stream);
+        h->launches += 12;
+        return;
+    }
     int *count = h->variant == MPM_VARIANT_SORTED ? h->off[h->ocur] : h->count;
     launch_key_rank(h->gd, src, h->key, h->rank, count, h->n, h->stream);
     launch_exclusive_scan(count, h->gd.Nc + 1, h->scan_aux, h->stream);
@@ -274,7 +301,7 @@ void step_sorted(mpm_handle *h)
     const PArr &p = h->pbuf[h->cur];
     const PArr &q = h->pbuf[h->cur ^ 1];
     int *off_old = h->off[h->ocur], *off_new = h->off[h->ocur ^ 1];
-    const SortedMap map{ h->groups, h->n_groups };
+    const SortedMap map{ h->groups, h->n_groups, nullptr };
     (void)off_old;
     {
         Timed t(h, MPM_K_MISC);
@@ -295,6 +322,35 @@ void step_sorted(mpm_handle *h)
       launch_build_groups(gd, off_new, h->goff, h->scan_aux, h->groups, h->n_groups, s); }                         // next step's groups
     h->cur ^= 1;
     h->ocur ^= 1;
+    h->launches += 16;
+}
+
+// one step of Algorithm 1 with the TILED kernel family (see mpm_kernels_tiled.cu)
+void step_tiled(mpm_handle *h)
+{
+    const GridDesc &gd = h->gd;
+    cudaStream_t s = h->stream;
+    const PArr &p = h->pbuf[h->cur];
+    const PArr &q = h->pbuf[h->cur ^ 1];
+    const SortedMap map{ h->groups, h->n_groups, h->goff };
+    {
+        Timed t(h, MPM_K_MISC);
+        launch_begin_step(h->sc, gd.h, s);                                                // dt (eq. 25/29)
+        launch_grid_clear(gd, h->g, s);                                                   // l.2
+        cudaMemsetAsync(h->count, 0, sizeof(int) * (size_t)(gd.Nkeys + 1), s);            // per-cell counters of l.12
+    }
+    { Timed t(h, MPM_K_P2G1); launch_p2g1_tiled(gd, p, h->S[h->cur], h->g, map, h->max_groups, s); }               // l.3
+    { Timed t(h, MPM_K_NODE1); launch_node1(gd, h->g, h->sc, s); }                                                 // l.4-5
+    { Timed t(h, MPM_K_G2P_P2G2);
+      launch_g2p_p2g2_tiled(gd, p, h->g, h->g.na, h->sc, map, h->count, h->dest, h->max_groups, s); }              // l.6-8
+    { Timed t(h, MPM_K_NODE2); launch_node2(gd, h->g, s); }                                                        // l.9
+    { Timed t(h, MPM_K_SORT); launch_exclusive_scan_from(h->count, h->off[0], gd.Nkeys + 1, h->scan_aux, true, s); }   // l.12 offsets
+    { Timed t(h, MPM_K_UPDATE);
+      launch_update_tiled(gd, p, q, h->g.na, h->g.nb, h->sc, map, h->off[0], h->dest, h->S[h->cur ^ 1], h->max_groups, s); }   // l.10-12
+    { Timed t(h, MPM_K_MISC); launch_end_step(h->sc, gd.h, s); }                                                   // l.13-14
+    { Timed t(h, MPM_K_SORT);
+      launch_build_groups_tiled(gd, h->count, h->off[0], h->goff, h->scan_aux, h->groups, h->n_groups, s); }       // next step's groups
+    h->cur ^= 1;
     h->launches += 16;
 }
 
@@ -342,7 +398,7 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
     for (int k = 0; k < MPM_K_COUNT; ++k) { h->kernel_ms[k] = 0.0; h->kernel_calls[k] = 0; }
     h->d_flag = nullptr; h->key = h->rank = h->count = h->scan_aux = nullptr; h->sc = nullptr;
     h->off[0] = h->off[1] = nullptr; h->ocur = 0; h->goff = h->n_groups = nullptr; h->groups = nullptr;
-    h->S[0] = h->S[1] = nullptr; h->dest = nullptr; h->max_groups = 0;
+    h->S[0] = h->S[1] = nullptr; h->dest = nullptr; h->max_groups = 0; h->coff = nullptr; h->slots = 0;
     std::memset(h->pbuf, 0, sizeof(h->pbuf));
     std::memset(&h->g, 0, sizeof(h->g));
     for (int a = 0; a < 3; ++a) h->d_normal[a] = nullptr;
@@ -384,13 +440,27 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
     gd.recycle_seed = cfg->recycle_seed;
     gd.has_obstacle = cfg->obstacle_mask != nullptr;
 
-    h->variant = cfg->variant == MPM_VARIANT_AUTO ? (cfg->sort_every == 1 ? MPM_VARIANT_SORTED : MPM_VARIANT_ATOMIC)
+    h->variant = cfg->variant == MPM_VARIANT_AUTO ? (cfg->sort_every == 1 ? MPM_VARIANT_TILED : MPM_VARIANT_ATOMIC)
                                                    : cfg->variant;
-    if (h->variant != MPM_VARIANT_ATOMIC && h->variant != MPM_VARIANT_SORTED) {
+    if (h->variant != MPM_VARIANT_ATOMIC && h->variant != MPM_VARIANT_SORTED && h->variant != MPM_VARIANT_TILED) {
         delete h;
         return fail(nullptr, MPM_E_ARG, "mpm_create: unknown kernel variant");
     }
-    const bool sorted = h->variant == MPM_VARIANT_SORTED;
+    const bool tiled = h->variant == MPM_VARIANT_TILED;
+    const bool sorted = h->variant == MPM_VARIANT_SORTED || tiled;
+    gd.tiled = tiled ? 1 : 0;
+    gd.Nkeys = gd.Nc;
+    if (tiled) {    // tile-major key space (TileGeo): whole tiles, so it can be larger than the number of cells
+        long long nt = 1;
+        for (int a = 0; a < 3; ++a) {
+            const int lt = gd.dim == 3 ? (a == 0 ? TileGeo<3>::LT0 : a == 1 ? TileGeo<3>::LT1 : TileGeo<3>::LT2)
+                                       : (a == 0 ? TileGeo<2>::LT0 : a == 1 ? TileGeo<2>::LT1 : 0);
+            gd.ntile[a] = a < gd.dim ? (gd.nc[a] + (1 << lt) - 1) >> lt : 1;
+            nt *= gd.ntile[a];
+        }
+        gd.Nkeys = nt * (gd.dim == 3 ? TileGeo<3>::TC : TileGeo<2>::TC);
+        if (gd.Nkeys >= (1ll << 31) - 2) { delete h; return fail(nullptr, MPM_E_ARG, "mpm_create: grid too large for 32-bit tile keys"); }
+    }
     if (sorted) {   // the group records pack the cell coordinates into one int
         const int lim = gd.dim == 3 ? 1024 : 65535;
         for (int a = 0; a < gd.dim; ++a)
@@ -408,10 +478,10 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
     }
     if (ok && sorted)
         ok = dev_alloc_t(h, &h->g.na, (size_t)gd.Nn * 2 * gd.dim) && dev_alloc_t(h, &h->g.nb, (size_t)gd.Nn * gd.dim) &&
-             dev_alloc_t(h, &h->off[0], (size_t)gd.Nc + 1) && dev_alloc_t(h, &h->off[1], (size_t)gd.Nc + 1) &&
-             dev_alloc_t(h, &h->goff, (size_t)gd.Nc + 1) && dev_alloc_t(h, &h->n_groups, 1);
+             dev_alloc_t(h, &h->off[0], (size_t)gd.Nkeys + 1) && dev_alloc_t(h, &h->off[1], (size_t)gd.Nkeys + 1) &&
+             dev_alloc_t(h, &h->goff, (size_t)gd.Nkeys + 1) && dev_alloc_t(h, &h->n_groups, 1);
     // the scan's block sums: one int per 4096 scanned elements
-    ok = ok && dev_alloc_t(h, &h->count, (size_t)gd.Nc + 1) && dev_alloc_t(h, &h->scan_aux, (size_t)gd.Nc / 4096 + 8) &&
+    ok = ok && dev_alloc_t(h, &h->count, (size_t)gd.Nkeys + 1) && dev_alloc_t(h, &h->scan_aux, (size_t)gd.Nkeys / 4096 + 8) &&
          dev_alloc_t(h, &h->sc, 1);
     if (gd.has_obstacle && ok) {
         build_obstacle(h, cfg->obstacle_mask, cfg->node_normals);
@@ -492,7 +562,7 @@ int mpm_load_particles(mpm_handle *h, int64_t n, const double *const *x, const d
     launch_initial_cfl(h->gd, p, h->sc, n, h->stream);
     h->launches += 3;
     h->steps_done = 0;
-    if ((h->cfg.sort_every > 0 || h->variant == MPM_VARIANT_SORTED) && n > 0) reorder(h);
+    if ((h->cfg.sort_every > 0 || h->variant != MPM_VARIANT_ATOMIC) && n > 0) reorder(h);
     MPM_CUDA(h, cudaGetLastError());
     if (ptr_location == MPM_HOST) MPM_CUDA(h, cudaStreamSynchronize(h->stream));   // caller may reuse its buffers
     return MPM_OK;
@@ -516,8 +586,8 @@ int mpm_step(mpm_handle *h, double dt, double cfl, int32_t nsteps, double *dt_la
     k_set_mode<<<1, 1, 0, s>>>(h->sc, dt > 0.0 ? dt : 0.0, cfl);
     h->launches += 1;
     for (int it = 0; it < nsteps; ++it) {
-        if (h->variant == MPM_VARIANT_SORTED) {
-            if (h->n > 0) step_sorted(h);
+        if (h->variant != MPM_VARIANT_ATOMIC) {
+            if (h->n > 0) { if (h->variant == MPM_VARIANT_TILED) step_tiled(h); else step_sorted(h); }
             else { launch_begin_step(h->sc, gd.h, s); launch_grid_clear(gd, h->g, s); launch_end_step(h->sc, gd.h, s); h->launches += 2; }
             h->steps_done += 1;
             continue;
@@ -561,10 +631,21 @@ int mpm_read_particles(mpm_handle *h, uint32_t field_mask, double *const *out, i
     if (field_mask & MPM_P_RHO) { src.push_back(p.rho); tmp.push_back(scratch.rho); }
     if (field_mask & MPM_P_E) { src.push_back(p.e); tmp.push_back(scratch.e); }
     if (field_mask & MPM_P_Q) { src.push_back(p.q); tmp.push_back(scratch.q); }
+    const bool tiled = h->variant == MPM_VARIANT_TILED && h->n > 0;
+    const SortedMap map{ h->groups, h->n_groups, h->goff };
+    if (tiled && order != 0) {   // storage order without the unused slots: compact offsets = scan of the per-key counts
+        if (!h->coff && !dev_alloc_t(h, &h->coff, (size_t)h->gd.Nkeys + 1)) return fail(h, MPM_E_OOM, "mpm_read_particles: out of device memory");
+        launch_exclusive_scan_from(h->count, h->coff, h->gd.Nkeys + 1, h->scan_aux, false, h->stream);
+        h->launches += 3;
+    }
     for (size_t j = 0; j < src.size(); ++j) {
         if (!out[j]) return fail(h, MPM_E_ARG, "mpm_read_particles: null output pointer");
         const double *from = src[j];
-        if (order == 0) {
+        if (tiled) {
+            launch_gather_by_id_groups(src[j], p.id, tmp[j], map, h->max_groups, order == 0 ? nullptr : h->coff, h->off[0], h->stream);
+            h->launches += 1;
+            from = tmp[j];
+        } else if (order == 0) {
             launch_gather_by_id(src[j], p.id, tmp[j], h->n, h->stream);
             h->launches += 1;
             from = tmp[j];
@@ -616,7 +697,10 @@ int mpm_get_stats(mpm_handle *h, mpm_stats *out)
     std::memset(out, 0, sizeof(*out));
     DevScalars host;
     if (h->pbuf[0].m) {
-        launch_stats_reduce(h->gd, h->pbuf[h->cur], h->sc, h->n, h->stream);
+        if (h->variant == MPM_VARIANT_TILED && h->n > 0)
+            launch_stats_reduce_groups(h->gd, h->pbuf[h->cur], h->sc, SortedMap{ h->groups, h->n_groups, h->goff }, h->max_groups, h->stream);
+        else
+            launch_stats_reduce(h->gd, h->pbuf[h->cur], h->sc, h->n, h->stream);
         h->launches += 2;
     }
     MPM_CUDA(h, cudaMemcpyAsync(&host, h->sc, sizeof(host), cudaMemcpyDeviceToHost, h->stream));

@@ -30,7 +30,49 @@ struct GridDesc {
     double inflow_rho, inflow_e, inflow_mass;
     int in_axis, in_side;   // first INFLOW face, -1 = none
     unsigned long long recycle_seed;
+    // TILED family: cell keys are tile-major (see TileGeo); ntile = tiles per axis, Nkeys = size of the key space
+    int tiled;
+    int ntile[3];
+    long long Nkeys;
 };
+
+// TILED family: the grid is cut into tiles of T0 x T1 (x T2) cells; the cell key is (tile index, cell inside the
+// tile), both x fastest, so that the particles of one tile are contiguous in the cell-sorted order (PAPER.md:745-748
+// applied per tile) and one thread block can keep the tile's (T+1)^d nodes in shared memory.
+template <int DIM>
+struct TileGeo {
+    static constexpr int LT0 = (DIM == 3) ? 3 : 4;
+    static constexpr int LT1 = (DIM == 3) ? 3 : 4;
+    static constexpr int LT2 = (DIM == 3) ? 2 : 0;
+    static constexpr int T0 = 1 << LT0, T1 = 1 << LT1, T2 = 1 << LT2;
+    static constexpr int LTC = LT0 + LT1 + LT2;
+    static constexpr int TC = 1 << LTC;                      // cells per tile
+    static constexpr int N0 = T0 + 1, N1 = T1 + 1, N2 = (DIM == 3) ? T2 + 1 : 1;
+    static constexpr int NN = N0 * N1 * N2;                  // nodes per tile
+};
+
+template <int DIM>
+__host__ __device__ __forceinline__ int tiled_key_of_cell(const GridDesc &gd, const int c[DIM])
+{
+    using TG = TileGeo<DIM>;
+    int tile = (c[0] >> TG::LT0) + gd.ntile[0] * (c[1] >> TG::LT1);
+    int local = (c[0] & (TG::T0 - 1)) | ((c[1] & (TG::T1 - 1)) << TG::LT0);
+    if (DIM == 3) {
+        tile += gd.ntile[0] * gd.ntile[1] * (c[DIM - 1] >> TG::LT2);
+        local |= (c[DIM - 1] & (TG::T2 - 1)) << (TG::LT0 + TG::LT1);
+    }
+    return (tile << TG::LTC) | local;
+}
+
+template <int DIM>
+__host__ __device__ __forceinline__ void tiled_cell_of_key(const GridDesc &gd, int key, int c[DIM])
+{
+    using TG = TileGeo<DIM>;
+    const int tile = key >> TG::LTC, local = key & (TG::TC - 1);
+    c[0] = ((tile % gd.ntile[0]) << TG::LT0) | (local & (TG::T0 - 1));
+    c[1] = (((tile / gd.ntile[0]) % gd.ntile[1]) << TG::LT1) | ((local >> TG::LT0) & (TG::T1 - 1));
+    if (DIM == 3) c[DIM - 1] = ((tile / (gd.ntile[0] * gd.ntile[1])) << TG::LT2) | (local >> (TG::LT0 + TG::LT1));
+}
 
 // particle SoA.  P, Vbar, A, grad V are transient and never stored.
 struct PArr {
@@ -150,6 +192,7 @@ __device__ __forceinline__ void atomic_max_nonneg(unsigned long long *addr, doub
 struct SortedMap {
     const int4 *groups;     // [n_groups]
     const int *n_groups;    // device scalar
+    const int *goff;        // TILED: first group of every key, [Nkeys + 1] (the groups of tile t are goff[t TC] .. goff[(t+1) TC])
 };
 
 // ---------------------------------------------------------------------------------------------- launchers
@@ -173,6 +216,24 @@ void launch_update_sorted(const GridDesc &gd, const PArr &p, const PArr &q, cons
                           const SortedMap &map, const int *off_new, const unsigned long long *dest, double *S_out,
                           long long max_groups, cudaStream_t s);
 
+// TILED family (tile-major cell order, even-aligned cell slots, tile nodes in shared memory) -- mpm_kernels_tiled.cu
+void launch_force_payload_slots(const GridDesc &gd, const PArr &p, double *S, long long nslots, cudaStream_t s);
+void launch_build_groups_tiled(const GridDesc &gd, const int *count, const int *off, int *goff, int *scan_aux, int4 *groups,
+                               int *n_groups, cudaStream_t s);
+void launch_p2g1_tiled(const GridDesc &gd, const PArr &p, const double *S, const GArr &g, const SortedMap &map,
+                       long long max_groups, cudaStream_t s);
+void launch_g2p_p2g2_tiled(const GridDesc &gd, const PArr &p, const GArr &g, const double *na, const DevScalars *sc,
+                           const SortedMap &map, int *count, unsigned long long *dest, long long max_groups, cudaStream_t s);
+void launch_update_tiled(const GridDesc &gd, const PArr &p, const PArr &q, const double *na, const double *nb, DevScalars *sc,
+                         const SortedMap &map, const int *off_new, const unsigned long long *dest, double *S_out,
+                         long long max_groups, cudaStream_t s);
+// dst[id] = src[slot] for every occupied slot; with coff (exclusive scan of the per-key counts) and off (slot offsets):
+// dst[compact storage index] = src[slot] instead
+void launch_gather_by_id_groups(const double *src, const int *id, double *dst, const SortedMap &map, long long max_groups,
+                                const int *coff, const int *off, cudaStream_t s);
+void launch_stats_reduce_groups(const GridDesc &gd, const PArr &p, DevScalars *sc, const SortedMap &map, long long max_groups,
+                                cudaStream_t s);
+
 // node kernels -- mpm_kernels_grid.cu
 void launch_grid_clear(const GridDesc &gd, const GArr &g, cudaStream_t s);
 void launch_node1(const GridDesc &gd, const GArr &g, const DevScalars *sc, cudaStream_t s);
@@ -188,6 +249,8 @@ void launch_stats_reduce(const GridDesc &gd, const PArr &p, DevScalars *sc, long
 void launch_iota(int *id, long long n, cudaStream_t s);
 void launch_key_rank(const GridDesc &gd, const PArr &p, int *key, int *rank, int *count, long long n, cudaStream_t s);
 void launch_exclusive_scan(int *data, long long n, int *aux, cudaStream_t s);   // in place, aux >= n/4096 + 2 ints
+// out = exclusive scan of in (round_even: of in rounded up to even); in == out allowed
+void launch_exclusive_scan_from(const int *in, int *out, long long n, int *aux, bool round_even, cudaStream_t s);
 void launch_permute(const GridDesc &gd, const PArr &src, const PArr &dst, const int *key, const int *rank,
                     const int *offset, long long n, cudaStream_t s);
 void launch_gather_by_id(const double *src, const int *id, double *dst, long long n, cudaStream_t s);

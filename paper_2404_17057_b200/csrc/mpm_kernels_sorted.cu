@@ -23,258 +23,17 @@
 //     loads is one load deep.
 // A particle whose true cell differs from its group's cell (never the case when the invariant holds; cheap to test)
 // takes a slow path with direct global reductions / gathers, so correctness never depends on the ordering.
-#include "mpm_internal.cuh"
+#include "mpm_lane_groups.cuh"
+
+#ifndef MPM_MINB
+#define MPM_MINB 2   // resident blocks per SM the particle kernels are compiled for (register budget)
+#endif
 
 namespace mpm {
 
 namespace {
 
-constexpr int kBlock = 256;
-constexpr unsigned kFull = 0xffffffffu;
-
-template <int DIM>
-struct Geo {
-    static constexpr int NB = 1 << DIM;            // corners per cell = particles per group
-    static constexpr int LG = NB / 2;              // lanes per group
-    static constexpr int NG = 32 / LG;             // groups per warp
-    static constexpr int GPB = kBlock / LG;        // groups per block and iteration
-    // shared staging of corner node values: [group][corner][channel]; the group stride is == 4 (mod 32) words so that
-    // the 16-byte broadcast reads of the groups of a warp fall into distinct banks
-    static constexpr int CH = (DIM == 3) ? 8 : 6;                       // doubles per corner (vbar, acc, dsum, pad)
-    static constexpr int GROUP_STRIDE = (DIM == 3) ? 66 : 34;           // doubles
-    static constexpr int WARP_DOUBLES = NG * GROUP_STRIDE;
-};
-
-__device__ __forceinline__ double shfl_xor_d(double v, int m) { return __shfl_xor_sync(kFull, v, m); }
-
-// Transposed butterfly over the LG lanes of a group.  Before: register r of lane l holds the lane's contribution to
-// corner r ^ l.  After: registers r = q * LG (q = 0, 1) hold the group totals of corners l + q * LG.
-template <int DIM>
-__device__ __forceinline__ void butterfly(double v[1 << DIM])
-{
-    constexpr int NB = 1 << DIM, LG = Geo<DIM>::LG;
-#pragma unroll
-    for (int m = LG / 2; m >= 1; m >>= 1) {
-#pragma unroll
-        for (int r = 0; r < NB; ++r)
-            if ((r & m) == 0 && (r & (LG - 1) & ~(2 * m - 1)) == 0) v[r] += shfl_xor_d(v[r | m], m);
-    }
-}
-
-struct Group {
-    int first;     // first particle of the group
-    int cnt;       // particles in the group (<= 2^d), 0 = idle
-    int cell;      // linear cell index
-    int cpack;     // packed cell coordinates (3D: 10 bits each, 2D: 16 bits each)
-};
-
-__device__ __forceinline__ Group fetch_group(const int4 *__restrict__ groups, long long gidx, int n_groups)
-{
-    Group g{ 0, 0, 0, 0 };
-    if (gidx < (long long)n_groups) {
-        const int4 r = __ldg(groups + gidx);
-        g.first = r.x; g.cnt = r.y; g.cell = r.z; g.cpack = r.w;
-    }
-    return g;
-}
-
-template <int DIM>
-__device__ __forceinline__ void unpack_coords(int cpack, int c[DIM])
-{
-    if (DIM == 3) { c[0] = cpack & 1023; c[1] = (cpack >> 10) & 1023; c[DIM - 1] = (cpack >> 20) & 1023; }
-    else { c[0] = cpack & 65535; c[1] = (cpack >> 16) & 65535; }
-}
-
-// node index of corner b of cell c (periodic wrap: node n == node 0, A11)
-template <int DIM>
-__device__ __forceinline__ int corner_node_i(const GridDesc &gd, const int c[DIM], int b)
-{
-    int idx = 0, stride = 1;
-#pragma unroll
-    for (int a = 0; a < DIM; ++a) {
-        int i = c[a] + ((b >> a) & 1);
-        if (gd.per[a] && i == gd.nc[a]) i = 0;
-        idx += stride * i;
-        stride *= gd.nn[a];
-    }
-    return idx;
-}
-
-// local coordinates w.r.t. the GROUP's cell; returns false if the particle's own cell (A6, A19) is a different one
-template <int DIM>
-__device__ __forceinline__ bool local_coords(const GridDesc &gd, const double X[DIM], const int c[DIM], double xi[DIM])
-{
-    bool same = true;
-#pragma unroll
-    for (int a = 0; a < DIM; ++a) {
-        int ci;
-        cell_1d(X[a], gd.inv_h, gd.nc[a], ci, xi[a]);
-        same = same && (ci == c[a]);
-    }
-    return same;
-}
-
-// weights in natural corner order (gathers) ...
-template <int DIM>
-__device__ __forceinline__ void natural_weights(const double xi[DIM], double w[1 << DIM])
-{
-#pragma unroll
-    for (int b = 0; b < (1 << DIM); ++b) w[b] = corner_phi<DIM>(xi, b);
-}
-// ... and in butterfly order (scatters): register r of lane l holds the weight of corner r ^ l (l < LG)
-template <int DIM>
-__device__ __forceinline__ void swizzled_weights(const double xi[DIM], int l, double w[1 << DIM])
-{
-    double p[DIM][2];
-#pragma unroll
-    for (int a = 0; a < DIM; ++a) {
-        const bool hi = (l >> a) & 1;       // l < LG: only the low axes are ever swapped
-        p[a][0] = hi ? xi[a] : 1.0 - xi[a];
-        p[a][1] = hi ? 1.0 - xi[a] : xi[a];
-    }
-#pragma unroll
-    for (int r = 0; r < (1 << DIM); ++r) {
-        double q = 1.0;
-#pragma unroll
-        for (int a = 0; a < DIM; ++a) q *= p[a][(r >> a) & 1];
-        w[r] = q;
-    }
-}
-
-// max over the warp of a NON-NEGATIVE double with two integer REDUX ops (bit patterns order like the values)
-__device__ __forceinline__ double warp_max_nonneg(double v)
-{
-    const unsigned hi = (unsigned)__double2hiint(v), lo = (unsigned)__double2loint(v);
-    const unsigned mhi = __reduce_max_sync(kFull, hi);
-    const unsigned mlo = __reduce_max_sync(kFull, hi == mhi ? lo : 0u);
-    return __hiloint2double((int)mhi, (int)mlo);
-}
-
-// ---------------------------------------------------------------------------------------------- slow paths
-template <int DIM>
-__device__ __forceinline__ void slow_p2g1(const GridDesc &gd, const GArr &g, const double X[DIM], const double V[DIM],
-                                          double M, double S)
-{
-    int c[DIM];
-    double xi[DIM];
-    particle_cell<DIM>(gd, X, c, xi);
-#pragma unroll 1
-    for (int ib = 0; ib < (1 << DIM); ++ib) {
-        const long long i = corner_node<DIM>(gd, c, ib);
-        const double phi = corner_phi<DIM>(xi, ib);
-        atomicAdd(&g.m[i], M * phi);
-#pragma unroll
-        for (int a = 0; a < DIM; ++a) {
-            atomicAdd(&g.mv[a][i], M * V[a] * phi);
-            atomicAdd(&g.f[a][i], S * corner_dphi<DIM>(xi, ib, a, gd.inv_h));
-        }
-    }
-}
-
-template <int DIM>
-__device__ __forceinline__ void slow_gather(const GridDesc &gd, const double *na, const double *nb, const double X[DIM],
-                                            double Vb[DIM], double A[DIM], double *D)
-{
-    int c[DIM];
-    double xi[DIM];
-    particle_cell<DIM>(gd, X, c, xi);
-    double d = 0.0;
-#pragma unroll
-    for (int a = 0; a < DIM; ++a) { Vb[a] = 0.0; A[a] = 0.0; }
-#pragma unroll 1
-    for (int ib = 0; ib < (1 << DIM); ++ib) {
-        const long long i = corner_node<DIM>(gd, c, ib);
-        const double phi = corner_phi<DIM>(xi, ib);
-#pragma unroll
-        for (int a = 0; a < DIM; ++a) {
-            Vb[a] += phi * na[i * (2 * DIM) + a];
-            A[a] += phi * na[i * (2 * DIM) + DIM + a];
-            if (nb) d += nb[i * DIM + a] * corner_dphi<DIM>(xi, ib, a, gd.inv_h);
-        }
-    }
-    if (D) *D = d;
-}
-
-template <int DIM>
-__device__ __forceinline__ void slow_p2g2(const GridDesc &gd, const GArr &g, const double X[DIM], const double MV[DIM])
-{
-    int c[DIM];
-    double xi[DIM];
-    particle_cell<DIM>(gd, X, c, xi);
-#pragma unroll 1
-    for (int ib = 0; ib < (1 << DIM); ++ib) {
-        const long long i = corner_node<DIM>(gd, c, ib);
-        const double phi = corner_phi<DIM>(xi, ib);
-#pragma unroll
-        for (int a = 0; a < DIM; ++a) atomicAdd(&g.mv2[a][i], MV[a] * phi);
-    }
-}
-
-// ---------------------------------------------------------------------------------------------- shared pieces
-
-// Alg. 1 l.11 for one particle: X' = X + dt Vbar, periodic wrap (A11), outflow detection, recycling position (A8),
-// clamp.  Used by BOTH the gather kernel (to find the new cell) and the update kernel (to write X'); the update kernel
-// places the particle by the key the gather kernel stored, so a last-bit disagreement could only cost a slow path.
-template <int DIM>
-__device__ __forceinline__ void move_particle(const GridDesc &gd, const double X[DIM], const double Vb[DIM], double dt,
-                                              long long id, long long step, double Xn[DIM], bool &recycled, int &nclamp)
-{
-    bool recycle = false;
-#pragma unroll
-    for (int a = 0; a < DIM; ++a) {
-        double x = fma(dt, Vb[a], X[a]);
-        if (gd.per[a]) {
-            if (x < 0.0 || x >= gd.L[a]) {
-                x = x - gd.L[a] * floor(x / gd.L[a]);
-                if (x >= gd.L[a]) x = 0.0;
-            }
-        } else {
-            if (x < 0.0 && gd.bc[a][0] == MPM_BC_OUTFLOW) recycle = true;
-            if (x > gd.L[a] && gd.bc[a][1] == MPM_BC_OUTFLOW) recycle = true;
-        }
-        Xn[a] = x;
-    }
-    recycled = recycle && gd.in_axis >= 0;
-    if (recycled) {
-        int jj = 0;
-        const double u0 = recycle_uniform(gd.recycle_seed, id, step, jj++);
-#pragma unroll
-        for (int a = 0; a < DIM; ++a) {
-            if (a == gd.in_axis) {
-                Xn[a] = (gd.in_side == 0) ? u0 * gd.h : gd.L[a] - u0 * gd.h;
-            } else {
-                const double u1 = recycle_uniform(gd.recycle_seed, id, step, jj++);
-                const double u2 = recycle_uniform(gd.recycle_seed, id, step, jj++);
-                int cell = (int)floor(u1 * (double)gd.nc[a]);
-                cell = min(cell, gd.nc[a] - 1);
-                Xn[a] = ((double)cell + u2) * gd.h;
-            }
-        }
-    }
-    nclamp = 0;
-#pragma unroll
-    for (int a = 0; a < DIM; ++a) {
-        if (!gd.per[a]) {
-            if (Xn[a] < 0.0) { Xn[a] = 0.0; nclamp++; }
-            if (Xn[a] > gd.L[a]) { Xn[a] = gd.L[a]; nclamp++; }
-        }
-    }
-}
-
-template <int DIM>
-__device__ __forceinline__ int cell_key(const GridDesc &gd, const double X[DIM])
-{
-    int key = 0, stride = 1;
-#pragma unroll
-    for (int a = 0; a < DIM; ++a) {
-        int c;
-        double xi;
-        cell_1d(X[a], gd.inv_h, gd.nc[a], c, xi);
-        key += stride * c;
-        stride *= gd.nc[a];
-    }
-    return key;
-}
+using namespace lg;
 
 // lane l stages vbar, acc of one corner (node-major array na[node][2 DIM]) into shared memory
 template <int DIM>
@@ -307,7 +66,7 @@ __device__ __forceinline__ void gather_pairs(const double *s_group, const double
 // ------------------------------------------------------------------------------------------------ Alg. 1 l.3
 // m, mv from phi-weighted channels (M, M V); f from the phi-weighted channel S = (P+Q) M / rho
 template <int DIM>
-__global__ void __launch_bounds__(kBlock) k_p2g1_sorted(GridDesc gd, PArr p, const double *__restrict__ Sarr, GArr g,
+__global__ void __launch_bounds__(kBlock, MPM_MINB) k_p2g1_sorted(GridDesc gd, PArr p, const double *__restrict__ Sarr, GArr g,
                                                         const int4 *__restrict__ groups, const int *__restrict__ n_groups_p)
 {
     constexpr int NB = 1 << DIM, LG = Geo<DIM>::LG, GPB = Geo<DIM>::GPB;
@@ -392,7 +151,7 @@ __global__ void __launch_bounds__(kBlock) k_p2g1_sorted(GridDesc gd, PArr p, con
 // A = G2P(f/m), Vbar = G2P(mv'/m); V' = V + dt A; mv2 += M V' phi.  Also: the particle's cell after the
 // move of l.11 and its rank inside that cell, for the fused re-ordering.  V' is NOT stored: the update kernel recomputes it.
 template <int DIM>
-__global__ void __launch_bounds__(kBlock) k_g2p_p2g2_sorted(GridDesc gd, PArr p, GArr g, const double *__restrict__ na,
+__global__ void __launch_bounds__(kBlock, MPM_MINB) k_g2p_p2g2_sorted(GridDesc gd, PArr p, GArr g, const double *__restrict__ na,
                                                             const DevScalars *__restrict__ sc,
                                                             const int4 *__restrict__ groups, const int *__restrict__ n_groups_p,
                                                             int *__restrict__ count, unsigned long long *__restrict__ dest)
@@ -496,7 +255,7 @@ __global__ void __launch_bounds__(kBlock) k_g2p_p2g2_sorted(GridDesc gd, PArr p,
 // X' = X + dt Vbar; the particle is written to its cell-sorted slot of the OTHER buffer (l.12),
 // together with next step's force payload S' = (P'+Q') M / rho' (eq. 13).
 template <int DIM>
-__global__ void __launch_bounds__(kBlock) k_update_sorted(GridDesc gd, PArr p, PArr q, const double *__restrict__ na,
+__global__ void __launch_bounds__(kBlock, MPM_MINB) k_update_sorted(GridDesc gd, PArr p, PArr q, const double *__restrict__ na,
                                                           const double *__restrict__ nb, DevScalars *sc,
                                                           const int4 *__restrict__ groups, const int *__restrict__ n_groups_p,
                                                           const int *__restrict__ off_new,

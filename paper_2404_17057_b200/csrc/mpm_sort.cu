@@ -28,20 +28,21 @@ __global__ void __launch_bounds__(kBlock) k_key_rank(GridDesc gd, PArr p, int *k
     long long k = (long long)blockIdx.x * kBlock + threadIdx.x;
     if (k >= n) return;
     long long cell = 0, stride = 1;
+    int cc[DIM];
 #pragma unroll
     for (int a = 0; a < DIM; ++a) {
-        int c;
         double xi;
-        cell_1d(p.x[a][k], gd.inv_h, gd.nc[a], c, xi);
-        cell += stride * c;
+        cell_1d(p.x[a][k], gd.inv_h, gd.nc[a], cc[a], xi);
+        cell += stride * cc[a];
         stride *= gd.nc[a];
     }
+    if (gd.tiled) cell = tiled_key_of_cell<DIM>(gd, cc);
     key[k] = (int)cell;
     rank[k] = atomicAdd(&count[cell], 1);
 }
 
 // block-wide exclusive scan of kScanTile ints; block sums go to aux[blockIdx.x]
-__global__ void __launch_bounds__(kScanBlock) k_scan_tiles(int *data, long long n, int *aux)
+__global__ void __launch_bounds__(kScanBlock) k_scan_tiles(const int *in, int *data, long long n, int *aux, bool round_even)
 {
     __shared__ int s_warp[kScanBlock / 32];
     const long long base = (long long)blockIdx.x * kScanTile + (long long)threadIdx.x * kScanItems;
@@ -49,7 +50,8 @@ __global__ void __launch_bounds__(kScanBlock) k_scan_tiles(int *data, long long 
     int sum = 0;
 #pragma unroll
     for (int j = 0; j < kScanItems; ++j) {
-        v[j] = (base + j < n) ? data[base + j] : 0;
+        v[j] = (base + j < n) ? in[base + j] : 0;
+        if (round_even) v[j] = (v[j] + 1) & ~1;
         sum += v[j];
     }
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -163,21 +165,26 @@ void launch_iota(int *id, long long n, cudaStream_t s)
 
 void launch_key_rank(const GridDesc &gd, const PArr &p, int *key, int *rank, int *count, long long n, cudaStream_t s)
 {
-    cudaMemsetAsync(count, 0, sizeof(int) * (size_t)(gd.Nc + 1), s);
+    cudaMemsetAsync(count, 0, sizeof(int) * (size_t)((gd.tiled ? gd.Nkeys : gd.Nc) + 1), s);
     if (n <= 0) return;
     if (gd.dim == 2) k_key_rank<2><<<grid_for(n, kBlock), kBlock, 0, s>>>(gd, p, key, rank, count, n);
     else k_key_rank<3><<<grid_for(n, kBlock), kBlock, 0, s>>>(gd, p, key, rank, count, n);
 }
 
-void launch_exclusive_scan(int *data, long long n, int *aux, cudaStream_t s)
+void launch_exclusive_scan_from(const int *in, int *out, long long n, int *aux, bool round_even, cudaStream_t s)
 {
     if (n <= 0) return;
     const unsigned tiles = grid_for(n, kScanTile);
-    k_scan_tiles<<<tiles, kScanBlock, 0, s>>>(data, n, aux);
+    k_scan_tiles<<<tiles, kScanBlock, 0, s>>>(in, out, n, aux, round_even);
     if (tiles > 1) {
         k_scan_aux<<<1, 1024, 0, s>>>(aux, (int)tiles);
-        k_scan_add<<<tiles, kScanBlock, 0, s>>>(data, n, aux);
+        k_scan_add<<<tiles, kScanBlock, 0, s>>>(out, n, aux);
     }
+}
+
+void launch_exclusive_scan(int *data, long long n, int *aux, cudaStream_t s)
+{
+    launch_exclusive_scan_from(data, data, n, aux, false, s);
 }
 
 void launch_permute(const GridDesc &gd, const PArr &src, const PArr &dst, const int *key, const int *rank,

@@ -50,8 +50,8 @@ def _make(po, mpm, w, sort_every, variant=0):
     return o, g
 
 
-# (sort_every, variant): ATOMIC unsorted / ATOMIC with a separate sort / SORTED family (binding.VARIANT_* = 1, 2)
-MODES = [(0, 1), (1, 1), (1, 2)]
+# (sort_every, variant): ATOMIC unsorted / ATOMIC with a separate sort / SORTED family / TILED family (binding.VARIANT_* = 1, 2, 3)
+MODES = [(0, 1), (1, 1), (1, 2), (1, 3)]
 
 
 @pytest.mark.parametrize("mode", MODES)
@@ -115,7 +115,7 @@ def test_reordering_does_not_change_results(mpm):
     """'Optional particles re-ordering' (Alg. 1 l.12) must leave the solution unchanged up to summation order."""
     w = inputs.periodic_box(n=64, perm_seed=7)
     res = []
-    for se, variant in ((0, 1), (1, 1), (5, 1), (1, 2)):
+    for se, variant in ((0, 1), (1, 1), (5, 1), (1, 2), (1, 3)):
         g = mpm.Solver(w["cfg"], sort_every=se, variant=variant)
         g.load_particles(w["x"], w["v"], w["mass"], w["rho"], w["e"])
         g.step(0.0, w["cfl"], 40)
@@ -171,7 +171,7 @@ def test_edge_cases(po, mpm):
     n = x.shape[1]
     v = np.array([[0.3, -0.2, 0.1, 0.0, -0.4, 0.2, 0.1], [0.1, -0.3, 0.0, 0.2, 0.3, -0.1, 0.2]])
     mass = np.full(n, 0.01); rho = np.full(n, 1.0); e = np.linspace(1.0, 2.0, n)
-    for se, variant in ((0, 1), (1, 1), (1, 2)):
+    for se, variant in ((0, 1), (1, 1), (1, 2), (1, 3)):
         o = po.Oracle(cfg); o.load_particles(x, v, mass, rho, e)
         g = mpm.Solver(cfg, sort_every=se, variant=variant); g.load_particles(x, v, mass, rho, e)
         o.step(1e-2, 0.3, 3); g.step(1e-2, 0.3, 3)
