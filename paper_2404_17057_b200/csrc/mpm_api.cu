@@ -30,6 +30,10 @@ struct mpm_handle {
     int *off[2];
     int ocur;
     int *coff;            // TILED: compact storage offsets, allocated on the first storage-order read
+    // TILED: the node accumulators m, mv, f are double-buffered: the update kernel of step n already scatters P2G#1 of
+    // step n+1 into the other set.  acc[acur] = the set the current / next mpm_step starts from (raw P2G#1).
+    double *acc_m[2], *acc_mv[2][3], *acc_f[2][3];
+    int acur;
     long long slots;      // TILED: allocated slots per particle array (particles + one spare slot per odd cell)
     int *goff, *n_groups;
     int4 *groups;
@@ -243,8 +247,8 @@ int alloc_particles(mpm_handle *h, long long n)
     if (ok && (h->variant == MPM_VARIANT_SORTED || tiled)) {
         const long long gs = 1ll << h->gd.dim;
         h->max_groups = n / gs + (n < h->gd.Nc ? n : h->gd.Nc) + 1;
-        ok = dev_alloc_t(h, &h->S[0], N) && dev_alloc_t(h, &h->S[1], N) && dev_alloc_t(h, &h->dest, N) &&
-             dev_alloc_t(h, &h->groups, (size_t)h->max_groups);
+        ok = dev_alloc_t(h, &h->dest, N) && dev_alloc_t(h, &h->groups, (size_t)h->max_groups);
+        if (ok && !tiled) ok = dev_alloc_t(h, &h->S[0], N) && dev_alloc_t(h, &h->S[1], N);
     }
     if (!ok) { free_particles(h); return fail(h, MPM_E_OOM, "out of device memory for particle arrays"); }
     if (tiled) {   // unused slots are read (and masked) by the 128-bit loads: keep them finite
@@ -254,12 +258,20 @@ int alloc_particles(mpm_handle *h, long long n)
             cudaMemsetAsync(p.m, 0, 8 * N, h->stream); cudaMemsetAsync(p.rho, 0, 8 * N, h->stream);
             cudaMemsetAsync(p.e, 0, 8 * N, h->stream); cudaMemsetAsync(p.q, 0, 8 * N, h->stream);
             cudaMemsetAsync(p.id, 0, 4 * N, h->stream);
-            cudaMemsetAsync(h->S[b], 0, 8 * N, h->stream);
         }
         cudaMemsetAsync(h->dest, 0, 8 * N, h->stream);
     }
     h->n = n; h->cap = n; h->cur = 0;
     return MPM_OK;
+}
+
+// TILED: view of the grid arrays with (m, mv, f) = accumulator set `which`
+GArr tiled_acc(const mpm_handle *h, int which)
+{
+    GArr g = h->g;
+    g.m = h->acc_m[which];
+    for (int a = 0; a < 3; ++a) { g.mv[a] = h->acc_mv[which][a]; g.f[a] = h->acc_f[which][a]; }
+    return g;
 }
 
 // cell-key counting sort of all particle arrays into the other buffer (Alg. 1 l.12).  SORTED family: only after a
@@ -275,8 +287,12 @@ void reorder(mpm_handle *h)
         launch_exclusive_scan_from(h->count, h->off[0], h->gd.Nkeys + 1, h->scan_aux, true, h->stream);
         launch_permute(h->gd, src, dst, h->key, h->rank, h->off[0], h->n, h->stream);
         h->cur ^= 1;
-        launch_force_payload_slots(h->gd, dst, h->S[h->cur], h->slots, h->stream);
         launch_build_groups_tiled(h->gd, h->count, h->off[0], h->goff, h->scan_aux, h->groups, h->n_groups, h->stream);
+        // P2G#1 of the first step (Alg. 1 l.3); every later one comes out of the update kernel of the step before
+        h->acur = 0;
+        GArr g0 = tiled_acc(h, 0);
+        launch_grid_clear(h->gd, g0, h->stream);
+        launch_p2g1_tiled(h->gd, dst, g0, SortedMap{ h->groups, h->n_groups, h->goff }, h->max_groups, h->stream);
         h->launches += 12;
         return;
     }
@@ -325,7 +341,8 @@ void step_sorted(mpm_handle *h)
     h->launches += 16;
 }
 
-// one step of Algorithm 1 with the TILED kernel family (see mpm_kernels_tiled.cu)
+// one step of Algorithm 1 with the TILED kernel family (see mpm_kernels_tiled.cu): l.3 of this step was done by the
+// previous step's update kernel (or by the load), l.3 of the next step is done by this step's update kernel
 void step_tiled(mpm_handle *h)
 {
     const GridDesc &gd = h->gd;
@@ -333,25 +350,26 @@ void step_tiled(mpm_handle *h)
     const PArr &p = h->pbuf[h->cur];
     const PArr &q = h->pbuf[h->cur ^ 1];
     const SortedMap map{ h->groups, h->n_groups, h->goff };
+    const GArr gc = tiled_acc(h, h->acur), gnx = tiled_acc(h, h->acur ^ 1);
     {
         Timed t(h, MPM_K_MISC);
         launch_begin_step(h->sc, gd.h, s);                                                // dt (eq. 25/29)
-        launch_grid_clear(gd, h->g, s);                                                   // l.2
+        launch_grid_clear(gd, gnx, s);                                                    // l.2 for the next step's l.3
         cudaMemsetAsync(h->count, 0, sizeof(int) * (size_t)(gd.Nkeys + 1), s);            // per-cell counters of l.12
     }
-    { Timed t(h, MPM_K_P2G1); launch_p2g1_tiled(gd, p, h->S[h->cur], h->g, map, h->max_groups, s); }               // l.3
-    { Timed t(h, MPM_K_NODE1); launch_node1(gd, h->g, h->sc, s); }                                                 // l.4-5
+    { Timed t(h, MPM_K_NODE1); launch_node1(gd, gc, h->sc, s); }                                                   // l.4-5
     { Timed t(h, MPM_K_G2P_P2G2);
-      launch_g2p_p2g2_tiled(gd, p, h->g, h->g.na, h->sc, map, h->count, h->dest, h->max_groups, s); }              // l.6-8
-    { Timed t(h, MPM_K_NODE2); launch_node2(gd, h->g, s); }                                                        // l.9
+      launch_g2p_p2g2_tiled(gd, p, gc, h->g.na, h->sc, map, h->count, h->dest, h->max_groups, s); }                // l.6-8
+    { Timed t(h, MPM_K_NODE2); launch_node2(gd, gc, s); }                                                          // l.9
     { Timed t(h, MPM_K_SORT); launch_exclusive_scan_from(h->count, h->off[0], gd.Nkeys + 1, h->scan_aux, true, s); }   // l.12 offsets
     { Timed t(h, MPM_K_UPDATE);
-      launch_update_tiled(gd, p, q, h->g.na, h->g.nb, h->sc, map, h->off[0], h->dest, h->S[h->cur ^ 1], h->max_groups, s); }   // l.10-12
+      launch_update_tiled(gd, p, q, h->g.na, h->g.nb, h->sc, map, h->off[0], h->dest, gnx, h->max_groups, s); }    // l.10-12, next l.3
     { Timed t(h, MPM_K_MISC); launch_end_step(h->sc, gd.h, s); }                                                   // l.13-14
     { Timed t(h, MPM_K_SORT);
       launch_build_groups_tiled(gd, h->count, h->off[0], h->goff, h->scan_aux, h->groups, h->n_groups, s); }       // next step's groups
     h->cur ^= 1;
-    h->launches += 16;
+    h->acur ^= 1;
+    h->launches += 22;
 }
 
 int copy_in(mpm_handle *h, double *dst, const double *src, long long n, int loc)
@@ -476,6 +494,14 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
             ok = dev_alloc_t(h, &h->g.vbar[a], (size_t)gd.Nn) && dev_alloc_t(h, &h->g.acc[a], (size_t)gd.Nn) &&
                  dev_alloc_t(h, &h->g.v2[a], (size_t)gd.Nn);
     }
+    h->acur = 0;
+    h->acc_m[0] = h->g.m; h->acc_m[1] = nullptr;
+    for (int a = 0; a < 3; ++a) { h->acc_mv[0][a] = h->g.mv[a]; h->acc_f[0][a] = h->g.f[a]; h->acc_mv[1][a] = h->acc_f[1][a] = nullptr; }
+    if (ok && tiled) {
+        ok = dev_alloc_t(h, &h->acc_m[1], (size_t)gd.Nn);
+        for (int a = 0; a < gd.dim && ok; ++a)
+            ok = dev_alloc_t(h, &h->acc_mv[1][a], (size_t)gd.Nn) && dev_alloc_t(h, &h->acc_f[1][a], (size_t)gd.Nn);
+    }
     if (ok && sorted)
         ok = dev_alloc_t(h, &h->g.na, (size_t)gd.Nn * 2 * gd.dim) && dev_alloc_t(h, &h->g.nb, (size_t)gd.Nn * gd.dim) &&
              dev_alloc_t(h, &h->off[0], (size_t)gd.Nkeys + 1) && dev_alloc_t(h, &h->off[1], (size_t)gd.Nkeys + 1) &&
@@ -510,6 +536,11 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
     if (sorted && e == cudaSuccess) e = cudaMemsetAsync(h->g.na, 0, sizeof(double) * (size_t)gd.Nn * 2 * gd.dim, h->stream);
     if (sorted && e == cudaSuccess) e = cudaMemsetAsync(h->g.nb, 0, sizeof(double) * (size_t)gd.Nn * gd.dim, h->stream);
     if (sorted && e == cudaSuccess) e = cudaMemsetAsync(h->n_groups, 0, sizeof(int), h->stream);
+    if (tiled && e == cudaSuccess) e = cudaMemsetAsync(h->acc_m[1], 0, sizeof(double) * (size_t)gd.Nn, h->stream);
+    for (int a = 0; a < gd.dim && tiled && e == cudaSuccess; ++a) {
+        e = cudaMemsetAsync(h->acc_mv[1][a], 0, sizeof(double) * (size_t)gd.Nn, h->stream);
+        if (e == cudaSuccess) e = cudaMemsetAsync(h->acc_f[1][a], 0, sizeof(double) * (size_t)gd.Nn, h->stream);
+    }
     if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
     if (e != cudaSuccess) {
         std::string msg = std::string("mpm_create: ") + cudaGetErrorString(e);
@@ -664,10 +695,12 @@ int mpm_read_grid(mpm_handle *h, int field, double *out, int ptr_location)
     const GridDesc &gd = h->gd;
     const size_t Nn = (size_t)gd.Nn;
     int rc = MPM_OK;
+    // TILED: the last completed step used the accumulator set that is no longer current
+    const GArr gl = (h->variant == MPM_VARIANT_TILED) ? tiled_acc(h, h->steps_done > 0 ? h->acur ^ 1 : h->acur) : h->g;
     switch (field) {
-    case MPM_G_MASS: rc = copy_out(h, out, h->g.m, gd.Nn, ptr_location); break;
-    case MPM_G_MOMENTUM: for (int a = 0; a < gd.dim && rc == MPM_OK; ++a) rc = copy_out(h, out + a * Nn, h->g.mv[a], gd.Nn, ptr_location); break;
-    case MPM_G_FORCE: for (int a = 0; a < gd.dim && rc == MPM_OK; ++a) rc = copy_out(h, out + a * Nn, h->g.f[a], gd.Nn, ptr_location); break;
+    case MPM_G_MASS: rc = copy_out(h, out, gl.m, gd.Nn, ptr_location); break;
+    case MPM_G_MOMENTUM: for (int a = 0; a < gd.dim && rc == MPM_OK; ++a) rc = copy_out(h, out + a * Nn, gl.mv[a], gd.Nn, ptr_location); break;
+    case MPM_G_FORCE: for (int a = 0; a < gd.dim && rc == MPM_OK; ++a) rc = copy_out(h, out + a * Nn, gl.f[a], gd.Nn, ptr_location); break;
     case MPM_G_MOMENTUM2: for (int a = 0; a < gd.dim && rc == MPM_OK; ++a) rc = copy_out(h, out + a * Nn, h->g.mv2[a], gd.Nn, ptr_location); break;
     case MPM_G_NORMAL:
     case MPM_G_FLAG: {

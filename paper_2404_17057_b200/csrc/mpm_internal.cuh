@@ -217,15 +217,15 @@ void launch_update_sorted(const GridDesc &gd, const PArr &p, const PArr &q, cons
                           long long max_groups, cudaStream_t s);
 
 // TILED family (tile-major cell order, even-aligned cell slots, tile nodes in shared memory) -- mpm_kernels_tiled.cu
-void launch_force_payload_slots(const GridDesc &gd, const PArr &p, double *S, long long nslots, cudaStream_t s);
 void launch_build_groups_tiled(const GridDesc &gd, const int *count, const int *off, int *goff, int *scan_aux, int4 *groups,
                                int *n_groups, cudaStream_t s);
-void launch_p2g1_tiled(const GridDesc &gd, const PArr &p, const double *S, const GArr &g, const SortedMap &map,
-                       long long max_groups, cudaStream_t s);
+// P2G#1 after a load (every later step gets it from launch_update_tiled of the step before); g.m, g.mv, g.f must be zero
+void launch_p2g1_tiled(const GridDesc &gd, const PArr &p, const GArr &g, const SortedMap &map, long long max_groups, cudaStream_t s);
 void launch_g2p_p2g2_tiled(const GridDesc &gd, const PArr &p, const GArr &g, const double *na, const DevScalars *sc,
                            const SortedMap &map, int *count, unsigned long long *dest, long long max_groups, cudaStream_t s);
+// update + re-ordering + P2G#1 of the next step into g_next.m, g_next.mv, g_next.f (zeroed by the caller)
 void launch_update_tiled(const GridDesc &gd, const PArr &p, const PArr &q, const double *na, const double *nb, DevScalars *sc,
-                         const SortedMap &map, const int *off_new, const unsigned long long *dest, double *S_out,
+                         const SortedMap &map, const int *off_new, const unsigned long long *dest, const GArr &g_next,
                          long long max_groups, cudaStream_t s);
 // dst[id] = src[slot] for every occupied slot; with coff (exclusive scan of the per-key counts) and off (slot offsets):
 // dst[compact storage index] = src[slot] instead

@@ -1,23 +1,22 @@
-// mpm_kernels_tiled.cu -- TILED kernel family: the SORTED family's lane groups (one cell per group, butterfly
-// reductions, fused re-ordering) re-organised around shared-memory grid tiles.
+// mpm_kernels_tiled.cu -- TILED kernel family: the SORTED family's lane groups (one cell per group of 2^d / 2 lanes, two
+// particles per lane, butterfly reductions, per-group staging of corner node values, fused re-ordering) with
 //
-//   * cell keys are tile-major (TileGeo: 8 x 8 x 4 cells in 3D, 16 x 16 in 2D), so the particles of one tile are one
-//     contiguous run of the cell-sorted order (the grid-to-particle connectivity of PAPER.md:745-748, per tile);
-//   * every cell's slot range starts at an EVEN slot (an odd cell leaves one unused slot), so that lane l of a group
-//     owns the two consecutive particles first + 2l, first + 2l + 1 and fetches each field with ONE aligned 128-bit load;
-//   * a thread block works on a chunk of consecutive groups, cut into segments at tile boundaries.  Per segment:
-//       gathers (Alg. 1 l.6, l.10): the tile's (T+1)^d node values are loaded once into shared memory and every lane
-//         reads its 2^d corners from there (no per-group staging, no redundant global node loads);
-//       scatters (l.3, l.8): group totals go into a shared-memory accumulator tile with fp64 atomicAdd (a CAS loop on
-//         sm_100a, measured 6 clk per conflict-free warp operation against 20 clk for a global RED), and the tile is
-//         flushed with ONE global fp64 reduction per touched node and channel: ~1.5 RED per particle instead of 7 + 3.
-//   * Alg. 1 l.12 is fused as in the SORTED family: the gather kernel ranks every particle in its new cell, a scan of
-//     the (even-rounded) counts gives the new slot offsets, the update kernel writes straight to the sorted slot.
+//   * tile-major cell keys (TileGeo: 8 x 8 x 4 cells in 3D, 16 x 16 in 2D): the particles of one tile are one contiguous
+//     run of the cell-sorted order (the grid-to-particle connectivity of PAPER.md:745-748, per tile), so the node lines a
+//     block touches stay in L2 while it works through the tile;
+//   * even-aligned cell slots: every cell's slot range starts at an EVEN slot (an odd cell leaves one unused slot), so
+//     that lane l of a group owns the two consecutive particles first + 2l, first + 2l + 1 and fetches each field with
+//     ONE aligned 128-bit load (half the load instructions of the SORTED family);
+//   * TWO particle sweeps per step instead of three: P2G#1 of step n+1 (Alg. 1 l.3) has no dt in it and
+//     only needs the state the update of step n has just produced, so it is fused into the update kernel (l.10-12):
+//     a particle that stays in its cell (the common case, CFL <= 0.5: PAPER.md:526) joins the group's butterfly with
+//     weights taken at its NEW position, a particle that changes cell adds its 2^d x (1 + 2d) contributions directly.
+//     The force payload S = (P+Q) M / rho never goes to memory.  Node accumulators m, mv, f are double-buffered.
+//
+// Shared-memory accumulator tiles with fp64 atomicAdd were measured and dropped (git history: CAS loops stall the
+// 16 resident warps; a global RED is asynchronous): scatters use global fp64 reductions as in the SORTED family.
 #include "mpm_lane_groups.cuh"
 
-#ifndef MPM_SCATTER_GLOBAL
-#define MPM_SCATTER_GLOBAL 0   // 1: group totals go straight to global memory (REDG), no shared accumulator tile
-#endif
 #ifndef MPM_MINB
 #define MPM_MINB 2   // resident blocks per SM the particle kernels are compiled for (register budget)
 #endif
@@ -27,65 +26,6 @@ namespace mpm {
 namespace {
 
 using namespace lg;
-
-template <int DIM>
-struct TK {
-    using TG = TileGeo<DIM>;
-    static constexpr int NB = 1 << DIM, LG = NB / 2, GPB = kBlock / LG;
-    static constexpr int CG = 8 * GPB;                      // groups per chunk (a multiple of the groups per iteration)
-    static constexpr int NA = 2 * DIM;                      // doubles per node in the (vbar, acc) tile
-    static constexpr int NBS = (DIM == 3) ? 4 : 2;          // doubles per node in the v2 tile (padded to 16 bytes)
-    static constexpr int NN = TG::NN;
-};
-
-template <int DIM>
-__device__ __forceinline__ void tile_origin(const GridDesc &gd, int tile, int o[DIM])
-{
-    using TG = TileGeo<DIM>;
-    o[0] = (tile % gd.ntile[0]) << TG::LT0;
-    o[1] = ((tile / gd.ntile[0]) % gd.ntile[1]) << TG::LT1;
-    if (DIM == 3) o[DIM - 1] = (tile / (gd.ntile[0] * gd.ntile[1])) << TG::LT2;
-}
-
-// global node index of local node ln of the tile with origin o; -1 if the node lies outside the grid (partial tile).
-// Periodic axes: node n == node 0 (A11).
-template <int DIM>
-__device__ __forceinline__ int tile_global_node(const GridDesc &gd, const int o[DIM], int ln)
-{
-    using TG = TileGeo<DIM>;
-    int i[3] = { ln % TG::N0, (ln / TG::N0) % TG::N1, ln / (TG::N0 * TG::N1) };
-    int idx = 0, stride = 1;
-    bool ok = true;
-#pragma unroll
-    for (int a = 0; a < DIM; ++a) {
-        int gi = o[a] + i[a];
-        if (gi > gd.nc[a]) ok = false;
-        if (gd.per[a] && gi == gd.nc[a]) gi = 0;
-        idx += stride * gi;
-        stride *= gd.nn[a];
-    }
-    return ok ? idx : -1;
-}
-
-// local node index of corner 0 of the cell with coordinates c (the tile origin is a multiple of the tile size)
-template <int DIM>
-__device__ __forceinline__ int tile_local_base(const int c[DIM])
-{
-    using TG = TileGeo<DIM>;
-    int ln = (c[0] & (TG::T0 - 1)) + TG::N0 * (c[1] & (TG::T1 - 1));
-    if (DIM == 3) ln += TG::N0 * TG::N1 * (c[DIM - 1] & (TG::T2 - 1));
-    return ln;
-}
-
-// first group index past the segment that starts at group seg_begin: the end of its tile or of the chunk
-template <int DIM>
-__device__ __forceinline__ int segment_end(const SortedMap &map, int seg_begin, int g_end, int &tile)
-{
-    using TG = TileGeo<DIM>;
-    const int key0 = __ldg(&map.groups[seg_begin].z);
-    tile = key0 >> TG::LTC;
-    return min(g_end, __ldg(&map.goff[(tile + 1) << TG::LTC]));
-}
 
 __device__ __forceinline__ double2 ld2(const double *__restrict__ p, long long k, bool ok)
 {
@@ -104,226 +44,100 @@ __device__ __forceinline__ int tiled_key_of_position(const GridDesc &gd, const d
     return tiled_key_of_cell<DIM>(gd, c);
 }
 
-// flush one accumulator channel of the tile: one global fp64 reduction per touched node (the data race
-// of P2G is closed with atomics; here once per tile and node instead of once per particle and node)
+// Group totals of the P2G#1 channels (m, mv, f) from per-lane payloads and butterfly-order weights, reduced into the node
+// accumulators g.m, g.mv, g.f with one global fp64 reduction per corner and channel (see mpm_kernels_sorted.cu):
+//   pay[i] = { M, M V_a, S } of the lane's particle i, w[i][r] = weight of corner r ^ l (0 for a particle that is not
+//   part of the group reduction).
 template <int DIM>
-__device__ __forceinline__ void flush_channel(const GridDesc &gd, const int o[DIM], const double *s_ch, double *__restrict__ dst)
+__device__ __forceinline__ void scatter_p2g1_group(const GridDesc &gd, const GArr &g, const int c[DIM], int l, bool any,
+                                                   const double pay[2][DIM + 2], const double w[2][1 << DIM])
 {
-    for (int ln = threadIdx.x; ln < TK<DIM>::NN; ln += kBlock) {
-        const double v = s_ch[ln];
-        if (v != 0.0) {
-            const int gn = tile_global_node<DIM>(gd, o, ln);
-            if (gn >= 0) atomicAdd(dst + gn, v);
+    constexpr int NB = 1 << DIM, LG = Geo<DIM>::LG;
+    double tot[DIM + 2][2];
+#pragma unroll
+    for (int ch = 0; ch < DIM + 2; ++ch) {
+        double v[NB];
+#pragma unroll
+        for (int r = 0; r < NB; ++r) v[r] = fma(pay[1][ch], w[1][r], pay[0][ch] * w[0][r]);
+        butterfly<DIM>(v);
+        tot[ch][0] = v[0];
+        tot[ch][1] = v[LG];
+    }
+    // forces of corners b_q = l + q LG: f_a = +-(1/h) (T_S(b) + T_S(b ^ bit_a)), + on the high side of axis a
+    double F[DIM][2];
+#pragma unroll
+    for (int a = 0; a < DIM; ++a) {
+#pragma unroll
+        for (int q = 0; q < 2; ++q) {
+            double other;
+            if ((1 << a) < LG) other = shfl_xor_d(tot[DIM + 1][q], 1 << a);
+            else other = tot[DIM + 1][q ^ 1];
+            const int b = l + q * LG;
+            const double pair = (tot[DIM + 1][q] + other) * gd.inv_h;
+            F[a][q] = ((b >> a) & 1) ? pair : -pair;
         }
     }
-}
-
-// ------------------------------------------------------------------------------------------------ Alg. 1 l.3
-template <int DIM>
-__global__ void __launch_bounds__(kBlock, MPM_MINB) k_p2g1_tiled(GridDesc gd, PArr p, const double *__restrict__ Sarr, GArr g, SortedMap map)
-{
-    using K = TK<DIM>;
-    constexpr int NB = K::NB, LG = K::LG, GPB = K::GPB, NN = K::NN, NCH = 1 + 2 * DIM;
-    __shared__ double s_acc[NCH * NN];
-    const int n_groups = *map.n_groups;
-    const int l = threadIdx.x % LG;
-    for (int chunk = blockIdx.x; (long long)chunk * K::CG < n_groups; chunk += gridDim.x) {
-        const int g_begin = chunk * K::CG, g_end = min(g_begin + K::CG, n_groups);
-        int seg_begin = g_begin;
-        while (seg_begin < g_end) {
-            int tile;
-            const int seg_end = segment_end<DIM>(map, seg_begin, g_end, tile);
-            int o[DIM];
-            tile_origin<DIM>(gd, tile, o);
-#if !MPM_SCATTER_GLOBAL
-            for (int i = threadIdx.x; i < NCH * NN; i += kBlock) s_acc[i] = 0.0;
-            __syncthreads();
-#endif
-            int gidx = seg_begin + threadIdx.x / LG;
-            Group next = fetch_group(map.groups, gidx, seg_end);
-            for (int gb = seg_begin; gb < seg_end; gb += GPB, gidx += GPB) {
-                const Group grp = next;
-                next = fetch_group(map.groups, (long long)gidx + GPB, seg_end);
-                int c[DIM];
-                unpack_coords<DIM>(grp.cpack, c);
-                const bool valid[2] = { 2 * l < grp.cnt, 2 * l + 1 < grp.cnt };
-                const long long k0 = (long long)grp.first + 2 * l;
-                double X[2][DIM], V[2][DIM], M[2], S[2];
+    if (any) {
 #pragma unroll
-                for (int a = 0; a < DIM; ++a) {
-                    const double2 tx = ld2(p.x[a], k0, valid[0]), tv = ld2(p.v[a], k0, valid[0]);
-                    X[0][a] = tx.x; X[1][a] = valid[1] ? tx.y : 0.0;
-                    V[0][a] = tv.x; V[1][a] = valid[1] ? tv.y : 0.0;
-                }
-                {
-                    const double2 tm = ld2(p.m, k0, valid[0]), ts = ld2(Sarr, k0, valid[0]);
-                    M[0] = tm.x; M[1] = valid[1] ? tm.y : 0.0;
-                    S[0] = ts.x; S[1] = valid[1] ? ts.y : 0.0;
-                }
-                double w[2][NB];
-#pragma unroll
-                for (int i = 0; i < 2; ++i) {
-                    double xi[DIM];
-                    const bool fast = valid[i] && local_coords<DIM>(gd, X[i], c, xi);
-                    if (valid[i] && !fast) { slow_p2g1<DIM>(gd, g, X[i], V[i], M[i], S[i]); M[i] = 0.0; S[i] = 0.0; }
-                    if (fast) swizzled_weights<DIM>(xi, l, w[i]);
-                    else {
-#pragma unroll
-                        for (int r = 0; r < NB; ++r) w[i][r] = 0.0;
-                    }
-                }
-                // lane totals per corner, then group totals: channels M, M V_a, S (see mpm_kernels_sorted.cu)
-                double tot[DIM + 2][2];
-#pragma unroll
-                for (int ch = 0; ch < DIM + 2; ++ch) {
-                    double pay[2];
-#pragma unroll
-                    for (int i = 0; i < 2; ++i) pay[i] = (ch == 0) ? M[i] : (ch == DIM + 1) ? S[i] : M[i] * V[i][ch - 1];
-                    double v[NB];
-#pragma unroll
-                    for (int r = 0; r < NB; ++r) v[r] = fma(pay[1], w[1][r], pay[0] * w[0][r]);
-                    butterfly<DIM>(v);
-                    tot[ch][0] = v[0];
-                    tot[ch][1] = v[LG];
-                }
-                double F[DIM][2];
-#pragma unroll
-                for (int a = 0; a < DIM; ++a) {
-#pragma unroll
-                    for (int q = 0; q < 2; ++q) {
-                        double other;
-                        if ((1 << a) < LG) other = shfl_xor_d(tot[DIM + 1][q], 1 << a);
-                        else other = tot[DIM + 1][q ^ 1];
-                        const int b = l + q * LG;
-                        const double pair = (tot[DIM + 1][q] + other) * gd.inv_h;
-                        F[a][q] = ((b >> a) & 1) ? pair : -pair;
-                    }
-                }
-                if (grp.cnt > 0) {
-#if MPM_SCATTER_GLOBAL
-#pragma unroll
-                    for (int q = 0; q < 2; ++q) {
-                        const int node = corner_node_i<DIM>(gd, c, l + q * LG);
-                        atomicAdd(&g.m[node], tot[0][q]);
-#pragma unroll
-                        for (int a = 0; a < DIM; ++a) {
-                            atomicAdd(&g.mv[a][node], tot[1 + a][q]);
-                            atomicAdd(&g.f[a][node], F[a][q]);
-                        }
-                    }
-#else
-                    const int base = tile_local_base<DIM>(c);
-#pragma unroll
-                    for (int q = 0; q < 2; ++q) {
-                        const int b = l + q * LG;
-                        const int ln = base + (b & 1) + TileGeo<DIM>::N0 * ((b >> 1) & 1) +
-                                       ((DIM == 3) ? TileGeo<DIM>::N0 * TileGeo<DIM>::N1 * ((b >> 2) & 1) : 0);
-                        atomicAdd(&s_acc[ln], tot[0][q]);
-#pragma unroll
-                        for (int a = 0; a < DIM; ++a) {
-                            atomicAdd(&s_acc[(1 + a) * NN + ln], tot[1 + a][q]);
-                            atomicAdd(&s_acc[(1 + DIM + a) * NN + ln], F[a][q]);
-                        }
-                    }
-#endif
-                }
-            }
-#if !MPM_SCATTER_GLOBAL
-            __syncthreads();
-            flush_channel<DIM>(gd, o, s_acc, g.m);
+        for (int q = 0; q < 2; ++q) {
+            const int node = corner_node_i<DIM>(gd, c, l + q * LG);
+            atomicAdd(&g.m[node], tot[0][q]);
 #pragma unroll
             for (int a = 0; a < DIM; ++a) {
-                flush_channel<DIM>(gd, o, s_acc + (1 + a) * NN, g.mv[a]);
-                flush_channel<DIM>(gd, o, s_acc + (1 + DIM + a) * NN, g.f[a]);
+                atomicAdd(&g.mv[a][node], tot[1 + a][q]);
+                atomicAdd(&g.f[a][node], F[a][q]);
             }
-            __syncthreads();
-#endif
-            seg_begin = seg_end;
         }
     }
 }
 
-// load the (vbar, acc) node values of a tile: node-major global array na[node][2 DIM] -> s_a[local node][2 DIM]
+// ------------------------------------------------------------------------------------------------ Alg. 1 l.3 (after a load only)
+// m, mv from phi-weighted channels (M, M V); f from the phi-weighted channel S = (P+Q) M / rho (eq. 13).
+// Every later step gets its P2G#1 from the update kernel of the step before.
 template <int DIM>
-__device__ __forceinline__ void load_tile_a(const GridDesc &gd, const int o[DIM], const double *__restrict__ na, double *s_a)
+__global__ void __launch_bounds__(kBlock, MPM_MINB) k_p2g1_tiled(GridDesc gd, PArr p, GArr g, SortedMap map)
 {
-    constexpr int NN = TK<DIM>::NN, U = DIM;    // double2 units per node
-    for (int i = threadIdx.x; i < NN * U; i += kBlock) {
-        const int ln = i / U, j = i % U;
-        const int gn = tile_global_node<DIM>(gd, o, ln);
-        double2 t = make_double2(0.0, 0.0);
-        if (gn >= 0) t = __ldg(reinterpret_cast<const double2 *>(na + (long long)gn * (2 * DIM)) + j);
-        reinterpret_cast<double2 *>(s_a)[i] = t;
-    }
-}
-
-// v2 = mv2/m of a tile: nb[node][DIM] -> s_b[local node][NBS]
-template <int DIM>
-__device__ __forceinline__ void load_tile_b(const GridDesc &gd, const int o[DIM], const double *__restrict__ nb, double *s_b)
-{
-    constexpr int NN = TK<DIM>::NN, NBS = TK<DIM>::NBS;
-    for (int ln = threadIdx.x; ln < NN; ln += kBlock) {
-        const int gn = tile_global_node<DIM>(gd, o, ln);
-#pragma unroll
-        for (int a = 0; a < NBS; ++a) s_b[ln * NBS + a] = (gn >= 0 && a < DIM) ? __ldg(nb + (long long)gn * DIM + a) : 0.0;
-    }
-}
-
-// phi-weighted gather of vbar, acc from the shared tile
-template <int DIM>
-__device__ __forceinline__ void gather_tile_a(const double *s_a, int base, const double w[1 << DIM], double Vb[DIM], double A[DIM])
-{
-    using TG = TileGeo<DIM>;
-    double out[2 * DIM];
-#pragma unroll
-    for (int cc = 0; cc < 2 * DIM; ++cc) out[cc] = 0.0;
-#pragma unroll
-    for (int b = 0; b < (1 << DIM); ++b) {
-        const int ln = base + (b & 1) + TG::N0 * ((b >> 1) & 1) + ((DIM == 3) ? TG::N0 * TG::N1 * ((b >> 2) & 1) : 0);
-        const double2 *row = reinterpret_cast<const double2 *>(s_a + ln * (2 * DIM));
-#pragma unroll
-        for (int j = 0; j < DIM; ++j) {
-            const double2 t = row[j];
-            out[2 * j] = fma(w[b], t.x, out[2 * j]);
-            out[2 * j + 1] = fma(w[b], t.y, out[2 * j + 1]);
-        }
-    }
-#pragma unroll
-    for (int a = 0; a < DIM; ++a) { Vb[a] = out[a]; A[a] = out[DIM + a]; }
-}
-
-// D = sum_b sum_a v2_a(b) d_a phi_b (eq. 19, trace only: PAPER.md:362-364) from the shared v2 tile
-template <int DIM>
-__device__ __forceinline__ double gather_divergence(const double *s_b, int base, const double xi[DIM], double inv_h)
-{
-    using TG = TileGeo<DIM>;
-    constexpr int NBS = TK<DIM>::NBS;
-    double wa[DIM][2];
-#pragma unroll
-    for (int a = 0; a < DIM; ++a) { wa[a][0] = 1.0 - xi[a]; wa[a][1] = xi[a]; }
-    double Da[DIM];
-#pragma unroll
-    for (int a = 0; a < DIM; ++a) Da[a] = 0.0;
-#pragma unroll
-    for (int b = 0; b < (1 << DIM); ++b) {
-        const int ln = base + (b & 1) + TG::N0 * ((b >> 1) & 1) + ((DIM == 3) ? TG::N0 * TG::N1 * ((b >> 2) & 1) : 0);
-        double v2[DIM];
-        const double2 t = *reinterpret_cast<const double2 *>(s_b + ln * NBS);
-        v2[0] = t.x; v2[1] = t.y;
-        if (DIM == 3) v2[DIM - 1] = s_b[ln * NBS + 2];
+    constexpr int NB = 1 << DIM, LG = Geo<DIM>::LG, GPB = Geo<DIM>::GPB;
+    const int n_groups = *map.n_groups;
+    const int l = threadIdx.x % LG;
+    const double gm1 = gd.gamma - 1.0;
+    const long long stride = (long long)gridDim.x * GPB;
+    long long gidx = (long long)blockIdx.x * GPB + threadIdx.x / LG;
+    for (long long g0 = (long long)blockIdx.x * GPB; g0 < n_groups; g0 += stride, gidx += stride) {
+        const Group grp = fetch_group(map.groups, gidx, n_groups);
+        int c[DIM];
+        unpack_coords<DIM>(grp.cpack, c);
+        const bool valid[2] = { 2 * l < grp.cnt, 2 * l + 1 < grp.cnt };
+        const long long k0 = (long long)grp.first + 2 * l;
+        double X[2][DIM], V[2][DIM], pay[2][DIM + 2], w[2][NB];
 #pragma unroll
         for (int a = 0; a < DIM; ++a) {
-            double q = 1.0;
-#pragma unroll
-            for (int a2 = 0; a2 < DIM; ++a2)
-                if (a2 != a) q *= wa[a2][(b >> a2) & 1];
-            Da[a] = ((b >> a) & 1) ? fma(q, v2[a], Da[a]) : fma(-q, v2[a], Da[a]);
+            const double2 tx = ld2(p.x[a], k0, valid[0]), tv = ld2(p.v[a], k0, valid[0]);
+            X[0][a] = tx.x; X[1][a] = valid[1] ? tx.y : 0.0;
+            V[0][a] = tv.x; V[1][a] = valid[1] ? tv.y : 0.0;
         }
-    }
-    double D = 0.0;
+        const double2 tm = ld2(p.m, k0, valid[0]), tr = ld2(p.rho, k0, valid[0]), te = ld2(p.e, k0, valid[0]),
+                      tq = ld2(p.q, k0, valid[0]);
 #pragma unroll
-    for (int a = 0; a < DIM; ++a) D += Da[a];
-    return D * inv_h;
+        for (int i = 0; i < 2; ++i) {
+            const double M = valid[i] ? (i ? tm.y : tm.x) : 0.0, rho = valid[i] ? (i ? tr.y : tr.x) : 1.0;
+            const double E = i ? te.y : te.x, Q = i ? tq.y : tq.x;
+            const double S = valid[i] ? (gm1 * rho * E + Q) * M / rho : 0.0;      // (P+Q) M / rho, P = (gamma-1) rho E (eq. 3)
+            double xi[DIM];
+            const bool fast = valid[i] && local_coords<DIM>(gd, X[i], c, xi);
+            if (valid[i] && !fast) slow_p2g1<DIM>(gd, g, X[i], V[i], M, S);
+            pay[i][0] = fast ? M : 0.0;
+            pay[i][DIM + 1] = fast ? S : 0.0;
+#pragma unroll
+            for (int a = 0; a < DIM; ++a) pay[i][1 + a] = fast ? M * V[i][a] : 0.0;
+            if (fast) swizzled_weights<DIM>(xi, l, w[i]);
+            else {
+#pragma unroll
+                for (int r = 0; r < NB; ++r) w[i][r] = 0.0;
+            }
+        }
+        scatter_p2g1_group<DIM>(gd, g, c, l, grp.cnt > 0, pay, w);
+    }
 }
 
 // Alg. 1 l.11 for one particle (see lg::move_particle); the persistent id is only needed by the recycling generator
@@ -348,257 +162,280 @@ __device__ __forceinline__ void move_particle_lazy_id(const GridDesc &gd, const 
 }
 
 // ------------------------------------------------------------------------------------------------ Alg. 1 l.6-8 (+ l.11-12 bookkeeping)
+// A = G2P(f/m), Vbar = G2P(mv'/m); V' = V + dt A; mv2 += M V' phi.  Also: the particle's cell after the
+// move of l.11 and its rank inside that cell, for the fused re-ordering.  V' is NOT stored: the update kernel recomputes it.
 template <int DIM>
 __global__ void __launch_bounds__(kBlock, MPM_MINB) k_g2p_p2g2_tiled(GridDesc gd, PArr p, GArr g, const double *__restrict__ na,
-                                                           const DevScalars *__restrict__ sc, SortedMap map,
-                                                           int *__restrict__ count, unsigned long long *__restrict__ dest)
+                                                                     const DevScalars *__restrict__ sc, SortedMap map,
+                                                                     int *__restrict__ count, unsigned long long *__restrict__ dest)
 {
-    using K = TK<DIM>;
-    using TG = TileGeo<DIM>;
-    constexpr int NB = K::NB, LG = K::LG, GPB = K::GPB, NN = K::NN;
-    __shared__ __align__(16) double s_a[NN * K::NA];
-    __shared__ double s_acc[DIM * NN];
+    constexpr int NB = 1 << DIM, LG = Geo<DIM>::LG, GPB = Geo<DIM>::GPB;
+    __shared__ __align__(16) double s_vals[(kBlock / 32) * Geo<DIM>::WARP_DOUBLES];
     const int n_groups = *map.n_groups;
     const double dt = sc->dt;
     const long long step = sc->step;
     const int l = threadIdx.x % LG;
-    for (int chunk = blockIdx.x; (long long)chunk * K::CG < n_groups; chunk += gridDim.x) {
-        const int g_begin = chunk * K::CG, g_end = min(g_begin + K::CG, n_groups);
-        int seg_begin = g_begin;
-        while (seg_begin < g_end) {
-            int tile;
-            const int seg_end = segment_end<DIM>(map, seg_begin, g_end, tile);
-            int o[DIM];
-            tile_origin<DIM>(gd, tile, o);
-            load_tile_a<DIM>(gd, o, na, s_a);
-#if !MPM_SCATTER_GLOBAL
-            for (int i = threadIdx.x; i < DIM * NN; i += kBlock) s_acc[i] = 0.0;
-#endif
-            __syncthreads();
-            int gidx = seg_begin + threadIdx.x / LG;
-            Group next = fetch_group(map.groups, gidx, seg_end);
-            for (int gb = seg_begin; gb < seg_end; gb += GPB, gidx += GPB) {
-                const Group grp = next;
-                next = fetch_group(map.groups, (long long)gidx + GPB, seg_end);
-                int c[DIM];
-                unpack_coords<DIM>(grp.cpack, c);
-                const bool valid[2] = { 2 * l < grp.cnt, 2 * l + 1 < grp.cnt };
-                const long long k0 = (long long)grp.first + 2 * l;
-                double X[2][DIM], V[2][DIM], M[2];
+    const int warp = threadIdx.x >> 5, gi = (threadIdx.x & 31) / LG;
+    double *s_group = s_vals + warp * Geo<DIM>::WARP_DOUBLES + gi * Geo<DIM>::GROUP_STRIDE;
+    const long long stride = (long long)gridDim.x * GPB;
+    long long gidx = (long long)blockIdx.x * GPB + threadIdx.x / LG;
+    Group next = fetch_group(map.groups, gidx, n_groups);
+    for (long long g0 = (long long)blockIdx.x * GPB; g0 < n_groups; g0 += stride, gidx += stride) {
+        const Group grp = next;
+        next = fetch_group(map.groups, gidx + stride, n_groups);
+        int c[DIM];
+        unpack_coords<DIM>(grp.cpack, c);
+        const bool valid[2] = { 2 * l < grp.cnt, 2 * l + 1 < grp.cnt };
+        const long long k0 = (long long)grp.first + 2 * l;
+        double X[2][DIM], V[2][DIM], M[2];
 #pragma unroll
-                for (int a = 0; a < DIM; ++a) {
-                    const double2 tx = ld2(p.x[a], k0, valid[0]), tv = ld2(p.v[a], k0, valid[0]);
-                    X[0][a] = tx.x; X[1][a] = valid[1] ? tx.y : 0.0;
-                    V[0][a] = tv.x; V[1][a] = valid[1] ? tv.y : 0.0;
+        for (int a = 0; a < DIM; ++a) {
+            const double2 tx = ld2(p.x[a], k0, valid[0]), tv = ld2(p.v[a], k0, valid[0]);
+            X[0][a] = tx.x; X[1][a] = valid[1] ? tx.y : 0.0;
+            V[0][a] = tv.x; V[1][a] = valid[1] ? tv.y : 0.0;
+        }
+        {
+            const double2 tm = ld2(p.m, k0, valid[0]);
+            M[0] = tm.x; M[1] = valid[1] ? tm.y : 0.0;
+        }
+        int node[2];
+#pragma unroll
+        for (int q = 0; q < 2; ++q) node[q] = corner_node_i<DIM>(gd, c, l + q * LG);
+        if (grp.cnt > 0) {
+#pragma unroll
+            for (int q = 0; q < 2; ++q) stage_na<DIM>(na, node[q], s_group + (l + q * LG) * Geo<DIM>::CH);
+        }
+        __syncwarp();
+        double ws[2][NB], MV[2][DIM];
+        unsigned long long dk[2] = { 0ull, 0ull };
+#pragma unroll
+        for (int i = 0; i < 2; ++i) {
+#pragma unroll
+            for (int r = 0; r < NB; ++r) ws[i][r] = 0.0;
+#pragma unroll
+            for (int a = 0; a < DIM; ++a) MV[i][a] = 0.0;
+            if (valid[i]) {
+                double xi[DIM], Vb[DIM], A[DIM];
+                const bool fast = local_coords<DIM>(gd, X[i], c, xi);
+                if (fast) {
+                    double w[NB], out[2 * DIM];
+                    natural_weights<DIM>(xi, w);
+                    gather_pairs<DIM, DIM>(s_group, w, out);
+#pragma unroll
+                    for (int a = 0; a < DIM; ++a) { Vb[a] = out[a]; A[a] = out[DIM + a]; }
+                    swizzled_weights<DIM>(xi, l, ws[i]);
+                } else {
+                    slow_gather<DIM>(gd, na, nullptr, X[i], Vb, A, nullptr);
                 }
-                {
-                    const double2 tm = ld2(p.m, k0, valid[0]);
-                    M[0] = tm.x; M[1] = valid[1] ? tm.y : 0.0;
-                }
-                const int base = tile_local_base<DIM>(c);
-                double ws[2][NB], MV[2][DIM];
-                unsigned long long dk[2] = { 0ull, 0ull };
 #pragma unroll
-                for (int i = 0; i < 2; ++i) {
-#pragma unroll
-                    for (int r = 0; r < NB; ++r) ws[i][r] = 0.0;
+                for (int a = 0; a < DIM; ++a) MV[i][a] = M[i] * fma(dt, A[a], V[i][a]);   // M V'
+                if (!fast) {
+                    slow_p2g2<DIM>(gd, g, X[i], MV[i]);
 #pragma unroll
                     for (int a = 0; a < DIM; ++a) MV[i][a] = 0.0;
-                    if (valid[i]) {
-                        double xi[DIM], Vb[DIM], A[DIM];
-                        const bool fast = local_coords<DIM>(gd, X[i], c, xi);
-                        if (fast) {
-                            double w[NB];
-                            natural_weights<DIM>(xi, w);
-                            gather_tile_a<DIM>(s_a, base, w, Vb, A);
-                            swizzled_weights<DIM>(xi, l, ws[i]);
-                        } else {
-                            slow_gather<DIM>(gd, na, nullptr, X[i], Vb, A, nullptr);
-                        }
-#pragma unroll
-                        for (int a = 0; a < DIM; ++a) MV[i][a] = M[i] * fma(dt, A[a], V[i][a]);   // M V'
-                        if (!fast) {
-                            slow_p2g2<DIM>(gd, g, X[i], MV[i]);
-#pragma unroll
-                            for (int a = 0; a < DIM; ++a) MV[i][a] = 0.0;
-                        }
-                        double Xn[DIM];
-                        move_particle_lazy_id<DIM>(gd, X[i], Vb, dt, p.id, k0 + i, step, Xn);
-                        const int key = tiled_key_of_position<DIM>(gd, Xn);
-                        const int rank = atomicAdd(&count[key], 1);
-                        dk[i] = ((unsigned long long)(unsigned)key << 32) | (unsigned)rank;
-                    }
                 }
-                if (valid[1]) *reinterpret_cast<ulonglong2 *>(dest + k0) = make_ulonglong2(dk[0], dk[1]);
-                else if (valid[0]) dest[k0] = dk[0];
-                double tot[DIM][2];
-#pragma unroll
-                for (int a = 0; a < DIM; ++a) {
-                    double v[NB];
-#pragma unroll
-                    for (int r = 0; r < NB; ++r) v[r] = fma(MV[1][a], ws[1][r], MV[0][a] * ws[0][r]);
-                    butterfly<DIM>(v);
-                    tot[a][0] = v[0];
-                    tot[a][1] = v[LG];
-                }
-                if (grp.cnt > 0) {
-#pragma unroll
-                    for (int q = 0; q < 2; ++q) {
-#if MPM_SCATTER_GLOBAL
-                        const int node = corner_node_i<DIM>(gd, c, l + q * LG);
-#pragma unroll
-                        for (int a = 0; a < DIM; ++a) atomicAdd(&g.mv2[a][node], tot[a][q]);
-#else
-                        const int b = l + q * LG;
-                        const int ln = base + (b & 1) + TG::N0 * ((b >> 1) & 1) + ((DIM == 3) ? TG::N0 * TG::N1 * ((b >> 2) & 1) : 0);
-#pragma unroll
-                        for (int a = 0; a < DIM; ++a) atomicAdd(&s_acc[a * NN + ln], tot[a][q]);
-#endif
-                    }
-                }
+                // where the particle will be after l.11, and its rank among the particles that end up in that cell
+                double Xn[DIM];
+                move_particle_lazy_id<DIM>(gd, X[i], Vb, dt, p.id, k0 + i, step, Xn);
+                const int key = tiled_key_of_position<DIM>(gd, Xn);
+                const int rank = atomicAdd(&count[key], 1);
+                dk[i] = ((unsigned long long)(unsigned)key << 32) | (unsigned)rank;
             }
-            __syncthreads();
-#if !MPM_SCATTER_GLOBAL
-#pragma unroll
-            for (int a = 0; a < DIM; ++a) flush_channel<DIM>(gd, o, s_acc + a * NN, g.mv2[a]);
-            __syncthreads();
-#endif
-            seg_begin = seg_end;
         }
+        if (valid[1]) *reinterpret_cast<ulonglong2 *>(dest + k0) = make_ulonglong2(dk[0], dk[1]);
+        else if (valid[0]) dest[k0] = dk[0];
+        double tot[DIM][2];
+#pragma unroll
+        for (int a = 0; a < DIM; ++a) {
+            double v[NB];
+#pragma unroll
+            for (int r = 0; r < NB; ++r) v[r] = fma(MV[1][a], ws[1][r], MV[0][a] * ws[0][r]);
+            butterfly<DIM>(v);
+            tot[a][0] = v[0];
+            tot[a][1] = v[LG];
+        }
+        if (grp.cnt > 0) {
+#pragma unroll
+            for (int q = 0; q < 2; ++q)
+#pragma unroll
+                for (int a = 0; a < DIM; ++a) atomicAdd(&g.mv2[a][node[q]], tot[a][q]);
+        }
+        __syncwarp();      // the staging area is rewritten by the next iteration
     }
 }
 
-// ------------------------------------------------------------------------------------------------ Alg. 1 l.10-13
+// ------------------------------------------------------------------------------------------------ Alg. 1 l.10-13 + l.3 of the next step
+// D = trace G2PD(mv2/m); Q (eq. 4), E', rho'; V' = V + dt A again; CFL maxima;
+// X' = X + dt Vbar; the particle is written to its cell-sorted slot of the OTHER buffer (l.12).
+// Then P2G#1 of the NEXT step at X' into the node accumulators `gn` (the other buffer of m, mv, f).
 template <int DIM>
 __global__ void __launch_bounds__(kBlock, MPM_MINB) k_update_tiled(GridDesc gd, PArr p, PArr q, const double *__restrict__ na,
-                                                         const double *__restrict__ nb, DevScalars *sc, SortedMap map,
-                                                         const int *__restrict__ off_new,
-                                                         const unsigned long long *__restrict__ dest, double *__restrict__ S_out)
+                                                                   const double *__restrict__ nb, DevScalars *sc, SortedMap map,
+                                                                   const int *__restrict__ off_new,
+                                                                   const unsigned long long *__restrict__ dest, GArr gn)
 {
-    using K = TK<DIM>;
-    constexpr int NB = K::NB, LG = K::LG, GPB = K::GPB, NN = K::NN;
-    __shared__ __align__(16) double s_a[NN * K::NA];
-    __shared__ __align__(16) double s_b[NN * K::NBS];
+    constexpr int NB = 1 << DIM, LG = Geo<DIM>::LG, GPB = Geo<DIM>::GPB;
+    constexpr int NPAIR = (DIM == 3) ? 4 : 3;
+    __shared__ __align__(16) double s_vals[(kBlock / 32) * Geo<DIM>::WARP_DOUBLES];
     __shared__ double s_v[kBlock / 32], s_c[kBlock / 32];
     const int n_groups = *map.n_groups;
     const double dt = sc->dt;
     const long long step = sc->step;
     const int l = threadIdx.x % LG;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, gi = lane / LG;
+    double *s_group = s_vals + warp * Geo<DIM>::WARP_DOUBLES + gi * Geo<DIM>::GROUP_STRIDE;
+    const long long stride = (long long)gridDim.x * GPB;
+    long long gidx = (long long)blockIdx.x * GPB + threadIdx.x / LG;
+    Group next = fetch_group(map.groups, gidx, n_groups);
     double vloc = 0.0, cloc = 0.0;
     int n_rec = 0, n_clamp = 0, n_neg = 0, n_nonfin = 0;
     const double gm1 = gd.gamma - 1.0;
-    for (int chunk = blockIdx.x; (long long)chunk * K::CG < n_groups; chunk += gridDim.x) {
-        const int g_begin = chunk * K::CG, g_end = min(g_begin + K::CG, n_groups);
-        int seg_begin = g_begin;
-        while (seg_begin < g_end) {
-            int tile;
-            const int seg_end = segment_end<DIM>(map, seg_begin, g_end, tile);
-            int o[DIM];
-            tile_origin<DIM>(gd, tile, o);
-            load_tile_a<DIM>(gd, o, na, s_a);
-            load_tile_b<DIM>(gd, o, nb, s_b);
-            __syncthreads();
-            int gidx = seg_begin + threadIdx.x / LG;
-            Group next = fetch_group(map.groups, gidx, seg_end);
-            for (int gb = seg_begin; gb < seg_end; gb += GPB, gidx += GPB) {
-                const Group grp = next;
-                next = fetch_group(map.groups, (long long)gidx + GPB, seg_end);
-                int c[DIM];
-                unpack_coords<DIM>(grp.cpack, c);
-                const bool valid[2] = { 2 * l < grp.cnt, 2 * l + 1 < grp.cnt };
-                const long long k0 = (long long)grp.first + 2 * l;
-                double X[2][DIM], V[2][DIM], M[2], rho[2], E[2];
-                int id[2];
-                unsigned long long dk[2];
+    for (long long g0 = (long long)blockIdx.x * GPB; g0 < n_groups; g0 += stride, gidx += stride) {
+        const Group grp = next;
+        next = fetch_group(map.groups, gidx + stride, n_groups);
+        int c[DIM];
+        unpack_coords<DIM>(grp.cpack, c);
+        const bool valid[2] = { 2 * l < grp.cnt, 2 * l + 1 < grp.cnt };
+        const long long k0 = (long long)grp.first + 2 * l;
+        double X[2][DIM], V[2][DIM], M[2], rho[2], E[2];
+        int id[2];
+        unsigned long long dk[2];
 #pragma unroll
-                for (int a = 0; a < DIM; ++a) {
-                    const double2 tx = ld2(p.x[a], k0, valid[0]), tv = ld2(p.v[a], k0, valid[0]);
-                    X[0][a] = tx.x; X[1][a] = valid[1] ? tx.y : 0.0;
-                    V[0][a] = tv.x; V[1][a] = valid[1] ? tv.y : 0.0;
+        for (int a = 0; a < DIM; ++a) {
+            const double2 tx = ld2(p.x[a], k0, valid[0]), tv = ld2(p.v[a], k0, valid[0]);
+            X[0][a] = tx.x; X[1][a] = valid[1] ? tx.y : 0.0;
+            V[0][a] = tv.x; V[1][a] = valid[1] ? tv.y : 0.0;
+        }
+        {
+            const double2 tm = ld2(p.m, k0, valid[0]), tr = ld2(p.rho, k0, valid[0]), te = ld2(p.e, k0, valid[0]);
+            M[0] = tm.x; M[1] = valid[1] ? tm.y : 0.0;
+            rho[0] = valid[0] ? tr.x : 1.0; rho[1] = valid[1] ? tr.y : 1.0;
+            E[0] = te.x; E[1] = valid[1] ? te.y : 0.0;
+            int2 ti = make_int2(0, 0);
+            ulonglong2 td = make_ulonglong2(0ull, 0ull);
+            if (valid[0]) {
+                ti = __ldg(reinterpret_cast<const int2 *>(p.id + k0));
+                td = __ldg(reinterpret_cast<const ulonglong2 *>(dest + k0));
+            }
+            id[0] = ti.x; id[1] = ti.y;
+            dk[0] = td.x; dk[1] = td.y;
+        }
+        // stage vbar, acc of corners l, l + LG, and dsum_b = sum_a (v2_a(high corner) - v2_a(low corner)) / h
+        double v2[2][DIM];
+        int node[2];
+#pragma unroll
+        for (int qq = 0; qq < 2; ++qq) {
+            node[qq] = corner_node_i<DIM>(gd, c, l + qq * LG);
+#pragma unroll
+            for (int a = 0; a < DIM; ++a) v2[qq][a] = (grp.cnt > 0) ? __ldg(nb + (long long)node[qq] * DIM + a) : 0.0;
+        }
+        double dsum[2] = { 0.0, 0.0 };
+#pragma unroll
+        for (int a = 0; a < DIM; ++a) {
+#pragma unroll
+            for (int qq = 0; qq < 2; ++qq) {
+                double other;
+                if ((1 << a) < LG) other = shfl_xor_d(v2[qq][a], 1 << a);
+                else other = v2[qq ^ 1][a];
+                const int b = l + qq * LG;
+                dsum[qq] += ((b >> a) & 1) ? (v2[qq][a] - other) : (other - v2[qq][a]);
+            }
+        }
+        if (grp.cnt > 0) {
+#pragma unroll
+            for (int qq = 0; qq < 2; ++qq) {
+                double *s_corner = s_group + (l + qq * LG) * Geo<DIM>::CH;
+                stage_na<DIM>(na, node[qq], s_corner);
+                *reinterpret_cast<double2 *>(s_corner + 2 * DIM) = make_double2(dsum[qq] * gd.inv_h, 0.0);
+            }
+        }
+        __syncwarp();
+        double pay[2][DIM + 2], wn[2][NB];      // next step's P2G#1: payload M, M V', S' and weights at X'
+#pragma unroll
+        for (int i = 0; i < 2; ++i) {
+#pragma unroll
+            for (int ch = 0; ch < DIM + 2; ++ch) pay[i][ch] = 0.0;
+#pragma unroll
+            for (int r = 0; r < NB; ++r) wn[i][r] = 0.0;
+            if (valid[i]) {
+                double xi[DIM], Vb[DIM], A[DIM], D;
+                if (local_coords<DIM>(gd, X[i], c, xi)) {
+                    double w[NB], out[2 * NPAIR];
+                    natural_weights<DIM>(xi, w);
+                    gather_pairs<DIM, NPAIR>(s_group, w, out);
+#pragma unroll
+                    for (int a = 0; a < DIM; ++a) { Vb[a] = out[a]; A[a] = out[DIM + a]; }
+                    D = out[2 * DIM];
+                } else {
+                    slow_gather<DIM>(gd, na, nb, X[i], Vb, A, &D);
                 }
-                {
-                    const double2 tm = ld2(p.m, k0, valid[0]), tr = ld2(p.rho, k0, valid[0]), te = ld2(p.e, k0, valid[0]);
-                    M[0] = tm.x; M[1] = valid[1] ? tm.y : 0.0;
-                    rho[0] = valid[0] ? tr.x : 1.0; rho[1] = valid[1] ? tr.y : 1.0;
-                    E[0] = te.x; E[1] = valid[1] ? te.y : 0.0;
-                    int2 ti = make_int2(0, 0);
-                    ulonglong2 td = make_ulonglong2(0ull, 0ull);
-                    if (valid[0]) {
-                        ti = __ldg(reinterpret_cast<const int2 *>(p.id + k0));
-                        td = __ldg(reinterpret_cast<const ulonglong2 *>(dest + k0));
+                double Vn[DIM];
+#pragma unroll
+                for (int a = 0; a < DIM; ++a) Vn[a] = fma(dt, A[a], V[i][a]);   // V'
+                // particle thermodynamics (eq. 4 with this step's D: reading A2).  P/rho = (gamma-1) E
+                // and gamma P/rho = gamma (gamma-1) E are used in place of the quotients (one rounding apart).
+                const double r = rho[i], e0 = E[i];
+                double Q = 0.0, Q_over_rho = 0.0;
+                if (D < 0.0) {
+                    const double cs0 = sqrt(gd.gamma * gm1 * e0);
+                    if (gd.visc_form == MPM_VISC_STANDARD) {
+                        Q_over_rho = gd.c0 * gd.h * gd.h * D * D - gd.c1 * gd.h * cs0 * D;
+                        Q = r * Q_over_rho;
+                    } else {
+                        Q = gd.c0 * (r * gd.h * D) * (r * gd.h * D) - gd.c1 * gd.h * cs0 * D;
+                        Q_over_rho = Q / r;
                     }
-                    id[0] = ti.x; id[1] = ti.y;
-                    dk[0] = td.x; dk[1] = td.y;
                 }
-                const int base = tile_local_base<DIM>(c);
+                double En = e0 - dt * (gm1 * e0 + Q_over_rho) * D;
+                const double jac = fma(dt, D, 1.0);
+                if (jac <= 0.0) n_neg++;
+                double rhon = r / jac;
+                const double cs = sqrt(gd.gamma * gm1 * En);
+                if (!isfinite(En) || !isfinite(rhon)) n_nonfin++;
+                double vv = 0.0, vb2 = 0.0;
 #pragma unroll
-                for (int i = 0; i < 2; ++i) {
-                    if (valid[i]) {
-                        double xi[DIM], Vb[DIM], A[DIM], D;
-                        if (local_coords<DIM>(gd, X[i], c, xi)) {
-                            double w[NB];
-                            natural_weights<DIM>(xi, w);
-                            gather_tile_a<DIM>(s_a, base, w, Vb, A);
-                            D = gather_divergence<DIM>(s_b, base, xi, gd.inv_h);
-                        } else {
-                            slow_gather<DIM>(gd, na, nb, X[i], Vb, A, &D);
-                        }
-                        double Vn[DIM];
+                for (int a = 0; a < DIM; ++a) { vv = fma(Vn[a], Vn[a], vv); vb2 = fma(Vb[a], Vb[a], vb2); }
+                vloc = fmax(vloc, fmax(vv, vb2));      // squared; the root is taken once at the end
+                cloc = fmax(cloc, cs);
+                double Xn[DIM];
+                bool recycled;
+                int nclamp;
+                move_particle<DIM>(gd, X[i], Vb, dt, (long long)id[i], step, Xn, recycled, nclamp);
+                n_clamp += nclamp;
+                double Mn = M[i];
+                if (recycled) {
 #pragma unroll
-                        for (int a = 0; a < DIM; ++a) Vn[a] = fma(dt, A[a], V[i][a]);   // V'
-                        // particle thermodynamics (eq. 4 with this step's D: reading A2)
-                        const double r = rho[i], e0 = E[i];
-                        double Q = 0.0, Q_over_rho = 0.0;
-                        if (D < 0.0) {
-                            const double cs0 = sqrt(gd.gamma * gm1 * e0);
-                            if (gd.visc_form == MPM_VISC_STANDARD) {
-                                Q_over_rho = gd.c0 * gd.h * gd.h * D * D - gd.c1 * gd.h * cs0 * D;
-                                Q = r * Q_over_rho;
-                            } else {
-                                Q = gd.c0 * (r * gd.h * D) * (r * gd.h * D) - gd.c1 * gd.h * cs0 * D;
-                                Q_over_rho = Q / r;
-                            }
-                        }
-                        double En = e0 - dt * (gm1 * e0 + Q_over_rho) * D;
-                        const double jac = fma(dt, D, 1.0);
-                        if (jac <= 0.0) n_neg++;
-                        double rhon = r / jac;
-                        const double cs = sqrt(gd.gamma * gm1 * En);
-                        if (!isfinite(En) || !isfinite(rhon)) n_nonfin++;
-                        double vv = 0.0, vb2 = 0.0;
+                    for (int a = 0; a < DIM; ++a) Vn[a] = gd.inflow_v[a];
+                    rhon = gd.inflow_rho; En = gd.inflow_e; Q = 0.0; Mn = gd.inflow_mass;
+                    n_rec++;
+                }
+                const long long dst = (long long)off_new[(int)(dk[i] >> 32)] + (long long)(unsigned)(dk[i] & 0xffffffffull);
 #pragma unroll
-                        for (int a = 0; a < DIM; ++a) { vv = fma(Vn[a], Vn[a], vv); vb2 = fma(Vb[a], Vb[a], vb2); }
-                        vloc = fmax(vloc, fmax(vv, vb2));      // squared; the root is taken once at the end
-                        cloc = fmax(cloc, cs);
-                        double Xn[DIM];
-                        bool recycled;
-                        int nclamp;
-                        move_particle<DIM>(gd, X[i], Vb, dt, (long long)id[i], step, Xn, recycled, nclamp);
-                        n_clamp += nclamp;
-                        double Mn = M[i];
-                        if (recycled) {
+                for (int a = 0; a < DIM; ++a) { q.x[a][dst] = Xn[a]; q.v[a][dst] = Vn[a]; }
+                q.m[dst] = Mn;
+                q.rho[dst] = rhon;
+                q.e[dst] = En;
+                q.q[dst] = Q;
+                q.id[dst] = id[i];
+                // P2G#1 of the next step (eq. 13, 14, 16, 18 at X'): in the group's butterfly if the particle stays in the
+                // group's cell, else directly
+                const double Sn = (gm1 * rhon * En + Q) * Mn / rhon;
+                double xin[DIM];
+                if (local_coords<DIM>(gd, Xn, c, xin)) {
+                    swizzled_weights<DIM>(xin, l, wn[i]);
+                    pay[i][0] = Mn;
+                    pay[i][DIM + 1] = Sn;
 #pragma unroll
-                            for (int a = 0; a < DIM; ++a) Vn[a] = gd.inflow_v[a];
-                            rhon = gd.inflow_rho; En = gd.inflow_e; Q = 0.0; Mn = gd.inflow_mass;
-                            n_rec++;
-                        }
-                        const long long dst = (long long)off_new[(int)(dk[i] >> 32)] + (long long)(unsigned)(dk[i] & 0xffffffffull);
-#pragma unroll
-                        for (int a = 0; a < DIM; ++a) { q.x[a][dst] = Xn[a]; q.v[a][dst] = Vn[a]; }
-                        q.m[dst] = Mn;
-                        q.rho[dst] = rhon;
-                        q.e[dst] = En;
-                        q.q[dst] = Q;
-                        q.id[dst] = id[i];
-                        S_out[dst] = (gm1 * rhon * En + Q) * Mn / rhon;     // eq. (13) payload of the next step
-                    }
+                    for (int a = 0; a < DIM; ++a) pay[i][1 + a] = Mn * Vn[a];
+                } else {
+                    slow_p2g1<DIM>(gd, gn, Xn, Vn, Mn, Sn);
                 }
             }
-            __syncthreads();      // the tiles are reloaded by the next segment
-            seg_begin = seg_end;
         }
+        scatter_p2g1_group<DIM>(gd, gn, c, l, grp.cnt > 0, pay, wn);
+        __syncwarp();      // the staging area is rewritten by the next iteration
     }
+    // block maxima -> one atomicMax per block (max is order-free, so this is exact)
     vloc = warp_max_nonneg(sqrt(vloc));
     cloc = warp_max_nonneg(cloc >= 0.0 ? cloc : 0.0);
     if (lane == 0) { s_v[warp] = vloc; s_c[warp] = cloc; }
@@ -621,13 +458,6 @@ __global__ void __launch_bounds__(kBlock, MPM_MINB) k_update_tiled(GridDesc gd, 
 }
 
 // ------------------------------------------------------------------------------------------------ bookkeeping kernels
-
-__global__ void __launch_bounds__(kBlock) k_force_payload_slots(double gamma, const double *m, const double *rho, const double *e,
-                                                                const double *q, double *S, long long n)
-{
-    const long long k = (long long)blockIdx.x * kBlock + threadIdx.x;
-    if (k < n) S[k] = ((gamma - 1.0) * rho[k] * e[k] + q[k]) * m[k] / rho[k];    // unused slots hold zeros -> NaN, never read
-}
 
 __global__ void __launch_bounds__(kBlock) k_group_counts_tiled(const int *count, int *gcount, int nkeys, int cap)
 {
@@ -712,23 +542,18 @@ inline unsigned blocks_for(long long n, int per) { return (unsigned)((n + per - 
 
 // persistent launch: as many blocks as are resident at once (occupancy query), never more than there are chunks
 template <typename Kernel>
-inline unsigned persistent_blocks(long long max_groups, int groups_per_chunk, Kernel kernel)
+inline unsigned persistent_blocks(long long max_groups, int groups_per_block, Kernel kernel)
 {
     int dev = 0, sms = 148, per_sm = 1;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, kBlock, 0) != cudaSuccess || per_sm < 1) per_sm = 1;
     const long long want = (long long)sms * per_sm;
-    const long long need = (max_groups + groups_per_chunk - 1) / groups_per_chunk;
+    const long long need = (max_groups + groups_per_block - 1) / groups_per_block;
     return (unsigned)(need < want ? (need > 0 ? need : 1) : want);
 }
 
 }  // namespace
-
-void launch_force_payload_slots(const GridDesc &gd, const PArr &p, double *S, long long nslots, cudaStream_t s)
-{
-    if (nslots > 0) k_force_payload_slots<<<blocks_for(nslots, kBlock), kBlock, 0, s>>>(gd.gamma, p.m, p.rho, p.e, p.q, S, nslots);
-}
 
 void launch_build_groups_tiled(const GridDesc &gd, const int *count, const int *off, int *goff, int *scan_aux, int4 *groups,
                                int *n_groups, cudaStream_t s)
@@ -741,12 +566,11 @@ void launch_build_groups_tiled(const GridDesc &gd, const int *count, const int *
     else k_group_fill_tiled<3><<<blocks_for(nkeys, kBlock), kBlock, 0, s>>>(gd, count, off, goff, groups, n_groups, nkeys);
 }
 
-void launch_p2g1_tiled(const GridDesc &gd, const PArr &p, const double *S, const GArr &g, const SortedMap &map,
-                       long long max_groups, cudaStream_t s)
+void launch_p2g1_tiled(const GridDesc &gd, const PArr &p, const GArr &g, const SortedMap &map, long long max_groups, cudaStream_t s)
 {
     if (max_groups <= 0) return;
-    if (gd.dim == 2) k_p2g1_tiled<2><<<persistent_blocks(max_groups, TK<2>::CG, k_p2g1_tiled<2>), kBlock, 0, s>>>(gd, p, S, g, map);
-    else k_p2g1_tiled<3><<<persistent_blocks(max_groups, TK<3>::CG, k_p2g1_tiled<3>), kBlock, 0, s>>>(gd, p, S, g, map);
+    if (gd.dim == 2) k_p2g1_tiled<2><<<persistent_blocks(max_groups, Geo<2>::GPB, k_p2g1_tiled<2>), kBlock, 0, s>>>(gd, p, g, map);
+    else k_p2g1_tiled<3><<<persistent_blocks(max_groups, Geo<3>::GPB, k_p2g1_tiled<3>), kBlock, 0, s>>>(gd, p, g, map);
 }
 
 void launch_g2p_p2g2_tiled(const GridDesc &gd, const PArr &p, const GArr &g, const double *na, const DevScalars *sc,
@@ -754,20 +578,20 @@ void launch_g2p_p2g2_tiled(const GridDesc &gd, const PArr &p, const GArr &g, con
 {
     if (max_groups <= 0) return;
     if (gd.dim == 2)
-        k_g2p_p2g2_tiled<2><<<persistent_blocks(max_groups, TK<2>::CG, k_g2p_p2g2_tiled<2>), kBlock, 0, s>>>(gd, p, g, na, sc, map, count, dest);
+        k_g2p_p2g2_tiled<2><<<persistent_blocks(max_groups, Geo<2>::GPB, k_g2p_p2g2_tiled<2>), kBlock, 0, s>>>(gd, p, g, na, sc, map, count, dest);
     else
-        k_g2p_p2g2_tiled<3><<<persistent_blocks(max_groups, TK<3>::CG, k_g2p_p2g2_tiled<3>), kBlock, 0, s>>>(gd, p, g, na, sc, map, count, dest);
+        k_g2p_p2g2_tiled<3><<<persistent_blocks(max_groups, Geo<3>::GPB, k_g2p_p2g2_tiled<3>), kBlock, 0, s>>>(gd, p, g, na, sc, map, count, dest);
 }
 
 void launch_update_tiled(const GridDesc &gd, const PArr &p, const PArr &q, const double *na, const double *nb, DevScalars *sc,
-                         const SortedMap &map, const int *off_new, const unsigned long long *dest, double *S_out,
+                         const SortedMap &map, const int *off_new, const unsigned long long *dest, const GArr &g_next,
                          long long max_groups, cudaStream_t s)
 {
     if (max_groups <= 0) return;
     if (gd.dim == 2)
-        k_update_tiled<2><<<persistent_blocks(max_groups, TK<2>::CG, k_update_tiled<2>), kBlock, 0, s>>>(gd, p, q, na, nb, sc, map, off_new, dest, S_out);
+        k_update_tiled<2><<<persistent_blocks(max_groups, Geo<2>::GPB, k_update_tiled<2>), kBlock, 0, s>>>(gd, p, q, na, nb, sc, map, off_new, dest, g_next);
     else
-        k_update_tiled<3><<<persistent_blocks(max_groups, TK<3>::CG, k_update_tiled<3>), kBlock, 0, s>>>(gd, p, q, na, nb, sc, map, off_new, dest, S_out);
+        k_update_tiled<3><<<persistent_blocks(max_groups, Geo<3>::GPB, k_update_tiled<3>), kBlock, 0, s>>>(gd, p, q, na, nb, sc, map, off_new, dest, g_next);
 }
 
 void launch_gather_by_id_groups(const double *src, const int *id, double *dst, const SortedMap &map, long long max_groups,

@@ -254,5 +254,33 @@ __device__ __forceinline__ int cell_key(const GridDesc &gd, const double X[DIM])
     return key;
 }
 
+// lane l stages vbar, acc of one corner (node-major array na[node][2 DIM]) into shared memory
+template <int DIM>
+__device__ __forceinline__ void stage_na(const double *__restrict__ na, int node, double *s_corner)
+{
+    const double2 *src = reinterpret_cast<const double2 *>(na + (long long)node * (2 * DIM));
+    double2 *dst = reinterpret_cast<double2 *>(s_corner);
+#pragma unroll
+    for (int q = 0; q < DIM; ++q) dst[q] = __ldg(src + q);
+}
+
+// phi-weighted gather of the staged channels: out[c] = sum_b w[b] vals[b][c], c < 2*NPAIR
+template <int DIM, int NPAIR>
+__device__ __forceinline__ void gather_pairs(const double *s_group, const double w[1 << DIM], double out[2 * NPAIR])
+{
+#pragma unroll
+    for (int c = 0; c < 2 * NPAIR; ++c) out[c] = 0.0;
+#pragma unroll
+    for (int b = 0; b < (1 << DIM); ++b) {
+        const double2 *row = reinterpret_cast<const double2 *>(s_group + b * Geo<DIM>::CH);
+#pragma unroll
+        for (int q = 0; q < NPAIR; ++q) {
+            const double2 t = row[q];
+            out[2 * q] = fma(w[b], t.x, out[2 * q]);
+            out[2 * q + 1] = fma(w[b], t.y, out[2 * q + 1]);
+        }
+    }
+}
+
 }  // namespace lg
 }  // namespace mpm
