@@ -37,6 +37,9 @@ struct mpm_handle {
     long long slots;      // TILED: allocated slots per particle array (particles + one spare slot per odd cell)
     int *goff, *n_groups;
     int4 *groups;
+    int4 *items;          // TILED: work items of the tile kernels (one block each), rebuilt with the groups
+    int *n_items;
+    long long max_items;
     double *S[2];
     unsigned long long *dest;
     long long max_groups;
@@ -226,6 +229,8 @@ void free_particles(mpm_handle *h)
     h->key = h->rank = nullptr;
     dev_free(h, h->S[0]); dev_free(h, h->S[1]); dev_free(h, h->dest); dev_free(h, h->groups);
     h->S[0] = h->S[1] = nullptr; h->dest = nullptr; h->groups = nullptr;
+    dev_free(h, h->items);
+    h->items = nullptr; h->max_items = 0;
     h->n = h->cap = 0;
 }
 
@@ -249,6 +254,10 @@ int alloc_particles(mpm_handle *h, long long n)
         h->max_groups = n / gs + (n < h->gd.Nc ? n : h->gd.Nc) + 1;
         ok = dev_alloc_t(h, &h->dest, N) && dev_alloc_t(h, &h->groups, (size_t)h->max_groups);
         if (ok && !tiled) ok = dev_alloc_t(h, &h->S[0], N) && dev_alloc_t(h, &h->S[1], N);
+        if (ok && tiled) {
+            h->max_items = max_items_tiled(h->gd, h->max_groups);
+            ok = dev_alloc_t(h, &h->items, (size_t)h->max_items);
+        }
     }
     if (!ok) { free_particles(h); return fail(h, MPM_E_OOM, "out of device memory for particle arrays"); }
     if (tiled) {   // unused slots are read (and masked) by the 128-bit loads: keep them finite
@@ -288,12 +297,13 @@ void reorder(mpm_handle *h)
         launch_permute(h->gd, src, dst, h->key, h->rank, h->off[0], h->n, h->stream);
         h->cur ^= 1;
         launch_build_groups_tiled(h->gd, h->count, h->off[0], h->goff, h->scan_aux, h->groups, h->n_groups, h->stream);
+        launch_build_items(h->gd, h->goff, h->items, h->n_items, h->stream);
         // P2G#1 of the first step (Alg. 1 l.3); every later one comes out of the update kernel of the step before
         h->acur = 0;
         GArr g0 = tiled_acc(h, 0);
         launch_grid_clear(h->gd, g0, h->stream);
         launch_p2g1_tiled(h->gd, dst, g0, SortedMap{ h->groups, h->n_groups, h->goff }, h->max_groups, h->stream);
-        h->launches += 12;
+        h->launches += 13;
         return;
     }
     int *count = h->variant == MPM_VARIANT_SORTED ? h->off[h->ocur] : h->count;
@@ -359,17 +369,18 @@ void step_tiled(mpm_handle *h)
     }
     { Timed t(h, MPM_K_NODE1); launch_node1(gd, gc, h->sc, s); }                                                   // l.4-5
     { Timed t(h, MPM_K_G2P_P2G2);
-      launch_g2p_p2g2_tiled(gd, p, gc, h->g.na, h->sc, map, h->count, h->dest, h->max_groups, s); }                // l.6-8
+      launch_g2p_p2g2_tiled(gd, p, gc, h->g.na, h->sc, map, h->items, h->n_items, h->max_items, h->count, h->dest, s); }   // l.6-8
     { Timed t(h, MPM_K_NODE2); launch_node2(gd, gc, s); }                                                          // l.9
     { Timed t(h, MPM_K_SORT); launch_exclusive_scan_from(h->count, h->off[0], gd.Nkeys + 1, h->scan_aux, true, s); }   // l.12 offsets
     { Timed t(h, MPM_K_UPDATE);
-      launch_update_tiled(gd, p, q, h->g.na, h->g.nb, h->sc, map, h->off[0], h->dest, gnx, h->max_groups, s); }    // l.10-12, next l.3
+      launch_update_tiled(gd, p, q, h->g.na, h->g.nb, h->sc, map, h->items, h->n_items, h->max_items, h->off[0], h->dest, gnx, s); }   // l.10-12, next l.3
     { Timed t(h, MPM_K_MISC); launch_end_step(h->sc, gd.h, s); }                                                   // l.13-14
     { Timed t(h, MPM_K_SORT);
-      launch_build_groups_tiled(gd, h->count, h->off[0], h->goff, h->scan_aux, h->groups, h->n_groups, s); }       // next step's groups
+      launch_build_groups_tiled(gd, h->count, h->off[0], h->goff, h->scan_aux, h->groups, h->n_groups, s);         // next step's groups
+      launch_build_items(gd, h->goff, h->items, h->n_items, s); }                                                  // ... and work items
     h->cur ^= 1;
     h->acur ^= 1;
-    h->launches += 22;
+    h->launches += 23;
 }
 
 int copy_in(mpm_handle *h, double *dst, const double *src, long long n, int loc)
@@ -416,6 +427,7 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
     for (int k = 0; k < MPM_K_COUNT; ++k) { h->kernel_ms[k] = 0.0; h->kernel_calls[k] = 0; }
     h->d_flag = nullptr; h->key = h->rank = h->count = h->scan_aux = nullptr; h->sc = nullptr;
     h->off[0] = h->off[1] = nullptr; h->ocur = 0; h->goff = h->n_groups = nullptr; h->groups = nullptr;
+    h->items = nullptr; h->n_items = nullptr; h->max_items = 0;
     h->S[0] = h->S[1] = nullptr; h->dest = nullptr; h->max_groups = 0; h->coff = nullptr; h->slots = 0;
     std::memset(h->pbuf, 0, sizeof(h->pbuf));
     std::memset(&h->g, 0, sizeof(h->g));
@@ -505,7 +517,7 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
     if (ok && sorted)
         ok = dev_alloc_t(h, &h->g.na, (size_t)gd.Nn * 2 * gd.dim) && dev_alloc_t(h, &h->g.nb, (size_t)gd.Nn * gd.dim) &&
              dev_alloc_t(h, &h->off[0], (size_t)gd.Nkeys + 1) && dev_alloc_t(h, &h->off[1], (size_t)gd.Nkeys + 1) &&
-             dev_alloc_t(h, &h->goff, (size_t)gd.Nkeys + 1) && dev_alloc_t(h, &h->n_groups, 1);
+             dev_alloc_t(h, &h->goff, (size_t)gd.Nkeys + 1) && dev_alloc_t(h, &h->n_groups, 1) && dev_alloc_t(h, &h->n_items, 1);
     // the scan's block sums: one int per 4096 scanned elements
     ok = ok && dev_alloc_t(h, &h->count, (size_t)gd.Nkeys + 1) && dev_alloc_t(h, &h->scan_aux, (size_t)gd.Nkeys / 4096 + 8) &&
          dev_alloc_t(h, &h->sc, 1);
@@ -536,6 +548,7 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
     if (sorted && e == cudaSuccess) e = cudaMemsetAsync(h->g.na, 0, sizeof(double) * (size_t)gd.Nn * 2 * gd.dim, h->stream);
     if (sorted && e == cudaSuccess) e = cudaMemsetAsync(h->g.nb, 0, sizeof(double) * (size_t)gd.Nn * gd.dim, h->stream);
     if (sorted && e == cudaSuccess) e = cudaMemsetAsync(h->n_groups, 0, sizeof(int), h->stream);
+    if (sorted && e == cudaSuccess) e = cudaMemsetAsync(h->n_items, 0, sizeof(int), h->stream);
     if (tiled && e == cudaSuccess) e = cudaMemsetAsync(h->acc_m[1], 0, sizeof(double) * (size_t)gd.Nn, h->stream);
     for (int a = 0; a < gd.dim && tiled && e == cudaSuccess; ++a) {
         e = cudaMemsetAsync(h->acc_mv[1][a], 0, sizeof(double) * (size_t)gd.Nn, h->stream);

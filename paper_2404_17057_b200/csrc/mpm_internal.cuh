@@ -110,10 +110,11 @@ struct DevScalars {
 
 // ---------------------------------------------------------------------------------------------- device helpers
 
-// Cell and local coordinate of a position along one axis (readings A6, A19)
+// Cell and local coordinate of a position along one axis (readings A6, A19).  The product is rounded on
+// its own (no contraction into s - c): every kernel that bins a position gets the same cell for it.
 __device__ __forceinline__ void cell_1d(double X, double inv_h, int ncell, int &c, double &xi)
 {
-    double s = X * inv_h;
+    double s = __dmul_rn(X, inv_h);
     int ci = (int)floor(s);
     ci = max(0, min(ci, ncell - 1));
     c = ci;
@@ -221,12 +222,16 @@ void launch_build_groups_tiled(const GridDesc &gd, const int *count, const int *
                                int *n_groups, cudaStream_t s);
 // P2G#1 after a load (every later step gets it from launch_update_tiled of the step before); g.m, g.mv, g.f must be zero
 void launch_p2g1_tiled(const GridDesc &gd, const PArr &p, const GArr &g, const SortedMap &map, long long max_groups, cudaStream_t s);
+// work items of the tile kernels: one block per item = <= Chunk::GROUPS groups of one tile; rebuilt every step
+void launch_build_items(const GridDesc &gd, const int *goff, int4 *items, int *n_items, cudaStream_t s);
+long long max_items_tiled(const GridDesc &gd, long long max_groups);   // upper bound of the item count (launch size)
 void launch_g2p_p2g2_tiled(const GridDesc &gd, const PArr &p, const GArr &g, const double *na, const DevScalars *sc,
-                           const SortedMap &map, int *count, unsigned long long *dest, long long max_groups, cudaStream_t s);
+                           const SortedMap &map, const int4 *items, const int *n_items, long long max_items, int *count,
+                           unsigned long long *dest, cudaStream_t s);
 // update + re-ordering + P2G#1 of the next step into g_next.m, g_next.mv, g_next.f (zeroed by the caller)
 void launch_update_tiled(const GridDesc &gd, const PArr &p, const PArr &q, const double *na, const double *nb, DevScalars *sc,
-                         const SortedMap &map, const int *off_new, const unsigned long long *dest, const GArr &g_next,
-                         long long max_groups, cudaStream_t s);
+                         const SortedMap &map, const int4 *items, const int *n_items, long long max_items, const int *off_new,
+                         const unsigned long long *dest, const GArr &g_next, cudaStream_t s);
 // dst[id] = src[slot] for every occupied slot; with coff (exclusive scan of the per-key counts) and off (slot offsets):
 // dst[compact storage index] = src[slot] instead
 void launch_gather_by_id_groups(const double *src, const int *id, double *dst, const SortedMap &map, long long max_groups,

@@ -2,8 +2,9 @@
 // particles per lane, butterfly reductions, per-group staging of corner node values, fused re-ordering) with
 //
 //   * tile-major cell keys (TileGeo: 8 x 8 x 4 cells in 3D, 16 x 16 in 2D): the particles of one tile are one contiguous
-//     run of the cell-sorted order (the grid-to-particle connectivity of PAPER.md:745-748, per tile), so the node lines a
-//     block touches stay in L2 while it works through the tile;
+//     run of the cell-sorted order (the grid-to-particle connectivity of PAPER.md:745-748, per tile).  One thread block
+//     works on one tile (or a chunk of a dense tile): the tile's (T+1)^d node velocities are staged ONCE in shared memory
+//     and every particle of the tile gathers from there (no per-group staging, each corner read once per lane);
 //   * even-aligned cell slots: every cell's slot range starts at an EVEN slot (an odd cell leaves one unused slot), so
 //     that lane l of a group owns the two consecutive particles first + 2l, first + 2l + 1 and fetches each field with
 //     ONE aligned 128-bit load (half the load instructions of the SORTED family);
@@ -140,6 +141,143 @@ __global__ void __launch_bounds__(kBlock, MPM_MINB) k_p2g1_tiled(GridDesc gd, PA
     }
 }
 
+// ------------------------------------------------------------------------------------------------ tile work items
+// A block works on one ITEM = up to Chunk<DIM>::GROUPS consecutive groups of ONE tile (a tile with more groups is cut into
+// several items, so that a dense tile does not serialise on one block).  The item list is rebuilt every step from the
+// per-key group offsets (k_build_items).
+template <int DIM>
+struct Chunk {
+    static constexpr int PASSES = 8;
+    static constexpr int GROUPS = PASSES * Geo<DIM>::GPB;
+};
+
+// tile-local node index j = lx + N0 (ly + N1 lz) of corner b of the cell with tile-local node index j0
+template <int DIM>
+__device__ __forceinline__ constexpr int corner_off(int b)
+{
+    using TG = TileGeo<DIM>;
+    return (b & 1) + TG::N0 * ((b >> 1) & 1) + ((DIM == 3) ? TG::N0 * TG::N1 * ((b >> 2) & 1) : 0);
+}
+
+template <int DIM>
+__device__ __forceinline__ void tile_origin(const GridDesc &gd, int tile, int org[DIM])
+{
+    using TG = TileGeo<DIM>;
+    org[0] = (tile % gd.ntile[0]) << TG::LT0;
+    org[1] = ((tile / gd.ntile[0]) % gd.ntile[1]) << TG::LT1;
+    if (DIM == 3) org[DIM - 1] = (tile / (gd.ntile[0] * gd.ntile[1])) << TG::LT2;
+}
+
+// global node index of tile-local node j (periodic wrap: node n == node 0, A11); -1 = outside the grid
+template <int DIM>
+__device__ __forceinline__ int tile_node_global(const GridDesc &gd, const int org[DIM], int j)
+{
+    using TG = TileGeo<DIM>;
+    int ln[3];
+    ln[0] = j % TG::N0;
+    ln[1] = (j / TG::N0) % TG::N1;
+    ln[2] = j / (TG::N0 * TG::N1);
+    int idx = 0, stride = 1;
+    bool ok = true;
+#pragma unroll
+    for (int a = 0; a < DIM; ++a) {
+        int i = org[a] + ln[a];
+        if (i > gd.nc[a]) ok = false;
+        if (gd.per[a] && i == gd.nc[a]) i = 0;
+        idx += stride * i;
+        stride *= gd.nn[a];
+    }
+    return ok ? idx : -1;
+}
+
+// Stage the node velocities of one tile in shared memory, node-major with CH doubles per node:
+//   [0, DIM) vbar = mv'/m, [DIM, 2 DIM) acc = f/m (from na), and with WITH_NB [2 DIM, 3 DIM) v2 = mv2/m (from nb), rest 0.
+template <int DIM, int CH, bool WITH_NB>
+__device__ __forceinline__ void stage_tile(const GridDesc &gd, const int org[DIM], const double *__restrict__ na,
+                                           const double *__restrict__ nb, double *s_tile)
+{
+    using TG = TileGeo<DIM>;
+    for (int j = threadIdx.x; j < TG::NN; j += kBlock) {
+        const int node = tile_node_global<DIM>(gd, org, j);
+        double2 *dst = reinterpret_cast<double2 *>(s_tile + j * CH);
+        double2 v[CH / 2];
+#pragma unroll
+        for (int q = 0; q < CH / 2; ++q) v[q] = make_double2(0.0, 0.0);
+        if (node >= 0) {
+            const double2 *src = reinterpret_cast<const double2 *>(na + (long long)node * (2 * DIM));
+#pragma unroll
+            for (int q = 0; q < DIM; ++q) v[q] = __ldg(src + q);
+            if (WITH_NB) {
+                double t[DIM + 1];
+#pragma unroll
+                for (int a = 0; a < DIM; ++a) t[a] = __ldg(nb + (long long)node * DIM + a);
+                t[DIM] = 0.0;
+#pragma unroll
+                for (int q = 0; q < (DIM + 1) / 2; ++q) v[DIM + q] = make_double2(t[2 * q], t[2 * q + 1]);
+            }
+        }
+#pragma unroll
+        for (int q = 0; q < CH / 2; ++q) dst[q] = v[q];
+    }
+}
+
+// 1D weights of a particle w.r.t. the GROUP's cell c (the particle is in that cell: exact sort, see move_particle):
+// W[a][0] = 1 - xi_a, W[a][1] = xi_a with xi = X / h - c (A19)
+template <int DIM>
+__device__ __forceinline__ void weights_1d(const GridDesc &gd, const double X[DIM], const int c[DIM], double xi[DIM], double W[DIM][2])
+{
+#pragma unroll
+    for (int a = 0; a < DIM; ++a) {
+        xi[a] = __dmul_rn(X[a], gd.inv_h) - (double)c[a];
+        W[a][0] = 1.0 - xi[a];
+        W[a][1] = xi[a];
+    }
+}
+
+// phi-weighted gather of the staged tile for the TWO particles of a lane (each corner is read once for both):
+//   out[i][ch] = sum_b phi_b(X_i) n_b[ch], ch < 2 DIM  (eq. 17: Vbar, A);
+//   with WITH_D also Dh[i] = h * sum_b sum_a v2_a(b) d_a phi_b(X_i)  (eq. 19, trace; the factor 1/h is applied by the caller)
+template <int DIM, int CH, bool WITH_D>
+__device__ __forceinline__ void gather_tile(const double *s_cell, const double W[2][DIM][2], double out[2][2 * DIM], double Dh[2])
+{
+#pragma unroll
+    for (int i = 0; i < 2; ++i) {
+        Dh[i] = 0.0;
+#pragma unroll
+        for (int ch = 0; ch < 2 * DIM; ++ch) out[i][ch] = 0.0;
+    }
+#pragma unroll
+    for (int b = 0; b < (1 << DIM); ++b) {
+        const double2 *row = reinterpret_cast<const double2 *>(s_cell + corner_off<DIM>(b) * CH);
+        double val[CH];
+#pragma unroll
+        for (int q = 0; q < CH / 2; ++q) {
+            const double2 t = row[q];
+            val[2 * q] = t.x;
+            val[2 * q + 1] = t.y;
+        }
+#pragma unroll
+        for (int i = 0; i < 2; ++i) {
+            double phi = W[i][0][b & 1];
+#pragma unroll
+            for (int a = 1; a < DIM; ++a) phi *= W[i][a][(b >> a) & 1];
+#pragma unroll
+            for (int ch = 0; ch < 2 * DIM; ++ch) out[i][ch] = fma(phi, val[ch], out[i][ch]);
+            if (WITH_D) {
+#pragma unroll
+                for (int a = 0; a < DIM; ++a) {
+                    double q = 1.0;
+#pragma unroll
+                    for (int a2 = 0; a2 < DIM; ++a2)
+                        if (a2 != a) q *= W[i][a2][(b >> a2) & 1];
+                    const double sv = ((b >> a) & 1) ? val[2 * DIM + a] : -val[2 * DIM + a];
+                    Dh[i] = fma(sv, q, Dh[i]);
+                }
+            }
+        }
+    }
+}
+
 // Alg. 1 l.11 for one particle (see lg::move_particle); the persistent id is only needed by the recycling generator
 // (A8), so it is fetched only when a particle actually leaves through an OUTFLOW face.
 template <int DIM>
@@ -161,30 +299,94 @@ __device__ __forceinline__ void move_particle_lazy_id(const GridDesc &gd, const 
     move_particle<DIM>(gd, X, Vb, dt, id, step, Xn, recycled, nclamp);
 }
 
+__device__ __forceinline__ double sel3(const double v[], int a, int dim)
+{
+    double r = v[0];
+    if (a == 1) r = v[1];
+    if (dim == 3 && a == 2) r = v[dim - 1];
+    return r;
+}
+__device__ __forceinline__ double *selp(double *const p[3], int a, int dim)
+{
+    double *r = p[0];
+    if (a == 1) r = p[1];
+    if (dim == 3 && a == 2) r = p[dim - 1];
+    return r;
+}
+
+// P2G#1 (eqs. 13, 14, 16, 18) of the particles flagged in `mask` (one bit per lane), done by the WHOLE warp: the
+// particle's data is broadcast, lane (corner b = lane % 2^d, q = lane / 2^d) adds the channels q, q + 32 / 2^d, ... of
+// corner b (channels: m, mv_a, f_a).  Used for particles that leave their group's cell (their contributions cannot
+// join the group's butterfly): 2 warp instructions instead of 2^d (1 + 2 d) per particle.
+template <int DIM>
+__device__ __forceinline__ void coop_p2g1(const GridDesc &gd, const GArr &gn, unsigned mask, const double Xn[DIM],
+                                          const double Vn[DIM], double Mn, double Sn, int lane)
+{
+    constexpr int NB = 1 << DIM, NQ = 32 / NB, NCH = 1 + 2 * DIM;
+    const int b = lane & (NB - 1), q = lane / NB;
+    while (mask) {
+        const int src = __ffs(mask) - 1;
+        mask &= mask - 1;
+        double X[DIM], V[DIM];
+#pragma unroll
+        for (int a = 0; a < DIM; ++a) {
+            X[a] = __shfl_sync(kFull, Xn[a], src);
+            V[a] = __shfl_sync(kFull, Vn[a], src);
+        }
+        const double M = __shfl_sync(kFull, Mn, src), S = __shfl_sync(kFull, Sn, src);
+        int c[DIM];
+        double xi[DIM];
+        particle_cell<DIM>(gd, X, c, xi);
+        const long long node = corner_node<DIM>(gd, c, b);
+        const double phi = corner_phi<DIM>(xi, b);
+#pragma unroll
+        for (int it = 0; it < (NCH + NQ - 1) / NQ; ++it) {
+            const int ch = q + it * NQ;
+            if (ch == 0) {
+                atomicAdd(gn.m + node, M * phi);
+            } else if (ch <= DIM) {
+                atomicAdd(selp(gn.mv, ch - 1, DIM) + node, M * sel3(V, ch - 1, DIM) * phi);
+            } else if (ch < NCH) {
+                atomicAdd(selp(gn.f, ch - 1 - DIM, DIM) + node, S * corner_dphi<DIM>(xi, b, ch - 1 - DIM, gd.inv_h));
+            }
+        }
+    }
+}
+
 // ------------------------------------------------------------------------------------------------ Alg. 1 l.6-8 (+ l.11-12 bookkeeping)
-// A = G2P(f/m), Vbar = G2P(mv'/m); V' = V + dt A; mv2 += M V' phi.  Also: the particle's cell after the
-// move of l.11 and its rank inside that cell, for the fused re-ordering.  V' is NOT stored: the update kernel recomputes it.
+// One block per item.  The tile's node velocities vbar = mv'/m, acc = f/m are staged once in shared memory; every lane
+// gathers A = G2P(f/m), Vbar = G2P(mv'/m) for its two particles from there (eq. 17), V' = V + dt A
+// (PAPER.md:776), mv2 += M V' phi through the group butterfly.  Also: the particle's cell after the
+// move of l.11 and its rank inside that cell, for the fused re-ordering (l.12): the particles of a group that stay in
+// their cell take consecutive ranks from ONE atomic per group (ballot + popc), only the others pay one atomic each.
+// V' is NOT stored: the update kernel recomputes it.
 template <int DIM>
 __global__ void __launch_bounds__(kBlock, MPM_MINB) k_g2p_p2g2_tiled(GridDesc gd, PArr p, GArr g, const double *__restrict__ na,
                                                                      const DevScalars *__restrict__ sc, SortedMap map,
+                                                                     const int4 *__restrict__ items, const int *__restrict__ n_items,
                                                                      int *__restrict__ count, unsigned long long *__restrict__ dest)
 {
-    constexpr int NB = 1 << DIM, LG = Geo<DIM>::LG, GPB = Geo<DIM>::GPB;
-    __shared__ __align__(16) double s_vals[(kBlock / 32) * Geo<DIM>::WARP_DOUBLES];
-    const int n_groups = *map.n_groups;
+    using TG = TileGeo<DIM>;
+    constexpr int NB = 1 << DIM, LG = Geo<DIM>::LG, GPB = Geo<DIM>::GPB, CH = 2 * DIM;
+    __shared__ __align__(16) double s_tile[TG::NN * CH];
+    if ((int)blockIdx.x >= *n_items) return;
+    const int4 item = __ldg(items + blockIdx.x);      // {tile, first group, groups, -}
+    int org[DIM];
+    tile_origin<DIM>(gd, item.x, org);
+    int gl = threadIdx.x / LG;
+    Group next = fetch_group(map.groups, (long long)item.y + gl, gl < item.z ? item.y + item.z : 0);
+    stage_tile<DIM, CH, false>(gd, org, na, nullptr, s_tile);
+    __syncthreads();
     const double dt = sc->dt;
     const long long step = sc->step;
-    const int l = threadIdx.x % LG;
-    const int warp = threadIdx.x >> 5, gi = (threadIdx.x & 31) / LG;
-    double *s_group = s_vals + warp * Geo<DIM>::WARP_DOUBLES + gi * Geo<DIM>::GROUP_STRIDE;
-    const long long stride = (long long)gridDim.x * GPB;
-    long long gidx = (long long)blockIdx.x * GPB + threadIdx.x / LG;
-    Group next = fetch_group(map.groups, gidx, n_groups);
-    for (long long g0 = (long long)blockIdx.x * GPB; g0 < n_groups; g0 += stride, gidx += stride) {
+    const int l = threadIdx.x % LG, lane = threadIdx.x & 31, sh = lane & ~(LG - 1);
+    for (int p0 = 0; p0 < item.z; p0 += GPB, gl += GPB) {
         const Group grp = next;
-        next = fetch_group(map.groups, gidx + stride, n_groups);
+        next = fetch_group(map.groups, (long long)item.y + gl + GPB, gl + GPB < item.z ? item.y + item.z : 0);
         int c[DIM];
         unpack_coords<DIM>(grp.cpack, c);
+        const int local = grp.cell & (TG::TC - 1);      // grp.cell = tile-major key
+        const int j0 = (local & (TG::T0 - 1)) + TG::N0 * (((local >> TG::LT0) & (TG::T1 - 1)) + TG::N1 * (local >> (TG::LT0 + TG::LT1)));
         const bool valid[2] = { 2 * l < grp.cnt, 2 * l + 1 < grp.cnt };
         const long long k0 = (long long)grp.first + 2 * l;
         double X[2][DIM], V[2][DIM], M[2];
@@ -198,52 +400,45 @@ __global__ void __launch_bounds__(kBlock, MPM_MINB) k_g2p_p2g2_tiled(GridDesc gd
             const double2 tm = ld2(p.m, k0, valid[0]);
             M[0] = tm.x; M[1] = valid[1] ? tm.y : 0.0;
         }
-        int node[2];
+        double W[2][DIM][2], xi[2][DIM], out[2][2 * DIM], Dh[2];
 #pragma unroll
-        for (int q = 0; q < 2; ++q) node[q] = corner_node_i<DIM>(gd, c, l + q * LG);
-        if (grp.cnt > 0) {
-#pragma unroll
-            for (int q = 0; q < 2; ++q) stage_na<DIM>(na, node[q], s_group + (l + q * LG) * Geo<DIM>::CH);
-        }
-        __syncwarp();
-        double ws[2][NB], MV[2][DIM];
-        unsigned long long dk[2] = { 0ull, 0ull };
+        for (int i = 0; i < 2; ++i) weights_1d<DIM>(gd, X[i], c, xi[i], W[i]);
+        gather_tile<DIM, CH, false>(s_tile + j0 * CH, W, out, Dh);
+        double MV[2][DIM];
+        int key[2] = { -1, -1 };
 #pragma unroll
         for (int i = 0; i < 2; ++i) {
 #pragma unroll
-            for (int r = 0; r < NB; ++r) ws[i][r] = 0.0;
-#pragma unroll
-            for (int a = 0; a < DIM; ++a) MV[i][a] = 0.0;
+            for (int a = 0; a < DIM; ++a) MV[i][a] = M[i] * fma(dt, out[i][DIM + a], V[i][a]);   // M V'
             if (valid[i]) {
-                double xi[DIM], Vb[DIM], A[DIM];
-                const bool fast = local_coords<DIM>(gd, X[i], c, xi);
-                if (fast) {
-                    double w[NB], out[2 * DIM];
-                    natural_weights<DIM>(xi, w);
-                    gather_pairs<DIM, DIM>(s_group, w, out);
-#pragma unroll
-                    for (int a = 0; a < DIM; ++a) { Vb[a] = out[a]; A[a] = out[DIM + a]; }
-                    swizzled_weights<DIM>(xi, l, ws[i]);
-                } else {
-                    slow_gather<DIM>(gd, na, nullptr, X[i], Vb, A, nullptr);
-                }
-#pragma unroll
-                for (int a = 0; a < DIM; ++a) MV[i][a] = M[i] * fma(dt, A[a], V[i][a]);   // M V'
-                if (!fast) {
-                    slow_p2g2<DIM>(gd, g, X[i], MV[i]);
-#pragma unroll
-                    for (int a = 0; a < DIM; ++a) MV[i][a] = 0.0;
-                }
-                // where the particle will be after l.11, and its rank among the particles that end up in that cell
+                // where the particle will be after l.11
                 double Xn[DIM];
-                move_particle_lazy_id<DIM>(gd, X[i], Vb, dt, p.id, k0 + i, step, Xn);
-                const int key = tiled_key_of_position<DIM>(gd, Xn);
-                const int rank = atomicAdd(&count[key], 1);
-                dk[i] = ((unsigned long long)(unsigned)key << 32) | (unsigned)rank;
+                move_particle_lazy_id<DIM>(gd, X[i], out[i], dt, p.id, k0 + i, step, Xn);
+                key[i] = tiled_key_of_position<DIM>(gd, Xn);
             }
         }
-        if (valid[1]) *reinterpret_cast<ulonglong2 *>(dest + k0) = make_ulonglong2(dk[0], dk[1]);
-        else if (valid[0]) dest[k0] = dk[0];
+        // ranks among the particles that end up in the same cell (arrival order of the atomics, A17)
+        const bool stay[2] = { valid[0] && key[0] == grp.cell, valid[1] && key[1] == grp.cell };
+        const unsigned gmask = (1u << LG) - 1u;
+        const unsigned g0 = (__ballot_sync(kFull, stay[0]) >> sh) & gmask, g1 = (__ballot_sync(kFull, stay[1]) >> sh) & gmask;
+        const int nstay = __popc(g0) + __popc(g1);
+        int base = 0;
+        if (l == 0 && nstay > 0) base = atomicAdd(&count[grp.cell], nstay);
+        base = __shfl_sync(kFull, base, sh);
+        const unsigned lower = (1u << l) - 1u;
+        const int pre = base + __popc(g0 & lower) + __popc(g1 & lower);
+        int rank[2] = { pre, pre + (int)((g0 >> l) & 1u) };
+#pragma unroll
+        for (int i = 0; i < 2; ++i)
+            if (valid[i] && !stay[i]) rank[i] = atomicAdd(&count[key[i]], 1);
+        const unsigned long long dk0 = ((unsigned long long)(unsigned)key[0] << 32) | (unsigned)rank[0];
+        const unsigned long long dk1 = ((unsigned long long)(unsigned)key[1] << 32) | (unsigned)rank[1];
+        if (valid[1]) *reinterpret_cast<ulonglong2 *>(dest + k0) = make_ulonglong2(dk0, dk1);
+        else if (valid[0]) dest[k0] = dk0;
+        // P2G#2: group totals of M V' phi per corner, one global reduction per corner and component
+        double ws[2][NB];
+#pragma unroll
+        for (int i = 0; i < 2; ++i) swizzled_weights<DIM>(xi[i], l, ws[i]);
         double tot[DIM][2];
 #pragma unroll
         for (int a = 0; a < DIM; ++a) {
@@ -256,45 +451,54 @@ __global__ void __launch_bounds__(kBlock, MPM_MINB) k_g2p_p2g2_tiled(GridDesc gd
         }
         if (grp.cnt > 0) {
 #pragma unroll
-            for (int q = 0; q < 2; ++q)
+            for (int q = 0; q < 2; ++q) {
+                const int node = corner_node_i<DIM>(gd, c, l + q * LG);
 #pragma unroll
-                for (int a = 0; a < DIM; ++a) atomicAdd(&g.mv2[a][node[q]], tot[a][q]);
+                for (int a = 0; a < DIM; ++a) atomicAdd(&g.mv2[a][node], tot[a][q]);
+            }
         }
-        __syncwarp();      // the staging area is rewritten by the next iteration
     }
 }
 
 // ------------------------------------------------------------------------------------------------ Alg. 1 l.10-13 + l.3 of the next step
-// D = trace G2PD(mv2/m); Q (eq. 4), E', rho'; V' = V + dt A again; CFL maxima;
-// X' = X + dt Vbar; the particle is written to its cell-sorted slot of the OTHER buffer (l.12).
-// Then P2G#1 of the NEXT step at X' into the node accumulators `gn` (the other buffer of m, mv, f).
+// One block per item; the tile's vbar, acc AND v2 = mv2/m are staged in shared memory.  D = trace G2PD(mv2/m) (eq. 19);
+// Q (eq. 4), E', rho'; V' = V + dt A again; CFL maxima; X' = X + dt Vbar
+// (PAPER.md:372-376); the particle is written to its cell-sorted slot of the OTHER buffer (l.12).  Then P2G#1 of the
+// NEXT step at X' into the node accumulators `gn` (the other buffer of m, mv, f): a particle that
+// stays in its cell joins the group's butterfly, the others are scattered by the whole warp (coop_p2g1).
 template <int DIM>
 __global__ void __launch_bounds__(kBlock, MPM_MINB) k_update_tiled(GridDesc gd, PArr p, PArr q, const double *__restrict__ na,
                                                                    const double *__restrict__ nb, DevScalars *sc, SortedMap map,
+                                                                   const int4 *__restrict__ items, const int *__restrict__ n_items,
                                                                    const int *__restrict__ off_new,
                                                                    const unsigned long long *__restrict__ dest, GArr gn)
 {
-    constexpr int NB = 1 << DIM, LG = Geo<DIM>::LG, GPB = Geo<DIM>::GPB;
-    constexpr int NPAIR = (DIM == 3) ? 4 : 3;
-    __shared__ __align__(16) double s_vals[(kBlock / 32) * Geo<DIM>::WARP_DOUBLES];
+    using TG = TileGeo<DIM>;
+    constexpr int NB = 1 << DIM, LG = Geo<DIM>::LG, GPB = Geo<DIM>::GPB, CH = (DIM == 3) ? 10 : 6;
+    __shared__ __align__(16) double s_tile[TG::NN * CH];
     __shared__ double s_v[kBlock / 32], s_c[kBlock / 32];
-    const int n_groups = *map.n_groups;
+    if ((int)blockIdx.x >= *n_items) return;
+    const int4 item = __ldg(items + blockIdx.x);
+    int org[DIM];
+    tile_origin<DIM>(gd, item.x, org);
+    int gl = threadIdx.x / LG;
+    const int g_end = item.y + item.z;
+    Group next = fetch_group(map.groups, (long long)item.y + gl, g_end);
+    stage_tile<DIM, CH, true>(gd, org, na, nb, s_tile);
+    __syncthreads();
     const double dt = sc->dt;
     const long long step = sc->step;
-    const int l = threadIdx.x % LG;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, gi = lane / LG;
-    double *s_group = s_vals + warp * Geo<DIM>::WARP_DOUBLES + gi * Geo<DIM>::GROUP_STRIDE;
-    const long long stride = (long long)gridDim.x * GPB;
-    long long gidx = (long long)blockIdx.x * GPB + threadIdx.x / LG;
-    Group next = fetch_group(map.groups, gidx, n_groups);
+    const int l = threadIdx.x % LG, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     double vloc = 0.0, cloc = 0.0;
     int n_rec = 0, n_clamp = 0, n_neg = 0, n_nonfin = 0;
     const double gm1 = gd.gamma - 1.0;
-    for (long long g0 = (long long)blockIdx.x * GPB; g0 < n_groups; g0 += stride, gidx += stride) {
+    for (int p0 = 0; p0 < item.z; p0 += GPB, gl += GPB) {
         const Group grp = next;
-        next = fetch_group(map.groups, gidx + stride, n_groups);
+        next = fetch_group(map.groups, (long long)item.y + gl + GPB, g_end);
         int c[DIM];
         unpack_coords<DIM>(grp.cpack, c);
+        const int local = grp.cell & (TG::TC - 1);
+        const int j0 = (local & (TG::T0 - 1)) + TG::N0 * (((local >> TG::LT0) & (TG::T1 - 1)) + TG::N1 * (local >> (TG::LT0 + TG::LT1)));
         const bool valid[2] = { 2 * l < grp.cnt, 2 * l + 1 < grp.cnt };
         const long long k0 = (long long)grp.first + 2 * l;
         double X[2][DIM], V[2][DIM], M[2], rho[2], E[2];
@@ -312,7 +516,7 @@ __global__ void __launch_bounds__(kBlock, MPM_MINB) k_update_tiled(GridDesc gd, 
             rho[0] = valid[0] ? tr.x : 1.0; rho[1] = valid[1] ? tr.y : 1.0;
             E[0] = te.x; E[1] = valid[1] ? te.y : 0.0;
             int2 ti = make_int2(0, 0);
-            ulonglong2 td = make_ulonglong2(0ull, 0ull);
+            ulonglong2 td = make_ulonglong2(~0ull, ~0ull);
             if (valid[0]) {
                 ti = __ldg(reinterpret_cast<const int2 *>(p.id + k0));
                 td = __ldg(reinterpret_cast<const ulonglong2 *>(dest + k0));
@@ -320,58 +524,27 @@ __global__ void __launch_bounds__(kBlock, MPM_MINB) k_update_tiled(GridDesc gd, 
             id[0] = ti.x; id[1] = ti.y;
             dk[0] = td.x; dk[1] = td.y;
         }
-        // stage vbar, acc of corners l, l + LG, and dsum_b = sum_a (v2_a(high corner) - v2_a(low corner)) / h
-        double v2[2][DIM];
-        int node[2];
+        double W[2][DIM][2], xi[2][DIM], out[2][2 * DIM], Dh[2];
 #pragma unroll
-        for (int qq = 0; qq < 2; ++qq) {
-            node[qq] = corner_node_i<DIM>(gd, c, l + qq * LG);
-#pragma unroll
-            for (int a = 0; a < DIM; ++a) v2[qq][a] = (grp.cnt > 0) ? __ldg(nb + (long long)node[qq] * DIM + a) : 0.0;
-        }
-        double dsum[2] = { 0.0, 0.0 };
-#pragma unroll
-        for (int a = 0; a < DIM; ++a) {
-#pragma unroll
-            for (int qq = 0; qq < 2; ++qq) {
-                double other;
-                if ((1 << a) < LG) other = shfl_xor_d(v2[qq][a], 1 << a);
-                else other = v2[qq ^ 1][a];
-                const int b = l + qq * LG;
-                dsum[qq] += ((b >> a) & 1) ? (v2[qq][a] - other) : (other - v2[qq][a]);
-            }
-        }
-        if (grp.cnt > 0) {
-#pragma unroll
-            for (int qq = 0; qq < 2; ++qq) {
-                double *s_corner = s_group + (l + qq * LG) * Geo<DIM>::CH;
-                stage_na<DIM>(na, node[qq], s_corner);
-                *reinterpret_cast<double2 *>(s_corner + 2 * DIM) = make_double2(dsum[qq] * gd.inv_h, 0.0);
-            }
-        }
-        __syncwarp();
+        for (int i = 0; i < 2; ++i) weights_1d<DIM>(gd, X[i], c, xi[i], W[i]);
+        gather_tile<DIM, CH, true>(s_tile + j0 * CH, W, out, Dh);
         double pay[2][DIM + 2], wn[2][NB];      // next step's P2G#1: payload M, M V', S' and weights at X'
+        double Xm[2][DIM], Vm[2][DIM], Mm[2], Sm[2];   // the same for a particle that leaves its cell
+        bool mover[2] = { false, false };
 #pragma unroll
         for (int i = 0; i < 2; ++i) {
 #pragma unroll
             for (int ch = 0; ch < DIM + 2; ++ch) pay[i][ch] = 0.0;
 #pragma unroll
             for (int r = 0; r < NB; ++r) wn[i][r] = 0.0;
-            if (valid[i]) {
-                double xi[DIM], Vb[DIM], A[DIM], D;
-                if (local_coords<DIM>(gd, X[i], c, xi)) {
-                    double w[NB], out[2 * NPAIR];
-                    natural_weights<DIM>(xi, w);
-                    gather_pairs<DIM, NPAIR>(s_group, w, out);
 #pragma unroll
-                    for (int a = 0; a < DIM; ++a) { Vb[a] = out[a]; A[a] = out[DIM + a]; }
-                    D = out[2 * DIM];
-                } else {
-                    slow_gather<DIM>(gd, na, nb, X[i], Vb, A, &D);
-                }
+            for (int a = 0; a < DIM; ++a) { Xm[i][a] = 0.0; Vm[i][a] = 0.0; }
+            Mm[i] = 0.0; Sm[i] = 0.0;
+            if (valid[i]) {
+                const double D = Dh[i] * gd.inv_h;
                 double Vn[DIM];
 #pragma unroll
-                for (int a = 0; a < DIM; ++a) Vn[a] = fma(dt, A[a], V[i][a]);   // V'
+                for (int a = 0; a < DIM; ++a) Vn[a] = fma(dt, out[i][DIM + a], V[i][a]);   // V'
                 // particle thermodynamics (eq. 4 with this step's D: reading A2).  P/rho = (gamma-1) E
                 // and gamma P/rho = gamma (gamma-1) E are used in place of the quotients (one rounding apart).
                 const double r = rho[i], e0 = E[i];
@@ -394,13 +567,13 @@ __global__ void __launch_bounds__(kBlock, MPM_MINB) k_update_tiled(GridDesc gd, 
                 if (!isfinite(En) || !isfinite(rhon)) n_nonfin++;
                 double vv = 0.0, vb2 = 0.0;
 #pragma unroll
-                for (int a = 0; a < DIM; ++a) { vv = fma(Vn[a], Vn[a], vv); vb2 = fma(Vb[a], Vb[a], vb2); }
+                for (int a = 0; a < DIM; ++a) { vv = fma(Vn[a], Vn[a], vv); vb2 = fma(out[i][a], out[i][a], vb2); }
                 vloc = fmax(vloc, fmax(vv, vb2));      // squared; the root is taken once at the end
                 cloc = fmax(cloc, cs);
                 double Xn[DIM];
                 bool recycled;
                 int nclamp;
-                move_particle<DIM>(gd, X[i], Vb, dt, (long long)id[i], step, Xn, recycled, nclamp);
+                move_particle<DIM>(gd, X[i], out[i], dt, (long long)id[i], step, Xn, recycled, nclamp);
                 n_clamp += nclamp;
                 double Mn = M[i];
                 if (recycled) {
@@ -409,7 +582,8 @@ __global__ void __launch_bounds__(kBlock, MPM_MINB) k_update_tiled(GridDesc gd, 
                     rhon = gd.inflow_rho; En = gd.inflow_e; Q = 0.0; Mn = gd.inflow_mass;
                     n_rec++;
                 }
-                const long long dst = (long long)off_new[(int)(dk[i] >> 32)] + (long long)(unsigned)(dk[i] & 0xffffffffull);
+                const int key = (int)(dk[i] >> 32);
+                const long long dst = (long long)__ldg(off_new + key) + (long long)(unsigned)(dk[i] & 0xffffffffull);
 #pragma unroll
                 for (int a = 0; a < DIM; ++a) { q.x[a][dst] = Xn[a]; q.v[a][dst] = Vn[a]; }
                 q.m[dst] = Mn;
@@ -417,25 +591,33 @@ __global__ void __launch_bounds__(kBlock, MPM_MINB) k_update_tiled(GridDesc gd, 
                 q.e[dst] = En;
                 q.q[dst] = Q;
                 q.id[dst] = id[i];
-                // P2G#1 of the next step (eq. 13, 14, 16, 18 at X'): in the group's butterfly if the particle stays in the
-                // group's cell, else directly
+                // P2G#1 of the next step (eq. 13, 14, 16, 18 at X')
                 const double Sn = (gm1 * rhon * En + Q) * Mn / rhon;
-                double xin[DIM];
-                if (local_coords<DIM>(gd, Xn, c, xin)) {
+                if (key == grp.cell) {
+                    double xin[DIM];
+#pragma unroll
+                    for (int a = 0; a < DIM; ++a) xin[a] = __dmul_rn(Xn[a], gd.inv_h) - (double)c[a];
                     swizzled_weights<DIM>(xin, l, wn[i]);
                     pay[i][0] = Mn;
                     pay[i][DIM + 1] = Sn;
 #pragma unroll
                     for (int a = 0; a < DIM; ++a) pay[i][1 + a] = Mn * Vn[a];
                 } else {
-                    slow_p2g1<DIM>(gd, gn, Xn, Vn, Mn, Sn);
+                    mover[i] = true;
+#pragma unroll
+                    for (int a = 0; a < DIM; ++a) { Xm[i][a] = Xn[a]; Vm[i][a] = Vn[a]; }
+                    Mm[i] = Mn; Sm[i] = Sn;
                 }
             }
         }
         scatter_p2g1_group<DIM>(gd, gn, c, l, grp.cnt > 0, pay, wn);
-        __syncwarp();      // the staging area is rewritten by the next iteration
+#pragma unroll
+        for (int i = 0; i < 2; ++i) {
+            const unsigned mm = __ballot_sync(kFull, mover[i]);
+            if (mm) coop_p2g1<DIM>(gd, gn, mm, Xm[i], Vm[i], Mm[i], Sm[i], lane);
+        }
     }
-    // block maxima -> one atomicMax per block (max is order-free, so this is exact)
+    // block maxima -> at most one atomicMax per block (max is order-free, so this is exact)
     vloc = warp_max_nonneg(sqrt(vloc));
     cloc = warp_max_nonneg(cloc >= 0.0 ? cloc : 0.0);
     if (lane == 0) { s_v[warp] = vloc; s_c[warp] = cloc; }
@@ -452,8 +634,51 @@ __global__ void __launch_bounds__(kBlock, MPM_MINB) k_update_tiled(GridDesc gd, 
         double v = s_v[0], cc = s_c[0];
 #pragma unroll
         for (int w = 1; w < kBlock / 32; ++w) { v = fmax(v, s_v[w]); cc = fmax(cc, s_c[w]); }
-        if (v > 0.0) atomic_max_nonneg(&sc->vmax_bits, v);
-        if (cc > 0.0) atomic_max_nonneg(&sc->cmax_bits, cc);
+        // a plain read filters out the blocks that cannot raise the maximum (it only ever grows during the kernel)
+        const unsigned long long vb = (unsigned long long)__double_as_longlong(v), cb = (unsigned long long)__double_as_longlong(cc);
+        if (vb > *(volatile unsigned long long *)&sc->vmax_bits) atomic_max_nonneg(&sc->vmax_bits, v);
+        if (cb > *(volatile unsigned long long *)&sc->cmax_bits) atomic_max_nonneg(&sc->cmax_bits, cc);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ work items
+// One block: items = for every tile, ceil(groups of the tile / per_item) chunks of its group range (in tile order).
+__global__ void __launch_bounds__(1024) k_build_items(const int *__restrict__ goff, int ntiles, int ltc, int per_item,
+                                                      int4 *__restrict__ items, int *__restrict__ n_items)
+{
+    __shared__ int s_warp[32];
+    const int per_thread = (ntiles + 1023) / 1024;
+    const int t0 = min(ntiles, (int)threadIdx.x * per_thread), t1 = min(ntiles, t0 + per_thread);
+    int mine = 0;
+    for (int t = t0; t < t1; ++t) {
+        const int ng = goff[(t + 1) << ltc] - goff[t << ltc];
+        mine += (ng + per_item - 1) / per_item;
+    }
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    int incl = mine;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int t = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += t;
+    }
+    if (lane == 31) s_warp[warp] = incl;
+    __syncthreads();
+    if (warp == 0) {
+        const int w = s_warp[lane];
+        int wi = w;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, wi, o);
+            if (lane >= o) wi += t;
+        }
+        s_warp[lane] = wi - w;
+        if (lane == 31) *n_items = wi;
+    }
+    __syncthreads();
+    int at = s_warp[warp] + incl - mine;
+    for (int t = t0; t < t1; ++t) {
+        const int gfirst = goff[t << ltc], ng = goff[(t + 1) << ltc] - gfirst;
+        for (int done = 0; done < ng; done += per_item) items[at++] = make_int4(t, gfirst + done, min(per_item, ng - done), 0);
     }
 }
 
@@ -573,25 +798,40 @@ void launch_p2g1_tiled(const GridDesc &gd, const PArr &p, const GArr &g, const S
     else k_p2g1_tiled<3><<<persistent_blocks(max_groups, Geo<3>::GPB, k_p2g1_tiled<3>), kBlock, 0, s>>>(gd, p, g, map);
 }
 
-void launch_g2p_p2g2_tiled(const GridDesc &gd, const PArr &p, const GArr &g, const double *na, const DevScalars *sc,
-                           const SortedMap &map, int *count, unsigned long long *dest, long long max_groups, cudaStream_t s)
+void launch_build_items(const GridDesc &gd, const int *goff, int4 *items, int *n_items, cudaStream_t s)
 {
-    if (max_groups <= 0) return;
-    if (gd.dim == 2)
-        k_g2p_p2g2_tiled<2><<<persistent_blocks(max_groups, Geo<2>::GPB, k_g2p_p2g2_tiled<2>), kBlock, 0, s>>>(gd, p, g, na, sc, map, count, dest);
-    else
-        k_g2p_p2g2_tiled<3><<<persistent_blocks(max_groups, Geo<3>::GPB, k_g2p_p2g2_tiled<3>), kBlock, 0, s>>>(gd, p, g, na, sc, map, count, dest);
+    long long ntiles = 1;
+    for (int a = 0; a < gd.dim; ++a) ntiles *= gd.ntile[a];
+    if (gd.dim == 2) k_build_items<<<1, 1024, 0, s>>>(goff, (int)ntiles, TileGeo<2>::LTC, Chunk<2>::GROUPS, items, n_items);
+    else k_build_items<<<1, 1024, 0, s>>>(goff, (int)ntiles, TileGeo<3>::LTC, Chunk<3>::GROUPS, items, n_items);
+}
+
+long long max_items_tiled(const GridDesc &gd, long long max_groups)
+{
+    long long ntiles = 1;
+    for (int a = 0; a < gd.dim; ++a) ntiles *= gd.ntile[a];
+    const int per = gd.dim == 2 ? Chunk<2>::GROUPS : Chunk<3>::GROUPS;
+    return (ntiles < max_groups ? ntiles : max_groups) + max_groups / per + 1;
+}
+
+void launch_g2p_p2g2_tiled(const GridDesc &gd, const PArr &p, const GArr &g, const double *na, const DevScalars *sc,
+                           const SortedMap &map, const int4 *items, const int *n_items, long long max_items, int *count,
+                           unsigned long long *dest, cudaStream_t s)
+{
+    if (max_items <= 0) return;
+    if (gd.dim == 2) k_g2p_p2g2_tiled<2><<<(unsigned)max_items, kBlock, 0, s>>>(gd, p, g, na, sc, map, items, n_items, count, dest);
+    else k_g2p_p2g2_tiled<3><<<(unsigned)max_items, kBlock, 0, s>>>(gd, p, g, na, sc, map, items, n_items, count, dest);
 }
 
 void launch_update_tiled(const GridDesc &gd, const PArr &p, const PArr &q, const double *na, const double *nb, DevScalars *sc,
-                         const SortedMap &map, const int *off_new, const unsigned long long *dest, const GArr &g_next,
-                         long long max_groups, cudaStream_t s)
+                         const SortedMap &map, const int4 *items, const int *n_items, long long max_items, const int *off_new,
+                         const unsigned long long *dest, const GArr &g_next, cudaStream_t s)
 {
-    if (max_groups <= 0) return;
+    if (max_items <= 0) return;
     if (gd.dim == 2)
-        k_update_tiled<2><<<persistent_blocks(max_groups, Geo<2>::GPB, k_update_tiled<2>), kBlock, 0, s>>>(gd, p, q, na, nb, sc, map, off_new, dest, g_next);
+        k_update_tiled<2><<<(unsigned)max_items, kBlock, 0, s>>>(gd, p, q, na, nb, sc, map, items, n_items, off_new, dest, g_next);
     else
-        k_update_tiled<3><<<persistent_blocks(max_groups, Geo<3>::GPB, k_update_tiled<3>), kBlock, 0, s>>>(gd, p, q, na, nb, sc, map, off_new, dest, g_next);
+        k_update_tiled<3><<<(unsigned)max_items, kBlock, 0, s>>>(gd, p, q, na, nb, sc, map, items, n_items, off_new, dest, g_next);
 }
 
 void launch_gather_by_id_groups(const double *src, const int *id, double *dst, const SortedMap &map, long long max_groups,

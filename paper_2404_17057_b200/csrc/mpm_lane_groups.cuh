@@ -191,8 +191,8 @@ __device__ __forceinline__ void slow_p2g2(const GridDesc &gd, const GArr &g, con
 // ---------------------------------------------------------------------------------------------- shared pieces
 
 // Alg. 1 l.11 for one particle: X' = X + dt Vbar, periodic wrap (A11), outflow detection, recycling position (A8),
-// clamp.  Used by BOTH the gather kernel (to find the new cell) and the update kernel (to write X'); the update kernel
-// places the particle by the key the gather kernel stored, so a last-bit disagreement could only cost a slow path.
+// clamp.  Used by BOTH the gather kernel (to find the new cell) and the update kernel (to write X'): every rounding is
+// explicit (fma / __dmul_rn / __dsub_rn), so that both kernels get the same X' bit for bit from the same inputs.
 template <int DIM>
 __device__ __forceinline__ void move_particle(const GridDesc &gd, const double X[DIM], const double Vb[DIM], double dt,
                                               long long id, long long step, double Xn[DIM], bool &recycled, int &nclamp)
@@ -203,7 +203,7 @@ __device__ __forceinline__ void move_particle(const GridDesc &gd, const double X
         double x = fma(dt, Vb[a], X[a]);
         if (gd.per[a]) {
             if (x < 0.0 || x >= gd.L[a]) {
-                x = x - gd.L[a] * floor(x / gd.L[a]);
+                x = __dsub_rn(x, __dmul_rn(gd.L[a], floor(x / gd.L[a])));
                 if (x >= gd.L[a]) x = 0.0;
             }
         } else {
@@ -214,19 +214,19 @@ __device__ __forceinline__ void move_particle(const GridDesc &gd, const double X
     }
     recycled = recycle && gd.in_axis >= 0;
     if (recycled) {
-        int jj = 0;
-        const double u0 = recycle_uniform(gd.recycle_seed, id, step, jj++);
+        // j = 0: offset normal to the inflow face; every other axis, in order, takes the next two numbers (cell, offset).
+        // Written as selects on a compile-time axis: an indexed store Xn[in_axis] would put Xn into local memory.
+        const double off = __dmul_rn(recycle_uniform(gd.recycle_seed, id, step, 0), gd.h);
 #pragma unroll
         for (int a = 0; a < DIM; ++a) {
-            if (a == gd.in_axis) {
-                Xn[a] = (gd.in_side == 0) ? u0 * gd.h : gd.L[a] - u0 * gd.h;
-            } else {
-                const double u1 = recycle_uniform(gd.recycle_seed, id, step, jj++);
-                const double u2 = recycle_uniform(gd.recycle_seed, id, step, jj++);
-                int cell = (int)floor(u1 * (double)gd.nc[a]);
-                cell = min(cell, gd.nc[a] - 1);
-                Xn[a] = ((double)cell + u2) * gd.h;
-            }
+            const int jb = 1 + 2 * (a - (a > gd.in_axis ? 1 : 0));
+            const double u1 = recycle_uniform(gd.recycle_seed, id, step, jb);
+            const double u2 = recycle_uniform(gd.recycle_seed, id, step, jb + 1);
+            int cell = (int)floor(u1 * (double)gd.nc[a]);
+            cell = min(cell, gd.nc[a] - 1);
+            const double x_face = (gd.in_side == 0) ? off : __dsub_rn(gd.L[a], off);
+            const double x_other = ((double)cell + u2) * gd.h;
+            Xn[a] = (a == gd.in_axis) ? x_face : x_other;
         }
     }
     nclamp = 0;
