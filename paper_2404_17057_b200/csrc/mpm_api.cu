@@ -353,7 +353,7 @@ void step_sorted(mpm_handle *h)
 
 // one step of Algorithm 1 with the TILED kernel family (see mpm_kernels_tiled.cu): l.3 of this step was done by the
 // previous step's update kernel (or by the load), l.3 of the next step is done by this step's update kernel
-void step_tiled(mpm_handle *h)
+void step_tiled(mpm_handle *h, bool last_of_call)
 {
     const GridDesc &gd = h->gd;
     cudaStream_t s = h->stream;
@@ -373,7 +373,7 @@ void step_tiled(mpm_handle *h)
     { Timed t(h, MPM_K_NODE2); launch_node2(gd, gc, s); }                                                          // l.9
     { Timed t(h, MPM_K_SORT); launch_exclusive_scan_from(h->count, h->off[0], gd.Nkeys + 1, h->scan_aux, true, s); }   // l.12 offsets
     { Timed t(h, MPM_K_UPDATE);
-      launch_update_tiled(gd, p, q, h->g.na, h->g.nb, h->sc, map, h->items, h->n_items, h->max_items, h->off[0], h->dest, gnx, s); }   // l.10-12, next l.3
+      launch_update_tiled(gd, p, q, h->g.na, h->g.nb, h->sc, map, h->items, h->n_items, h->max_items, h->off[0], h->dest, gnx, last_of_call, s); }   // l.10-12, next l.3
     { Timed t(h, MPM_K_MISC); launch_end_step(h->sc, gd.h, s); }                                                   // l.13-14
     { Timed t(h, MPM_K_SORT);
       launch_build_groups_tiled(gd, h->count, h->off[0], h->goff, h->scan_aux, h->groups, h->n_groups, s);         // next step's groups
@@ -631,7 +631,7 @@ int mpm_step(mpm_handle *h, double dt, double cfl, int32_t nsteps, double *dt_la
     h->launches += 1;
     for (int it = 0; it < nsteps; ++it) {
         if (h->variant != MPM_VARIANT_ATOMIC) {
-            if (h->n > 0) { if (h->variant == MPM_VARIANT_TILED) step_tiled(h); else step_sorted(h); }
+            if (h->n > 0) { if (h->variant == MPM_VARIANT_TILED) step_tiled(h, it == nsteps - 1); else step_sorted(h); }
             else { launch_begin_step(h->sc, gd.h, s); launch_grid_clear(gd, h->g, s); launch_end_step(h->sc, gd.h, s); h->launches += 2; }
             h->steps_done += 1;
             continue;

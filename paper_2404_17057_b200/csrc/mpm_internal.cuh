@@ -228,10 +228,12 @@ long long max_items_tiled(const GridDesc &gd, long long max_groups);   // upper 
 void launch_g2p_p2g2_tiled(const GridDesc &gd, const PArr &p, const GArr &g, const double *na, const DevScalars *sc,
                            const SortedMap &map, const int4 *items, const int *n_items, long long max_items, int *count,
                            unsigned long long *dest, cudaStream_t s);
-// update + re-ordering + P2G#1 of the next step into g_next.m, g_next.mv, g_next.f (zeroed by the caller)
+// update + re-ordering + P2G#1 of the next step into g_next.m, g_next.mv, g_next.f (zeroed by the caller).  store_q:
+// write Q' to memory (only needed when the state can be read back or re-loaded before the next step: the fused P2G#1
+// has already consumed it)
 void launch_update_tiled(const GridDesc &gd, const PArr &p, const PArr &q, const double *na, const double *nb, DevScalars *sc,
                          const SortedMap &map, const int4 *items, const int *n_items, long long max_items, const int *off_new,
-                         const unsigned long long *dest, const GArr &g_next, cudaStream_t s);
+                         const unsigned long long *dest, const GArr &g_next, bool store_q, cudaStream_t s);
 // dst[id] = src[slot] for every occupied slot; with coff (exclusive scan of the per-key counts) and off (slot offsets):
 // dst[compact storage index] = src[slot] instead
 void launch_gather_by_id_groups(const double *src, const int *id, double *dst, const SortedMap &map, long long max_groups,

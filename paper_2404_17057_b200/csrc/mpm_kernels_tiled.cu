@@ -32,6 +32,22 @@ __device__ __forceinline__ double2 ld2(const double *__restrict__ p, long long k
 {
     return ok ? __ldg(reinterpret_cast<const double2 *>(p + k)) : make_double2(0.0, 0.0);
 }
+__device__ __forceinline__ void st2(double *p, long long k, double a, double b)
+{
+    *reinterpret_cast<double2 *>(p + k) = make_double2(a, b);
+}
+
+// cp.async: 16 / 8 bytes from global memory straight into shared memory, L2 only (streamed particle data)
+__device__ __forceinline__ void cp_async16(void *smem, const void *gmem)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async8(void *smem, const void *gmem)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
 template <int DIM>
 __device__ __forceinline__ int tiled_key_of_position(const GridDesc &gd, const double X[DIM])
@@ -145,10 +161,23 @@ __global__ void __launch_bounds__(kBlock, MPM_MINB) k_p2g1_tiled(GridDesc gd, PA
 // A block works on one ITEM = up to Chunk<DIM>::GROUPS consecutive groups of ONE tile (a tile with more groups is cut into
 // several items, so that a dense tile does not serialise on one block).  The item list is rebuilt every step from the
 // per-key group offsets (k_build_items).
+#ifndef MPM_TB
+#define MPM_TB 128
+#endif
+#ifndef MPM_TBMIN_G
+#define MPM_TBMIN_G 4
+#endif
+#ifndef MPM_TBMIN_U
+#define MPM_TBMIN_U 3
+#endif
+constexpr int kTB = MPM_TB;              // threads per block of the tile kernels
+constexpr int kTBMinG = MPM_TBMIN_G;     // resident blocks per SM the gather kernel is compiled for (128 registers)
+constexpr int kTBMinU = MPM_TBMIN_U;     // ... and the update kernel (168 registers: it spills at 128)
+
 template <int DIM>
 struct Chunk {
-    static constexpr int PASSES = 8;
-    static constexpr int GROUPS = PASSES * Geo<DIM>::GPB;
+    static constexpr int PASSES = 16;
+    static constexpr int GROUPS = PASSES * (kTB / Geo<DIM>::LG);
 };
 
 // tile-local node index j = lx + N0 (ly + N1 lz) of corner b of the cell with tile-local node index j0
@@ -197,7 +226,7 @@ __device__ __forceinline__ void stage_tile(const GridDesc &gd, const int org[DIM
                                            const double *__restrict__ nb, double *s_tile)
 {
     using TG = TileGeo<DIM>;
-    for (int j = threadIdx.x; j < TG::NN; j += kBlock) {
+    for (int j = threadIdx.x; j < TG::NN; j += kTB) {
         const int node = tile_node_global<DIM>(gd, org, j);
         double2 *dst = reinterpret_cast<double2 *>(s_tile + j * CH);
         double2 v[CH / 2];
@@ -354,35 +383,51 @@ __device__ __forceinline__ void coop_p2g1(const GridDesc &gd, const GArr &gn, un
 }
 
 // ------------------------------------------------------------------------------------------------ Alg. 1 l.6-8 (+ l.11-12 bookkeeping)
-// One block per item.  The tile's node velocities vbar = mv'/m, acc = f/m are staged once in shared memory; every lane
-// gathers A = G2P(f/m), Vbar = G2P(mv'/m) for its two particles from there (eq. 17), V' = V + dt A
-// (PAPER.md:776), mv2 += M V' phi through the group butterfly.  Also: the particle's cell after the
-// move of l.11 and its rank inside that cell, for the fused re-ordering (l.12): the particles of a group that stay in
-// their cell take consecutive ranks from ONE atomic per group (ballot + popc), only the others pay one atomic each.
-// V' is NOT stored: the update kernel recomputes it.
+// One block (kTB threads) per item.  The tile's node velocities vbar = mv'/m, acc = f/m are staged once in shared memory;
+// every lane gathers A = G2P(f/m), Vbar = G2P(mv'/m) for its two particles from there (eq. 17),
+// V' = V + dt A, mv2 += M V' phi through the group butterfly.  Also: the particle's
+// cell after the move of l.11 and its rank inside that cell, for the fused re-ordering (l.12): the particles of a group
+// that stay in their cell take consecutive ranks from ONE atomic per group (ballot + popc), only the others pay one
+// atomic each; the atomics are issued before the scatter and their results consumed after it.
+// The particle fields of the NEXT pass are copied into the thread's own shared-memory slots with cp.async while the
+// current pass computes (PfSlots).  V' is NOT stored: the update kernel recomputes it.
 template <int DIM>
-__global__ void __launch_bounds__(kBlock, MPM_MINB) k_g2p_p2g2_tiled(GridDesc gd, PArr p, GArr g, const double *__restrict__ na,
-                                                                     const DevScalars *__restrict__ sc, SortedMap map,
-                                                                     const int4 *__restrict__ items, const int *__restrict__ n_items,
-                                                                     int *__restrict__ count, unsigned long long *__restrict__ dest)
+__global__ void __launch_bounds__(kTB, kTBMinG) k_g2p_p2g2_tiled(GridDesc gd, PArr p, GArr g, const double *__restrict__ na,
+                                                                const DevScalars *__restrict__ sc, SortedMap map,
+                                                                const int4 *__restrict__ items, const int *__restrict__ n_items,
+                                                                int *__restrict__ count, unsigned long long *__restrict__ dest)
 {
     using TG = TileGeo<DIM>;
-    constexpr int NB = 1 << DIM, LG = Geo<DIM>::LG, GPB = Geo<DIM>::GPB, CH = 2 * DIM;
+    constexpr int NB = 1 << DIM, LG = Geo<DIM>::LG, GPB = kTB / LG, CH = 2 * DIM, NF = 2 * DIM + 1;
     __shared__ __align__(16) double s_tile[TG::NN * CH];
+    __shared__ __align__(16) double2 s_pf[NF][kTB];      // x[d], v[d], m of the thread's two particles
     if ((int)blockIdx.x >= *n_items) return;
     const int4 item = __ldg(items + blockIdx.x);      // {tile, first group, groups, -}
+    const int l = threadIdx.x % LG, lane = threadIdx.x & 31, sh = lane & ~(LG - 1);
+    const int g_end = item.y + item.z;
+    int gl = threadIdx.x / LG;
+    Group grp = fetch_group(map.groups, (long long)item.y + gl, g_end);
+    Group nxt = fetch_group(map.groups, (long long)item.y + gl + GPB, g_end);
+    auto issue = [&](const Group &gr) {
+        if (2 * l < gr.cnt) {
+            const long long k0 = (long long)gr.first + 2 * l;
+#pragma unroll
+            for (int a = 0; a < DIM; ++a) {
+                cp_async16(&s_pf[a][threadIdx.x], p.x[a] + k0);
+                cp_async16(&s_pf[DIM + a][threadIdx.x], p.v[a] + k0);
+            }
+            cp_async16(&s_pf[2 * DIM][threadIdx.x], p.m + k0);
+        }
+        cp_async_commit();
+    };
+    issue(grp);
     int org[DIM];
     tile_origin<DIM>(gd, item.x, org);
-    int gl = threadIdx.x / LG;
-    Group next = fetch_group(map.groups, (long long)item.y + gl, gl < item.z ? item.y + item.z : 0);
     stage_tile<DIM, CH, false>(gd, org, na, nullptr, s_tile);
     __syncthreads();
     const double dt = sc->dt;
     const long long step = sc->step;
-    const int l = threadIdx.x % LG, lane = threadIdx.x & 31, sh = lane & ~(LG - 1);
     for (int p0 = 0; p0 < item.z; p0 += GPB, gl += GPB) {
-        const Group grp = next;
-        next = fetch_group(map.groups, (long long)item.y + gl + GPB, gl + GPB < item.z ? item.y + item.z : 0);
         int c[DIM];
         unpack_coords<DIM>(grp.cpack, c);
         const int local = grp.cell & (TG::TC - 1);      // grp.cell = tile-major key
@@ -390,16 +435,19 @@ __global__ void __launch_bounds__(kBlock, MPM_MINB) k_g2p_p2g2_tiled(GridDesc gd
         const bool valid[2] = { 2 * l < grp.cnt, 2 * l + 1 < grp.cnt };
         const long long k0 = (long long)grp.first + 2 * l;
         double X[2][DIM], V[2][DIM], M[2];
+        cp_async_wait_all();
 #pragma unroll
         for (int a = 0; a < DIM; ++a) {
-            const double2 tx = ld2(p.x[a], k0, valid[0]), tv = ld2(p.v[a], k0, valid[0]);
-            X[0][a] = tx.x; X[1][a] = valid[1] ? tx.y : 0.0;
-            V[0][a] = tv.x; V[1][a] = valid[1] ? tv.y : 0.0;
+            const double2 tx = s_pf[a][threadIdx.x], tv = s_pf[DIM + a][threadIdx.x];
+            X[0][a] = valid[0] ? tx.x : 0.0; X[1][a] = valid[1] ? tx.y : 0.0;
+            V[0][a] = valid[0] ? tv.x : 0.0; V[1][a] = valid[1] ? tv.y : 0.0;
         }
         {
-            const double2 tm = ld2(p.m, k0, valid[0]);
-            M[0] = tm.x; M[1] = valid[1] ? tm.y : 0.0;
+            const double2 tm = s_pf[2 * DIM][threadIdx.x];
+            M[0] = valid[0] ? tm.x : 0.0; M[1] = valid[1] ? tm.y : 0.0;
         }
+        issue(nxt);                                   // the slots have been read: refill them for the next pass
+        const Group nn = fetch_group(map.groups, (long long)item.y + gl + 2 * GPB, g_end);
         double W[2][DIM][2], xi[2][DIM], out[2][2 * DIM], Dh[2];
 #pragma unroll
         for (int i = 0; i < 2; ++i) weights_1d<DIM>(gd, X[i], c, xi[i], W[i]);
@@ -417,134 +465,180 @@ __global__ void __launch_bounds__(kBlock, MPM_MINB) k_g2p_p2g2_tiled(GridDesc gd
                 key[i] = tiled_key_of_position<DIM>(gd, Xn);
             }
         }
-        // ranks among the particles that end up in the same cell (arrival order of the atomics, A17)
+        // ranks among the particles that end up in the same cell (arrival order of the atomics, A17): issue the atomics
         const bool stay[2] = { valid[0] && key[0] == grp.cell, valid[1] && key[1] == grp.cell };
         const unsigned gmask = (1u << LG) - 1u;
         const unsigned g0 = (__ballot_sync(kFull, stay[0]) >> sh) & gmask, g1 = (__ballot_sync(kFull, stay[1]) >> sh) & gmask;
         const int nstay = __popc(g0) + __popc(g1);
-        int base = 0;
+        int base = 0, rank_m[2] = { 0, 0 };
         if (l == 0 && nstay > 0) base = atomicAdd(&count[grp.cell], nstay);
+#pragma unroll
+        for (int i = 0; i < 2; ++i)
+            if (valid[i] && !stay[i]) rank_m[i] = atomicAdd(&count[key[i]], 1);
+        // P2G#2: group totals of M V' phi per corner, one global reduction per corner and component
+        {
+            double ws[2][NB];
+#pragma unroll
+            for (int i = 0; i < 2; ++i) swizzled_weights<DIM>(xi[i], l, ws[i]);
+            double tot[DIM][2];
+#pragma unroll
+            for (int a = 0; a < DIM; ++a) {
+                double v[NB];
+#pragma unroll
+                for (int r = 0; r < NB; ++r) v[r] = fma(MV[1][a], ws[1][r], MV[0][a] * ws[0][r]);
+                butterfly<DIM>(v);
+                tot[a][0] = v[0];
+                tot[a][1] = v[LG];
+            }
+            if (grp.cnt > 0) {
+#pragma unroll
+                for (int q = 0; q < 2; ++q) {
+                    const int node = corner_node_i<DIM>(gd, c, l + q * LG);
+#pragma unroll
+                    for (int a = 0; a < DIM; ++a) atomicAdd(&g.mv2[a][node], tot[a][q]);
+                }
+            }
+        }
+        // ... and only now use what they returned
         base = __shfl_sync(kFull, base, sh);
         const unsigned lower = (1u << l) - 1u;
         const int pre = base + __popc(g0 & lower) + __popc(g1 & lower);
-        int rank[2] = { pre, pre + (int)((g0 >> l) & 1u) };
-#pragma unroll
-        for (int i = 0; i < 2; ++i)
-            if (valid[i] && !stay[i]) rank[i] = atomicAdd(&count[key[i]], 1);
-        const unsigned long long dk0 = ((unsigned long long)(unsigned)key[0] << 32) | (unsigned)rank[0];
-        const unsigned long long dk1 = ((unsigned long long)(unsigned)key[1] << 32) | (unsigned)rank[1];
+        const int rank0 = stay[0] ? pre : rank_m[0], rank1 = stay[1] ? pre + (int)((g0 >> l) & 1u) : rank_m[1];
+        const unsigned long long dk0 = ((unsigned long long)(unsigned)key[0] << 32) | (unsigned)rank0;
+        const unsigned long long dk1 = ((unsigned long long)(unsigned)key[1] << 32) | (unsigned)rank1;
         if (valid[1]) *reinterpret_cast<ulonglong2 *>(dest + k0) = make_ulonglong2(dk0, dk1);
         else if (valid[0]) dest[k0] = dk0;
-        // P2G#2: group totals of M V' phi per corner, one global reduction per corner and component
-        double ws[2][NB];
-#pragma unroll
-        for (int i = 0; i < 2; ++i) swizzled_weights<DIM>(xi[i], l, ws[i]);
-        double tot[DIM][2];
-#pragma unroll
-        for (int a = 0; a < DIM; ++a) {
-            double v[NB];
-#pragma unroll
-            for (int r = 0; r < NB; ++r) v[r] = fma(MV[1][a], ws[1][r], MV[0][a] * ws[0][r]);
-            butterfly<DIM>(v);
-            tot[a][0] = v[0];
-            tot[a][1] = v[LG];
-        }
-        if (grp.cnt > 0) {
-#pragma unroll
-            for (int q = 0; q < 2; ++q) {
-                const int node = corner_node_i<DIM>(gd, c, l + q * LG);
-#pragma unroll
-                for (int a = 0; a < DIM; ++a) atomicAdd(&g.mv2[a][node], tot[a][q]);
-            }
-        }
+        grp = nxt;
+        nxt = nn;
     }
 }
 
 // ------------------------------------------------------------------------------------------------ Alg. 1 l.10-13 + l.3 of the next step
-// One block per item; the tile's vbar, acc AND v2 = mv2/m are staged in shared memory.  D = trace G2PD(mv2/m) (eq. 19);
-// Q (eq. 4), E', rho'; V' = V + dt A again; CFL maxima; X' = X + dt Vbar
-// (PAPER.md:372-376); the particle is written to its cell-sorted slot of the OTHER buffer (l.12).  Then P2G#1 of the
-// NEXT step at X' into the node accumulators `gn` (the other buffer of m, mv, f): a particle that
-// stays in its cell joins the group's butterfly, the others are scattered by the whole warp (coop_p2g1).
+// One block (kTB threads) per item; the tile's vbar, acc AND v2 = mv2/m are staged in shared memory.  D = trace
+// G2PD(mv2/m) (eq. 19); Q (eq. 4), E', rho'; V' = V + dt A again; CFL maxima;
+// X' = X + dt Vbar; the particle is written to its cell-sorted slot of the OTHER buffer (l.12).  Then
+// P2G#1 of the NEXT step at X' into the node accumulators `gn` (the other buffer of m, mv, f): a
+// particle that stays in its cell joins the group's butterfly, the others are scattered by the whole warp (coop_p2g1).
+// Particle fields of the next pass arrive through cp.async in the thread's own shared-memory slots, as in the gather kernel.
 template <int DIM>
-__global__ void __launch_bounds__(kBlock, MPM_MINB) k_update_tiled(GridDesc gd, PArr p, PArr q, const double *__restrict__ na,
-                                                                   const double *__restrict__ nb, DevScalars *sc, SortedMap map,
-                                                                   const int4 *__restrict__ items, const int *__restrict__ n_items,
-                                                                   const int *__restrict__ off_new,
-                                                                   const unsigned long long *__restrict__ dest, GArr gn)
+struct UpdSmem {
+    using TG = TileGeo<DIM>;
+    static constexpr int CH = (DIM == 3) ? 10 : 6;          // doubles per staged node: vbar, acc, v2, pad
+    static constexpr int NF = 2 * DIM + 3;                  // x[d], v[d], m, rho, e
+    static constexpr size_t TILE = sizeof(double) * TG::NN * CH;
+    static constexpr size_t PF = sizeof(double2) * NF * kTB;
+    static constexpr size_t DEST = sizeof(ulonglong2) * kTB;
+    static constexpr size_t ID = sizeof(int2) * kTB;
+    static constexpr size_t BYTES = TILE + PF + DEST + ID;
+};
+
+template <int DIM>
+__global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr p, PArr q, const double *__restrict__ na,
+                                                              const double *__restrict__ nb, DevScalars *sc, SortedMap map,
+                                                              const int4 *__restrict__ items, const int *__restrict__ n_items,
+                                                              const int *__restrict__ off_new,
+                                                              const unsigned long long *__restrict__ dest, GArr gn, int store_q)
 {
     using TG = TileGeo<DIM>;
-    constexpr int NB = 1 << DIM, LG = Geo<DIM>::LG, GPB = Geo<DIM>::GPB, CH = (DIM == 3) ? 10 : 6;
-    __shared__ __align__(16) double s_tile[TG::NN * CH];
-    __shared__ double s_v[kBlock / 32], s_c[kBlock / 32];
+    using SM = UpdSmem<DIM>;
+    constexpr int NB = 1 << DIM, LG = Geo<DIM>::LG, GPB = kTB / LG, CH = SM::CH;
+    extern __shared__ __align__(16) unsigned char s_raw[];
+    double *s_tile = reinterpret_cast<double *>(s_raw);
+    double2 (*s_pf)[kTB] = reinterpret_cast<double2 (*)[kTB]>(s_raw + SM::TILE);
+    ulonglong2 *s_dest = reinterpret_cast<ulonglong2 *>(s_raw + SM::TILE + SM::PF);
+    int2 *s_id = reinterpret_cast<int2 *>(s_raw + SM::TILE + SM::PF + SM::DEST);
+    __shared__ double s_v[kTB / 32], s_c[kTB / 32];
     if ((int)blockIdx.x >= *n_items) return;
     const int4 item = __ldg(items + blockIdx.x);
+    const int l = threadIdx.x % LG, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int g_end = item.y + item.z;
+    int gl = threadIdx.x / LG;
+    Group grp = fetch_group(map.groups, (long long)item.y + gl, g_end);
+    Group nxt = fetch_group(map.groups, (long long)item.y + gl + GPB, g_end);
+    auto issue = [&](const Group &gr) {
+        if (2 * l < gr.cnt) {
+            const long long k0 = (long long)gr.first + 2 * l;
+#pragma unroll
+            for (int a = 0; a < DIM; ++a) {
+                cp_async16(&s_pf[a][threadIdx.x], p.x[a] + k0);
+                cp_async16(&s_pf[DIM + a][threadIdx.x], p.v[a] + k0);
+            }
+            cp_async16(&s_pf[2 * DIM][threadIdx.x], p.m + k0);
+            cp_async16(&s_pf[2 * DIM + 1][threadIdx.x], p.rho + k0);
+            cp_async16(&s_pf[2 * DIM + 2][threadIdx.x], p.e + k0);
+            cp_async16(&s_dest[threadIdx.x], dest + k0);
+            cp_async8(&s_id[threadIdx.x], p.id + k0);
+        }
+        cp_async_commit();
+    };
+    issue(grp);
     int org[DIM];
     tile_origin<DIM>(gd, item.x, org);
-    int gl = threadIdx.x / LG;
-    const int g_end = item.y + item.z;
-    Group next = fetch_group(map.groups, (long long)item.y + gl, g_end);
     stage_tile<DIM, CH, true>(gd, org, na, nb, s_tile);
     __syncthreads();
     const double dt = sc->dt;
     const long long step = sc->step;
-    const int l = threadIdx.x % LG, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     double vloc = 0.0, cloc = 0.0;
     int n_rec = 0, n_clamp = 0, n_neg = 0, n_nonfin = 0;
     const double gm1 = gd.gamma - 1.0;
     for (int p0 = 0; p0 < item.z; p0 += GPB, gl += GPB) {
-        const Group grp = next;
-        next = fetch_group(map.groups, (long long)item.y + gl + GPB, g_end);
         int c[DIM];
         unpack_coords<DIM>(grp.cpack, c);
         const int local = grp.cell & (TG::TC - 1);
         const int j0 = (local & (TG::T0 - 1)) + TG::N0 * (((local >> TG::LT0) & (TG::T1 - 1)) + TG::N1 * (local >> (TG::LT0 + TG::LT1)));
         const bool valid[2] = { 2 * l < grp.cnt, 2 * l + 1 < grp.cnt };
-        const long long k0 = (long long)grp.first + 2 * l;
-        double X[2][DIM], V[2][DIM], M[2], rho[2], E[2];
-        int id[2];
-        unsigned long long dk[2];
+        double X[2][DIM];
+        int key[2];
+        long long dst[2] = { -1, -1 };
+        cp_async_wait_all();
+        {   // l.12: slot of the particle in the other buffer = offset of its new cell + its rank there; the offset load
+            // is issued first so that it overlaps the gather
+            const ulonglong2 td = s_dest[threadIdx.x];
+            key[0] = valid[0] ? (int)(td.x >> 32) : -1;
+            key[1] = valid[1] ? (int)(td.y >> 32) : -1;
+            if (valid[0]) dst[0] = (long long)__ldg(off_new + key[0]) + (long long)(unsigned)(td.x & 0xffffffffull);
+            if (valid[1]) dst[1] = (long long)__ldg(off_new + key[1]) + (long long)(unsigned)(td.y & 0xffffffffull);
+        }
 #pragma unroll
         for (int a = 0; a < DIM; ++a) {
-            const double2 tx = ld2(p.x[a], k0, valid[0]), tv = ld2(p.v[a], k0, valid[0]);
-            X[0][a] = tx.x; X[1][a] = valid[1] ? tx.y : 0.0;
-            V[0][a] = tv.x; V[1][a] = valid[1] ? tv.y : 0.0;
-        }
-        {
-            const double2 tm = ld2(p.m, k0, valid[0]), tr = ld2(p.rho, k0, valid[0]), te = ld2(p.e, k0, valid[0]);
-            M[0] = tm.x; M[1] = valid[1] ? tm.y : 0.0;
-            rho[0] = valid[0] ? tr.x : 1.0; rho[1] = valid[1] ? tr.y : 1.0;
-            E[0] = te.x; E[1] = valid[1] ? te.y : 0.0;
-            int2 ti = make_int2(0, 0);
-            ulonglong2 td = make_ulonglong2(~0ull, ~0ull);
-            if (valid[0]) {
-                ti = __ldg(reinterpret_cast<const int2 *>(p.id + k0));
-                td = __ldg(reinterpret_cast<const ulonglong2 *>(dest + k0));
-            }
-            id[0] = ti.x; id[1] = ti.y;
-            dk[0] = td.x; dk[1] = td.y;
+            const double2 tx = s_pf[a][threadIdx.x];
+            X[0][a] = valid[0] ? tx.x : 0.0; X[1][a] = valid[1] ? tx.y : 0.0;
         }
         double W[2][DIM][2], xi[2][DIM], out[2][2 * DIM], Dh[2];
 #pragma unroll
         for (int i = 0; i < 2; ++i) weights_1d<DIM>(gd, X[i], c, xi[i], W[i]);
         gather_tile<DIM, CH, true>(s_tile + j0 * CH, W, out, Dh);
-        double pay[2][DIM + 2], wn[2][NB];      // next step's P2G#1: payload M, M V', S' and weights at X'
-        double Xm[2][DIM], Vm[2][DIM], Mm[2], Sm[2];   // the same for a particle that leaves its cell
-        bool mover[2] = { false, false };
+        // the fields that are only needed from here on stay in shared memory during the gather (register budget)
+        asm volatile("" ::: "memory");
+        double V[2][DIM], M[2], rho[2], E[2];
+        int id[2];
+#pragma unroll
+        for (int a = 0; a < DIM; ++a) {
+            const double2 tv = s_pf[DIM + a][threadIdx.x];
+            V[0][a] = valid[0] ? tv.x : 0.0; V[1][a] = valid[1] ? tv.y : 0.0;
+        }
+        {
+            const double2 tm = s_pf[2 * DIM][threadIdx.x], tr = s_pf[2 * DIM + 1][threadIdx.x], te = s_pf[2 * DIM + 2][threadIdx.x];
+            M[0] = valid[0] ? tm.x : 0.0; M[1] = valid[1] ? tm.y : 0.0;
+            rho[0] = valid[0] ? tr.x : 1.0; rho[1] = valid[1] ? tr.y : 1.0;
+            E[0] = valid[0] ? te.x : 0.0; E[1] = valid[1] ? te.y : 0.0;
+            const int2 ti = s_id[threadIdx.x];
+            id[0] = ti.x; id[1] = ti.y;
+        }
+        issue(nxt);                                   // the slots have been read: refill them for the next pass
+        const Group nn = fetch_group(map.groups, (long long)item.y + gl + 2 * GPB, g_end);
+        // per particle: the new state (what goes to memory), its slot, and whether it stays in the group's cell
+        double Xo[2][DIM], Vo[2][DIM], Mo[2], Ro[2], Eo[2], Qo[2];
+        bool stay[2] = { false, false };
 #pragma unroll
         for (int i = 0; i < 2; ++i) {
 #pragma unroll
-            for (int ch = 0; ch < DIM + 2; ++ch) pay[i][ch] = 0.0;
-#pragma unroll
-            for (int r = 0; r < NB; ++r) wn[i][r] = 0.0;
-#pragma unroll
-            for (int a = 0; a < DIM; ++a) { Xm[i][a] = 0.0; Vm[i][a] = 0.0; }
-            Mm[i] = 0.0; Sm[i] = 0.0;
+            for (int a = 0; a < DIM; ++a) { Xo[i][a] = 0.0; Vo[i][a] = 0.0; }
+            Mo[i] = 0.0; Ro[i] = 1.0; Eo[i] = 0.0; Qo[i] = 0.0;
             if (valid[i]) {
                 const double D = Dh[i] * gd.inv_h;
-                double Vn[DIM];
 #pragma unroll
-                for (int a = 0; a < DIM; ++a) Vn[a] = fma(dt, out[i][DIM + a], V[i][a]);   // V'
+                for (int a = 0; a < DIM; ++a) Vo[i][a] = fma(dt, out[i][DIM + a], V[i][a]);   // V'
                 // particle thermodynamics (eq. 4 with this step's D: reading A2).  P/rho = (gamma-1) E
                 // and gamma P/rho = gamma (gamma-1) E are used in place of the quotients (one rounding apart).
                 const double r = rho[i], e0 = E[i];
@@ -567,55 +661,76 @@ __global__ void __launch_bounds__(kBlock, MPM_MINB) k_update_tiled(GridDesc gd, 
                 if (!isfinite(En) || !isfinite(rhon)) n_nonfin++;
                 double vv = 0.0, vb2 = 0.0;
 #pragma unroll
-                for (int a = 0; a < DIM; ++a) { vv = fma(Vn[a], Vn[a], vv); vb2 = fma(out[i][a], out[i][a], vb2); }
+                for (int a = 0; a < DIM; ++a) { vv = fma(Vo[i][a], Vo[i][a], vv); vb2 = fma(out[i][a], out[i][a], vb2); }
                 vloc = fmax(vloc, fmax(vv, vb2));      // squared; the root is taken once at the end
                 cloc = fmax(cloc, cs);
-                double Xn[DIM];
                 bool recycled;
                 int nclamp;
-                move_particle<DIM>(gd, X[i], out[i], dt, (long long)id[i], step, Xn, recycled, nclamp);
+                move_particle<DIM>(gd, X[i], out[i], dt, (long long)id[i], step, Xo[i], recycled, nclamp);
                 n_clamp += nclamp;
                 double Mn = M[i];
                 if (recycled) {
 #pragma unroll
-                    for (int a = 0; a < DIM; ++a) Vn[a] = gd.inflow_v[a];
+                    for (int a = 0; a < DIM; ++a) Vo[i][a] = gd.inflow_v[a];
                     rhon = gd.inflow_rho; En = gd.inflow_e; Q = 0.0; Mn = gd.inflow_mass;
                     n_rec++;
                 }
-                const int key = (int)(dk[i] >> 32);
-                const long long dst = (long long)__ldg(off_new + key) + (long long)(unsigned)(dk[i] & 0xffffffffull);
-#pragma unroll
-                for (int a = 0; a < DIM; ++a) { q.x[a][dst] = Xn[a]; q.v[a][dst] = Vn[a]; }
-                q.m[dst] = Mn;
-                q.rho[dst] = rhon;
-                q.e[dst] = En;
-                q.q[dst] = Q;
-                q.id[dst] = id[i];
-                // P2G#1 of the next step (eq. 13, 14, 16, 18 at X')
-                const double Sn = (gm1 * rhon * En + Q) * Mn / rhon;
-                if (key == grp.cell) {
-                    double xin[DIM];
-#pragma unroll
-                    for (int a = 0; a < DIM; ++a) xin[a] = __dmul_rn(Xn[a], gd.inv_h) - (double)c[a];
-                    swizzled_weights<DIM>(xin, l, wn[i]);
-                    pay[i][0] = Mn;
-                    pay[i][DIM + 1] = Sn;
-#pragma unroll
-                    for (int a = 0; a < DIM; ++a) pay[i][1 + a] = Mn * Vn[a];
-                } else {
-                    mover[i] = true;
-#pragma unroll
-                    for (int a = 0; a < DIM; ++a) { Xm[i][a] = Xn[a]; Vm[i][a] = Vn[a]; }
-                    Mm[i] = Mn; Sm[i] = Sn;
-                }
+                Mo[i] = Mn; Ro[i] = rhon; Eo[i] = En; Qo[i] = Q;
+                stay[i] = key[i] == grp.cell;
             }
         }
-        scatter_p2g1_group<DIM>(gd, gn, c, l, grp.cnt > 0, pay, wn);
+        // l.12: the particle goes to its cell-sorted slot of the other buffer; the two particles of a lane usually
+        // keep adjacent slots (ranks of the stayers are consecutive), then each field is ONE 16-byte store
+        if (valid[1] && dst[1] == dst[0] + 1 && (dst[0] & 1) == 0) {
+            const long long d0 = dst[0];
+#pragma unroll
+            for (int a = 0; a < DIM; ++a) {
+                st2(q.x[a], d0, Xo[0][a], Xo[1][a]);
+                st2(q.v[a], d0, Vo[0][a], Vo[1][a]);
+            }
+            st2(q.m, d0, Mo[0], Mo[1]);
+            st2(q.rho, d0, Ro[0], Ro[1]);
+            st2(q.e, d0, Eo[0], Eo[1]);
+            if (store_q) st2(q.q, d0, Qo[0], Qo[1]);
+            *reinterpret_cast<int2 *>(q.id + d0) = make_int2(id[0], id[1]);
+        } else {
+#pragma unroll
+            for (int i = 0; i < 2; ++i) {
+                if (!valid[i]) continue;
+                const long long d = dst[i];
+#pragma unroll
+                for (int a = 0; a < DIM; ++a) { q.x[a][d] = Xo[i][a]; q.v[a][d] = Vo[i][a]; }
+                q.m[d] = Mo[i];
+                q.rho[d] = Ro[i];
+                q.e[d] = Eo[i];
+                if (store_q) q.q[d] = Qo[i];
+                q.id[d] = id[i];
+            }
+        }
+        // P2G#1 of the next step (eqs. 13, 14, 16, 18 at X'): S' = (P' + Q') M / rho', P' = (gamma-1) rho' E' (eq. 3)
+        double Sn[2];
+#pragma unroll
+        for (int i = 0; i < 2; ++i) Sn[i] = (gm1 * Ro[i] * Eo[i] + Qo[i]) * Mo[i] / Ro[i];
+#pragma unroll
+        for (int i = 0; i < 2; ++i) {      // particles that leave the group's cell: scattered by the whole warp
+            const unsigned mm = __ballot_sync(kFull, valid[i] && !stay[i]);
+            if (mm) coop_p2g1<DIM>(gd, gn, mm, Xo[i], Vo[i], Mo[i], Sn[i], lane);
+        }
+        double pay[2][DIM + 2], wn[2][NB];      // the others join the group's butterfly: payload M, M V', S', weights at X'
 #pragma unroll
         for (int i = 0; i < 2; ++i) {
-            const unsigned mm = __ballot_sync(kFull, mover[i]);
-            if (mm) coop_p2g1<DIM>(gd, gn, mm, Xm[i], Vm[i], Mm[i], Sm[i], lane);
+            double xin[DIM];
+#pragma unroll
+            for (int a = 0; a < DIM; ++a) xin[a] = __dmul_rn(Xo[i][a], gd.inv_h) - (double)c[a];
+            swizzled_weights<DIM>(xin, l, wn[i]);
+            pay[i][0] = stay[i] ? Mo[i] : 0.0;
+            pay[i][DIM + 1] = stay[i] ? Sn[i] : 0.0;
+#pragma unroll
+            for (int a = 0; a < DIM; ++a) pay[i][1 + a] = stay[i] ? Mo[i] * Vo[i][a] : 0.0;
         }
+        scatter_p2g1_group<DIM>(gd, gn, c, l, grp.cnt > 0, pay, wn);
+        grp = nxt;
+        nxt = nn;
     }
     // block maxima -> at most one atomicMax per block (max is order-free, so this is exact)
     vloc = warp_max_nonneg(sqrt(vloc));
@@ -633,7 +748,7 @@ __global__ void __launch_bounds__(kBlock, MPM_MINB) k_update_tiled(GridDesc gd, 
     if (threadIdx.x == 0) {
         double v = s_v[0], cc = s_c[0];
 #pragma unroll
-        for (int w = 1; w < kBlock / 32; ++w) { v = fmax(v, s_v[w]); cc = fmax(cc, s_c[w]); }
+        for (int w = 1; w < kTB / 32; ++w) { v = fmax(v, s_v[w]); cc = fmax(cc, s_c[w]); }
         // a plain read filters out the blocks that cannot raise the maximum (it only ever grows during the kernel)
         const unsigned long long vb = (unsigned long long)__double_as_longlong(v), cb = (unsigned long long)__double_as_longlong(cc);
         if (vb > *(volatile unsigned long long *)&sc->vmax_bits) atomic_max_nonneg(&sc->vmax_bits, v);
@@ -819,19 +934,26 @@ void launch_g2p_p2g2_tiled(const GridDesc &gd, const PArr &p, const GArr &g, con
                            unsigned long long *dest, cudaStream_t s)
 {
     if (max_items <= 0) return;
-    if (gd.dim == 2) k_g2p_p2g2_tiled<2><<<(unsigned)max_items, kBlock, 0, s>>>(gd, p, g, na, sc, map, items, n_items, count, dest);
-    else k_g2p_p2g2_tiled<3><<<(unsigned)max_items, kBlock, 0, s>>>(gd, p, g, na, sc, map, items, n_items, count, dest);
+    if (gd.dim == 2) k_g2p_p2g2_tiled<2><<<(unsigned)max_items, kTB, 0, s>>>(gd, p, g, na, sc, map, items, n_items, count, dest);
+    else k_g2p_p2g2_tiled<3><<<(unsigned)max_items, kTB, 0, s>>>(gd, p, g, na, sc, map, items, n_items, count, dest);
 }
 
 void launch_update_tiled(const GridDesc &gd, const PArr &p, const PArr &q, const double *na, const double *nb, DevScalars *sc,
                          const SortedMap &map, const int4 *items, const int *n_items, long long max_items, const int *off_new,
-                         const unsigned long long *dest, const GArr &g_next, cudaStream_t s)
+                         const unsigned long long *dest, const GArr &g_next, bool store_q, cudaStream_t s)
 {
     if (max_items <= 0) return;
+    const int sq = store_q ? 1 : 0;
+    static bool attr_set = false;      // more than 48 KB of dynamic shared memory needs the opt-in, once per process
+    if (!attr_set) {
+        cudaFuncSetAttribute(k_update_tiled<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UpdSmem<2>::BYTES);
+        cudaFuncSetAttribute(k_update_tiled<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UpdSmem<3>::BYTES);
+        attr_set = true;
+    }
     if (gd.dim == 2)
-        k_update_tiled<2><<<(unsigned)max_items, kBlock, 0, s>>>(gd, p, q, na, nb, sc, map, items, n_items, off_new, dest, g_next);
+        k_update_tiled<2><<<(unsigned)max_items, kTB, UpdSmem<2>::BYTES, s>>>(gd, p, q, na, nb, sc, map, items, n_items, off_new, dest, g_next, sq);
     else
-        k_update_tiled<3><<<(unsigned)max_items, kBlock, 0, s>>>(gd, p, q, na, nb, sc, map, items, n_items, off_new, dest, g_next);
+        k_update_tiled<3><<<(unsigned)max_items, kTB, UpdSmem<3>::BYTES, s>>>(gd, p, q, na, nb, sc, map, items, n_items, off_new, dest, g_next, sq);
 }
 
 void launch_gather_by_id_groups(const double *src, const int *id, double *dst, const SortedMap &map, long long max_groups,
