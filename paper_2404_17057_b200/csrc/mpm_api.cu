@@ -34,6 +34,7 @@ struct mpm_handle {
     // step n+1 into the other set.  acc[acur] = the set the current / next mpm_step starts from (raw P2G#1).
     double *acc_m[2], *acc_mv[2][3], *acc_f[2][3];
     int acur;
+    bool grid_final;      // TILED: the last step's m, mv, f, mv2 have been brought to their post-BC form for mpm_read_grid
     long long slots;      // TILED: allocated slots per particle array (particles + one spare slot per odd cell)
     int *goff, *n_groups;
     int4 *groups;
@@ -365,22 +366,24 @@ void step_tiled(mpm_handle *h, bool last_of_call)
         Timed t(h, MPM_K_MISC);
         launch_begin_step(h->sc, gd.h, s);                                                // dt (eq. 25/29)
         launch_grid_clear(gd, gnx, s);                                                    // l.2 for the next step's l.3
+        for (int a = 0; a < gd.dim; ++a) cudaMemsetAsync(h->g.mv2[a], 0, sizeof(double) * (size_t)gd.Nn, s);   // ... and for l.8
         cudaMemsetAsync(h->count, 0, sizeof(int) * (size_t)(gd.Nkeys + 1), s);            // per-cell counters of l.12
     }
-    { Timed t(h, MPM_K_NODE1); launch_node1(gd, gc, h->sc, s); }                                                   // l.4-5
+    // l.4-5 and l.9 (BC, obstacle, mv' = mv + dt f, the quotients by m) have no kernel of their own: the two particle
+    // kernels evaluate them per tile node while staging the tile (stage_tile)
     { Timed t(h, MPM_K_G2P_P2G2);
-      launch_g2p_p2g2_tiled(gd, p, gc, h->g.na, h->sc, map, h->items, h->n_items, h->max_items, h->count, h->dest, s); }   // l.6-8
-    { Timed t(h, MPM_K_NODE2); launch_node2(gd, gc, s); }                                                          // l.9
+      launch_g2p_p2g2_tiled(gd, p, gc, h->sc, map, h->items, h->n_items, h->max_items, h->count, h->dest, s); }          // l.4-8
     { Timed t(h, MPM_K_SORT); launch_exclusive_scan_from(h->count, h->off[0], gd.Nkeys + 1, h->scan_aux, true, s); }   // l.12 offsets
     { Timed t(h, MPM_K_UPDATE);
-      launch_update_tiled(gd, p, q, h->g.na, h->g.nb, h->sc, map, h->items, h->n_items, h->max_items, h->off[0], h->dest, gnx, last_of_call, s); }   // l.10-12, next l.3
+      launch_update_tiled(gd, p, q, gc, h->sc, map, h->items, h->n_items, h->max_items, h->off[0], h->dest, gnx, last_of_call, s); }   // l.9-12, next l.3
     { Timed t(h, MPM_K_MISC); launch_end_step(h->sc, gd.h, s); }                                                   // l.13-14
     { Timed t(h, MPM_K_SORT);
       launch_build_groups_tiled(gd, h->count, h->off[0], h->goff, h->scan_aux, h->groups, h->n_groups, s);         // next step's groups
       launch_build_items(gd, h->goff, h->items, h->n_items, s); }                                                  // ... and work items
     h->cur ^= 1;
     h->acur ^= 1;
-    h->launches += 23;
+    h->grid_final = false;
+    h->launches += 24;
 }
 
 int copy_in(mpm_handle *h, double *dst, const double *src, long long n, int loc)
@@ -506,7 +509,7 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
             ok = dev_alloc_t(h, &h->g.vbar[a], (size_t)gd.Nn) && dev_alloc_t(h, &h->g.acc[a], (size_t)gd.Nn) &&
                  dev_alloc_t(h, &h->g.v2[a], (size_t)gd.Nn);
     }
-    h->acur = 0;
+    h->acur = 0; h->grid_final = true;
     h->acc_m[0] = h->g.m; h->acc_m[1] = nullptr;
     for (int a = 0; a < 3; ++a) { h->acc_mv[0][a] = h->g.mv[a]; h->acc_f[0][a] = h->g.f[a]; h->acc_mv[1][a] = h->acc_f[1][a] = nullptr; }
     if (ok && tiled) {
@@ -514,9 +517,10 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
         for (int a = 0; a < gd.dim && ok; ++a)
             ok = dev_alloc_t(h, &h->acc_mv[1][a], (size_t)gd.Nn) && dev_alloc_t(h, &h->acc_f[1][a], (size_t)gd.Nn);
     }
+    if (ok && sorted && !tiled)   // node-major node velocities; the TILED kernels form them per tile in shared memory
+        ok = dev_alloc_t(h, &h->g.na, (size_t)gd.Nn * 2 * gd.dim) && dev_alloc_t(h, &h->g.nb, (size_t)gd.Nn * gd.dim);
     if (ok && sorted)
-        ok = dev_alloc_t(h, &h->g.na, (size_t)gd.Nn * 2 * gd.dim) && dev_alloc_t(h, &h->g.nb, (size_t)gd.Nn * gd.dim) &&
-             dev_alloc_t(h, &h->off[0], (size_t)gd.Nkeys + 1) && dev_alloc_t(h, &h->off[1], (size_t)gd.Nkeys + 1) &&
+        ok = dev_alloc_t(h, &h->off[0], (size_t)gd.Nkeys + 1) && dev_alloc_t(h, &h->off[1], (size_t)gd.Nkeys + 1) &&
              dev_alloc_t(h, &h->goff, (size_t)gd.Nkeys + 1) && dev_alloc_t(h, &h->n_groups, 1) && dev_alloc_t(h, &h->n_items, 1);
     // the scan's block sums: one int per 4096 scanned elements
     ok = ok && dev_alloc_t(h, &h->count, (size_t)gd.Nkeys + 1) && dev_alloc_t(h, &h->scan_aux, (size_t)gd.Nkeys / 4096 + 8) &&
@@ -545,8 +549,8 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
         for (int j = 0; j < 6 && e == cudaSuccess; ++j)
             if (arrs[j]) e = cudaMemsetAsync(arrs[j], 0, sizeof(double) * (size_t)gd.Nn, h->stream);
     }
-    if (sorted && e == cudaSuccess) e = cudaMemsetAsync(h->g.na, 0, sizeof(double) * (size_t)gd.Nn * 2 * gd.dim, h->stream);
-    if (sorted && e == cudaSuccess) e = cudaMemsetAsync(h->g.nb, 0, sizeof(double) * (size_t)gd.Nn * gd.dim, h->stream);
+    if (sorted && !tiled && e == cudaSuccess) e = cudaMemsetAsync(h->g.na, 0, sizeof(double) * (size_t)gd.Nn * 2 * gd.dim, h->stream);
+    if (sorted && !tiled && e == cudaSuccess) e = cudaMemsetAsync(h->g.nb, 0, sizeof(double) * (size_t)gd.Nn * gd.dim, h->stream);
     if (sorted && e == cudaSuccess) e = cudaMemsetAsync(h->n_groups, 0, sizeof(int), h->stream);
     if (sorted && e == cudaSuccess) e = cudaMemsetAsync(h->n_items, 0, sizeof(int), h->stream);
     if (tiled && e == cudaSuccess) e = cudaMemsetAsync(h->acc_m[1], 0, sizeof(double) * (size_t)gd.Nn, h->stream);
@@ -710,6 +714,14 @@ int mpm_read_grid(mpm_handle *h, int field, double *out, int ptr_location)
     int rc = MPM_OK;
     // TILED: the last completed step used the accumulator set that is no longer current
     const GArr gl = (h->variant == MPM_VARIANT_TILED) ? tiled_acc(h, h->steps_done > 0 ? h->acur ^ 1 : h->acur) : h->g;
+    if (h->variant == MPM_VARIANT_TILED && !h->grid_final && h->steps_done > 0) {
+        // the step left the raw sums; l.4-5 and l.9 are replayed in place with the node kernels (dt of that step is
+        // still in the device scalars).  That accumulator set is cleared before it is used again.
+        launch_node1(gd, gl, h->sc, h->stream, false);
+        launch_node2(gd, gl, h->stream);
+        h->grid_final = true;
+        h->launches += 2;
+    }
     switch (field) {
     case MPM_G_MASS: rc = copy_out(h, out, gl.m, gd.Nn, ptr_location); break;
     case MPM_G_MOMENTUM: for (int a = 0; a < gd.dim && rc == MPM_OK; ++a) rc = copy_out(h, out + a * Nn, gl.mv[a], gd.Nn, ptr_location); break;

@@ -225,13 +225,14 @@ void launch_p2g1_tiled(const GridDesc &gd, const PArr &p, const GArr &g, const S
 // work items of the tile kernels: one block per item = <= Chunk::GROUPS groups of one tile; rebuilt every step
 void launch_build_items(const GridDesc &gd, const int *goff, int4 *items, int *n_items, cudaStream_t s);
 long long max_items_tiled(const GridDesc &gd, long long max_groups);   // upper bound of the item count (launch size)
-void launch_g2p_p2g2_tiled(const GridDesc &gd, const PArr &p, const GArr &g, const double *na, const DevScalars *sc,
+// g: the node accumulators m, mv, f of this step (raw P2G#1) and mv2; the kernels apply l.4-5 / l.9 while staging a tile
+void launch_g2p_p2g2_tiled(const GridDesc &gd, const PArr &p, const GArr &g, const DevScalars *sc,
                            const SortedMap &map, const int4 *items, const int *n_items, long long max_items, int *count,
                            unsigned long long *dest, cudaStream_t s);
 // update + re-ordering + P2G#1 of the next step into g_next.m, g_next.mv, g_next.f (zeroed by the caller).  store_q:
 // write Q' to memory (only needed when the state can be read back or re-loaded before the next step: the fused P2G#1
 // has already consumed it)
-void launch_update_tiled(const GridDesc &gd, const PArr &p, const PArr &q, const double *na, const double *nb, DevScalars *sc,
+void launch_update_tiled(const GridDesc &gd, const PArr &p, const PArr &q, const GArr &g, DevScalars *sc,
                          const SortedMap &map, const int4 *items, const int *n_items, long long max_items, const int *off_new,
                          const unsigned long long *dest, const GArr &g_next, bool store_q, cudaStream_t s);
 // dst[id] = src[slot] for every occupied slot; with coff (exclusive scan of the per-key counts) and off (slot offsets):
@@ -243,7 +244,8 @@ void launch_stats_reduce_groups(const GridDesc &gd, const PArr &p, DevScalars *s
 
 // node kernels -- mpm_kernels_grid.cu
 void launch_grid_clear(const GridDesc &gd, const GArr &g, cudaStream_t s);
-void launch_node1(const GridDesc &gd, const GArr &g, const DevScalars *sc, cudaStream_t s);
+// zero_mv2: also reset mv2 for l.8 (false when the kernel only replays l.4-5 for mpm_read_grid)
+void launch_node1(const GridDesc &gd, const GArr &g, const DevScalars *sc, cudaStream_t s, bool zero_mv2 = true);
 void launch_node2(const GridDesc &gd, const GArr &g, cudaStream_t s);
 
 // time loop scalars -- mpm_kernels_grid.cu

@@ -5,59 +5,13 @@
 //           m = 0, reading A5) and the reset of mv2 for l.8.
 //   node2 : Alg. 1 l.9    BC on mv2, v2 = mv2/m.
 //   begin/end_step : dt from the CFL reduction (eq. 25/29), t += dt -- no host round trip.
-#include "mpm_internal.cuh"
+#include "mpm_node_bc.cuh"
 
 namespace mpm {
 
 namespace {
 
 constexpr int kBlock = 256;
-
-// Domain-face and obstacle conditions on one node's (mv, f) pair, in the order x, y, z faces then obstacle (A9, A14).
-// WITH_F = false is the second application (momentum only).
-template <int DIM, bool WITH_F>
-__device__ __forceinline__ void apply_bc(const GridDesc &gd, const GArr &g, long long i, const int idx[DIM], double m,
-                                         double mv[DIM], double f[DIM])
-{
-#pragma unroll
-    for (int a = 0; a < DIM; ++a) {
-        if (gd.per[a]) continue;
-#pragma unroll
-        for (int s = 0; s < 2; ++s) {
-            const bool on_face = (s == 0) ? (idx[a] == 0) : (idx[a] == gd.nn[a] - 1);
-            if (!on_face) continue;
-            const int bc = gd.bc[a][s];
-            if (bc == MPM_BC_REFLECT) {            // eq. (30): v.n = 0
-                mv[a] = 0.0;
-                if (WITH_F) f[a] = 0.0;
-            } else if (bc == MPM_BC_INFLOW) {      // Dirichlet inflow
-#pragma unroll
-                for (int a2 = 0; a2 < DIM; ++a2) {
-                    mv[a2] = m * gd.inflow_v[a2];
-                    if (WITH_F) f[a2] = 0.0;
-                }
-            } else if (bc == MPM_BC_OUTFLOW) {     // A10
-                if (WITH_F) f[a] = 0.0;
-            }
-        }
-    }
-    if (gd.has_obstacle && g.flag[i]) {
-        double nrm[DIM], dot = 0.0, dotf = 0.0;
-#pragma unroll
-        for (int a = 0; a < DIM; ++a) {
-            nrm[a] = g.normal[a][i];
-            dot += mv[a] * nrm[a];
-            if (WITH_F) dotf += f[a] * nrm[a];
-        }
-        const double half = (dot - fabs(dot)) / 2.0;       // eq. (21)
-        const double halff = (dotf - fabs(dotf)) / 2.0;    // eq. (22)
-#pragma unroll
-        for (int a = 0; a < DIM; ++a) {
-            mv[a] -= half * nrm[a];
-            if (WITH_F) f[a] -= halff * nrm[a];
-        }
-    }
-}
 
 template <int DIM>
 __device__ __forceinline__ void node_coords(const GridDesc &gd, long long i, int idx[DIM])
@@ -71,7 +25,7 @@ __device__ __forceinline__ void node_coords(const GridDesc &gd, long long i, int
 }
 
 template <int DIM>
-__global__ void __launch_bounds__(kBlock) k_node1(GridDesc gd, GArr g, const DevScalars *sc)
+__global__ void __launch_bounds__(kBlock) k_node1(GridDesc gd, GArr g, const DevScalars *sc, bool zero_mv2)
 {
     const long long i = (long long)blockIdx.x * kBlock + threadIdx.x;
     if (i >= gd.Nn) return;
@@ -93,11 +47,11 @@ __global__ void __launch_bounds__(kBlock) k_node1(GridDesc gd, GArr g, const Dev
         if (g.na) {
             g.na[i * (2 * DIM) + a] = vb;
             g.na[i * (2 * DIM) + DIM + a] = ac;
-        } else {
+        } else if (g.vbar[a]) {
             g.vbar[a][i] = vb;
             g.acc[a][i] = ac;
         }
-        g.mv2[a][i] = 0.0;
+        if (zero_mv2) g.mv2[a][i] = 0.0;
     }
 }
 
@@ -117,7 +71,7 @@ __global__ void __launch_bounds__(kBlock) k_node2(GridDesc gd, GArr g)
     for (int a = 0; a < DIM; ++a) {
         g.mv2[a][i] = mv[a];
         const double v2 = (m != 0.0) ? mv[a] / m : 0.0;
-        if (g.nb) g.nb[i * DIM + a] = v2; else g.v2[a][i] = v2;
+        if (g.nb) g.nb[i * DIM + a] = v2; else if (g.v2[a]) g.v2[a][i] = v2;
     }
 }
 
@@ -221,10 +175,10 @@ void launch_grid_clear(const GridDesc &gd, const GArr &g, cudaStream_t s)
     }
 }
 
-void launch_node1(const GridDesc &gd, const GArr &g, const DevScalars *sc, cudaStream_t s)
+void launch_node1(const GridDesc &gd, const GArr &g, const DevScalars *sc, cudaStream_t s, bool zero_mv2)
 {
-    if (gd.dim == 2) k_node1<2><<<grid_for(gd.Nn), kBlock, 0, s>>>(gd, g, sc);
-    else k_node1<3><<<grid_for(gd.Nn), kBlock, 0, s>>>(gd, g, sc);
+    if (gd.dim == 2) k_node1<2><<<grid_for(gd.Nn), kBlock, 0, s>>>(gd, g, sc, zero_mv2);
+    else k_node1<3><<<grid_for(gd.Nn), kBlock, 0, s>>>(gd, g, sc, zero_mv2);
 }
 
 void launch_node2(const GridDesc &gd, const GArr &g, cudaStream_t s)

@@ -17,6 +17,7 @@
 // Shared-memory accumulator tiles with fp64 atomicAdd were measured and dropped (git history: CAS loops stall the
 // 16 resident warps; a global RED is asynchronous): scatters use global fp64 reductions as in the SORTED family.
 #include "mpm_lane_groups.cuh"
+#include "mpm_node_bc.cuh"
 
 #ifndef MPM_MINB
 #define MPM_MINB 2   // resident blocks per SM the particle kernels are compiled for (register budget)
@@ -197,56 +198,69 @@ __device__ __forceinline__ void tile_origin(const GridDesc &gd, int tile, int or
     if (DIM == 3) org[DIM - 1] = (tile / (gd.ntile[0] * gd.ntile[1])) << TG::LT2;
 }
 
-// global node index of tile-local node j (periodic wrap: node n == node 0, A11); -1 = outside the grid
+// global node index and node coordinates of tile-local node j (periodic wrap: node n == node 0, A11); -1 = outside the grid
 template <int DIM>
-__device__ __forceinline__ int tile_node_global(const GridDesc &gd, const int org[DIM], int j)
+__device__ __forceinline__ int tile_node_global(const GridDesc &gd, const int org[DIM], int j, int idx[DIM])
 {
     using TG = TileGeo<DIM>;
     int ln[3];
     ln[0] = j % TG::N0;
     ln[1] = (j / TG::N0) % TG::N1;
     ln[2] = j / (TG::N0 * TG::N1);
-    int idx = 0, stride = 1;
+    int node = 0, stride = 1;
     bool ok = true;
 #pragma unroll
     for (int a = 0; a < DIM; ++a) {
         int i = org[a] + ln[a];
         if (i > gd.nc[a]) ok = false;
         if (gd.per[a] && i == gd.nc[a]) i = 0;
-        idx += stride * i;
+        idx[a] = i;
+        node += stride * i;
         stride *= gd.nn[a];
     }
-    return ok ? idx : -1;
+    return ok ? node : -1;
 }
 
-// Stage the node velocities of one tile in shared memory, node-major with CH doubles per node:
-//   [0, DIM) vbar = mv'/m, [DIM, 2 DIM) acc = f/m (from na), and with WITH_NB [2 DIM, 3 DIM) v2 = mv2/m (from nb), rest 0.
-template <int DIM, int CH, bool WITH_NB>
-__device__ __forceinline__ void stage_tile(const GridDesc &gd, const int org[DIM], const double *__restrict__ na,
-                                           const double *__restrict__ nb, double *s_tile)
+// Stage the node velocities of one tile in shared memory, node-major with CH doubles per node, straight from the raw
+// node accumulators m, mv, f (and mv2): Alg. 1 l.4 (BC + obstacle on mv, f: eqs. 21, 22, 30), l.5
+// (mv' = mv + dt f) and the quotients the gathers read (theta of PAPER.md:295, ratio := 0 where m = 0,
+// reading A5) are evaluated HERE, per tile node, instead of in a node kernel that writes them to memory first:
+//   [0, DIM) vbar = mv'/m, [DIM, 2 DIM) acc = f/m, and with WITH_V2 [2 DIM, 3 DIM) v2 = BC(mv2)/m (l.9), rest 0.
+// One reciprocal per node (1 ulp from the true quotients of the node kernels, far inside the parity tolerance).
+template <int DIM, int CH, bool WITH_V2>
+__device__ __forceinline__ void stage_tile(const GridDesc &gd, const int org[DIM], const GArr &g, double dt, double *s_tile)
 {
     using TG = TileGeo<DIM>;
     for (int j = threadIdx.x; j < TG::NN; j += kTB) {
-        const int node = tile_node_global<DIM>(gd, org, j);
-        double2 *dst = reinterpret_cast<double2 *>(s_tile + j * CH);
-        double2 v[CH / 2];
+        int idx[DIM];
+        const int node = tile_node_global<DIM>(gd, org, j, idx);
+        double v[CH];
 #pragma unroll
-        for (int q = 0; q < CH / 2; ++q) v[q] = make_double2(0.0, 0.0);
+        for (int q = 0; q < CH; ++q) v[q] = 0.0;
         if (node >= 0) {
-            const double2 *src = reinterpret_cast<const double2 *>(na + (long long)node * (2 * DIM));
+            const double m = __ldg(g.m + node);
+            double mv[DIM], f[DIM];
 #pragma unroll
-            for (int q = 0; q < DIM; ++q) v[q] = __ldg(src + q);
-            if (WITH_NB) {
-                double t[DIM + 1];
+            for (int a = 0; a < DIM; ++a) { mv[a] = __ldg(g.mv[a] + node); f[a] = __ldg(g.f[a] + node); }
+            apply_bc<DIM, true>(gd, g, node, idx, m, mv, f);
+            const double inv = (m != 0.0) ? 1.0 / m : 0.0;
 #pragma unroll
-                for (int a = 0; a < DIM; ++a) t[a] = __ldg(nb + (long long)node * DIM + a);
-                t[DIM] = 0.0;
+            for (int a = 0; a < DIM; ++a) {
+                v[a] = (mv[a] + dt * f[a]) * inv;
+                v[DIM + a] = f[a] * inv;
+            }
+            if (WITH_V2) {
+                double mv2[DIM], none[DIM];
 #pragma unroll
-                for (int q = 0; q < (DIM + 1) / 2; ++q) v[DIM + q] = make_double2(t[2 * q], t[2 * q + 1]);
+                for (int a = 0; a < DIM; ++a) { mv2[a] = __ldg(g.mv2[a] + node); none[a] = 0.0; }
+                apply_bc<DIM, false>(gd, g, node, idx, m, mv2, none);
+#pragma unroll
+                for (int a = 0; a < DIM; ++a) v[2 * DIM + a] = mv2[a] * inv;
             }
         }
+        double2 *dst = reinterpret_cast<double2 *>(s_tile + j * CH);
 #pragma unroll
-        for (int q = 0; q < CH / 2; ++q) dst[q] = v[q];
+        for (int q = 0; q < CH / 2; ++q) dst[q] = make_double2(v[2 * q], v[2 * q + 1]);
     }
 }
 
@@ -392,7 +406,7 @@ __device__ __forceinline__ void coop_p2g1(const GridDesc &gd, const GArr &gn, un
 // The particle fields of the NEXT pass are copied into the thread's own shared-memory slots with cp.async while the
 // current pass computes (PfSlots).  V' is NOT stored: the update kernel recomputes it.
 template <int DIM>
-__global__ void __launch_bounds__(kTB, kTBMinG) k_g2p_p2g2_tiled(GridDesc gd, PArr p, GArr g, const double *__restrict__ na,
+__global__ void __launch_bounds__(kTB, kTBMinG) k_g2p_p2g2_tiled(GridDesc gd, PArr p, GArr g,
                                                                 const DevScalars *__restrict__ sc, SortedMap map,
                                                                 const int4 *__restrict__ items, const int *__restrict__ n_items,
                                                                 int *__restrict__ count, unsigned long long *__restrict__ dest)
@@ -423,10 +437,10 @@ __global__ void __launch_bounds__(kTB, kTBMinG) k_g2p_p2g2_tiled(GridDesc gd, PA
     issue(grp);
     int org[DIM];
     tile_origin<DIM>(gd, item.x, org);
-    stage_tile<DIM, CH, false>(gd, org, na, nullptr, s_tile);
-    __syncthreads();
     const double dt = sc->dt;
     const long long step = sc->step;
+    stage_tile<DIM, CH, false>(gd, org, g, dt, s_tile);
+    __syncthreads();
     for (int p0 = 0; p0 < item.z; p0 += GPB, gl += GPB) {
         int c[DIM];
         unpack_coords<DIM>(grp.cpack, c);
@@ -533,8 +547,7 @@ struct UpdSmem {
 };
 
 template <int DIM>
-__global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr p, PArr q, const double *__restrict__ na,
-                                                              const double *__restrict__ nb, DevScalars *sc, SortedMap map,
+__global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr p, PArr q, GArr g, DevScalars *sc, SortedMap map,
                                                               const int4 *__restrict__ items, const int *__restrict__ n_items,
                                                               const int *__restrict__ off_new,
                                                               const unsigned long long *__restrict__ dest, GArr gn, int store_q)
@@ -574,10 +587,10 @@ __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr
     issue(grp);
     int org[DIM];
     tile_origin<DIM>(gd, item.x, org);
-    stage_tile<DIM, CH, true>(gd, org, na, nb, s_tile);
-    __syncthreads();
     const double dt = sc->dt;
     const long long step = sc->step;
+    stage_tile<DIM, CH, true>(gd, org, g, dt, s_tile);
+    __syncthreads();
     double vloc = 0.0, cloc = 0.0;
     int n_rec = 0, n_clamp = 0, n_neg = 0, n_nonfin = 0;
     const double gm1 = gd.gamma - 1.0;
@@ -929,16 +942,16 @@ long long max_items_tiled(const GridDesc &gd, long long max_groups)
     return (ntiles < max_groups ? ntiles : max_groups) + max_groups / per + 1;
 }
 
-void launch_g2p_p2g2_tiled(const GridDesc &gd, const PArr &p, const GArr &g, const double *na, const DevScalars *sc,
+void launch_g2p_p2g2_tiled(const GridDesc &gd, const PArr &p, const GArr &g, const DevScalars *sc,
                            const SortedMap &map, const int4 *items, const int *n_items, long long max_items, int *count,
                            unsigned long long *dest, cudaStream_t s)
 {
     if (max_items <= 0) return;
-    if (gd.dim == 2) k_g2p_p2g2_tiled<2><<<(unsigned)max_items, kTB, 0, s>>>(gd, p, g, na, sc, map, items, n_items, count, dest);
-    else k_g2p_p2g2_tiled<3><<<(unsigned)max_items, kTB, 0, s>>>(gd, p, g, na, sc, map, items, n_items, count, dest);
+    if (gd.dim == 2) k_g2p_p2g2_tiled<2><<<(unsigned)max_items, kTB, 0, s>>>(gd, p, g, sc, map, items, n_items, count, dest);
+    else k_g2p_p2g2_tiled<3><<<(unsigned)max_items, kTB, 0, s>>>(gd, p, g, sc, map, items, n_items, count, dest);
 }
 
-void launch_update_tiled(const GridDesc &gd, const PArr &p, const PArr &q, const double *na, const double *nb, DevScalars *sc,
+void launch_update_tiled(const GridDesc &gd, const PArr &p, const PArr &q, const GArr &g, DevScalars *sc,
                          const SortedMap &map, const int4 *items, const int *n_items, long long max_items, const int *off_new,
                          const unsigned long long *dest, const GArr &g_next, bool store_q, cudaStream_t s)
 {
@@ -951,9 +964,9 @@ void launch_update_tiled(const GridDesc &gd, const PArr &p, const PArr &q, const
         attr_set = true;
     }
     if (gd.dim == 2)
-        k_update_tiled<2><<<(unsigned)max_items, kTB, UpdSmem<2>::BYTES, s>>>(gd, p, q, na, nb, sc, map, items, n_items, off_new, dest, g_next, sq);
+        k_update_tiled<2><<<(unsigned)max_items, kTB, UpdSmem<2>::BYTES, s>>>(gd, p, q, g, sc, map, items, n_items, off_new, dest, g_next, sq);
     else
-        k_update_tiled<3><<<(unsigned)max_items, kTB, UpdSmem<3>::BYTES, s>>>(gd, p, q, na, nb, sc, map, items, n_items, off_new, dest, g_next, sq);
+        k_update_tiled<3><<<(unsigned)max_items, kTB, UpdSmem<3>::BYTES, s>>>(gd, p, q, g, sc, map, items, n_items, off_new, dest, g_next, sq);
 }
 
 void launch_gather_by_id_groups(const double *src, const int *id, double *dst, const SortedMap &map, long long max_groups,
