@@ -132,12 +132,12 @@ def measured_peak_gbs():
         return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
 
 
-def ncu_traffic(kernel, workload_name):
+def ncu_traffic(kernel, workload_name, variant):
     """dram bytes per launch of the dominant kernel from the committed ncu --set full summary, if there is one."""
     path = os.path.join(ROOT, "profiles", "traffic.json")
     try:
         table = json.load(open(path))
-        return table.get(workload_name, {}).get(kernel)
+        return table.get(variant, {}).get(workload_name, {}).get(kernel)
     except Exception:
         return None
 
@@ -250,7 +250,7 @@ def run_ours(args):
     peak, peak_src = measured_peak_gbs()
     achieved = per_kernel[dom] / (kms[dom] * 1e-3) / 1e9
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": ncu_traffic(dom, args.workload), "peak_source": peak_src,
+                "frac": achieved / peak, "traffic": ncu_traffic(dom, args.workload, args.variant) if not args.size else None, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": per_kernel[dom], "kernel_ms": kms[dom]}
     step_gbs = step_bytes * args.steps / (ms * 1e-3) / 1e9
     step_roofline = {"bytes_per_step": step_bytes, "achieved_gbs": step_gbs, "frac_of_measured_peak": step_gbs / peak,
