@@ -321,25 +321,20 @@ __device__ __forceinline__ void gather_tile(const double *s_cell, const double W
     }
 }
 
-// Alg. 1 l.11 for one particle (see lg::move_particle); the persistent id is only needed by the recycling generator
-// (A8), so it is fetched only when a particle actually leaves through an OUTFLOW face.
+// Fast path of Alg. 1 l.11: X' = X + dt Vbar.  When X' lies in [0, L) on every axis, neither the
+// periodic wrap (A11), nor the outflow test (A8), nor the clamp of lg::move_particle changes it, so that function
+// returns exactly this X'; the caller takes move_particle only when this returns false (rare: particles next to a
+// domain face).  Both tile kernels use the same two functions on the same inputs, so they agree on X' bit for bit.
 template <int DIM>
-__device__ __forceinline__ void move_particle_lazy_id(const GridDesc &gd, const double X[DIM], const double Vb[DIM], double dt,
-                                                      const int *__restrict__ idarr, long long k, long long step, double Xn[DIM])
+__device__ __forceinline__ bool move_inside(const GridDesc &gd, const double X[DIM], const double Vb[DIM], double dt, double Xn[DIM])
 {
-    bool leaves = false;
+    bool in = true;
 #pragma unroll
     for (int a = 0; a < DIM; ++a) {
-        const double x = fma(dt, Vb[a], X[a]);
-        if (!gd.per[a]) {
-            if (x < 0.0 && gd.bc[a][0] == MPM_BC_OUTFLOW) leaves = true;
-            if (x > gd.L[a] && gd.bc[a][1] == MPM_BC_OUTFLOW) leaves = true;
-        }
+        Xn[a] = fma(dt, Vb[a], X[a]);
+        in = in && (Xn[a] >= 0.0) && (Xn[a] < gd.L[a]);
     }
-    const long long id = (leaves && gd.in_axis >= 0) ? (long long)idarr[k] : 0;
-    bool recycled;
-    int nclamp;
-    move_particle<DIM>(gd, X, Vb, dt, id, step, Xn, recycled, nclamp);
+    return in;
 }
 
 __device__ __forceinline__ double sel3(const double v[], int a, int dim)
@@ -467,17 +462,19 @@ __global__ void __launch_bounds__(kTB, kTBMinG) k_g2p_p2g2_tiled(GridDesc gd, PA
         for (int i = 0; i < 2; ++i) weights_1d<DIM>(gd, X[i], c, xi[i], W[i]);
         gather_tile<DIM, CH, false>(s_tile + j0 * CH, W, out, Dh);
         double MV[2][DIM];
-        int key[2] = { -1, -1 };
+        int key[2];
 #pragma unroll
         for (int i = 0; i < 2; ++i) {
 #pragma unroll
             for (int a = 0; a < DIM; ++a) MV[i][a] = M[i] * fma(dt, out[i][DIM + a], V[i][a]);   // M V'
-            if (valid[i]) {
-                // where the particle will be after l.11
-                double Xn[DIM];
-                move_particle_lazy_id<DIM>(gd, X[i], out[i], dt, p.id, k0 + i, step, Xn);
-                key[i] = tiled_key_of_position<DIM>(gd, Xn);
+            // where the particle will be after l.11 (the persistent id is only needed by the recycling generator, A8)
+            double Xn[DIM];
+            if (!move_inside<DIM>(gd, X[i], out[i], dt, Xn) && valid[i]) {
+                bool recycled;
+                int nclamp;
+                move_particle<DIM>(gd, X[i], out[i], dt, gd.in_axis >= 0 ? (long long)p.id[k0 + i] : 0, step, Xn, recycled, nclamp);
             }
+            key[i] = valid[i] ? tiled_key_of_position<DIM>(gd, Xn) : -1;
         }
         // ranks among the particles that end up in the same cell (arrival order of the atomics, A17): issue the atomics
         const bool stay[2] = { valid[0] && key[0] == grp.cell, valid[1] && key[1] == grp.cell };
@@ -640,57 +637,58 @@ __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr
         }
         issue(nxt);                                   // the slots have been read: refill them for the next pass
         const Group nn = fetch_group(map.groups, (long long)item.y + gl + 2 * GPB, g_end);
-        // per particle: the new state (what goes to memory), its slot, and whether it stays in the group's cell
-        double Xo[2][DIM], Vo[2][DIM], Mo[2], Ro[2], Eo[2], Qo[2];
-        bool stay[2] = { false, false };
+        // per particle: the new state (what goes to memory), S' for the next step's force, and whether it stays in the
+        // group's cell.  Straight-line code for both particles of the lane (an unused slot computes on M = 0, rho = 1,
+        // E = 0, X = 0 and is masked where it could be seen: counters, maxima, stores, scatter payloads).
+        double Xo[2][DIM], Vo[2][DIM], Mo[2], Ro[2], Eo[2], Qo[2], Sn[2];
+        bool stay[2];
 #pragma unroll
         for (int i = 0; i < 2; ++i) {
+            const double D = Dh[i] * gd.inv_h;
 #pragma unroll
-            for (int a = 0; a < DIM; ++a) { Xo[i][a] = 0.0; Vo[i][a] = 0.0; }
-            Mo[i] = 0.0; Ro[i] = 1.0; Eo[i] = 0.0; Qo[i] = 0.0;
+            for (int a = 0; a < DIM; ++a) Vo[i][a] = fma(dt, out[i][DIM + a], V[i][a]);   // V'
+            // particle thermodynamics (eq. 4 with this step's D: reading A2).  P/rho = (gamma-1) E
+            // and gamma P/rho = gamma (gamma-1) E are used in place of the quotients (one rounding apart).
+            const double r = rho[i], e0 = E[i];
+            const double cs0 = sqrt(gd.gamma * gm1 * e0);
+            double Q, Q_over_rho;
+            if (gd.visc_form == MPM_VISC_STANDARD) {
+                Q_over_rho = gd.c0 * gd.h * gd.h * D * D - gd.c1 * gd.h * cs0 * D;
+                Q = r * Q_over_rho;
+            } else {
+                Q = gd.c0 * (r * gd.h * D) * (r * gd.h * D) - gd.c1 * gd.h * cs0 * D;
+                Q_over_rho = Q / r;
+            }
+            if (!(D < 0.0)) { Q = 0.0; Q_over_rho = 0.0; }      // eq. (4): only in compression
+            double En = e0 - dt * (gm1 * e0 + Q_over_rho) * D;
+            const double jac = fma(dt, D, 1.0);
+            double rhon = r / jac;
             if (valid[i]) {
-                const double D = Dh[i] * gd.inv_h;
-#pragma unroll
-                for (int a = 0; a < DIM; ++a) Vo[i][a] = fma(dt, out[i][DIM + a], V[i][a]);   // V'
-                // particle thermodynamics (eq. 4 with this step's D: reading A2).  P/rho = (gamma-1) E
-                // and gamma P/rho = gamma (gamma-1) E are used in place of the quotients (one rounding apart).
-                const double r = rho[i], e0 = E[i];
-                double Q = 0.0, Q_over_rho = 0.0;
-                if (D < 0.0) {
-                    const double cs0 = sqrt(gd.gamma * gm1 * e0);
-                    if (gd.visc_form == MPM_VISC_STANDARD) {
-                        Q_over_rho = gd.c0 * gd.h * gd.h * D * D - gd.c1 * gd.h * cs0 * D;
-                        Q = r * Q_over_rho;
-                    } else {
-                        Q = gd.c0 * (r * gd.h * D) * (r * gd.h * D) - gd.c1 * gd.h * cs0 * D;
-                        Q_over_rho = Q / r;
-                    }
-                }
-                double En = e0 - dt * (gm1 * e0 + Q_over_rho) * D;
-                const double jac = fma(dt, D, 1.0);
                 if (jac <= 0.0) n_neg++;
-                double rhon = r / jac;
-                const double cs = sqrt(gd.gamma * gm1 * En);
                 if (!isfinite(En) || !isfinite(rhon)) n_nonfin++;
                 double vv = 0.0, vb2 = 0.0;
 #pragma unroll
                 for (int a = 0; a < DIM; ++a) { vv = fma(Vo[i][a], Vo[i][a], vv); vb2 = fma(out[i][a], out[i][a], vb2); }
-                vloc = fmax(vloc, fmax(vv, vb2));      // squared; the root is taken once at the end
-                cloc = fmax(cloc, cs);
+                vloc = fmax(vloc, fmax(vv, vb2));                // squared; the root is taken once at the end
+                cloc = fmax(cloc, gd.gamma * gm1 * En);          // c_s^2 = gamma P'/rho' (the root is monotone: taken at the end)
+            }
+            double Mn = M[i];
+            if (!move_inside<DIM>(gd, X[i], out[i], dt, Xo[i]) && valid[i]) {      // next to a domain face (rare)
                 bool recycled;
                 int nclamp;
                 move_particle<DIM>(gd, X[i], out[i], dt, (long long)id[i], step, Xo[i], recycled, nclamp);
                 n_clamp += nclamp;
-                double Mn = M[i];
                 if (recycled) {
 #pragma unroll
                     for (int a = 0; a < DIM; ++a) Vo[i][a] = gd.inflow_v[a];
-                    rhon = gd.inflow_rho; En = gd.inflow_e; Q = 0.0; Mn = gd.inflow_mass;
+                    rhon = gd.inflow_rho; En = gd.inflow_e; Q = 0.0; Q_over_rho = 0.0; Mn = gd.inflow_mass;
                     n_rec++;
                 }
-                Mo[i] = Mn; Ro[i] = rhon; Eo[i] = En; Qo[i] = Q;
-                stay[i] = key[i] == grp.cell;
             }
+            Mo[i] = Mn; Ro[i] = rhon; Eo[i] = En; Qo[i] = Q;
+            // S' = (P' + Q') M / rho' with P' = (gamma-1) rho' E' (eq. 3) and Q'/rho' = (Q'/rho) (1 + dt D)  (rho' = rho / (1 + dt D))
+            Sn[i] = (gm1 * En + Q_over_rho * jac) * Mn;
+            stay[i] = valid[i] && key[i] == grp.cell;
         }
         // l.12: the particle goes to its cell-sorted slot of the other buffer; the two particles of a lane usually
         // keep adjacent slots (ranks of the stayers are consecutive), then each field is ONE 16-byte store
@@ -720,10 +718,7 @@ __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr
                 q.id[d] = id[i];
             }
         }
-        // P2G#1 of the next step (eqs. 13, 14, 16, 18 at X'): S' = (P' + Q') M / rho', P' = (gamma-1) rho' E' (eq. 3)
-        double Sn[2];
-#pragma unroll
-        for (int i = 0; i < 2; ++i) Sn[i] = (gm1 * Ro[i] * Eo[i] + Qo[i]) * Mo[i] / Ro[i];
+        // P2G#1 of the next step (eqs. 13, 14, 16, 18 at X')
 #pragma unroll
         for (int i = 0; i < 2; ++i) {      // particles that leave the group's cell: scattered by the whole warp
             const unsigned mm = __ballot_sync(kFull, valid[i] && !stay[i]);
@@ -747,7 +742,7 @@ __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr
     }
     // block maxima -> at most one atomicMax per block (max is order-free, so this is exact)
     vloc = warp_max_nonneg(sqrt(vloc));
-    cloc = warp_max_nonneg(cloc >= 0.0 ? cloc : 0.0);
+    cloc = warp_max_nonneg(cloc > 0.0 ? sqrt(cloc) : 0.0);
     if (lane == 0) { s_v[warp] = vloc; s_c[warp] = cloc; }
     const int rec_sum = __reduce_add_sync(kFull, n_rec), neg_sum = __reduce_add_sync(kFull, n_neg),
               nf_sum = __reduce_add_sync(kFull, n_nonfin), clamp_sum = __reduce_add_sync(kFull, n_clamp);
