@@ -169,11 +169,11 @@ __global__ void __launch_bounds__(kBlock, MPM_MINB) k_p2g1_tiled(GridDesc gd, PA
 #define MPM_TBMIN_G 4
 #endif
 #ifndef MPM_TBMIN_U
-#define MPM_TBMIN_U 3
+#define MPM_TBMIN_U 4
 #endif
 constexpr int kTB = MPM_TB;              // threads per block of the tile kernels
 constexpr int kTBMinG = MPM_TBMIN_G;     // resident blocks per SM the gather kernel is compiled for (128 registers)
-constexpr int kTBMinU = MPM_TBMIN_U;     // ... and the update kernel (168 registers: it spills at 128)
+constexpr int kTBMinU = MPM_TBMIN_U;     // ... and the update kernel (128 registers, no spills)
 
 template <int DIM>
 struct Chunk {
@@ -225,7 +225,8 @@ __device__ __forceinline__ int tile_node_global(const GridDesc &gd, const int or
 // node accumulators m, mv, f (and mv2): Alg. 1 l.4 (BC + obstacle on mv, f: eqs. 21, 22, 30), l.5
 // (mv' = mv + dt f) and the quotients the gathers read (theta of PAPER.md:295, ratio := 0 where m = 0,
 // reading A5) are evaluated HERE, per tile node, instead of in a node kernel that writes them to memory first:
-//   [0, DIM) vbar = mv'/m, [DIM, 2 DIM) acc = f/m, and with WITH_V2 [2 DIM, 3 DIM) v2 = BC(mv2)/m (l.9), rest 0.
+//   WITH_V2 = false (gather kernel): [0, DIM) vbar = mv'/m, [DIM, 2 DIM) acc = f/m;
+//   WITH_V2 = true  (update kernel): [0, DIM) vbar = mv'/m, [DIM, 2 DIM) v2 = BC(mv2)/m (l.9); rest 0.
 // One reciprocal per node (1 ulp from the true quotients of the node kernels, far inside the parity tolerance).
 template <int DIM, int CH, bool WITH_V2>
 __device__ __forceinline__ void stage_tile(const GridDesc &gd, const int org[DIM], const GArr &g, double dt, double *s_tile)
@@ -239,23 +240,27 @@ __device__ __forceinline__ void stage_tile(const GridDesc &gd, const int org[DIM
         for (int q = 0; q < CH; ++q) v[q] = 0.0;
         if (node >= 0) {
             const double m = __ldg(g.m + node);
-            double mv[DIM], f[DIM];
+            double mv[DIM], f[DIM], mv2[DIM];
 #pragma unroll
             for (int a = 0; a < DIM; ++a) { mv[a] = __ldg(g.mv[a] + node); f[a] = __ldg(g.f[a] + node); }
+            if (WITH_V2) {
+#pragma unroll
+                for (int a = 0; a < DIM; ++a) mv2[a] = __ldg(g.mv2[a] + node);
+            }
             apply_bc<DIM, true>(gd, g, node, idx, m, mv, f);
             const double inv = (m != 0.0) ? 1.0 / m : 0.0;
 #pragma unroll
-            for (int a = 0; a < DIM; ++a) {
-                v[a] = (mv[a] + dt * f[a]) * inv;
-                v[DIM + a] = f[a] * inv;
-            }
+            for (int a = 0; a < DIM; ++a) v[a] = (mv[a] + dt * f[a]) * inv;
             if (WITH_V2) {
-                double mv2[DIM], none[DIM];
+                double none[DIM];
 #pragma unroll
-                for (int a = 0; a < DIM; ++a) { mv2[a] = __ldg(g.mv2[a] + node); none[a] = 0.0; }
+                for (int a = 0; a < DIM; ++a) none[a] = 0.0;
                 apply_bc<DIM, false>(gd, g, node, idx, m, mv2, none);
 #pragma unroll
-                for (int a = 0; a < DIM; ++a) v[2 * DIM + a] = mv2[a] * inv;
+                for (int a = 0; a < DIM; ++a) v[DIM + a] = mv2[a] * inv;
+            } else {
+#pragma unroll
+                for (int a = 0; a < DIM; ++a) v[DIM + a] = f[a] * inv;
             }
         }
         double2 *dst = reinterpret_cast<double2 *>(s_tile + j * CH);
@@ -278,11 +283,13 @@ __device__ __forceinline__ void weights_1d(const GridDesc &gd, const double X[DI
 }
 
 // phi-weighted gather of the staged tile for the TWO particles of a lane (each corner is read once for both):
-//   out[i][ch] = sum_b phi_b(X_i) n_b[ch], ch < 2 DIM  (eq. 17: Vbar, A);
-//   with WITH_D also Dh[i] = h * sum_b sum_a v2_a(b) d_a phi_b(X_i)  (eq. 19, trace; the factor 1/h is applied by the caller)
+//   out[i][ch] = sum_b phi_b(X_i) n_b[ch]  (eq. 17), ch < 2 DIM (Vbar, A) without WITH_D, ch < DIM (Vbar) with it;
+//   with WITH_D also Dh[i] = h * sum_b sum_a v2_a(b) d_a phi_b(X_i), v2 = channels [DIM, 2 DIM)  (eq. 19, trace; the
+//   factor 1/h is applied by the caller)
 template <int DIM, int CH, bool WITH_D>
 __device__ __forceinline__ void gather_tile(const double *s_cell, const double W[2][DIM][2], double out[2][2 * DIM], double Dh[2])
 {
+    constexpr int NPHI = WITH_D ? DIM : 2 * DIM;
 #pragma unroll
     for (int i = 0; i < 2; ++i) {
         Dh[i] = 0.0;
@@ -305,7 +312,7 @@ __device__ __forceinline__ void gather_tile(const double *s_cell, const double W
 #pragma unroll
             for (int a = 1; a < DIM; ++a) phi *= W[i][a][(b >> a) & 1];
 #pragma unroll
-            for (int ch = 0; ch < 2 * DIM; ++ch) out[i][ch] = fma(phi, val[ch], out[i][ch]);
+            for (int ch = 0; ch < NPHI; ++ch) out[i][ch] = fma(phi, val[ch], out[i][ch]);
             if (WITH_D) {
 #pragma unroll
                 for (int a = 0; a < DIM; ++a) {
@@ -313,7 +320,7 @@ __device__ __forceinline__ void gather_tile(const double *s_cell, const double W
 #pragma unroll
                     for (int a2 = 0; a2 < DIM; ++a2)
                         if (a2 != a) q *= W[i][a2][(b >> a2) & 1];
-                    const double sv = ((b >> a) & 1) ? val[2 * DIM + a] : -val[2 * DIM + a];
+                    const double sv = ((b >> a) & 1) ? val[DIM + a] : -val[DIM + a];
                     Dh[i] = fma(sv, q, Dh[i]);
                 }
             }
@@ -399,7 +406,7 @@ __device__ __forceinline__ void coop_p2g1(const GridDesc &gd, const GArr &gn, un
 // that stay in their cell take consecutive ranks from ONE atomic per group (ballot + popc), only the others pay one
 // atomic each; the atomics are issued before the scatter and their results consumed after it.
 // The particle fields of the NEXT pass are copied into the thread's own shared-memory slots with cp.async while the
-// current pass computes (PfSlots).  V' is NOT stored: the update kernel recomputes it.
+// current pass computes (PfSlots).  V' overwrites V in place (the slots are this thread's own).
 template <int DIM>
 __global__ void __launch_bounds__(kTB, kTBMinG) k_g2p_p2g2_tiled(GridDesc gd, PArr p, GArr g,
                                                                 const DevScalars *__restrict__ sc, SortedMap map,
@@ -466,7 +473,10 @@ __global__ void __launch_bounds__(kTB, kTBMinG) k_g2p_p2g2_tiled(GridDesc gd, PA
 #pragma unroll
         for (int i = 0; i < 2; ++i) {
 #pragma unroll
-            for (int a = 0; a < DIM; ++a) MV[i][a] = M[i] * fma(dt, out[i][DIM + a], V[i][a]);   // M V'
+            for (int a = 0; a < DIM; ++a) {
+                V[i][a] = fma(dt, out[i][DIM + a], V[i][a]);      // V' = V + dt A
+                MV[i][a] = M[i] * V[i][a];                        // M V'
+            }
             // where the particle will be after l.11 (the persistent id is only needed by the recycling generator, A8)
             double Xn[DIM];
             if (!move_inside<DIM>(gd, X[i], out[i], dt, Xn) && valid[i]) {
@@ -475,6 +485,12 @@ __global__ void __launch_bounds__(kTB, kTBMinG) k_g2p_p2g2_tiled(GridDesc gd, PA
                 move_particle<DIM>(gd, X[i], out[i], dt, gd.in_axis >= 0 ? (long long)p.id[k0 + i] : 0, step, Xn, recycled, nclamp);
             }
             key[i] = valid[i] ? tiled_key_of_position<DIM>(gd, Xn) : -1;
+        }
+        // V' replaces V in memory (the update kernel reads it back instead of gathering A again)
+#pragma unroll
+        for (int a = 0; a < DIM; ++a) {
+            if (valid[1]) st2(p.v[a], k0, V[0][a], V[1][a]);
+            else if (valid[0]) p.v[a][k0] = V[0][a];
         }
         // ranks among the particles that end up in the same cell (arrival order of the atomics, A17): issue the atomics
         const bool stay[2] = { valid[0] && key[0] == grp.cell, valid[1] && key[1] == grp.cell };
@@ -525,8 +541,8 @@ __global__ void __launch_bounds__(kTB, kTBMinG) k_g2p_p2g2_tiled(GridDesc gd, PA
 }
 
 // ------------------------------------------------------------------------------------------------ Alg. 1 l.10-13 + l.3 of the next step
-// One block (kTB threads) per item; the tile's vbar, acc AND v2 = mv2/m are staged in shared memory.  D = trace
-// G2PD(mv2/m) (eq. 19); Q (eq. 4), E', rho'; V' = V + dt A again; CFL maxima;
+// One block (kTB threads) per item; the tile's vbar and v2 = mv2/m are staged in shared memory.  D = trace
+// G2PD(mv2/m) (eq. 19); Q (eq. 4), E', rho'; V' is read back from the gather kernel; CFL maxima;
 // X' = X + dt Vbar; the particle is written to its cell-sorted slot of the OTHER buffer (l.12).  Then
 // P2G#1 of the NEXT step at X' into the node accumulators `gn` (the other buffer of m, mv, f): a
 // particle that stays in its cell joins the group's butterfly, the others are scattered by the whole warp (coop_p2g1).
@@ -534,7 +550,7 @@ __global__ void __launch_bounds__(kTB, kTBMinG) k_g2p_p2g2_tiled(GridDesc gd, PA
 template <int DIM>
 struct UpdSmem {
     using TG = TileGeo<DIM>;
-    static constexpr int CH = (DIM == 3) ? 10 : 6;          // doubles per staged node: vbar, acc, v2, pad
+    static constexpr int CH = 2 * DIM;                      // doubles per staged node: vbar, v2
     static constexpr int NF = 2 * DIM + 3;                  // x[d], v[d], m, rho, e
     static constexpr size_t TILE = sizeof(double) * TG::NN * CH;
     static constexpr size_t PF = sizeof(double2) * NF * kTB;
@@ -646,7 +662,7 @@ __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr
         for (int i = 0; i < 2; ++i) {
             const double D = Dh[i] * gd.inv_h;
 #pragma unroll
-            for (int a = 0; a < DIM; ++a) Vo[i][a] = fma(dt, out[i][DIM + a], V[i][a]);   // V'
+            for (int a = 0; a < DIM; ++a) Vo[i][a] = V[i][a];      // V' = V + dt A, stored by the gather kernel
             // particle thermodynamics (eq. 4 with this step's D: reading A2).  P/rho = (gamma-1) E
             // and gamma P/rho = gamma (gamma-1) E are used in place of the quotients (one rounding apart).
             const double r = rho[i], e0 = E[i];
