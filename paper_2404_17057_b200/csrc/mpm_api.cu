@@ -40,6 +40,11 @@ struct mpm_handle {
     int4 *groups;
     int4 *items;          // TILED: work items of the tile kernels (one block each), rebuilt with the groups
     int *n_items;
+    // TILED: the cell map (groups, items) of the NEXT step is built between the two sweeps of a step, while the update
+    // kernel still walks the current one: second set, swapped at the end of the step
+    int4 *groups_alt, *items_alt;
+    int *n_groups_alt, *n_items_alt;
+    void *map_state;      // scratch of launch_cell_map_tiled
     long long max_items;
     double *S[2];
     unsigned long long *dest;
@@ -230,8 +235,8 @@ void free_particles(mpm_handle *h)
     h->key = h->rank = nullptr;
     dev_free(h, h->S[0]); dev_free(h, h->S[1]); dev_free(h, h->dest); dev_free(h, h->groups);
     h->S[0] = h->S[1] = nullptr; h->dest = nullptr; h->groups = nullptr;
-    dev_free(h, h->items);
-    h->items = nullptr; h->max_items = 0;
+    dev_free(h, h->items); dev_free(h, h->items_alt); dev_free(h, h->groups_alt);
+    h->items = h->items_alt = nullptr; h->groups_alt = nullptr; h->max_items = 0;
     h->n = h->cap = 0;
 }
 
@@ -257,7 +262,8 @@ int alloc_particles(mpm_handle *h, long long n)
         if (ok && !tiled) ok = dev_alloc_t(h, &h->S[0], N) && dev_alloc_t(h, &h->S[1], N);
         if (ok && tiled) {
             h->max_items = max_items_tiled(h->gd, h->max_groups);
-            ok = dev_alloc_t(h, &h->items, (size_t)h->max_items);
+            ok = dev_alloc_t(h, &h->items, (size_t)h->max_items) && dev_alloc_t(h, &h->items_alt, (size_t)h->max_items) &&
+                 dev_alloc_t(h, &h->groups_alt, (size_t)h->max_groups);
         }
     }
     if (!ok) { free_particles(h); return fail(h, MPM_E_OOM, "out of device memory for particle arrays"); }
@@ -294,17 +300,15 @@ void reorder(mpm_handle *h)
     if (h->variant == MPM_VARIANT_TILED) {
         // counts per tile-major key -> even-rounded slot offsets -> permutation; then groups and the force payload
         launch_key_rank(h->gd, src, h->key, h->rank, h->count, h->n, h->stream);
-        launch_exclusive_scan_from(h->count, h->off[0], h->gd.Nkeys + 1, h->scan_aux, true, h->stream);
+        launch_cell_map_tiled(h->gd, h->count, h->off[0], h->groups, h->n_groups, h->items, h->n_items, h->map_state, h->stream);
         launch_permute(h->gd, src, dst, h->key, h->rank, h->off[0], h->n, h->stream);
         h->cur ^= 1;
-        launch_build_groups_tiled(h->gd, h->count, h->off[0], h->goff, h->scan_aux, h->groups, h->n_groups, h->stream);
-        launch_build_items(h->gd, h->goff, h->items, h->n_items, h->stream);
         // P2G#1 of the first step (Alg. 1 l.3); every later one comes out of the update kernel of the step before
         h->acur = 0;
         GArr g0 = tiled_acc(h, 0);
         launch_grid_clear(h->gd, g0, h->stream);
         launch_p2g1_tiled(h->gd, dst, g0, SortedMap{ h->groups, h->n_groups, h->goff }, h->max_groups, h->stream);
-        h->launches += 13;
+        h->launches += 6;
         return;
     }
     int *count = h->variant == MPM_VARIANT_SORTED ? h->off[h->ocur] : h->count;
@@ -373,17 +377,17 @@ void step_tiled(mpm_handle *h, bool last_of_call)
     // kernels evaluate them per tile node while staging the tile (stage_tile)
     { Timed t(h, MPM_K_G2P_P2G2);
       launch_g2p_p2g2_tiled(gd, p, gc, h->sc, map, h->items, h->n_items, h->max_items, h->count, h->dest, s); }          // l.4-8
-    { Timed t(h, MPM_K_SORT); launch_exclusive_scan_from(h->count, h->off[0], gd.Nkeys + 1, h->scan_aux, true, s); }   // l.12 offsets
+    { Timed t(h, MPM_K_SORT);                                                         // l.12: offsets, next step's groups and work items
+      launch_cell_map_tiled(gd, h->count, h->off[0], h->groups_alt, h->n_groups_alt, h->items_alt, h->n_items_alt, h->map_state, s); }
     { Timed t(h, MPM_K_UPDATE);
       launch_update_tiled(gd, p, q, gc, h->sc, map, h->items, h->n_items, h->max_items, h->off[0], h->dest, gnx, last_of_call, s); }   // l.9-12, next l.3
     { Timed t(h, MPM_K_MISC); launch_end_step(h->sc, gd.h, s); }                                                   // l.13-14
-    { Timed t(h, MPM_K_SORT);
-      launch_build_groups_tiled(gd, h->count, h->off[0], h->goff, h->scan_aux, h->groups, h->n_groups, s);         // next step's groups
-      launch_build_items(gd, h->goff, h->items, h->n_items, s); }                                                  // ... and work items
+    { int4 *t4 = h->groups; h->groups = h->groups_alt; h->groups_alt = t4; t4 = h->items; h->items = h->items_alt; h->items_alt = t4;
+      int *t1 = h->n_groups; h->n_groups = h->n_groups_alt; h->n_groups_alt = t1; t1 = h->n_items; h->n_items = h->n_items_alt; h->n_items_alt = t1; }
     h->cur ^= 1;
     h->acur ^= 1;
     h->grid_final = false;
-    h->launches += 24;
+    h->launches += 11;
 }
 
 int copy_in(mpm_handle *h, double *dst, const double *src, long long n, int loc)
@@ -431,6 +435,7 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
     h->d_flag = nullptr; h->key = h->rank = h->count = h->scan_aux = nullptr; h->sc = nullptr;
     h->off[0] = h->off[1] = nullptr; h->ocur = 0; h->goff = h->n_groups = nullptr; h->groups = nullptr;
     h->items = nullptr; h->n_items = nullptr; h->max_items = 0;
+    h->groups_alt = h->items_alt = nullptr; h->n_groups_alt = h->n_items_alt = nullptr; h->map_state = nullptr;
     h->S[0] = h->S[1] = nullptr; h->dest = nullptr; h->max_groups = 0; h->coff = nullptr; h->slots = 0;
     std::memset(h->pbuf, 0, sizeof(h->pbuf));
     std::memset(&h->g, 0, sizeof(h->g));
@@ -522,6 +527,11 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
     if (ok && sorted)
         ok = dev_alloc_t(h, &h->off[0], (size_t)gd.Nkeys + 1) && dev_alloc_t(h, &h->off[1], (size_t)gd.Nkeys + 1) &&
              dev_alloc_t(h, &h->goff, (size_t)gd.Nkeys + 1) && dev_alloc_t(h, &h->n_groups, 1) && dev_alloc_t(h, &h->n_items, 1);
+    if (ok && tiled) {
+        unsigned char *st = nullptr;
+        ok = dev_alloc_t(h, &h->n_groups_alt, 1) && dev_alloc_t(h, &h->n_items_alt, 1) && dev_alloc_t(h, &st, cell_map_state_bytes(gd));
+        h->map_state = st;
+    }
     // the scan's block sums: one int per 4096 scanned elements
     ok = ok && dev_alloc_t(h, &h->count, (size_t)gd.Nkeys + 1) && dev_alloc_t(h, &h->scan_aux, (size_t)gd.Nkeys / 4096 + 8) &&
          dev_alloc_t(h, &h->sc, 1);

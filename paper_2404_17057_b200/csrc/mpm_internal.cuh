@@ -218,12 +218,14 @@ void launch_update_sorted(const GridDesc &gd, const PArr &p, const PArr &q, cons
                           long long max_groups, cudaStream_t s);
 
 // TILED family (tile-major cell order, even-aligned cell slots, tile nodes in shared memory) -- mpm_kernels_tiled.cu
-void launch_build_groups_tiled(const GridDesc &gd, const int *count, const int *off, int *goff, int *scan_aux, int4 *groups,
-                               int *n_groups, cudaStream_t s);
+// Alg. 1 l.12 bookkeeping in one kernel: per-key counts -> even-aligned slot offsets off[Nkeys + 1], group records, work
+// items of the tile kernels (one block per item = <= Chunk::GROUPS groups of one tile).  `state`: scratch of
+// cell_map_state_bytes(gd) bytes (zeroed by the launcher).
+size_t cell_map_state_bytes(const GridDesc &gd);
+void launch_cell_map_tiled(const GridDesc &gd, const int *count, int *off, int4 *groups, int *n_groups, int4 *items, int *n_items,
+                           void *state, cudaStream_t s);
 // P2G#1 after a load (every later step gets it from launch_update_tiled of the step before); g.m, g.mv, g.f must be zero
 void launch_p2g1_tiled(const GridDesc &gd, const PArr &p, const GArr &g, const SortedMap &map, long long max_groups, cudaStream_t s);
-// work items of the tile kernels: one block per item = <= Chunk::GROUPS groups of one tile; rebuilt every step
-void launch_build_items(const GridDesc &gd, const int *goff, int4 *items, int *n_items, cudaStream_t s);
 long long max_items_tiled(const GridDesc &gd, long long max_groups);   // upper bound of the item count (launch size)
 // g: the node accumulators m, mv, f of this step (raw P2G#1) and mv2; the kernels apply l.4-5 / l.9 while staging a tile
 void launch_g2p_p2g2_tiled(const GridDesc &gd, const PArr &p, const GArr &g, const DevScalars *sc,

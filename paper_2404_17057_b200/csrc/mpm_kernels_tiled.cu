@@ -161,7 +161,7 @@ __global__ void __launch_bounds__(kBlock, MPM_MINB) k_p2g1_tiled(GridDesc gd, PA
 // ------------------------------------------------------------------------------------------------ tile work items
 // A block works on one ITEM = up to Chunk<DIM>::GROUPS consecutive groups of ONE tile (a tile with more groups is cut into
 // several items, so that a dense tile does not serialise on one block).  The item list is rebuilt every step from the
-// per-key group offsets (k_build_items).
+// per-key particle counts (k_cell_map_tiled).
 #ifndef MPM_TB
 #define MPM_TB 128
 #endif
@@ -419,6 +419,7 @@ __global__ void __launch_bounds__(kTB, kTBMinG) k_g2p_p2g2_tiled(GridDesc gd, PA
     __shared__ __align__(16) double2 s_pf[NF][kTB];      // x[d], v[d], m of the thread's two particles
     if ((int)blockIdx.x >= *n_items) return;
     const int4 item = __ldg(items + blockIdx.x);      // {tile, first group, groups, -}
+    if (item.z == 0) return;                          // a tile without particles
     const int l = threadIdx.x % LG, lane = threadIdx.x & 31, sh = lane & ~(LG - 1);
     const int g_end = item.y + item.z;
     int gl = threadIdx.x / LG;
@@ -576,6 +577,7 @@ __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr
     __shared__ double s_v[kTB / 32], s_c[kTB / 32];
     if ((int)blockIdx.x >= *n_items) return;
     const int4 item = __ldg(items + blockIdx.x);
+    if (item.z == 0) return;
     const int l = threadIdx.x % LG, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int g_end = item.y + item.z;
     int gl = threadIdx.x / LG;
@@ -780,72 +782,131 @@ __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr
     }
 }
 
-// ------------------------------------------------------------------------------------------------ work items
-// One block: items = for every tile, ceil(groups of the tile / per_item) chunks of its group range (in tile order).
-__global__ void __launch_bounds__(1024) k_build_items(const int *__restrict__ goff, int ntiles, int ltc, int per_item,
-                                                      int4 *__restrict__ items, int *__restrict__ n_items)
+// ------------------------------------------------------------------------------------------------ cell map (Alg. 1 l.12)
+// ONE kernel turns the per-key particle counts of the re-ordering into everything the next sweeps need (the grid-to-
+// particle connectivity of PAPER.md:745-748: "count ... cumulative sum"):
+//   off[key]    first slot of the key's particles: exclusive scan of the counts rounded up to even (even-aligned slots);
+//   groups[]    one record {first slot, count, key, packed cell coordinates} per <= 2^d particles of a cell, key order;
+//   items[]     work items of the tile kernels {tile, first group, groups, -}: item t < ntiles is the first
+//               Chunk::GROUPS groups of tile t (possibly none), the further chunks of dense tiles are appended behind.
+// Single pass: a block takes 4 tiles (1024 keys, 4 per thread) in ticket order, scans (slots, groups) packed in one
+// 64-bit word and gets its exclusive prefix by decoupled look-back over the published block states
+// (flag << 62 | slots << 31 | groups; flag 1 = block aggregate, 2 = inclusive prefix).  `state` must be zero at launch.
+struct CellMapState {
+    unsigned long long ticket_done;      // low 32 bits: next block ticket; the kernel's last block resets nothing (memset per launch)
+    int extra;                           // chunks appended behind the per-tile items
+    int done;                            // blocks finished
+    unsigned long long block[1];         // [n_blocks]
+};
+constexpr int kMapBlock = 256, kMapKeysPerThread = 4, kMapKeys = kMapBlock * kMapKeysPerThread;
+
+template <int DIM>
+__global__ void __launch_bounds__(kMapBlock) k_cell_map_tiled(GridDesc gd, const int *__restrict__ count, int *__restrict__ off,
+                                                              int4 *__restrict__ groups, int *__restrict__ n_groups,
+                                                              int4 *__restrict__ items, int *__restrict__ n_items,
+                                                              CellMapState *state, int nkeys, int ntiles, int n_blocks, int per_item)
 {
-    __shared__ int s_warp[32];
-    const int per_thread = (ntiles + 1023) / 1024;
-    const int t0 = min(ntiles, (int)threadIdx.x * per_thread), t1 = min(ntiles, t0 + per_thread);
-    int mine = 0;
-    for (int t = t0; t < t1; ++t) {
-        const int ng = goff[(t + 1) << ltc] - goff[t << ltc];
-        mine += (ng + per_item - 1) / per_item;
+    constexpr int CAP = 1 << DIM, TPT = TileGeo<DIM>::TC / kMapKeysPerThread;      // threads per tile (64)
+    constexpr unsigned long long FIELD = (1ull << 31) - 1ull;
+    __shared__ unsigned long long s_warp[kMapBlock / 32], s_excl[kMapBlock + 1], s_prefix;
+    __shared__ int s_bid;
+    if (threadIdx.x == 0) s_bid = (int)atomicAdd(&state->ticket_done, 1ull);
+    __syncthreads();
+    const int bid = s_bid;
+    const int key0 = bid * kMapKeys + (int)threadIdx.x * kMapKeysPerThread;
+    int c[kMapKeysPerThread] = { 0, 0, 0, 0 };
+    if (key0 < nkeys) {      // nkeys is a multiple of the tile size, hence of 4
+        const int4 t = __ldg(reinterpret_cast<const int4 *>(count + key0));
+        c[0] = t.x; c[1] = t.y; c[2] = t.z; c[3] = t.w;
     }
+    unsigned long long mine = 0ull;
+#pragma unroll
+    for (int j = 0; j < kMapKeysPerThread; ++j)
+        mine += ((unsigned long long)((c[j] + 1) & ~1) << 31) | (unsigned long long)((c[j] + CAP - 1) / CAP);
+    // block-wide exclusive scan of `mine`
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    int incl = mine;
+    unsigned long long incl = mine;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
-        const int t = __shfl_up_sync(0xffffffffu, incl, o);
+        const unsigned long long t = __shfl_up_sync(0xffffffffu, incl, o);
         if (lane >= o) incl += t;
     }
     if (lane == 31) s_warp[warp] = incl;
     __syncthreads();
-    if (warp == 0) {
-        const int w = s_warp[lane];
-        int wi = w;
+    unsigned long long wbase = 0ull, total = 0ull;
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const int t = __shfl_up_sync(0xffffffffu, wi, o);
-            if (lane >= o) wi += t;
+    for (int w = 0; w < kMapBlock / 32; ++w) {
+        if (w < warp) wbase += s_warp[w];
+        total += s_warp[w];
+    }
+    const unsigned long long excl_local = wbase + incl - mine;
+    s_excl[threadIdx.x] = excl_local;
+    if (warp == 0) {      // decoupled look-back, 32 predecessors at a time
+        volatile unsigned long long *st = state->block;
+        constexpr unsigned long long VAL = (1ull << 62) - 1ull;
+        unsigned long long prefix = 0ull;
+        if (bid > 0 && lane == 0) st[bid] = (1ull << 62) | total;
+        for (int j = bid - 1; j >= 0; j -= 32) {
+            const int idx = j - lane;
+            unsigned long long v;
+            do { v = (idx >= 0) ? st[idx] : (2ull << 62); } while (__any_sync(0xffffffffu, (v >> 62) == 0ull));
+            const unsigned full = __ballot_sync(0xffffffffu, (v >> 62) == 2ull);      // lanes that hold an inclusive prefix
+            const int stop = full ? __ffs(full) - 1 : 32;                             // the nearest one ends the walk
+            unsigned long long val = (lane <= stop) ? (v & VAL) : 0ull;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) val += __shfl_xor_sync(0xffffffffu, val, o);
+            prefix += val;
+            if (full) break;
         }
-        s_warp[lane] = wi - w;
-        if (lane == 31) *n_items = wi;
+        if (lane == 0) {
+            __threadfence();
+            st[bid] = (2ull << 62) | (prefix + total);
+            s_prefix = prefix;
+            s_excl[kMapBlock] = total;
+        }
     }
     __syncthreads();
-    int at = s_warp[warp] + incl - mine;
-    for (int t = t0; t < t1; ++t) {
-        const int gfirst = goff[t << ltc], ng = goff[(t + 1) << ltc] - gfirst;
-        for (int done = 0; done < ng; done += per_item) items[at++] = make_int4(t, gfirst + done, min(per_item, ng - done), 0);
+    const unsigned long long base = s_prefix + excl_local;
+    int slot = (int)(base >> 31), g = (int)(base & FIELD);
+    if (key0 < nkeys) {
+        int o4[kMapKeysPerThread];
+#pragma unroll
+        for (int j = 0; j < kMapKeysPerThread; ++j) {
+            o4[j] = slot;
+            const int key = key0 + j;
+            if (c[j] > 0) {
+                int cc[DIM];
+                tiled_cell_of_key<DIM>(gd, key, cc);
+                const int cpack = (DIM == 3) ? (cc[0] | (cc[1] << 10) | (cc[DIM - 1] << 20)) : (cc[0] | (cc[1] << 16));
+                for (int first = 0; first < c[j]; first += CAP, ++g) groups[g] = make_int4(slot + first, min(CAP, c[j] - first), key, cpack);
+            }
+            slot += (c[j] + 1) & ~1;
+        }
+        *reinterpret_cast<int4 *>(off + key0) = make_int4(o4[0], o4[1], o4[2], o4[3]);
+        // work items of the tile this thread starts
+        if ((threadIdx.x % TPT) == 0) {
+            const int tile = key0 >> TileGeo<DIM>::LTC;
+            const int gfirst = (int)((s_prefix + excl_local) & FIELD);
+            const int ng = (int)((s_excl[threadIdx.x + TPT] - excl_local) & FIELD);
+            items[tile] = make_int4(tile, gfirst, min(ng, per_item), 0);
+            if (ng > per_item) {
+                const int more = (ng - 1) / per_item;
+                int at = ntiles + atomicAdd(&state->extra, more);
+                for (int done = per_item; done < ng; done += per_item) items[at++] = make_int4(tile, gfirst + done, min(per_item, ng - done), 0);
+            }
+        }
     }
-}
-
-// ------------------------------------------------------------------------------------------------ bookkeeping kernels
-
-__global__ void __launch_bounds__(kBlock) k_group_counts_tiled(const int *count, int *gcount, int nkeys, int cap)
-{
-    const int c = blockIdx.x * kBlock + threadIdx.x;
-    if (c < nkeys) gcount[c] = (count[c] + cap - 1) / cap;
-    else if (c == nkeys) gcount[c] = 0;
-}
-
-template <int DIM>
-__global__ void __launch_bounds__(kBlock) k_group_fill_tiled(GridDesc gd, const int *count, const int *off, const int *goff,
-                                                             int4 *groups, int *n_groups, int nkeys)
-{
-    constexpr int CAP = 1 << DIM;
-    const int key = blockIdx.x * kBlock + threadIdx.x;
-    if (key == 0) *n_groups = goff[nkeys];
-    if (key >= nkeys) return;
-    const int g0 = goff[key], g1 = goff[key + 1];
-    if (g0 == g1) return;
-    int c[DIM];
-    tiled_cell_of_key<DIM>(gd, key, c);
-    const int cpack = (DIM == 3) ? (c[0] | (c[1] << 10) | (c[DIM - 1] << 20)) : (c[0] | (c[1] << 16));
-    int first = off[key];
-    const int end = first + count[key];
-    for (int gq = g0; gq < g1; ++gq, first += CAP) groups[gq] = make_int4(first, min(CAP, end - first), key, cpack);
+    if (bid == n_blocks - 1 && threadIdx.x == 0) {
+        const unsigned long long all = s_prefix + s_excl[kMapBlock];
+        off[nkeys] = (int)(all >> 31);
+        *n_groups = (int)(all & FIELD);
+    }
+    // the last block to finish publishes the item count
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        if (atomicAdd(&state->done, 1) == n_blocks - 1) *n_items = ntiles + atomicAdd(&state->extra, 0);
+    }
 }
 
 // dst[id] = src[slot] for every occupied slot (one thread per group); coff != NULL: dst[compact storage index] instead
@@ -902,7 +963,6 @@ __global__ void k_stats_clear_t(DevScalars *sc)
     sc->sum_mom[0] = sc->sum_mom[1] = sc->sum_mom[2] = 0.0;
 }
 
-inline unsigned blocks_for(long long n, int per) { return (unsigned)((n + per - 1) / per); }
 
 // persistent launch: as many blocks as are resident at once (occupancy query), never more than there are chunks
 template <typename Kernel>
@@ -919,15 +979,24 @@ inline unsigned persistent_blocks(long long max_groups, int groups_per_block, Ke
 
 }  // namespace
 
-void launch_build_groups_tiled(const GridDesc &gd, const int *count, const int *off, int *goff, int *scan_aux, int4 *groups,
-                               int *n_groups, cudaStream_t s)
+size_t cell_map_state_bytes(const GridDesc &gd)
 {
-    const int cap = 1 << gd.dim;
-    const int nkeys = (int)gd.Nkeys;
-    k_group_counts_tiled<<<blocks_for(nkeys + 1, kBlock), kBlock, 0, s>>>(count, goff, nkeys, cap);
-    launch_exclusive_scan(goff, nkeys + 1, scan_aux, s);
-    if (gd.dim == 2) k_group_fill_tiled<2><<<blocks_for(nkeys, kBlock), kBlock, 0, s>>>(gd, count, off, goff, groups, n_groups, nkeys);
-    else k_group_fill_tiled<3><<<blocks_for(nkeys, kBlock), kBlock, 0, s>>>(gd, count, off, goff, groups, n_groups, nkeys);
+    const long long n_blocks = (gd.Nkeys + kMapKeys - 1) / kMapKeys;
+    return sizeof(CellMapState) + sizeof(unsigned long long) * (size_t)n_blocks;
+}
+
+void launch_cell_map_tiled(const GridDesc &gd, const int *count, int *off, int4 *groups, int *n_groups, int4 *items, int *n_items,
+                           void *state, cudaStream_t s)
+{
+    long long ntiles = 1;
+    for (int a = 0; a < gd.dim; ++a) ntiles *= gd.ntile[a];
+    const int nkeys = (int)gd.Nkeys, n_blocks = (nkeys + kMapKeys - 1) / kMapKeys;
+    cudaMemsetAsync(state, 0, cell_map_state_bytes(gd), s);
+    CellMapState *st = reinterpret_cast<CellMapState *>(state);
+    if (gd.dim == 2)
+        k_cell_map_tiled<2><<<n_blocks, kMapBlock, 0, s>>>(gd, count, off, groups, n_groups, items, n_items, st, nkeys, (int)ntiles, n_blocks, Chunk<2>::GROUPS);
+    else
+        k_cell_map_tiled<3><<<n_blocks, kMapBlock, 0, s>>>(gd, count, off, groups, n_groups, items, n_items, st, nkeys, (int)ntiles, n_blocks, Chunk<3>::GROUPS);
 }
 
 void launch_p2g1_tiled(const GridDesc &gd, const PArr &p, const GArr &g, const SortedMap &map, long long max_groups, cudaStream_t s)
@@ -937,20 +1006,12 @@ void launch_p2g1_tiled(const GridDesc &gd, const PArr &p, const GArr &g, const S
     else k_p2g1_tiled<3><<<persistent_blocks(max_groups, Geo<3>::GPB, k_p2g1_tiled<3>), kBlock, 0, s>>>(gd, p, g, map);
 }
 
-void launch_build_items(const GridDesc &gd, const int *goff, int4 *items, int *n_items, cudaStream_t s)
-{
-    long long ntiles = 1;
-    for (int a = 0; a < gd.dim; ++a) ntiles *= gd.ntile[a];
-    if (gd.dim == 2) k_build_items<<<1, 1024, 0, s>>>(goff, (int)ntiles, TileGeo<2>::LTC, Chunk<2>::GROUPS, items, n_items);
-    else k_build_items<<<1, 1024, 0, s>>>(goff, (int)ntiles, TileGeo<3>::LTC, Chunk<3>::GROUPS, items, n_items);
-}
-
 long long max_items_tiled(const GridDesc &gd, long long max_groups)
 {
     long long ntiles = 1;
     for (int a = 0; a < gd.dim; ++a) ntiles *= gd.ntile[a];
     const int per = gd.dim == 2 ? Chunk<2>::GROUPS : Chunk<3>::GROUPS;
-    return (ntiles < max_groups ? ntiles : max_groups) + max_groups / per + 1;
+    return ntiles + max_groups / per + 1;      // one item per tile + the further chunks of dense tiles
 }
 
 void launch_g2p_p2g2_tiled(const GridDesc &gd, const PArr &p, const GArr &g, const DevScalars *sc,
