@@ -62,13 +62,38 @@ __device__ __forceinline__ int tiled_key_of_position(const GridDesc &gd, const d
     return tiled_key_of_cell<DIM>(gd, c);
 }
 
+// A dense cell fills whole warps with its groups.  Then the groups' corner totals are added up across the warp first
+// (xor shuffles over the group index) and the first group alone issues the reductions: 32 / LG times fewer fp64
+// reductions on the same 2^d nodes.  Returns whether this lane's group still has to issue them.
+template <int DIM, int NCH>
+__device__ __forceinline__ bool fold_warp_one_cell(double tot[NCH][2], int lane, bool one_cell, bool any)
+{
+    if (!one_cell) return any;
+#pragma unroll
+    for (int m = Geo<DIM>::LG; m < 32; m <<= 1) {
+#pragma unroll
+        for (int ch = 0; ch < NCH; ++ch) {
+            tot[ch][0] += shfl_xor_d(tot[ch][0], m);
+            tot[ch][1] += shfl_xor_d(tot[ch][1], m);
+        }
+    }
+    return lane < Geo<DIM>::LG;      // lane 0's group is never idle unless the whole warp is (then every total is 0)
+}
+
+// warp-uniform: do all groups of this warp (idle ones aside) sit in the same cell?
+__device__ __forceinline__ bool warp_one_cell(int cell, int cnt)
+{
+    const int first = __shfl_sync(kFull, cell, 0);
+    return __all_sync(kFull, cnt == 0 || cell == first);
+}
+
 // Group totals of the P2G#1 channels (m, mv, f) from per-lane payloads and butterfly-order weights, reduced into the node
 // accumulators g.m, g.mv, g.f with one global fp64 reduction per corner and channel (see mpm_kernels_sorted.cu):
 //   pay[i] = { M, M V_a, S } of the lane's particle i, w[i][r] = weight of corner r ^ l (0 for a particle that is not
 //   part of the group reduction).
 template <int DIM>
 __device__ __forceinline__ void scatter_p2g1_group(const GridDesc &gd, const GArr &g, const int c[DIM], int l, bool any,
-                                                   const double pay[2][DIM + 2], const double w[2][1 << DIM])
+                                                   const double pay[2][DIM + 2], const double w[2][1 << DIM], bool one_cell = false)
 {
     constexpr int NB = 1 << DIM, LG = Geo<DIM>::LG;
     double tot[DIM + 2][2];
@@ -81,6 +106,7 @@ __device__ __forceinline__ void scatter_p2g1_group(const GridDesc &gd, const GAr
         tot[ch][0] = v[0];
         tot[ch][1] = v[LG];
     }
+    any = fold_warp_one_cell<DIM, DIM + 2>(tot, threadIdx.x & 31, one_cell, any);
     // forces of corners b_q = l + q LG: f_a = +-(1/h) (T_S(b) + T_S(b ^ bit_a)), + on the high side of axis a
     double F[DIM][2];
 #pragma unroll
@@ -344,55 +370,43 @@ __device__ __forceinline__ bool move_inside(const GridDesc &gd, const double X[D
     return in;
 }
 
-__device__ __forceinline__ double sel3(const double v[], int a, int dim)
-{
-    double r = v[0];
-    if (a == 1) r = v[1];
-    if (dim == 3 && a == 2) r = v[dim - 1];
-    return r;
-}
-__device__ __forceinline__ double *selp(double *const p[3], int a, int dim)
-{
-    double *r = p[0];
-    if (a == 1) r = p[1];
-    if (dim == 3 && a == 2) r = p[dim - 1];
-    return r;
-}
-
-// P2G#1 (eqs. 13, 14, 16, 18) of the particles flagged in `mask` (one bit per lane), done by the WHOLE warp: the
-// particle's data is broadcast, lane (corner b = lane % 2^d, q = lane / 2^d) adds the channels q, q + 32 / 2^d, ... of
-// corner b (channels: m, mv_a, f_a).  Used for particles that leave their group's cell (their contributions cannot
-// join the group's butterfly): 2 warp instructions instead of 2^d (1 + 2 d) per particle.
+// P2G#1 (eqs. 13, 14, 16, 18) of the particles flagged in `mask` (one bit per lane), done by the WHOLE warp, 32 / 2^d
+// particles per round: lane (slot = lane / 2^d, corner b = lane % 2^d) gets the data of the slot's particle by shuffle
+// and adds its 1 + 2 d channels (m, mv_a, f_a) to corner b.  Used for particles that leave their group's cell (their
+// contributions cannot join the group's butterfly).
 template <int DIM>
 __device__ __forceinline__ void coop_p2g1(const GridDesc &gd, const GArr &gn, unsigned mask, const double Xn[DIM],
                                           const double Vn[DIM], double Mn, double Sn, int lane)
 {
-    constexpr int NB = 1 << DIM, NQ = 32 / NB, NCH = 1 + 2 * DIM;
-    const int b = lane & (NB - 1), q = lane / NB;
+    constexpr int NB = 1 << DIM, SLOTS = 32 / NB;
+    const int b = lane & (NB - 1), slot = lane / NB;
     while (mask) {
-        const int src = __ffs(mask) - 1;
-        mask &= mask - 1;
+        int src = -1;
+#pragma unroll
+        for (int s = 0; s < SLOTS; ++s) {      // the slot's particle = the s-th flagged lane (mask is warp-uniform)
+            const int f = mask ? __ffs(mask) - 1 : -1;
+            if (s == slot) src = f;
+            mask &= mask - 1u;
+        }
+        const int from = src < 0 ? 0 : src;
         double X[DIM], V[DIM];
 #pragma unroll
         for (int a = 0; a < DIM; ++a) {
-            X[a] = __shfl_sync(kFull, Xn[a], src);
-            V[a] = __shfl_sync(kFull, Vn[a], src);
+            X[a] = __shfl_sync(kFull, Xn[a], from);
+            V[a] = __shfl_sync(kFull, Vn[a], from);
         }
-        const double M = __shfl_sync(kFull, Mn, src), S = __shfl_sync(kFull, Sn, src);
-        int c[DIM];
-        double xi[DIM];
-        particle_cell<DIM>(gd, X, c, xi);
-        const long long node = corner_node<DIM>(gd, c, b);
-        const double phi = corner_phi<DIM>(xi, b);
+        const double M = __shfl_sync(kFull, Mn, from), S = __shfl_sync(kFull, Sn, from);
+        if (src >= 0) {
+            int c[DIM];
+            double xi[DIM];
+            particle_cell<DIM>(gd, X, c, xi);
+            const long long node = corner_node<DIM>(gd, c, b);
+            const double Mphi = M * corner_phi<DIM>(xi, b);
+            atomicAdd(gn.m + node, Mphi);
 #pragma unroll
-        for (int it = 0; it < (NCH + NQ - 1) / NQ; ++it) {
-            const int ch = q + it * NQ;
-            if (ch == 0) {
-                atomicAdd(gn.m + node, M * phi);
-            } else if (ch <= DIM) {
-                atomicAdd(selp(gn.mv, ch - 1, DIM) + node, M * sel3(V, ch - 1, DIM) * phi);
-            } else if (ch < NCH) {
-                atomicAdd(selp(gn.f, ch - 1 - DIM, DIM) + node, S * corner_dphi<DIM>(xi, b, ch - 1 - DIM, gd.inv_h));
+            for (int a = 0; a < DIM; ++a) {
+                atomicAdd(gn.mv[a] + node, V[a] * Mphi);
+                atomicAdd(gn.f[a] + node, S * corner_dphi<DIM>(xi, b, a, gd.inv_h));
             }
         }
     }
@@ -496,10 +510,16 @@ __global__ void __launch_bounds__(kTB, kTBMinG) k_g2p_p2g2_tiled(GridDesc gd, PA
         // ranks among the particles that end up in the same cell (arrival order of the atomics, A17): issue the atomics
         const bool stay[2] = { valid[0] && key[0] == grp.cell, valid[1] && key[1] == grp.cell };
         const unsigned gmask = (1u << LG) - 1u;
-        const unsigned g0 = (__ballot_sync(kFull, stay[0]) >> sh) & gmask, g1 = (__ballot_sync(kFull, stay[1]) >> sh) & gmask;
+        const unsigned b0 = __ballot_sync(kFull, stay[0]), b1 = __ballot_sync(kFull, stay[1]);
+        const unsigned g0 = (b0 >> sh) & gmask, g1 = (b1 >> sh) & gmask;
         const int nstay = __popc(g0) + __popc(g1);
         int base = 0, rank_m[2] = { 0, 0 };
-        if (l == 0 && nstay > 0) base = atomicAdd(&count[grp.cell], nstay);
+        // a dense cell fills whole warps with its groups: then ONE atomic serves the warp (the groups' shares follow
+        // from the ballots), instead of one per group on the same counter
+        const bool one_cell = warp_one_cell(grp.cell, grp.cnt);
+        if (one_cell) {
+            if (lane == 0 && (b0 | b1)) base = atomicAdd(&count[grp.cell], __popc(b0) + __popc(b1));
+        } else if (l == 0 && nstay > 0) base = atomicAdd(&count[grp.cell], nstay);
 #pragma unroll
         for (int i = 0; i < 2; ++i)
             if (valid[i] && !stay[i]) rank_m[i] = atomicAdd(&count[key[i]], 1);
@@ -518,7 +538,7 @@ __global__ void __launch_bounds__(kTB, kTBMinG) k_g2p_p2g2_tiled(GridDesc gd, PA
                 tot[a][0] = v[0];
                 tot[a][1] = v[LG];
             }
-            if (grp.cnt > 0) {
+            if (fold_warp_one_cell<DIM, DIM>(tot, lane, one_cell, grp.cnt > 0)) {
 #pragma unroll
                 for (int q = 0; q < 2; ++q) {
                     const int node = corner_node_i<DIM>(gd, c, l + q * LG);
@@ -528,7 +548,8 @@ __global__ void __launch_bounds__(kTB, kTBMinG) k_g2p_p2g2_tiled(GridDesc gd, PA
             }
         }
         // ... and only now use what they returned
-        base = __shfl_sync(kFull, base, sh);
+        if (one_cell) base = __shfl_sync(kFull, base, 0) + __popc(b0 & ((1u << sh) - 1u)) + __popc(b1 & ((1u << sh) - 1u));
+        else base = __shfl_sync(kFull, base, sh);
         const unsigned lower = (1u << l) - 1u;
         const int pre = base + __popc(g0 & lower) + __popc(g1 & lower);
         const int rank0 = stay[0] ? pre : rank_m[0], rank1 = stay[1] ? pre + (int)((g0 >> l) & 1u) : rank_m[1];
@@ -754,7 +775,7 @@ __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr
 #pragma unroll
             for (int a = 0; a < DIM; ++a) pay[i][1 + a] = stay[i] ? Mo[i] * Vo[i][a] : 0.0;
         }
-        scatter_p2g1_group<DIM>(gd, gn, c, l, grp.cnt > 0, pay, wn);
+        scatter_p2g1_group<DIM>(gd, gn, c, l, grp.cnt > 0, pay, wn, warp_one_cell(grp.cell, grp.cnt));
         grp = nxt;
         nxt = nn;
     }
