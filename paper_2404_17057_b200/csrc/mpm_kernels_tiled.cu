@@ -49,6 +49,8 @@ __device__ __forceinline__ void cp_async8(void *smem, const void *gmem)
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+// all committed groups but the most recent one have landed
+__device__ __forceinline__ void cp_async_wait_but_one() { asm volatile("cp.async.wait_group 1;" ::: "memory"); }
 
 template <int DIM>
 __device__ __forceinline__ int tiled_key_of_position(const GridDesc &gd, const double X[DIM])
@@ -258,40 +260,58 @@ template <int DIM, int CH, bool WITH_V2>
 __device__ __forceinline__ void stage_tile(const GridDesc &gd, const int org[DIM], const GArr &g, double dt, double *s_tile)
 {
     using TG = TileGeo<DIM>;
-    for (int j = threadIdx.x; j < TG::NN; j += kTB) {
-        int idx[DIM];
-        const int node = tile_node_global<DIM>(gd, org, j, idx);
+    constexpr int BATCH = WITH_V2 ? 2 : 4;              // measured: the update kernel has no registers to spare for 4
+    constexpr int NALL = (TG::NN + kTB - 1) / kTB;      // nodes per thread
+    constexpr int NIT = NALL < BATCH ? NALL : BATCH;    // ... loaded together
+    for (int j0 = 0; j0 < TG::NN; j0 += NIT * kTB) {
+    // the loads of NIT nodes are issued before the first one is used (fewer exposed memory latencies per tile)
+    int node[NIT], idx[NIT][DIM];
+    double m[NIT], mv[NIT][DIM], f[NIT][DIM], mv2[NIT][DIM];
+#pragma unroll
+    for (int it = 0; it < NIT; ++it) {
+        const int j = j0 + threadIdx.x + it * kTB;
+        node[it] = (j < TG::NN) ? tile_node_global<DIM>(gd, org, j, idx[it]) : -1;
+        m[it] = 0.0;
+#pragma unroll
+        for (int a = 0; a < DIM; ++a) { mv[it][a] = 0.0; f[it][a] = 0.0; mv2[it][a] = 0.0; }
+        if (node[it] >= 0) {
+            m[it] = __ldg(g.m + node[it]);
+#pragma unroll
+            for (int a = 0; a < DIM; ++a) { mv[it][a] = __ldg(g.mv[a] + node[it]); f[it][a] = __ldg(g.f[a] + node[it]); }
+            if (WITH_V2) {
+#pragma unroll
+                for (int a = 0; a < DIM; ++a) mv2[it][a] = __ldg(g.mv2[a] + node[it]);
+            }
+        }
+    }
+#pragma unroll
+    for (int it = 0; it < NIT; ++it) {
+        const int j = j0 + threadIdx.x + it * kTB;
+        if (j >= TG::NN) break;
         double v[CH];
 #pragma unroll
         for (int q = 0; q < CH; ++q) v[q] = 0.0;
-        if (node >= 0) {
-            const double m = __ldg(g.m + node);
-            double mv[DIM], f[DIM], mv2[DIM];
+        if (node[it] >= 0) {
+            apply_bc<DIM, true>(gd, g, node[it], idx[it], m[it], mv[it], f[it]);
+            const double inv = (m[it] != 0.0) ? 1.0 / m[it] : 0.0;
 #pragma unroll
-            for (int a = 0; a < DIM; ++a) { mv[a] = __ldg(g.mv[a] + node); f[a] = __ldg(g.f[a] + node); }
-            if (WITH_V2) {
-#pragma unroll
-                for (int a = 0; a < DIM; ++a) mv2[a] = __ldg(g.mv2[a] + node);
-            }
-            apply_bc<DIM, true>(gd, g, node, idx, m, mv, f);
-            const double inv = (m != 0.0) ? 1.0 / m : 0.0;
-#pragma unroll
-            for (int a = 0; a < DIM; ++a) v[a] = (mv[a] + dt * f[a]) * inv;
+            for (int a = 0; a < DIM; ++a) v[a] = (mv[it][a] + dt * f[it][a]) * inv;
             if (WITH_V2) {
                 double none[DIM];
 #pragma unroll
                 for (int a = 0; a < DIM; ++a) none[a] = 0.0;
-                apply_bc<DIM, false>(gd, g, node, idx, m, mv2, none);
+                apply_bc<DIM, false>(gd, g, node[it], idx[it], m[it], mv2[it], none);
 #pragma unroll
-                for (int a = 0; a < DIM; ++a) v[DIM + a] = mv2[a] * inv;
+                for (int a = 0; a < DIM; ++a) v[DIM + a] = mv2[it][a] * inv;
             } else {
 #pragma unroll
-                for (int a = 0; a < DIM; ++a) v[DIM + a] = f[a] * inv;
+                for (int a = 0; a < DIM; ++a) v[DIM + a] = f[it][a] * inv;
             }
         }
         double2 *dst = reinterpret_cast<double2 *>(s_tile + j * CH);
 #pragma unroll
         for (int q = 0; q < CH / 2; ++q) dst[q] = make_double2(v[2 * q], v[2 * q + 1]);
+    }
     }
 }
 
@@ -439,19 +459,26 @@ __global__ void __launch_bounds__(kTB, kTBMinG) k_g2p_p2g2_tiled(GridDesc gd, PA
     int gl = threadIdx.x / LG;
     Group grp = fetch_group(map.groups, (long long)item.y + gl, g_end);
     Group nxt = fetch_group(map.groups, (long long)item.y + gl + GPB, g_end);
-    auto issue = [&](const Group &gr) {
+    // two copy groups per pass: X (needed first, refilled as soon as it has been read: a whole pass of lead time) and V, M
+    auto issue_x = [&](const Group &gr) {
         if (2 * l < gr.cnt) {
             const long long k0 = (long long)gr.first + 2 * l;
 #pragma unroll
-            for (int a = 0; a < DIM; ++a) {
-                cp_async16(&s_pf[a][threadIdx.x], p.x[a] + k0);
-                cp_async16(&s_pf[DIM + a][threadIdx.x], p.v[a] + k0);
-            }
+            for (int a = 0; a < DIM; ++a) cp_async16(&s_pf[a][threadIdx.x], p.x[a] + k0);
+        }
+        cp_async_commit();
+    };
+    auto issue_vm = [&](const Group &gr) {
+        if (2 * l < gr.cnt) {
+            const long long k0 = (long long)gr.first + 2 * l;
+#pragma unroll
+            for (int a = 0; a < DIM; ++a) cp_async16(&s_pf[DIM + a][threadIdx.x], p.v[a] + k0);
             cp_async16(&s_pf[2 * DIM][threadIdx.x], p.m + k0);
         }
         cp_async_commit();
     };
-    issue(grp);
+    issue_x(grp);
+    issue_vm(grp);
     int org[DIM];
     tile_origin<DIM>(gd, item.x, org);
     const double dt = sc->dt;
@@ -466,23 +493,29 @@ __global__ void __launch_bounds__(kTB, kTBMinG) k_g2p_p2g2_tiled(GridDesc gd, PA
         const bool valid[2] = { 2 * l < grp.cnt, 2 * l + 1 < grp.cnt };
         const long long k0 = (long long)grp.first + 2 * l;
         double X[2][DIM], V[2][DIM], M[2];
-        cp_async_wait_all();
+        cp_async_wait_but_one();                      // this pass's X has landed (its V, M may still be in flight)
 #pragma unroll
         for (int a = 0; a < DIM; ++a) {
-            const double2 tx = s_pf[a][threadIdx.x], tv = s_pf[DIM + a][threadIdx.x];
+            const double2 tx = s_pf[a][threadIdx.x];
             X[0][a] = valid[0] ? tx.x : 0.0; X[1][a] = valid[1] ? tx.y : 0.0;
+        }
+        issue_x(nxt);                                 // the slots have been read: refill them for the next pass
+        const Group nn = fetch_group(map.groups, (long long)item.y + gl + 2 * GPB, g_end);
+        double W[2][DIM][2], xi[2][DIM], out[2][2 * DIM], Dh[2];
+#pragma unroll
+        for (int i = 0; i < 2; ++i) weights_1d<DIM>(gd, X[i], c, xi[i], W[i]);
+        gather_tile<DIM, CH, false>(s_tile + j0 * CH, W, out, Dh);
+        cp_async_wait_but_one();                      // this pass's V, M have landed (the next X may still be in flight)
+#pragma unroll
+        for (int a = 0; a < DIM; ++a) {
+            const double2 tv = s_pf[DIM + a][threadIdx.x];
             V[0][a] = valid[0] ? tv.x : 0.0; V[1][a] = valid[1] ? tv.y : 0.0;
         }
         {
             const double2 tm = s_pf[2 * DIM][threadIdx.x];
             M[0] = valid[0] ? tm.x : 0.0; M[1] = valid[1] ? tm.y : 0.0;
         }
-        issue(nxt);                                   // the slots have been read: refill them for the next pass
-        const Group nn = fetch_group(map.groups, (long long)item.y + gl + 2 * GPB, g_end);
-        double W[2][DIM][2], xi[2][DIM], out[2][2 * DIM], Dh[2];
-#pragma unroll
-        for (int i = 0; i < 2; ++i) weights_1d<DIM>(gd, X[i], c, xi[i], W[i]);
-        gather_tile<DIM, CH, false>(s_tile + j0 * CH, W, out, Dh);
+        issue_vm(nxt);
         double MV[2][DIM];
         int key[2];
 #pragma unroll
@@ -604,23 +637,31 @@ __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr
     int gl = threadIdx.x / LG;
     Group grp = fetch_group(map.groups, (long long)item.y + gl, g_end);
     Group nxt = fetch_group(map.groups, (long long)item.y + gl + GPB, g_end);
-    auto issue = [&](const Group &gr) {
+    // two copy groups per pass: X and the destination record (needed first, refilled as soon as they have been read: a
+    // whole pass of lead time) and the fields that are only needed after the gather
+    auto issue_x = [&](const Group &gr) {
         if (2 * l < gr.cnt) {
             const long long k0 = (long long)gr.first + 2 * l;
 #pragma unroll
-            for (int a = 0; a < DIM; ++a) {
-                cp_async16(&s_pf[a][threadIdx.x], p.x[a] + k0);
-                cp_async16(&s_pf[DIM + a][threadIdx.x], p.v[a] + k0);
-            }
+            for (int a = 0; a < DIM; ++a) cp_async16(&s_pf[a][threadIdx.x], p.x[a] + k0);
+            cp_async16(&s_dest[threadIdx.x], dest + k0);
+        }
+        cp_async_commit();
+    };
+    auto issue_rest = [&](const Group &gr) {
+        if (2 * l < gr.cnt) {
+            const long long k0 = (long long)gr.first + 2 * l;
+#pragma unroll
+            for (int a = 0; a < DIM; ++a) cp_async16(&s_pf[DIM + a][threadIdx.x], p.v[a] + k0);
             cp_async16(&s_pf[2 * DIM][threadIdx.x], p.m + k0);
             cp_async16(&s_pf[2 * DIM + 1][threadIdx.x], p.rho + k0);
             cp_async16(&s_pf[2 * DIM + 2][threadIdx.x], p.e + k0);
-            cp_async16(&s_dest[threadIdx.x], dest + k0);
             cp_async8(&s_id[threadIdx.x], p.id + k0);
         }
         cp_async_commit();
     };
-    issue(grp);
+    issue_x(grp);
+    issue_rest(grp);
     int org[DIM];
     tile_origin<DIM>(gd, item.x, org);
     const double dt = sc->dt;
@@ -639,7 +680,7 @@ __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr
         double X[2][DIM];
         int key[2];
         long long dst[2] = { -1, -1 };
-        cp_async_wait_all();
+        cp_async_wait_but_one();                      // this pass's X and destination records have landed
         {   // l.12: slot of the particle in the other buffer = offset of its new cell + its rank there; the offset load
             // is issued first so that it overlaps the gather
             const ulonglong2 td = s_dest[threadIdx.x];
@@ -653,12 +694,13 @@ __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr
             const double2 tx = s_pf[a][threadIdx.x];
             X[0][a] = valid[0] ? tx.x : 0.0; X[1][a] = valid[1] ? tx.y : 0.0;
         }
+        issue_x(nxt);                                 // the slots have been read: refill them for the next pass
         double W[2][DIM][2], xi[2][DIM], out[2][2 * DIM], Dh[2];
 #pragma unroll
         for (int i = 0; i < 2; ++i) weights_1d<DIM>(gd, X[i], c, xi[i], W[i]);
         gather_tile<DIM, CH, true>(s_tile + j0 * CH, W, out, Dh);
         // the fields that are only needed from here on stay in shared memory during the gather (register budget)
-        asm volatile("" ::: "memory");
+        cp_async_wait_but_one();                      // ... they have landed (the next X may still be in flight)
         double V[2][DIM], M[2], rho[2], E[2];
         int id[2];
 #pragma unroll
@@ -674,7 +716,7 @@ __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr
             const int2 ti = s_id[threadIdx.x];
             id[0] = ti.x; id[1] = ti.y;
         }
-        issue(nxt);                                   // the slots have been read: refill them for the next pass
+        issue_rest(nxt);
         const Group nn = fetch_group(map.groups, (long long)item.y + gl + 2 * GPB, g_end);
         // per particle: the new state (what goes to memory), S' for the next step's force, and whether it stays in the
         // group's cell.  Straight-line code for both particles of the lane (an unused slot computes on M = 0, rho = 1,
