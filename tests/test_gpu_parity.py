@@ -23,6 +23,8 @@ def small_workloads():
         "cylinder": lambda: inputs.cylinder(nx=200, ny=100),
         "sedov": lambda: inputs.sedov(n=20),
         "clumps": lambda: inputs.clumps(n=20, num_particles=150_001),     # odd particle count
+        # thousands of particles per cell: whole warps of groups in ONE cell (warp-folded reductions, shared rank atomics)
+        "clumps_dense": lambda: inputs.clumps(n=16, num_particles=200_001, nclumps=3, sigma_cells=1.0),
     }
 
 
@@ -79,7 +81,7 @@ def test_one_step_grid_parity(po, mpm, name, mode):
     assert so.n_recycled == sg.n_recycled and so.n_clamped == sg.n_clamped
 
 
-STEPS = {"sod": 100, "box": 100, "box_shuffled": 100, "cylinder": 100, "sedov": 100, "clumps": 50}
+STEPS = {"sod": 100, "box": 100, "box_shuffled": 100, "cylinder": 100, "sedov": 100, "clumps": 50, "clumps_dense": 30}
 
 
 @pytest.mark.parametrize("mode", MODES + [(3, 1)])
@@ -109,6 +111,55 @@ def test_many_step_particle_parity(po, mpm, name, mode):
         if w["cfg"]["bc"][a][0] == 0:
             dx[a] = np.minimum(dx[a], L[a] - dx[a])
     assert dx.sum() <= PART_TOL * np.abs(x).sum(), name
+
+
+@pytest.mark.parametrize("name", ["sedov", "clumps"])
+def test_full_size_properties(mpm, name):
+    """BASELINE.json configs 4 and 5 at full size in the launch configuration bench.py times (TILED family, re-ordering
+    every step): properties that hold at any size.  Exact conservation of mass (M_k untouched, sum_i m_i = sum_k M_k:
+    PAPER.md:205, partition of unity), sum_i f_i = 0 and sum_i mv_i = sum_k M_k V_k in the periodic box (PAPER.md:200,
+    :224), the CFL identity dt_next (v_max + c_max) = alpha h (eq. 25/29) with exact maxima, ids a permutation, storage
+    order cell-sorted."""
+    w = inputs.sedov() if name == "sedov" else inputs.clumps()
+    cfg, d, h = w["cfg"], w["cfg"]["dim"], w["cfg"]["dx"]
+    n = w["mass"].shape[0]
+    g = mpm.Solver(cfg, sort_every=1, variant=mpm.VARIANT_TILED)
+    g.load_particles(w["x"], w["v"], w["mass"], w["rho"], w["e"])
+    nsteps = 3
+    g.step(0.0, w["cfl"], nsteps)
+    st = g.stats()
+    assert st.step == nsteps and st.n_nonfinite == 0 and st.n_negjac == 0
+    assert abs(st.dt_next * (st.vmax + st.cmax) / h - w["cfl"]) <= 4e-16 * 8
+    msum = float(np.sum(w["mass"], dtype=np.longdouble))
+    gm = g.read_grid(mpm.G_MASS)
+    assert abs(float(np.sum(gm, dtype=np.longdouble)) - msum) <= 1e-12 * msum
+    assert abs(st.sum_mass - msum) <= 1e-12 * msum
+    gf = g.read_grid(mpm.G_FORCE)
+    gmom = g.read_grid(mpm.G_MOMENTUM2)
+    if name == "clumps":            # periodic box: no boundary node takes momentum or force out
+        fabs = float(np.abs(gf).sum())
+        for a in range(d):
+            assert abs(float(np.sum(gf[a], dtype=np.longdouble))) <= 1e-12 * fabs
+    p = g.read_particles()
+    np.testing.assert_array_equal(p["mass"], w["mass"])                      # M_k never changes, ids intact
+    if name == "clumps":
+        mom = (p["mass"][None, :] * p["v"]).sum(axis=1, dtype=np.longdouble)
+        scale = float(np.abs(p["mass"][None, :] * p["v"]).sum())
+        for a in range(d):
+            assert abs(float(np.sum(gmom[a], dtype=np.longdouble)) - float(mom[a])) <= 1e-11 * scale
+    vmax = float(np.sqrt((p["v"] ** 2).sum(axis=0)).max())
+    cmax = float(np.sqrt(cfg["gamma"] * (cfg["gamma"] - 1.0) * p["e"]).max())
+    assert st.vmax >= vmax * (1 - 1e-15) and abs(st.cmax - cmax) <= 1e-14 * cmax
+    assert np.isfinite(p["rho"]).all() and (p["rho"] > 0).all() and np.isfinite(p["e"]).all()
+    del p
+    s = g.read_particles(order=1)                                            # storage order: cell-sorted, tile-major
+    c = np.clip(np.floor(s["x"] / h).astype(np.int64), 0, np.array(cfg["n"][:d])[:, None] - 1)
+    t = (8, 8, 4)
+    nt = [-(-cfg["n"][a] // t[a]) for a in range(d)]
+    tile = (c[0] // t[0]) + nt[0] * ((c[1] // t[1]) + nt[1] * (c[2] // t[2]))
+    local = (c[0] % t[0]) + t[0] * ((c[1] % t[1]) + t[1] * (c[2] % t[2]))
+    key = tile * (t[0] * t[1] * t[2]) + local
+    assert s["mass"].shape[0] == n and (np.diff(key) >= 0).all()
 
 
 def test_reordering_does_not_change_results(mpm):
