@@ -32,7 +32,10 @@ struct mpm_handle {
     int *coff;            // TILED: compact storage offsets, allocated on the first storage-order read
     // TILED: the node accumulators m, mv, f are double-buffered: the update kernel of step n already scatters P2G#1 of
     // step n+1 into the other set.  acc[acur] = the set the current / next mpm_step starts from (raw P2G#1).
-    double *acc_m[2], *acc_mv[2][3], *acc_f[2][3];
+    double *acc_m[2], *acc_mv[2][3], *acc_f[2][3], *acc_mv2[2][3];
+    // TILED: the next step's accumulator set is cleared on a second stream while the gather kernel runs
+    cudaStream_t side;
+    cudaEvent_t ev_fork, ev_join;
     int acur;
     bool grid_final;      // TILED: the last step's m, mv, f, mv2 have been brought to their post-BC form for mpm_read_grid
     long long slots;      // TILED: allocated slots per particle array (particles + one spare slot per odd cell)
@@ -286,7 +289,7 @@ GArr tiled_acc(const mpm_handle *h, int which)
 {
     GArr g = h->g;
     g.m = h->acc_m[which];
-    for (int a = 0; a < 3; ++a) { g.mv[a] = h->acc_mv[which][a]; g.f[a] = h->acc_f[which][a]; }
+    for (int a = 0; a < 3; ++a) { g.mv[a] = h->acc_mv[which][a]; g.f[a] = h->acc_f[which][a]; g.mv2[a] = h->acc_mv2[which][a]; }
     return g;
 }
 
@@ -307,6 +310,7 @@ void reorder(mpm_handle *h)
         h->acur = 0;
         GArr g0 = tiled_acc(h, 0);
         launch_grid_clear(h->gd, g0, h->stream);
+        for (int a = 0; a < h->gd.dim; ++a) cudaMemsetAsync(g0.mv2[a], 0, sizeof(double) * (size_t)h->gd.Nn, h->stream);
         launch_p2g1_tiled(h->gd, dst, g0, SortedMap{ h->groups, h->n_groups, h->goff }, h->max_groups, h->stream);
         h->launches += 6;
         return;
@@ -369,8 +373,13 @@ void step_tiled(mpm_handle *h, bool last_of_call)
     {
         Timed t(h, MPM_K_MISC);
         launch_begin_step(h->sc, gd.h, s);                                                // dt (eq. 25/29)
-        launch_grid_clear(gd, gnx, s);                                                    // l.2 for the next step's l.3
-        for (int a = 0; a < gd.dim; ++a) cudaMemsetAsync(h->g.mv2[a], 0, sizeof(double) * (size_t)gd.Nn, s);   // ... and for l.8
+        // l.2 for the next step: its accumulator set (m, mv, f for l.3, mv2 for l.8; last read by the previous step's
+        // update kernel) is cleared on the second stream while this step's gather kernel runs
+        cudaEventRecord(h->ev_fork, s);
+        cudaStreamWaitEvent(h->side, h->ev_fork, 0);
+        launch_grid_clear(gd, gnx, h->side);
+        for (int a = 0; a < gd.dim; ++a) cudaMemsetAsync(gnx.mv2[a], 0, sizeof(double) * (size_t)gd.Nn, h->side);
+        cudaEventRecord(h->ev_join, h->side);
         cudaMemsetAsync(h->count, 0, sizeof(int) * (size_t)(gd.Nkeys + 1), s);            // per-cell counters of l.12
     }
     // l.4-5 and l.9 (BC, obstacle, mv' = mv + dt f, the quotients by m) have no kernel of their own: the two particle
@@ -379,6 +388,7 @@ void step_tiled(mpm_handle *h, bool last_of_call)
       launch_g2p_p2g2_tiled(gd, p, gc, h->sc, map, h->items, h->n_items, h->max_items, h->count, h->dest, s); }          // l.4-8
     { Timed t(h, MPM_K_SORT);                                                         // l.12: offsets, next step's groups and work items
       launch_cell_map_tiled(gd, h->count, h->off[0], h->groups_alt, h->n_groups_alt, h->items_alt, h->n_items_alt, h->map_state, s); }
+    cudaStreamWaitEvent(s, h->ev_join, 0);
     { Timed t(h, MPM_K_UPDATE);
       launch_update_tiled(gd, p, q, gc, h->sc, map, h->items, h->n_items, h->max_items, h->off[0], h->dest, gnx, last_of_call, s); }   // l.9-12, next l.3
     { Timed t(h, MPM_K_MISC); launch_end_step(h->sc, gd.h, s); }                                                   // l.13-14
@@ -429,6 +439,13 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
     if (!h) return fail(nullptr, MPM_E_OOM, "mpm_create: host allocation failed");
     h->cfg = *cfg;
     h->stream = (cudaStream_t)cfg->stream;
+    h->side = nullptr; h->ev_fork = h->ev_join = nullptr;
+    if (cudaStreamCreateWithFlags(&h->side, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming) != cudaSuccess) {
+        delete h;
+        return fail(nullptr, MPM_E_CUDA, "mpm_create: cannot create the second stream");
+    }
     h->cur = 0; h->n = h->cap = 0; h->launches = 0; h->steps_done = 0;
     h->profiling = false;
     for (int k = 0; k < MPM_K_COUNT; ++k) { h->kernel_ms[k] = 0.0; h->kernel_calls[k] = 0; }
@@ -516,11 +533,13 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
     }
     h->acur = 0; h->grid_final = true;
     h->acc_m[0] = h->g.m; h->acc_m[1] = nullptr;
+    for (int a = 0; a < 3; ++a) { h->acc_mv2[0][a] = h->g.mv2[a]; h->acc_mv2[1][a] = nullptr; }
     for (int a = 0; a < 3; ++a) { h->acc_mv[0][a] = h->g.mv[a]; h->acc_f[0][a] = h->g.f[a]; h->acc_mv[1][a] = h->acc_f[1][a] = nullptr; }
     if (ok && tiled) {
         ok = dev_alloc_t(h, &h->acc_m[1], (size_t)gd.Nn);
         for (int a = 0; a < gd.dim && ok; ++a)
-            ok = dev_alloc_t(h, &h->acc_mv[1][a], (size_t)gd.Nn) && dev_alloc_t(h, &h->acc_f[1][a], (size_t)gd.Nn);
+            ok = dev_alloc_t(h, &h->acc_mv[1][a], (size_t)gd.Nn) && dev_alloc_t(h, &h->acc_f[1][a], (size_t)gd.Nn) &&
+                 dev_alloc_t(h, &h->acc_mv2[1][a], (size_t)gd.Nn);
     }
     if (ok && sorted && !tiled)   // node-major node velocities; the TILED kernels form them per tile in shared memory
         ok = dev_alloc_t(h, &h->g.na, (size_t)gd.Nn * 2 * gd.dim) && dev_alloc_t(h, &h->g.nb, (size_t)gd.Nn * gd.dim);
@@ -567,6 +586,7 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
     for (int a = 0; a < gd.dim && tiled && e == cudaSuccess; ++a) {
         e = cudaMemsetAsync(h->acc_mv[1][a], 0, sizeof(double) * (size_t)gd.Nn, h->stream);
         if (e == cudaSuccess) e = cudaMemsetAsync(h->acc_f[1][a], 0, sizeof(double) * (size_t)gd.Nn, h->stream);
+        if (e == cudaSuccess) e = cudaMemsetAsync(h->acc_mv2[1][a], 0, sizeof(double) * (size_t)gd.Nn, h->stream);
     }
     if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
     if (e != cudaSuccess) {
@@ -584,6 +604,9 @@ void mpm_destroy(mpm_handle *h)
     drain_spans(h);
     cudaStreamSynchronize(h->stream);
     for (cudaEvent_t e : h->event_pool) cudaEventDestroy(e);
+    if (h->side) { cudaStreamSynchronize(h->side); cudaStreamDestroy(h->side); }
+    if (h->ev_fork) cudaEventDestroy(h->ev_fork);
+    if (h->ev_join) cudaEventDestroy(h->ev_join);
     std::vector<void *> all = h->allocations;
     for (void *p : all) dev_free(h, p);
     delete h;
@@ -615,12 +638,32 @@ int mpm_load_particles(mpm_handle *h, int64_t n, const double *const *x, const d
     if (rc != MPM_OK) return rc;
     if (q) { rc = copy_in(h, p.q, q, n, ptr_location); if (rc != MPM_OK) return rc; }
     else MPM_CUDA(h, cudaMemsetAsync(p.q, 0, sizeof(double) * (size_t)(n > 0 ? n : 1), h->stream));
+    h->gd.uniform_mass = 0;
+    h->gd.um = 0.0;
+    if (h->variant == MPM_VARIANT_TILED && n > 0) {
+        // equal particle masses (configs 4 and 5; with an inflow face the recycled mass must be the same too): the sweeps
+        // then neither read nor write the mass array -- 24 B per particle and step less
+        struct { int differs; int pad; double first; } probe = { 0, 0, 0.0 };
+        MPM_CUDA(h, cudaMemsetAsync(h->n_items_alt, 0, sizeof(int), h->stream));      // free until the first step
+        launch_mass_differs(p.m, n, h->n_items_alt, h->stream);
+        MPM_CUDA(h, cudaMemcpyAsync(&probe.differs, h->n_items_alt, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+        MPM_CUDA(h, cudaMemcpyAsync(&probe.first, p.m, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+        MPM_CUDA(h, cudaStreamSynchronize(h->stream));
+        const bool inflow_ok = h->gd.in_axis < 0 || h->gd.inflow_mass == probe.first;
+        if (!probe.differs && inflow_ok) { h->gd.uniform_mass = 1; h->gd.um = probe.first; }
+        h->launches += 1;
+    }
     launch_iota(p.id, n, h->stream);
     MPM_CUDA(h, cudaMemsetAsync(h->sc, 0, sizeof(DevScalars), h->stream));
     launch_initial_cfl(h->gd, p, h->sc, n, h->stream);
     h->launches += 3;
     h->steps_done = 0;
     if ((h->cfg.sort_every > 0 || h->variant != MPM_VARIANT_ATOMIC) && n > 0) reorder(h);
+    if (h->gd.uniform_mass) {      // every slot of both buffers holds the mass: nothing moves it any more
+        launch_fill(h->pbuf[0].m, h->slots, h->gd.um, h->stream);
+        launch_fill(h->pbuf[1].m, h->slots, h->gd.um, h->stream);
+        h->launches += 2;
+    }
     MPM_CUDA(h, cudaGetLastError());
     if (ptr_location == MPM_HOST) MPM_CUDA(h, cudaStreamSynchronize(h->stream));   // caller may reuse its buffers
     return MPM_OK;
@@ -736,7 +779,7 @@ int mpm_read_grid(mpm_handle *h, int field, double *out, int ptr_location)
     case MPM_G_MASS: rc = copy_out(h, out, gl.m, gd.Nn, ptr_location); break;
     case MPM_G_MOMENTUM: for (int a = 0; a < gd.dim && rc == MPM_OK; ++a) rc = copy_out(h, out + a * Nn, gl.mv[a], gd.Nn, ptr_location); break;
     case MPM_G_FORCE: for (int a = 0; a < gd.dim && rc == MPM_OK; ++a) rc = copy_out(h, out + a * Nn, gl.f[a], gd.Nn, ptr_location); break;
-    case MPM_G_MOMENTUM2: for (int a = 0; a < gd.dim && rc == MPM_OK; ++a) rc = copy_out(h, out + a * Nn, h->g.mv2[a], gd.Nn, ptr_location); break;
+    case MPM_G_MOMENTUM2: for (int a = 0; a < gd.dim && rc == MPM_OK; ++a) rc = copy_out(h, out + a * Nn, gl.mv2[a], gd.Nn, ptr_location); break;
     case MPM_G_NORMAL:
     case MPM_G_FLAG: {
         const int nc = field == MPM_G_NORMAL ? gd.dim : 1;

@@ -34,6 +34,10 @@ struct GridDesc {
     int tiled;
     int ntile[3];
     long long Nkeys;
+    // TILED: every loaded particle has the same mass (bit for bit; with an inflow face, the recycled mass too): the
+    // kernels then take M from here and neither read nor write the mass array (it stays filled with this value)
+    int uniform_mass;
+    double um;
 };
 
 // TILED family: the grid is cut into tiles of T0 x T1 (x T2) cells; the cell key is (tile index, cell inside the
@@ -226,6 +230,9 @@ void launch_cell_map_tiled(const GridDesc &gd, const int *count, int *off, int4 
                            void *state, cudaStream_t s);
 // P2G#1 after a load (every later step gets it from launch_update_tiled of the step before); g.m, g.mv, g.f must be zero
 void launch_p2g1_tiled(const GridDesc &gd, const PArr &p, const GArr &g, const SortedMap &map, long long max_groups, cudaStream_t s);
+// flag[0] |= 1 if any of m[0..n) differs from m[0] bit for bit (flag zeroed by the caller); fill: m[0..n) = value
+void launch_mass_differs(const double *m, long long n, int *flag, cudaStream_t s);
+void launch_fill(double *m, long long n, double value, cudaStream_t s);
 long long max_items_tiled(const GridDesc &gd, long long max_groups);   // upper bound of the item count (launch size)
 // g: the node accumulators m, mv, f of this step (raw P2G#1) and mv2; the kernels apply l.4-5 / l.9 while staging a tile
 void launch_g2p_p2g2_tiled(const GridDesc &gd, const PArr &p, const GArr &g, const DevScalars *sc,

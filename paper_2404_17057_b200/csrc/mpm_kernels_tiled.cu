@@ -473,7 +473,7 @@ __global__ void __launch_bounds__(kTB, kTBMinG) k_g2p_p2g2_tiled(GridDesc gd, PA
             const long long k0 = (long long)gr.first + 2 * l;
 #pragma unroll
             for (int a = 0; a < DIM; ++a) cp_async16(&s_pf[DIM + a][threadIdx.x], p.v[a] + k0);
-            cp_async16(&s_pf[2 * DIM][threadIdx.x], p.m + k0);
+            if (!gd.uniform_mass) cp_async16(&s_pf[2 * DIM][threadIdx.x], p.m + k0);
         }
         cp_async_commit();
     };
@@ -512,7 +512,7 @@ __global__ void __launch_bounds__(kTB, kTBMinG) k_g2p_p2g2_tiled(GridDesc gd, PA
             V[0][a] = valid[0] ? tv.x : 0.0; V[1][a] = valid[1] ? tv.y : 0.0;
         }
         {
-            const double2 tm = s_pf[2 * DIM][threadIdx.x];
+            const double2 tm = gd.uniform_mass ? make_double2(gd.um, gd.um) : s_pf[2 * DIM][threadIdx.x];
             M[0] = valid[0] ? tm.x : 0.0; M[1] = valid[1] ? tm.y : 0.0;
         }
         issue_vm(nxt);
@@ -653,7 +653,7 @@ __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr
             const long long k0 = (long long)gr.first + 2 * l;
 #pragma unroll
             for (int a = 0; a < DIM; ++a) cp_async16(&s_pf[DIM + a][threadIdx.x], p.v[a] + k0);
-            cp_async16(&s_pf[2 * DIM][threadIdx.x], p.m + k0);
+            if (!gd.uniform_mass) cp_async16(&s_pf[2 * DIM][threadIdx.x], p.m + k0);
             cp_async16(&s_pf[2 * DIM + 1][threadIdx.x], p.rho + k0);
             cp_async16(&s_pf[2 * DIM + 2][threadIdx.x], p.e + k0);
             cp_async8(&s_id[threadIdx.x], p.id + k0);
@@ -709,7 +709,8 @@ __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr
             V[0][a] = valid[0] ? tv.x : 0.0; V[1][a] = valid[1] ? tv.y : 0.0;
         }
         {
-            const double2 tm = s_pf[2 * DIM][threadIdx.x], tr = s_pf[2 * DIM + 1][threadIdx.x], te = s_pf[2 * DIM + 2][threadIdx.x];
+            const double2 tm = gd.uniform_mass ? make_double2(gd.um, gd.um) : s_pf[2 * DIM][threadIdx.x];
+            const double2 tr = s_pf[2 * DIM + 1][threadIdx.x], te = s_pf[2 * DIM + 2][threadIdx.x];
             M[0] = valid[0] ? tm.x : 0.0; M[1] = valid[1] ? tm.y : 0.0;
             rho[0] = valid[0] ? tr.x : 1.0; rho[1] = valid[1] ? tr.y : 1.0;
             E[0] = valid[0] ? te.x : 0.0; E[1] = valid[1] ? te.y : 0.0;
@@ -780,7 +781,7 @@ __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr
                 st2(q.x[a], d0, Xo[0][a], Xo[1][a]);
                 st2(q.v[a], d0, Vo[0][a], Vo[1][a]);
             }
-            st2(q.m, d0, Mo[0], Mo[1]);
+            if (!gd.uniform_mass) st2(q.m, d0, Mo[0], Mo[1]);
             st2(q.rho, d0, Ro[0], Ro[1]);
             st2(q.e, d0, Eo[0], Eo[1]);
             if (store_q) st2(q.q, d0, Qo[0], Qo[1]);
@@ -792,7 +793,7 @@ __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr
                 const long long d = dst[i];
 #pragma unroll
                 for (int a = 0; a < DIM; ++a) { q.x[a][d] = Xo[i][a]; q.v[a][d] = Vo[i][a]; }
-                q.m[d] = Mo[i];
+                if (!gd.uniform_mass) q.m[d] = Mo[i];
                 q.rho[d] = Ro[i];
                 q.e[d] = Eo[i];
                 if (store_q) q.q[d] = Qo[i];
@@ -1027,6 +1028,20 @@ __global__ void k_stats_clear_t(DevScalars *sc)
 }
 
 
+__global__ void __launch_bounds__(kBlock) k_mass_differs(const double *__restrict__ m, long long n, int *flag)
+{
+    const long long first = __double_as_longlong(m[0]);
+    bool differs = false;
+    for (long long k = (long long)blockIdx.x * kBlock + threadIdx.x; k < n; k += (long long)gridDim.x * kBlock)
+        differs = differs || __double_as_longlong(m[k]) != first;
+    if (__any_sync(0xffffffffu, differs) && (threadIdx.x & 31) == 0) atomicOr(flag, 1);
+}
+
+__global__ void __launch_bounds__(kBlock) k_fill(double *m, long long n, double value)
+{
+    for (long long k = (long long)blockIdx.x * kBlock + threadIdx.x; k < n; k += (long long)gridDim.x * kBlock) m[k] = value;
+}
+
 // persistent launch: as many blocks as are resident at once (occupancy query), never more than there are chunks
 template <typename Kernel>
 inline unsigned persistent_blocks(long long max_groups, int groups_per_block, Kernel kernel)
@@ -1067,6 +1082,16 @@ void launch_p2g1_tiled(const GridDesc &gd, const PArr &p, const GArr &g, const S
     if (max_groups <= 0) return;
     if (gd.dim == 2) k_p2g1_tiled<2><<<persistent_blocks(max_groups, Geo<2>::GPB, k_p2g1_tiled<2>), kBlock, 0, s>>>(gd, p, g, map);
     else k_p2g1_tiled<3><<<persistent_blocks(max_groups, Geo<3>::GPB, k_p2g1_tiled<3>), kBlock, 0, s>>>(gd, p, g, map);
+}
+
+void launch_mass_differs(const double *m, long long n, int *flag, cudaStream_t s)
+{
+    if (n > 0) k_mass_differs<<<148 * 8, kBlock, 0, s>>>(m, n, flag);
+}
+
+void launch_fill(double *m, long long n, double value, cudaStream_t s)
+{
+    if (n > 0) k_fill<<<148 * 8, kBlock, 0, s>>>(m, n, value);
 }
 
 long long max_items_tiled(const GridDesc &gd, long long max_groups)
