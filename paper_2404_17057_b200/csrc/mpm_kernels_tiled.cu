@@ -853,7 +853,7 @@ __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr
 //   groups[]    one record {first slot, count, key, packed cell coordinates} per <= 2^d particles of a cell, key order;
 //   items[]     work items of the tile kernels {tile, first group, groups, -}: item t < ntiles is the first
 //               Chunk::GROUPS groups of tile t (possibly none), the further chunks of dense tiles are appended behind.
-// Single pass: a block takes 4 tiles (1024 keys, 4 per thread) in ticket order, scans (slots, groups) packed in one
+// Single pass: a block takes kMapKeys keys (whole tiles, kMapKeysPerThread per thread) in ticket order, scans (slots, groups) packed in one
 // 64-bit word and gets its exclusive prefix by decoupled look-back over the published block states
 // (flag << 62 | slots << 31 | groups; flag 1 = block aggregate, 2 = inclusive prefix).  `state` must be zero at launch.
 struct CellMapState {
@@ -862,7 +862,10 @@ struct CellMapState {
     int done;                            // blocks finished
     unsigned long long block[1];         // [n_blocks]
 };
-constexpr int kMapBlock = 256, kMapKeysPerThread = 4, kMapKeys = kMapBlock * kMapKeysPerThread;
+#ifndef MPM_MAP_KPT
+#define MPM_MAP_KPT 16
+#endif
+constexpr int kMapBlock = 256, kMapKeysPerThread = MPM_MAP_KPT, kMapKeys = kMapBlock * kMapKeysPerThread;
 
 template <int DIM>
 __global__ void __launch_bounds__(kMapBlock) k_cell_map_tiled(GridDesc gd, const int *__restrict__ count, int *__restrict__ off,
@@ -878,10 +881,15 @@ __global__ void __launch_bounds__(kMapBlock) k_cell_map_tiled(GridDesc gd, const
     __syncthreads();
     const int bid = s_bid;
     const int key0 = bid * kMapKeys + (int)threadIdx.x * kMapKeysPerThread;
-    int c[kMapKeysPerThread] = { 0, 0, 0, 0 };
-    if (key0 < nkeys) {      // nkeys is a multiple of the tile size, hence of 4
-        const int4 t = __ldg(reinterpret_cast<const int4 *>(count + key0));
-        c[0] = t.x; c[1] = t.y; c[2] = t.z; c[3] = t.w;
+    int c[kMapKeysPerThread];
+#pragma unroll
+    for (int j = 0; j < kMapKeysPerThread; ++j) c[j] = 0;
+    if (key0 < nkeys) {      // nkeys is a multiple of the tile size, hence of the keys per thread
+#pragma unroll
+        for (int j = 0; j < kMapKeysPerThread; j += 4) {
+            const int4 t = __ldg(reinterpret_cast<const int4 *>(count + key0 + j));
+            c[j] = t.x; c[j + 1] = t.y; c[j + 2] = t.z; c[j + 3] = t.w;
+        }
     }
     unsigned long long mine = 0ull;
 #pragma unroll
@@ -946,7 +954,8 @@ __global__ void __launch_bounds__(kMapBlock) k_cell_map_tiled(GridDesc gd, const
             }
             slot += (c[j] + 1) & ~1;
         }
-        *reinterpret_cast<int4 *>(off + key0) = make_int4(o4[0], o4[1], o4[2], o4[3]);
+#pragma unroll
+        for (int j = 0; j < kMapKeysPerThread; j += 4) *reinterpret_cast<int4 *>(off + key0 + j) = make_int4(o4[j], o4[j + 1], o4[j + 2], o4[j + 3]);
         // work items of the tile this thread starts
         if ((threadIdx.x % TPT) == 0) {
             const int tile = key0 >> TileGeo<DIM>::LTC;
