@@ -215,7 +215,8 @@ def run_ours(args):
     cfg, dim = w["cfg"], w["cfg"]["dim"]
     n_p = int(w["mass"].shape[0])
     variant = {"tiled": mpm.VARIANT_TILED, "sorted": mpm.VARIANT_SORTED, "atomic": mpm.VARIANT_ATOMIC}[args.variant]
-    g = mpm.Solver(cfg, sort_every=1, variant=variant, device=local)
+    accum = mpm.ACCUM_FP32 if args.grid_accum == "fp32" else mpm.ACCUM_FP64
+    g = mpm.Solver(cfg, sort_every=1, variant=variant, device=local, grid_accum=accum)
     n_n = g.num_nodes
     g.load_particles(w["x"], w["v"], w["mass"], w["rho"], w["e"])          # inputs resident in HBM before timing
     stream = g.stream
@@ -250,7 +251,7 @@ def run_ours(args):
     peak, peak_src = measured_peak_gbs()
     achieved = per_kernel[dom] / (kms[dom] * 1e-3) / 1e9
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": ncu_traffic(dom, args.workload, args.variant) if not args.size else None, "peak_source": peak_src,
+                "frac": achieved / peak, "traffic": ncu_traffic(dom, args.workload, args.variant) if not args.size and args.grid_accum == "fp64" else None, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": per_kernel[dom], "kernel_ms": kms[dom]}
     step_gbs = step_bytes * args.steps / (ms * 1e-3) / 1e9
     step_roofline = {"bytes_per_step": step_bytes, "achieved_gbs": step_gbs, "frac_of_measured_peak": step_gbs / peak,
@@ -259,8 +260,8 @@ def run_ours(args):
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f64", "data": "synthetic",
-        "config": {"workload": w["name"], "particles_per_gpu": n_p, "nodes": n_n, "dim": dim,
+        "dtype": "f64" if args.grid_accum == "fp64" else "f64 particles, f32 grid accumulation (separate variant)", "data": "synthetic",
+        "config": {"workload": w["name"], "grid_accum": args.grid_accum, "particles_per_gpu": n_p, "nodes": n_n, "dim": dim,
                    "kernel_family": args.variant, "parallelism": f"replicas x{world}",
                    "l2": "inputs (%.1f GB particle state) exceed the 126 MB L2; no flush" % (n_p * (2 * dim + 5) * 8 / 1e9)},
         "clocks": clocks, "gpu_launches": launches, "roofline": roofline, "step_roofline": step_roofline,
@@ -316,6 +317,8 @@ def main():
     ap.add_argument("--workload", default="sedov", choices=["sedov", "clumps", "cylinder", "box", "sod"])
     ap.add_argument("--size", type=int, default=0, help="grid resolution override (0 = BASELINE.json size)")
     ap.add_argument("--variant", default="tiled", choices=["tiled", "sorted", "atomic"])
+    ap.add_argument("--grid-accum", default="fp64", choices=["fp64", "fp32"],
+                    help="fp32: the fp32 grid-accumulation variant of config 5 (tiled family), reported separately")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")

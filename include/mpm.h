@@ -59,9 +59,14 @@ enum { MPM_VISC_PRINTED = 0, MPM_VISC_STANDARD = 1 };
  *         group of 2^dim lanes, contributions summed inside the group before one global reduction per corner and
  *         channel, corner node values staged once per group.  Ignores sort_every (always 1).
  * TILED:  SORTED's lane groups with tile-major cell order, even-aligned cell slots (128-bit particle loads) and
- *         shared-memory grid tiles: node values of a tile are loaded once per block, scatters accumulate in shared
- *         memory and reach global memory as one reduction per tile node.  Ignores sort_every (always 1). */
+ *         shared-memory grid tiles: the node velocities of a tile are formed once per block from the raw sums (BC,
+ *         momentum advance and quotients included), two particle sweeps per step (the next step's first P2G is fused
+ *         into the particle update).  Ignores sort_every (always 1). */
 enum { MPM_VARIANT_AUTO = 0, MPM_VARIANT_ATOMIC = 1, MPM_VARIANT_SORTED = 2, MPM_VARIANT_TILED = 3 };
+/* precision of the node sums m, mv, f, mv2 ("the code supports different choices"): FP64 (default), or FP32
+ * = the fp32 grid-accumulation variant of the clustered stress workload: the scatters reduce in fp32 and the sums are
+ * kept in fp32, all particle arithmetic stays fp64.  TILED family only (MPM_E_ARG otherwise). */
+enum { MPM_ACCUM_FP64 = 0, MPM_ACCUM_FP32 = 1 };
 /* particle fields (bit mask for mpm_read_particles; output pointers are consumed in this order, a vector field
  * takes `dim` pointers) */
 enum { MPM_P_X = 1, MPM_P_V = 2, MPM_P_M = 4, MPM_P_RHO = 8, MPM_P_E = 16, MPM_P_Q = 32 };
@@ -95,7 +100,7 @@ typedef struct mpm_config {
     int32_t sort_every;       /* 0 = never re-order; k > 0 = cell-key re-ordering every k steps */
     int32_t variant;          /* MPM_VARIANT_* */
     int32_t device;           /* CUDA device ordinal */
-    int32_t reserved;
+    int32_t grid_accum;       /* MPM_ACCUM_* (this field was `reserved`, 0, in ABI version 1) */
     void *stream;             /* cudaStream_t; NULL = the legacy default stream */
     mpm_alloc_fn alloc;       /* NULL = cudaMalloc */
     mpm_free_fn free;         /* NULL = cudaFree */

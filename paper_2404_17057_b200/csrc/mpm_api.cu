@@ -48,6 +48,8 @@ struct mpm_handle {
     int4 *groups_alt, *items_alt;
     int *n_groups_alt, *n_items_alt;
     void *map_state;      // scratch of launch_cell_map_tiled
+    // TILED with fp32 accumulators: fp64 copies of the last step's m, mv, f, mv2 for mpm_read_grid (allocated on first use)
+    double *rg_m, *rg_mv[3], *rg_f[3], *rg_mv2[3];
     long long max_items;
     double *S[2];
     unsigned long long *dest;
@@ -308,6 +310,7 @@ void reorder(mpm_handle *h)
         h->cur ^= 1;
         // P2G#1 of the first step (Alg. 1 l.3); every later one comes out of the update kernel of the step before
         h->acur = 0;
+        h->grid_final = false;
         GArr g0 = tiled_acc(h, 0);
         launch_grid_clear(h->gd, g0, h->stream);
         for (int a = 0; a < h->gd.dim; ++a) cudaMemsetAsync(g0.mv2[a], 0, sizeof(double) * (size_t)h->gd.Nn, h->stream);
@@ -452,6 +455,7 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
     h->d_flag = nullptr; h->key = h->rank = h->count = h->scan_aux = nullptr; h->sc = nullptr;
     h->off[0] = h->off[1] = nullptr; h->ocur = 0; h->goff = h->n_groups = nullptr; h->groups = nullptr;
     h->items = nullptr; h->n_items = nullptr; h->max_items = 0;
+    h->rg_m = nullptr; for (int a = 0; a < 3; ++a) h->rg_mv[a] = h->rg_f[a] = h->rg_mv2[a] = nullptr;
     h->groups_alt = h->items_alt = nullptr; h->n_groups_alt = h->n_items_alt = nullptr; h->map_state = nullptr;
     h->S[0] = h->S[1] = nullptr; h->dest = nullptr; h->max_groups = 0; h->coff = nullptr; h->slots = 0;
     std::memset(h->pbuf, 0, sizeof(h->pbuf));
@@ -503,7 +507,12 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
     }
     const bool tiled = h->variant == MPM_VARIANT_TILED;
     const bool sorted = h->variant == MPM_VARIANT_SORTED || tiled;
+    if (cfg->grid_accum != MPM_ACCUM_FP64 && !(cfg->grid_accum == MPM_ACCUM_FP32 && tiled)) {
+        delete h;
+        return fail(nullptr, MPM_E_ARG, "mpm_create: grid_accum must be MPM_ACCUM_FP64, or MPM_ACCUM_FP32 with the TILED family");
+    }
     gd.tiled = tiled ? 1 : 0;
+    gd.acc32 = cfg->grid_accum == MPM_ACCUM_FP32 ? 1 : 0;
     gd.Nkeys = gd.Nc;
     if (tiled) {    // tile-major key space (TileGeo): whole tiles, so it can be larger than the number of cells
         long long nt = 1;
@@ -766,8 +775,32 @@ int mpm_read_grid(mpm_handle *h, int field, double *out, int ptr_location)
     const size_t Nn = (size_t)gd.Nn;
     int rc = MPM_OK;
     // TILED: the last completed step used the accumulator set that is no longer current
-    const GArr gl = (h->variant == MPM_VARIANT_TILED) ? tiled_acc(h, h->steps_done > 0 ? h->acur ^ 1 : h->acur) : h->g;
-    if (h->variant == MPM_VARIANT_TILED && !h->grid_final && h->steps_done > 0) {
+    GArr gl = (h->variant == MPM_VARIANT_TILED) ? tiled_acc(h, h->steps_done > 0 ? h->acur ^ 1 : h->acur) : h->g;
+    if (gd.acc32) {
+        // fp32 accumulators: widen the last step's sums into fp64 copies and replay the node conditions there
+        if (!h->rg_m) {
+            bool ok = dev_alloc_t(h, &h->rg_m, Nn);
+            for (int a = 0; a < gd.dim && ok; ++a)
+                ok = dev_alloc_t(h, &h->rg_mv[a], Nn) && dev_alloc_t(h, &h->rg_f[a], Nn) && dev_alloc_t(h, &h->rg_mv2[a], Nn);
+            if (!ok) return fail(h, MPM_E_OOM, "mpm_read_grid: out of device memory");
+            h->grid_final = false;
+        }
+        GArr gw = gl;
+        gw.m = h->rg_m;
+        for (int a = 0; a < gd.dim; ++a) { gw.mv[a] = h->rg_mv[a]; gw.f[a] = h->rg_f[a]; gw.mv2[a] = h->rg_mv2[a]; }
+        if (!h->grid_final) {
+            launch_widen(gl.m, gw.m, gd.Nn, h->stream);
+            for (int a = 0; a < gd.dim; ++a) {
+                launch_widen(gl.mv[a], gw.mv[a], gd.Nn, h->stream);
+                launch_widen(gl.f[a], gw.f[a], gd.Nn, h->stream);
+                launch_widen(gl.mv2[a], gw.mv2[a], gd.Nn, h->stream);
+            }
+            if (h->steps_done > 0) { launch_node1(gd, gw, h->sc, h->stream, false); launch_node2(gd, gw, h->stream); }
+            h->grid_final = true;
+            h->launches += 3 + 3 * gd.dim;
+        }
+        gl = gw;
+    } else if (h->variant == MPM_VARIANT_TILED && !h->grid_final && h->steps_done > 0) {
         // the step left the raw sums; l.4-5 and l.9 are replayed in place with the node kernels (dt of that step is
         // still in the device scalars).  That accumulator set is cleared before it is used again.
         launch_node1(gd, gl, h->sc, h->stream, false);

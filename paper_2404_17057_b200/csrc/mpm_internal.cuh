@@ -38,6 +38,8 @@ struct GridDesc {
     // kernels then take M from here and neither read nor write the mass array (it stays filled with this value)
     int uniform_mass;
     double um;
+    // TILED: node accumulators m, mv, f, mv2 are fp32 (mpm_config.grid_accum = MPM_ACCUM_FP32)
+    int acc32;
 };
 
 // TILED family: the grid is cut into tiles of T0 x T1 (x T2) cells; the cell key is (tile index, cell inside the
@@ -233,6 +235,8 @@ void launch_p2g1_tiled(const GridDesc &gd, const PArr &p, const GArr &g, const S
 // flag[0] |= 1 if any of m[0..n) differs from m[0] bit for bit (flag zeroed by the caller); fill: m[0..n) = value
 void launch_mass_differs(const double *m, long long n, int *flag, cudaStream_t s);
 void launch_fill(double *m, long long n, double value, cudaStream_t s);
+// dst[i] = (double)((const float *)src)[i]: fp32 accumulators widened for mpm_read_grid
+void launch_widen(const double *src_as_float, double *dst, long long n, cudaStream_t s);
 long long max_items_tiled(const GridDesc &gd, long long max_groups);   // upper bound of the item count (launch size)
 // g: the node accumulators m, mv, f of this step (raw P2G#1) and mv2; the kernels apply l.4-5 / l.9 while staging a tile
 void launch_g2p_p2g2_tiled(const GridDesc &gd, const PArr &p, const GArr &g, const DevScalars *sc,

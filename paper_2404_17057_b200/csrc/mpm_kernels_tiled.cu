@@ -52,6 +52,22 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 // all committed groups but the most recent one have landed
 __device__ __forceinline__ void cp_async_wait_but_one() { asm volatile("cp.async.wait_group 1;" ::: "memory"); }
 
+// Node accumulators m, mv, f, mv2: fp64 (default) or, with ACC32, fp32 values in the same allocations (the fp32
+// grid-accumulation variant of BASELINE.json config 5: particle arithmetic stays fp64, the sums on the grid and the
+// reductions that form them are fp32)
+template <bool ACC32>
+__device__ __forceinline__ void acc_add(double *arr, long long i, double v)
+{
+    if (ACC32) atomicAdd(reinterpret_cast<float *>(arr) + i, (float)v);
+    else atomicAdd(arr + i, v);
+}
+template <bool ACC32>
+__device__ __forceinline__ double acc_ld(const double *arr, long long i)
+{
+    if (ACC32) return (double)__ldg(reinterpret_cast<const float *>(arr) + i);
+    return __ldg(arr + i);
+}
+
 template <int DIM>
 __device__ __forceinline__ int tiled_key_of_position(const GridDesc &gd, const double X[DIM])
 {
@@ -93,7 +109,7 @@ __device__ __forceinline__ bool warp_one_cell(int cell, int cnt)
 // accumulators g.m, g.mv, g.f with one global fp64 reduction per corner and channel (see mpm_kernels_sorted.cu):
 //   pay[i] = { M, M V_a, S } of the lane's particle i, w[i][r] = weight of corner r ^ l (0 for a particle that is not
 //   part of the group reduction).
-template <int DIM>
+template <int DIM, bool ACC32>
 __device__ __forceinline__ void scatter_p2g1_group(const GridDesc &gd, const GArr &g, const int c[DIM], int l, bool any,
                                                    const double pay[2][DIM + 2], const double w[2][1 << DIM], bool one_cell = false)
 {
@@ -127,11 +143,11 @@ __device__ __forceinline__ void scatter_p2g1_group(const GridDesc &gd, const GAr
 #pragma unroll
         for (int q = 0; q < 2; ++q) {
             const int node = corner_node_i<DIM>(gd, c, l + q * LG);
-            atomicAdd(&g.m[node], tot[0][q]);
+            acc_add<ACC32>(g.m, node, tot[0][q]);
 #pragma unroll
             for (int a = 0; a < DIM; ++a) {
-                atomicAdd(&g.mv[a][node], tot[1 + a][q]);
-                atomicAdd(&g.f[a][node], F[a][q]);
+                acc_add<ACC32>(g.mv[a], node, tot[1 + a][q]);
+                acc_add<ACC32>(g.f[a], node, F[a][q]);
             }
         }
     }
@@ -140,7 +156,7 @@ __device__ __forceinline__ void scatter_p2g1_group(const GridDesc &gd, const GAr
 // ------------------------------------------------------------------------------------------------ Alg. 1 l.3 (after a load only)
 // m, mv from phi-weighted channels (M, M V); f from the phi-weighted channel S = (P+Q) M / rho (eq. 13).
 // Every later step gets its P2G#1 from the update kernel of the step before.
-template <int DIM>
+template <int DIM, bool ACC32>
 __global__ void __launch_bounds__(kBlock, MPM_MINB) k_p2g1_tiled(GridDesc gd, PArr p, GArr g, SortedMap map)
 {
     constexpr int NB = 1 << DIM, LG = Geo<DIM>::LG, GPB = Geo<DIM>::GPB;
@@ -171,7 +187,7 @@ __global__ void __launch_bounds__(kBlock, MPM_MINB) k_p2g1_tiled(GridDesc gd, PA
             const double S = valid[i] ? (gm1 * rho * E + Q) * M / rho : 0.0;      // (P+Q) M / rho, P = (gamma-1) rho E (eq. 3)
             double xi[DIM];
             const bool fast = valid[i] && local_coords<DIM>(gd, X[i], c, xi);
-            if (valid[i] && !fast) slow_p2g1<DIM>(gd, g, X[i], V[i], M, S);
+            if (valid[i] && !fast) slow_p2g1<DIM, ACC32>(gd, g, X[i], V[i], M, S);
             pay[i][0] = fast ? M : 0.0;
             pay[i][DIM + 1] = fast ? S : 0.0;
 #pragma unroll
@@ -182,7 +198,7 @@ __global__ void __launch_bounds__(kBlock, MPM_MINB) k_p2g1_tiled(GridDesc gd, PA
                 for (int r = 0; r < NB; ++r) w[i][r] = 0.0;
             }
         }
-        scatter_p2g1_group<DIM>(gd, g, c, l, grp.cnt > 0, pay, w);
+        scatter_p2g1_group<DIM, ACC32>(gd, g, c, l, grp.cnt > 0, pay, w);
     }
 }
 
@@ -256,7 +272,7 @@ __device__ __forceinline__ int tile_node_global(const GridDesc &gd, const int or
 //   WITH_V2 = false (gather kernel): [0, DIM) vbar = mv'/m, [DIM, 2 DIM) acc = f/m;
 //   WITH_V2 = true  (update kernel): [0, DIM) vbar = mv'/m, [DIM, 2 DIM) v2 = BC(mv2)/m (l.9); rest 0.
 // One reciprocal per node (1 ulp from the true quotients of the node kernels, far inside the parity tolerance).
-template <int DIM, int CH, bool WITH_V2>
+template <int DIM, int CH, bool WITH_V2, bool ACC32>
 __device__ __forceinline__ void stage_tile(const GridDesc &gd, const int org[DIM], const GArr &g, double dt, double *s_tile)
 {
     using TG = TileGeo<DIM>;
@@ -275,12 +291,12 @@ __device__ __forceinline__ void stage_tile(const GridDesc &gd, const int org[DIM
 #pragma unroll
         for (int a = 0; a < DIM; ++a) { mv[it][a] = 0.0; f[it][a] = 0.0; mv2[it][a] = 0.0; }
         if (node[it] >= 0) {
-            m[it] = __ldg(g.m + node[it]);
+            m[it] = acc_ld<ACC32>(g.m, node[it]);
 #pragma unroll
-            for (int a = 0; a < DIM; ++a) { mv[it][a] = __ldg(g.mv[a] + node[it]); f[it][a] = __ldg(g.f[a] + node[it]); }
+            for (int a = 0; a < DIM; ++a) { mv[it][a] = acc_ld<ACC32>(g.mv[a], node[it]); f[it][a] = acc_ld<ACC32>(g.f[a], node[it]); }
             if (WITH_V2) {
 #pragma unroll
-                for (int a = 0; a < DIM; ++a) mv2[it][a] = __ldg(g.mv2[a] + node[it]);
+                for (int a = 0; a < DIM; ++a) mv2[it][a] = acc_ld<ACC32>(g.mv2[a], node[it]);
             }
         }
     }
@@ -394,7 +410,7 @@ __device__ __forceinline__ bool move_inside(const GridDesc &gd, const double X[D
 // particles per round: lane (slot = lane / 2^d, corner b = lane % 2^d) gets the data of the slot's particle by shuffle
 // and adds its 1 + 2 d channels (m, mv_a, f_a) to corner b.  Used for particles that leave their group's cell (their
 // contributions cannot join the group's butterfly).
-template <int DIM>
+template <int DIM, bool ACC32>
 __device__ __forceinline__ void coop_p2g1(const GridDesc &gd, const GArr &gn, unsigned mask, const double Xn[DIM],
                                           const double Vn[DIM], double Mn, double Sn, int lane)
 {
@@ -422,11 +438,11 @@ __device__ __forceinline__ void coop_p2g1(const GridDesc &gd, const GArr &gn, un
             particle_cell<DIM>(gd, X, c, xi);
             const long long node = corner_node<DIM>(gd, c, b);
             const double Mphi = M * corner_phi<DIM>(xi, b);
-            atomicAdd(gn.m + node, Mphi);
+            acc_add<ACC32>(gn.m, node, Mphi);
 #pragma unroll
             for (int a = 0; a < DIM; ++a) {
-                atomicAdd(gn.mv[a] + node, V[a] * Mphi);
-                atomicAdd(gn.f[a] + node, S * corner_dphi<DIM>(xi, b, a, gd.inv_h));
+                acc_add<ACC32>(gn.mv[a], node, V[a] * Mphi);
+                acc_add<ACC32>(gn.f[a], node, S * corner_dphi<DIM>(xi, b, a, gd.inv_h));
             }
         }
     }
@@ -441,7 +457,7 @@ __device__ __forceinline__ void coop_p2g1(const GridDesc &gd, const GArr &gn, un
 // atomic each; the atomics are issued before the scatter and their results consumed after it.
 // The particle fields of the NEXT pass are copied into the thread's own shared-memory slots with cp.async while the
 // current pass computes (PfSlots).  V' overwrites V in place (the slots are this thread's own).
-template <int DIM>
+template <int DIM, bool ACC32>
 __global__ void __launch_bounds__(kTB, kTBMinG) k_g2p_p2g2_tiled(GridDesc gd, PArr p, GArr g,
                                                                 const DevScalars *__restrict__ sc, SortedMap map,
                                                                 const int4 *__restrict__ items, const int *__restrict__ n_items,
@@ -483,7 +499,7 @@ __global__ void __launch_bounds__(kTB, kTBMinG) k_g2p_p2g2_tiled(GridDesc gd, PA
     tile_origin<DIM>(gd, item.x, org);
     const double dt = sc->dt;
     const long long step = sc->step;
-    stage_tile<DIM, CH, false>(gd, org, g, dt, s_tile);
+    stage_tile<DIM, CH, false, ACC32>(gd, org, g, dt, s_tile);
     __syncthreads();
     for (int p0 = 0; p0 < item.z; p0 += GPB, gl += GPB) {
         int c[DIM];
@@ -576,7 +592,7 @@ __global__ void __launch_bounds__(kTB, kTBMinG) k_g2p_p2g2_tiled(GridDesc gd, PA
                 for (int q = 0; q < 2; ++q) {
                     const int node = corner_node_i<DIM>(gd, c, l + q * LG);
 #pragma unroll
-                    for (int a = 0; a < DIM; ++a) atomicAdd(&g.mv2[a][node], tot[a][q]);
+                    for (int a = 0; a < DIM; ++a) acc_add<ACC32>(g.mv2[a], node, tot[a][q]);
                 }
             }
         }
@@ -614,7 +630,7 @@ struct UpdSmem {
     static constexpr size_t BYTES = TILE + PF + DEST + ID;
 };
 
-template <int DIM>
+template <int DIM, bool ACC32>
 __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr p, PArr q, GArr g, DevScalars *sc, SortedMap map,
                                                               const int4 *__restrict__ items, const int *__restrict__ n_items,
                                                               const int *__restrict__ off_new,
@@ -666,7 +682,7 @@ __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr
     tile_origin<DIM>(gd, item.x, org);
     const double dt = sc->dt;
     const long long step = sc->step;
-    stage_tile<DIM, CH, true>(gd, org, g, dt, s_tile);
+    stage_tile<DIM, CH, true, ACC32>(gd, org, g, dt, s_tile);
     __syncthreads();
     double vloc = 0.0, cloc = 0.0;
     int n_rec = 0, n_clamp = 0, n_neg = 0, n_nonfin = 0;
@@ -804,7 +820,7 @@ __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr
 #pragma unroll
         for (int i = 0; i < 2; ++i) {      // particles that leave the group's cell: scattered by the whole warp
             const unsigned mm = __ballot_sync(kFull, valid[i] && !stay[i]);
-            if (mm) coop_p2g1<DIM>(gd, gn, mm, Xo[i], Vo[i], Mo[i], Sn[i], lane);
+            if (mm) coop_p2g1<DIM, ACC32>(gd, gn, mm, Xo[i], Vo[i], Mo[i], Sn[i], lane);
         }
         double pay[2][DIM + 2], wn[2][NB];      // the others join the group's butterfly: payload M, M V', S', weights at X'
 #pragma unroll
@@ -818,7 +834,7 @@ __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr
 #pragma unroll
             for (int a = 0; a < DIM; ++a) pay[i][1 + a] = stay[i] ? Mo[i] * Vo[i][a] : 0.0;
         }
-        scatter_p2g1_group<DIM>(gd, gn, c, l, grp.cnt > 0, pay, wn, warp_one_cell(grp.cell, grp.cnt));
+        scatter_p2g1_group<DIM, ACC32>(gd, gn, c, l, grp.cnt > 0, pay, wn, warp_one_cell(grp.cell, grp.cnt));
         grp = nxt;
         nxt = nn;
     }
@@ -1089,8 +1105,11 @@ void launch_cell_map_tiled(const GridDesc &gd, const int *count, int *off, int4 
 void launch_p2g1_tiled(const GridDesc &gd, const PArr &p, const GArr &g, const SortedMap &map, long long max_groups, cudaStream_t s)
 {
     if (max_groups <= 0) return;
-    if (gd.dim == 2) k_p2g1_tiled<2><<<persistent_blocks(max_groups, Geo<2>::GPB, k_p2g1_tiled<2>), kBlock, 0, s>>>(gd, p, g, map);
-    else k_p2g1_tiled<3><<<persistent_blocks(max_groups, Geo<3>::GPB, k_p2g1_tiled<3>), kBlock, 0, s>>>(gd, p, g, map);
+#define MPM_LAUNCH_P2G1(D, A) \
+    k_p2g1_tiled<D, A><<<persistent_blocks(max_groups, Geo<D>::GPB, k_p2g1_tiled<D, A>), kBlock, 0, s>>>(gd, p, g, map)
+    if (gd.dim == 2) { if (gd.acc32) MPM_LAUNCH_P2G1(2, true); else MPM_LAUNCH_P2G1(2, false); }
+    else { if (gd.acc32) MPM_LAUNCH_P2G1(3, true); else MPM_LAUNCH_P2G1(3, false); }
+#undef MPM_LAUNCH_P2G1
 }
 
 void launch_mass_differs(const double *m, long long n, int *flag, cudaStream_t s)
@@ -1116,8 +1135,10 @@ void launch_g2p_p2g2_tiled(const GridDesc &gd, const PArr &p, const GArr &g, con
                            unsigned long long *dest, cudaStream_t s)
 {
     if (max_items <= 0) return;
-    if (gd.dim == 2) k_g2p_p2g2_tiled<2><<<(unsigned)max_items, kTB, 0, s>>>(gd, p, g, sc, map, items, n_items, count, dest);
-    else k_g2p_p2g2_tiled<3><<<(unsigned)max_items, kTB, 0, s>>>(gd, p, g, sc, map, items, n_items, count, dest);
+#define MPM_LAUNCH_G2P(D, A) k_g2p_p2g2_tiled<D, A><<<(unsigned)max_items, kTB, 0, s>>>(gd, p, g, sc, map, items, n_items, count, dest)
+    if (gd.dim == 2) { if (gd.acc32) MPM_LAUNCH_G2P(2, true); else MPM_LAUNCH_G2P(2, false); }
+    else { if (gd.acc32) MPM_LAUNCH_G2P(3, true); else MPM_LAUNCH_G2P(3, false); }
+#undef MPM_LAUNCH_G2P
 }
 
 void launch_update_tiled(const GridDesc &gd, const PArr &p, const PArr &q, const GArr &g, DevScalars *sc,
@@ -1128,14 +1149,27 @@ void launch_update_tiled(const GridDesc &gd, const PArr &p, const PArr &q, const
     const int sq = store_q ? 1 : 0;
     static bool attr_set = false;      // more than 48 KB of dynamic shared memory needs the opt-in, once per process
     if (!attr_set) {
-        cudaFuncSetAttribute(k_update_tiled<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UpdSmem<2>::BYTES);
-        cudaFuncSetAttribute(k_update_tiled<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UpdSmem<3>::BYTES);
+        cudaFuncSetAttribute(k_update_tiled<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UpdSmem<2>::BYTES);
+        cudaFuncSetAttribute(k_update_tiled<3, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UpdSmem<3>::BYTES);
+        cudaFuncSetAttribute(k_update_tiled<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UpdSmem<2>::BYTES);
+        cudaFuncSetAttribute(k_update_tiled<3, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UpdSmem<3>::BYTES);
         attr_set = true;
     }
-    if (gd.dim == 2)
-        k_update_tiled<2><<<(unsigned)max_items, kTB, UpdSmem<2>::BYTES, s>>>(gd, p, q, g, sc, map, items, n_items, off_new, dest, g_next, sq);
-    else
-        k_update_tiled<3><<<(unsigned)max_items, kTB, UpdSmem<3>::BYTES, s>>>(gd, p, q, g, sc, map, items, n_items, off_new, dest, g_next, sq);
+#define MPM_LAUNCH_UPD(D, A) \
+    k_update_tiled<D, A><<<(unsigned)max_items, kTB, UpdSmem<D>::BYTES, s>>>(gd, p, q, g, sc, map, items, n_items, off_new, dest, g_next, sq)
+    if (gd.dim == 2) { if (gd.acc32) MPM_LAUNCH_UPD(2, true); else MPM_LAUNCH_UPD(2, false); }
+    else { if (gd.acc32) MPM_LAUNCH_UPD(3, true); else MPM_LAUNCH_UPD(3, false); }
+#undef MPM_LAUNCH_UPD
+}
+
+// dst[i] = (double)src[i], i < n (fp32 accumulators brought to fp64 for mpm_read_grid)
+__global__ void __launch_bounds__(256) k_widen(const float *__restrict__ src, double *__restrict__ dst, long long n)
+{
+    for (long long i = (long long)blockIdx.x * 256 + threadIdx.x; i < n; i += (long long)gridDim.x * 256) dst[i] = (double)src[i];
+}
+void launch_widen(const double *src_as_float, double *dst, long long n, cudaStream_t s)
+{
+    if (n > 0) k_widen<<<148 * 8, 256, 0, s>>>(reinterpret_cast<const float *>(src_as_float), dst, n);
 }
 
 void launch_gather_by_id_groups(const double *src, const int *id, double *dst, const SortedMap &map, long long max_groups,

@@ -129,7 +129,7 @@ __device__ __forceinline__ double warp_max_nonneg(double v)
 }
 
 // ---------------------------------------------------------------------------------------------- slow paths
-template <int DIM>
+template <int DIM, bool ACC32 = false>
 __device__ __forceinline__ void slow_p2g1(const GridDesc &gd, const GArr &g, const double X[DIM], const double V[DIM],
                                           double M, double S)
 {
@@ -140,6 +140,15 @@ __device__ __forceinline__ void slow_p2g1(const GridDesc &gd, const GArr &g, con
     for (int ib = 0; ib < (1 << DIM); ++ib) {
         const long long i = corner_node<DIM>(gd, c, ib);
         const double phi = corner_phi<DIM>(xi, ib);
+        if (ACC32) {      // fp32 grid accumulation (TILED family only)
+            atomicAdd(reinterpret_cast<float *>(g.m) + i, (float)(M * phi));
+#pragma unroll
+            for (int a = 0; a < DIM; ++a) {
+                atomicAdd(reinterpret_cast<float *>(g.mv[a]) + i, (float)(M * V[a] * phi));
+                atomicAdd(reinterpret_cast<float *>(g.f[a]) + i, (float)(S * corner_dphi<DIM>(xi, ib, a, gd.inv_h)));
+            }
+            continue;
+        }
         atomicAdd(&g.m[i], M * phi);
 #pragma unroll
         for (int a = 0; a < DIM; ++a) {

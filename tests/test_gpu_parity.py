@@ -162,6 +162,47 @@ def test_full_size_properties(mpm, name):
     assert s["mass"].shape[0] == n and (np.diff(key) >= 0).all()
 
 
+@pytest.mark.parametrize("name", ["clumps", "clumps_dense", "sedov", "cylinder"])
+def test_fp32_grid_accumulation_variant(po, mpm, name):
+    """The fp32 grid-accumulation variant of BASELINE.json config 5 (node sums m, mv, f, mv2 reduced and kept in fp32,
+    particle arithmetic fp64; TILED family) against the fp64 oracle: same norms as the fp64 parity tests at 1e-5
+    (SURVEY.md section 8(c)-D).  An fp32 sum of n terms of one sign carries a relative error of about sqrt(n) 2^-24
+    (n <= a few hundred reductions per node, since the lane groups and dense-cell warps add in fp64 first): ~1e-6."""
+    w = small_workloads()[name]()
+    o = po.Oracle(w["cfg"])
+    o.load_particles(w["x"], w["v"], w["mass"], w["rho"], w["e"])
+    g = mpm.Solver(w["cfg"], sort_every=1, variant=mpm.VARIANT_TILED, grid_accum=mpm.ACCUM_FP32)
+    g.load_particles(w["x"], w["v"], w["mass"], w["rho"], w["e"])
+    o.step(0.0, w["cfl"], 1)
+    g.step(0.0, w["cfl"], 1)
+    tol = 1e-5
+    fscale = _force_scale(w)
+    for fo, fg, scale in ((po.G_MASS, mpm.G_MASS, None), (po.G_MOM, mpm.G_MOMENTUM, None),
+                          (po.G_MOM2, mpm.G_MOMENTUM2, None), (po.G_FORCE, mpm.G_FORCE, fscale)):
+        a, b = o.grid(fo), g.read_grid(fg)
+        sc = scale if scale is not None else np.abs(a).max()
+        err = np.abs(a - b).max()
+        assert err <= tol * sc, (name, fo, err, sc)
+        assert err > 1e-12 * sc            # it really is the fp32 path
+    nsteps = STEPS[name]
+    o.step(0.0, w["cfl"], nsteps - 1)
+    g.step(0.0, w["cfl"], nsteps - 1)
+    assert g.stats().n_nonfinite == 0
+    p = g.read_particles()
+    for key, fo in (("rho", po.P_RHO), ("e", po.P_E), ("x", po.P_X)):
+        a = o.particles(fo)
+        assert np.abs(a - p[key]).sum() <= tol * np.abs(a).sum(), (name, key)
+    v = o.particles(po.P_V)
+    assert np.abs(v - p["v"]).sum() <= tol * np.sqrt((v ** 2).sum(axis=0)).sum() * w["cfg"]["dim"], name
+    np.testing.assert_array_equal(o.particles(po.P_M), p["mass"])
+
+
+def test_fp32_grid_accumulation_needs_tiled(mpm):
+    cfg = dict(dim=2, n=[8, 8], dx=0.125, gamma=1.4, bc=[[0, 0], [0, 0]])
+    with pytest.raises(mpm.MpmError):
+        mpm.Solver(cfg, sort_every=0, variant=mpm.VARIANT_ATOMIC, grid_accum=mpm.ACCUM_FP32)
+
+
 def test_reordering_does_not_change_results(mpm):
     """'Optional particles re-ordering' (Alg. 1 l.12) must leave the solution unchanged up to summation order."""
     w = inputs.periodic_box(n=64, perm_seed=7)
