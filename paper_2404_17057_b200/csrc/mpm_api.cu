@@ -425,6 +425,19 @@ int mpm_abi_version(void) { return MPM_ABI_VERSION; }
 
 const char *mpm_last_error(const mpm_handle *h) { return h ? h->err.c_str() : g_create_error.c_str(); }
 
+namespace {
+// a handle that never became visible to the caller: release what mpm_create has made so far
+void discard(mpm_handle *h)
+{
+    if (h->side) cudaStreamDestroy(h->side);
+    if (h->ev_fork) cudaEventDestroy(h->ev_fork);
+    if (h->ev_join) cudaEventDestroy(h->ev_join);
+    std::vector<void *> all = h->allocations;
+    for (void *p : all) dev_free(h, p);
+    delete h;
+}
+}  // namespace
+
 int mpm_create(const mpm_config *cfg, mpm_handle **out)
 {
     if (!cfg || !out) return fail(nullptr, MPM_E_ARG, "mpm_create: null argument");
@@ -446,7 +459,7 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
     if (cudaStreamCreateWithFlags(&h->side, cudaStreamNonBlocking) != cudaSuccess ||
         cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
         cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming) != cudaSuccess) {
-        delete h;
+        discard(h);
         return fail(nullptr, MPM_E_CUDA, "mpm_create: cannot create the second stream");
     }
     h->cur = 0; h->n = h->cap = 0; h->launches = 0; h->steps_done = 0;
@@ -471,7 +484,7 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
         if (a < gd.dim) {
             const bool p0 = cfg->bc[a][0] == MPM_BC_PERIODIC, p1 = cfg->bc[a][1] == MPM_BC_PERIODIC;
             if (cfg->n[a] < 1 || p0 != p1) {
-                delete h;
+                discard(h);
                 return fail(nullptr, MPM_E_ARG, "mpm_create: n[a] >= 1 and PERIODIC on both sides of an axis required");
             }
             gd.nc[a] = cfg->n[a]; gd.per[a] = p0; gd.nn[a] = p0 ? cfg->n[a] : cfg->n[a] + 1;
@@ -483,7 +496,7 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
         gd.Nn *= gd.nn[a]; gd.Nc *= gd.nc[a];
     }
     if (gd.Nc >= (1ll << 31) - 2 || gd.Nn >= (1ll << 31) - 2) {
-        delete h;
+        discard(h);
         return fail(nullptr, MPM_E_ARG, "mpm_create: grid too large for 32-bit cell keys");
     }
     gd.in_axis = -1; gd.in_side = 0;
@@ -502,13 +515,13 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
     h->variant = cfg->variant == MPM_VARIANT_AUTO ? (cfg->sort_every == 1 ? MPM_VARIANT_TILED : MPM_VARIANT_ATOMIC)
                                                    : cfg->variant;
     if (h->variant != MPM_VARIANT_ATOMIC && h->variant != MPM_VARIANT_SORTED && h->variant != MPM_VARIANT_TILED) {
-        delete h;
+        discard(h);
         return fail(nullptr, MPM_E_ARG, "mpm_create: unknown kernel variant");
     }
     const bool tiled = h->variant == MPM_VARIANT_TILED;
     const bool sorted = h->variant == MPM_VARIANT_SORTED || tiled;
     if (cfg->grid_accum != MPM_ACCUM_FP64 && !(cfg->grid_accum == MPM_ACCUM_FP32 && tiled)) {
-        delete h;
+        discard(h);
         return fail(nullptr, MPM_E_ARG, "mpm_create: grid_accum must be MPM_ACCUM_FP64, or MPM_ACCUM_FP32 with the TILED family");
     }
     gd.tiled = tiled ? 1 : 0;
@@ -523,12 +536,12 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
             nt *= gd.ntile[a];
         }
         gd.Nkeys = nt * (gd.dim == 3 ? TileGeo<3>::TC : TileGeo<2>::TC);
-        if (gd.Nkeys >= (1ll << 31) - 2) { delete h; return fail(nullptr, MPM_E_ARG, "mpm_create: grid too large for 32-bit tile keys"); }
+        if (gd.Nkeys >= (1ll << 31) - 2) { discard(h); return fail(nullptr, MPM_E_ARG, "mpm_create: grid too large for 32-bit tile keys"); }
     }
     if (sorted) {   // the group records pack the cell coordinates into one int
         const int lim = gd.dim == 3 ? 1024 : 65535;
         for (int a = 0; a < gd.dim; ++a)
-            if (gd.nc[a] > lim) { delete h; return fail(nullptr, MPM_E_ARG, "mpm_create: SORTED family needs n[a] <= 1024 (3D) / 65535 (2D)"); }
+            if (gd.nc[a] > lim) { discard(h); return fail(nullptr, MPM_E_ARG, "mpm_create: SORTED family needs n[a] <= 1024 (3D) / 65535 (2D)"); }
     }
 
     // grid arrays
