@@ -137,6 +137,37 @@ def cylinder(nx=2048, ny=1024, seed=3003, recycle_seed=3004, ppc=9, steps=500):
     return dict(name=f"cylinder2d_{nx}x{ny}", cfg=cfg, x=x, v=v, mass=mass, rho=rho, e=e, cfl=0.3, steps=steps)
 
 
+def sphere_tunnel(nx=48, ny=24, nz=24, seed=6006, recycle_seed=6007, ppc=8, steps=60, mach=2.0):
+    """3D counterpart of the cylinder case (PAPER.md:543-554 with the z repetition of PAPER.md:729-733): supersonic flow
+    past a solid sphere, radius ny/6 cells, centred at (nx/3, ny/2, nz/2) cells, given as a cell mask WITHOUT node normals
+    (the library derives them from the mask, reading A7); inflow x-low, outflow x-high with recycling,
+    reflecting y and z; ppc particles uniform in every free cell.  A parity workload, not one of the BASELINE configs."""
+    h = 1.0 / ny
+    gamma = 1.4
+    u = mach * np.sqrt(gamma * 1.0 / 1.4)
+    cfg = _base_cfg(3, [nx, ny, nz], h, gamma, [[BC_INFLOW, BC_OUTFLOW], [BC_REFLECT, BC_REFLECT], [BC_REFLECT, BC_REFLECT]])
+    cfg.update(inflow_rho=1.4, inflow_p=1.0, inflow_v=[u, 0.0, 0.0], recycle_seed=recycle_seed, ppc_inflow=float(ppc))
+    ix, iy, iz = np.arange(nx) + 0.5, np.arange(ny) + 0.5, np.arange(nz) + 0.5
+    r_cells = ny / 6.0
+    mask = ((ix[None, None, :] - nx / 3.0) ** 2 + (iy[None, :, None] - ny / 2.0) ** 2 +
+            (iz[:, None, None] - nz / 2.0) ** 2) <= r_cells ** 2                    # [nz, ny, nx], x fastest
+    cfg["obstacle_mask"] = mask.astype(np.uint8).ravel()
+    rng = _rng(seed)
+    free = np.flatnonzero(~mask.ravel())
+    N = free.size * ppc
+    cell = np.repeat(free, ppc)
+    x = np.empty((3, N))
+    x[0] = ((cell % nx) + rng.uniform(0.0, 1.0, N)) * h
+    x[1] = (((cell // nx) % ny) + rng.uniform(0.0, 1.0, N)) * h
+    x[2] = ((cell // (nx * ny)) + rng.uniform(0.0, 1.0, N)) * h
+    rho = np.full(N, 1.4)
+    v = np.zeros((3, N))
+    v[0] = u
+    mass = rho * h ** 3 / ppc
+    e = np.full(N, 1.0 / ((gamma - 1.0) * 1.4))
+    return dict(name=f"sphere3d_{nx}x{ny}x{nz}", cfg=cfg, x=x, v=v, mass=mass, rho=rho, e=e, cfl=0.3, steps=steps)
+
+
 def sedov(n=256, seed=4004, jitter=0.1, steps=100, e_total=1.0, p_ambient=1e-5):
     """Config 4: 3D Sedov-type blast, n^3 cells, 8 particles/cell on a jittered 2x2x2 lattice, rho=1,
     p=1e-5, total energy 1 deposited on the particles within 2 cells of the centre; reflecting walls, CFL 0.25."""

@@ -25,6 +25,8 @@ def small_workloads():
         "clumps": lambda: inputs.clumps(n=20, num_particles=150_001),     # odd particle count
         # thousands of particles per cell: whole warps of groups in ONE cell (warp-folded reductions, shared rank atomics)
         "clumps_dense": lambda: inputs.clumps(n=16, num_particles=200_001, nclumps=3, sigma_cells=1.0),
+        # 3D inflow / outflow with recycling, reflecting walls and a sphere given as a cell mask (normals derived, A7)
+        "sphere3d": lambda: inputs.sphere_tunnel(),
     }
 
 
@@ -81,7 +83,7 @@ def test_one_step_grid_parity(po, mpm, name, mode):
     assert so.n_recycled == sg.n_recycled and so.n_clamped == sg.n_clamped
 
 
-STEPS = {"sod": 100, "box": 100, "box_shuffled": 100, "cylinder": 100, "sedov": 100, "clumps": 50, "clumps_dense": 30}
+STEPS = {"sod": 100, "box": 100, "box_shuffled": 100, "cylinder": 100, "sedov": 100, "clumps": 50, "clumps_dense": 30, "sphere3d": 40}
 
 
 @pytest.mark.parametrize("mode", MODES + [(3, 1)])
