@@ -55,7 +55,7 @@ def make_workload(name, size, rank=0):
 
 def sample_size(name):
     """Bounded sample of the same workload for the CPU oracle (about 10-30 s of single-core work)."""
-    return {"sedov": 72, "clumps": 48, "cylinder": 512, "box": 512, "sod": 256}[name]
+    return {"sedov": 96, "clumps": 64, "cylinder": 768, "box": 1024, "sod": 256}[name]
 
 
 def algorithmic_bytes(dim, n_p, n_n):
