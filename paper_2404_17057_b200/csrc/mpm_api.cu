@@ -251,6 +251,8 @@ int alloc_particles(mpm_handle *h, long long n)
     // TILED: every cell's slot range starts at an even slot -> at most one unused slot per occupied cell
     const bool tiled = h->variant == MPM_VARIANT_TILED;
     h->slots = tiled ? n + (n < h->gd.Nc ? n : h->gd.Nc) + 8 : n;
+    // slot indices, slot offsets and the look-back state of the cell map are 32-bit / 31-bit quantities
+    if (h->slots >= (1ll << 31) - 1) return fail(h, MPM_E_ARG, "mpm_load_particles: too many particles for 32-bit slot indices");
     const size_t N = (size_t)(h->slots > 0 ? h->slots : 1);
     bool ok = true;
     for (int b = 0; b < 2 && ok; ++b) {
