@@ -47,7 +47,8 @@ def _load():
     spec = importlib.util.spec_from_file_location("_oracle_build", os.path.join(_HERE, "build.py"))
     mod = importlib.util.module_from_spec(spec)
     spec.loader.exec_module(mod)
-    lib = C.CDLL(mod.build())
+    # MPM_ORACLE_LIB: a differently built copy of the same source (tests/test_oracle_sanitizers.py: ASan + UBSan)
+    lib = C.CDLL(os.environ.get("MPM_ORACLE_LIB") or mod.build())
     vp, dp = C.c_void_p, C.POINTER(C.c_double)
     lib.oracle_create.restype = vp
     lib.oracle_create.argtypes = [C.POINTER(_Config)]
