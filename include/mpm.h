@@ -32,7 +32,7 @@
 extern "C" {
 #endif
 
-#define MPM_ABI_VERSION 1
+#define MPM_ABI_VERSION 2   /* 2: mpm_stats grew three counters; the SORTED kernel family was retired */
 
 #if defined(__GNUC__)
 #define MPM_API __attribute__((visibility("default")))
@@ -55,14 +55,14 @@ enum { MPM_VISC_PRINTED = 0, MPM_VISC_STANDARD = 1 };
 /* kernel family.  AUTO = TILED when sort_every == 1, else ATOMIC.
  * ATOMIC: one thread per particle, global fp64 atomics (the paper's design); any particle order;
  *         sort_every = k > 0 adds a separate cell-key counting sort every k steps.
- * SORTED: particles are kept exactly cell-sorted every step (the re-ordering is fused into the sweeps); one cell per
- *         group of 2^dim lanes, contributions summed inside the group before one global reduction per corner and
- *         channel, corner node values staged once per group.  Ignores sort_every (always 1).
- * TILED:  SORTED's lane groups with tile-major cell order, even-aligned cell slots (128-bit particle loads) and
- *         shared-memory grid tiles: the node velocities of a tile are formed once per block from the raw sums (BC,
- *         momentum advance and quotients included), two particle sweeps per step (the next step's first P2G is fused
- *         into the particle update).  Ignores sort_every (always 1). */
-enum { MPM_VARIANT_AUTO = 0, MPM_VARIANT_ATOMIC = 1, MPM_VARIANT_SORTED = 2, MPM_VARIANT_TILED = 3 };
+ * TILED:  particles are kept exactly cell-sorted every step, in tile-major cell order with even-aligned cell slots
+ *         (128-bit particle loads); the re-ordering is fused into the sweeps; one cell per group of 2^dim / 2 lanes,
+ *         contributions summed inside the group before they reach the grid; shared-memory grid tiles: the node
+ *         velocities of a tile are formed once per block from the raw sums (BC, momentum advance and quotients
+ *         included); two particle sweeps per step (the next step's first P2G is fused into the particle update).
+ *         Ignores sort_every (always 1).
+ * (2 was the SORTED family of ABI version 1, an intermediate of TILED; mpm_create now rejects it.) */
+enum { MPM_VARIANT_AUTO = 0, MPM_VARIANT_ATOMIC = 1, MPM_VARIANT_SORTED_RETIRED = 2, MPM_VARIANT_TILED = 3 };
 /* precision of the node sums m, mv, f, mv2 ("the code supports different choices"): FP64 (default), or FP32
  * = the fp32 grid-accumulation variant of the clustered stress workload: the scatters reduce in fp32 and the sums are
  * kept in fp32, all particle arithmetic stays fp64.  TILED family only (MPM_E_ARG otherwise). */
@@ -125,6 +125,11 @@ typedef struct mpm_stats {
     int64_t launches;         /* kernels launched by this handle so far */
     double kernel_ms[8];      /* with profiling on: device time per kernel class (MPM_K_*), CUDA events on `stream` */
     int64_t kernel_calls[8];  /* ... and how many timed launches (groups) went into it */
+    /* ABI version 2 */
+    int64_t n_cell_changes;   /* cumulative: particles whose cell changed in a step (Alg. 1 l.12); TILED family only */
+    int64_t n_out_of_cell;    /* cumulative: particles a TILED kernel found outside their group's cell (debug counter of
+                                 the exact-sort invariant; must be 0) */
+    int64_t n_bad_dt;         /* cumulative: CFL steps with v_max + c_max = 0 or non-finite; such a step runs with dt = 0 */
 } mpm_stats;
 
 typedef struct mpm_handle mpm_handle;
@@ -141,7 +146,8 @@ MPM_API int mpm_load_particles(mpm_handle *h, int64_t n, const double *const *x,
 
 /* Advance nsteps time steps of Algorithm 1.  dt > 0: fixed step.  dt <= 0: CFL mode, each step uses
  * dt = cfl * h / (vmax + cmax) from the latest device-side reduction (eq. 25/29); `cfl` is alpha.
- * dt_last: HOST, NULL = do not synchronise. */
+ * dt_last: HOST, NULL = do not synchronise.  With dt_last != NULL the call returns MPM_E_NONFINITE if a non-finite
+ * particle state or a CFL step without a positive finite dt (mpm_stats.n_bad_dt) has been seen so far. */
 MPM_API int mpm_step(mpm_handle *h, double dt, double cfl, int32_t nsteps, double *dt_last);
 
 /* Read particle fields selected by field_mask (MPM_P_*).  out: HOST array of pointers (see MPM_P_* order), each

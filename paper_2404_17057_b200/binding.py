@@ -16,7 +16,7 @@ OK, E_ARG, E_CUDA, E_OOM, E_STATE, E_NONFINITE = 0, -1, -2, -3, -4, -5
 HOST, DEVICE = 0, 1
 BC_PERIODIC, BC_REFLECT, BC_INFLOW, BC_OUTFLOW = 0, 1, 2, 3
 VISC_PRINTED, VISC_STANDARD = 0, 1
-VARIANT_AUTO, VARIANT_ATOMIC, VARIANT_SORTED, VARIANT_TILED = 0, 1, 2, 3
+VARIANT_AUTO, VARIANT_ATOMIC, VARIANT_SORTED_RETIRED, VARIANT_TILED = 0, 1, 2, 3
 ACCUM_FP64, ACCUM_FP32 = 0, 1
 P_X, P_V, P_M, P_RHO, P_E, P_Q = 1, 2, 4, 8, 16, 32
 G_MASS, G_MOMENTUM, G_FORCE, G_MOMENTUM2, G_NORMAL, G_FLAG = 0, 1, 2, 3, 4, 5
@@ -51,6 +51,7 @@ class Stats(C.Structure):
         ("sum_mass", C.c_double), ("sum_momentum", C.c_double * 3), ("sum_energy", C.c_double),
         ("num_particles", C.c_int64), ("num_nodes", C.c_int64), ("nn", C.c_int32 * 3), ("variant", C.c_int32),
         ("launches", C.c_int64), ("kernel_ms", C.c_double * 8), ("kernel_calls", C.c_int64 * 8),
+        ("n_cell_changes", C.c_int64), ("n_out_of_cell", C.c_int64), ("n_bad_dt", C.c_int64),
     ]
 
 

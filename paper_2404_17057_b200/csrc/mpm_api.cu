@@ -25,10 +25,8 @@ struct mpm_handle {
     std::vector<unsigned char> h_flag;
     std::vector<double> h_normal;   // [dim][Nn]
     int *key, *rank, *count, *scan_aux;
-    // SORTED family: cell offsets (double-buffered; the inactive one doubles as the per-cell counter of the fused
-    // re-ordering), group map, force payload S (double-buffered with the particles), destination records
-    int *off[2];
-    int ocur;
+    // TILED family: even-aligned slot offsets of the cell keys, group map, destination records
+    int *off[1];
     int *coff;            // TILED: compact storage offsets, allocated on the first storage-order read
     // TILED: the node accumulators m, mv, f are double-buffered: the update kernel of step n already scatters P2G#1 of
     // step n+1 into the other set.  acc[acur] = the set the current / next mpm_step starts from (raw P2G#1).
@@ -39,7 +37,7 @@ struct mpm_handle {
     int acur;
     bool grid_final;      // TILED: the last step's m, mv, f, mv2 have been brought to their post-BC form for mpm_read_grid
     long long slots;      // TILED: allocated slots per particle array (particles + one spare slot per odd cell)
-    int *goff, *n_groups;
+    int *n_groups;
     int4 *groups;
     int4 *items;          // TILED: work items of the tile kernels (one block each), rebuilt with the groups
     int *n_items;
@@ -51,7 +49,6 @@ struct mpm_handle {
     // TILED with fp32 accumulators: fp64 copies of the last step's m, mv, f, mv2 for mpm_read_grid (allocated on first use)
     double *rg_m, *rg_mv[3], *rg_f[3], *rg_mv2[3];
     long long max_items;
-    double *S[2];
     unsigned long long *dest;
     long long max_groups;
     DevScalars *sc;
@@ -71,6 +68,20 @@ struct mpm_handle {
 static std::string g_create_error = "";
 
 namespace {
+
+// Every entry point runs on the handle's device whatever the caller's current device is, and restores the caller's
+// device on return (one process may drive handles on several GPUs).
+struct DeviceGuard {
+    int prev;
+    bool switched;
+    explicit DeviceGuard(int device) : prev(-1), switched(false)
+    {
+        if (cudaGetDevice(&prev) == cudaSuccess && prev != device) switched = cudaSetDevice(device) == cudaSuccess;
+    }
+    ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+    DeviceGuard(const DeviceGuard &) = delete;
+    DeviceGuard &operator=(const DeviceGuard &) = delete;
+};
 
 int fail(mpm_handle *h, int code, const std::string &msg)
 {
@@ -238,8 +249,8 @@ void free_particles(mpm_handle *h)
     }
     dev_free(h, h->key); dev_free(h, h->rank);
     h->key = h->rank = nullptr;
-    dev_free(h, h->S[0]); dev_free(h, h->S[1]); dev_free(h, h->dest); dev_free(h, h->groups);
-    h->S[0] = h->S[1] = nullptr; h->dest = nullptr; h->groups = nullptr;
+    dev_free(h, h->dest); dev_free(h, h->groups);
+    h->dest = nullptr; h->groups = nullptr;
     dev_free(h, h->items); dev_free(h, h->items_alt); dev_free(h, h->groups_alt);
     h->items = h->items_alt = nullptr; h->groups_alt = nullptr; h->max_items = 0;
     h->n = h->cap = 0;
@@ -262,12 +273,11 @@ int alloc_particles(mpm_handle *h, long long n)
              dev_alloc_t(h, &p.q, N) && dev_alloc_t(h, &p.id, N);
     }
     ok = ok && dev_alloc_t(h, &h->key, N) && dev_alloc_t(h, &h->rank, N);
-    if (ok && (h->variant == MPM_VARIANT_SORTED || tiled)) {
+    if (ok && tiled) {
         const long long gs = 1ll << h->gd.dim;
         h->max_groups = n / gs + (n < h->gd.Nc ? n : h->gd.Nc) + 1;
         ok = dev_alloc_t(h, &h->dest, N) && dev_alloc_t(h, &h->groups, (size_t)h->max_groups);
-        if (ok && !tiled) ok = dev_alloc_t(h, &h->S[0], N) && dev_alloc_t(h, &h->S[1], N);
-        if (ok && tiled) {
+        if (ok) {
             h->max_items = max_items_tiled(h->gd, h->max_groups);
             ok = dev_alloc_t(h, &h->items, (size_t)h->max_items) && dev_alloc_t(h, &h->items_alt, (size_t)h->max_items) &&
                  dev_alloc_t(h, &h->groups_alt, (size_t)h->max_groups);
@@ -297,8 +307,8 @@ GArr tiled_acc(const mpm_handle *h, int which)
     return g;
 }
 
-// cell-key counting sort of all particle arrays into the other buffer (Alg. 1 l.12).  SORTED family: only after a
-// load (every later step re-orders inside its own sweeps); it also builds the group map and the force payload.
+// cell-key counting sort of all particle arrays into the other buffer (Alg. 1 l.12).  TILED family: only after a
+// load (every later step re-orders inside its own sweeps); it also builds the cell map and does the first P2G#1.
 void reorder(mpm_handle *h)
 {
     Timed timer(h, MPM_K_SORT);
@@ -316,53 +326,15 @@ void reorder(mpm_handle *h)
         GArr g0 = tiled_acc(h, 0);
         launch_grid_clear(h->gd, g0, h->stream);
         for (int a = 0; a < h->gd.dim; ++a) cudaMemsetAsync(g0.mv2[a], 0, sizeof(double) * (size_t)h->gd.Nn, h->stream);
-        launch_p2g1_tiled(h->gd, dst, g0, SortedMap{ h->groups, h->n_groups, h->goff }, h->max_groups, h->stream);
+        launch_p2g1_tiled(h->gd, dst, g0, SortedMap{ h->groups, h->n_groups }, h->max_groups, h->stream);
         h->launches += 6;
         return;
     }
-    int *count = h->variant == MPM_VARIANT_SORTED ? h->off[h->ocur] : h->count;
-    launch_key_rank(h->gd, src, h->key, h->rank, count, h->n, h->stream);
-    launch_exclusive_scan(count, h->gd.Nc + 1, h->scan_aux, h->stream);
-    launch_permute(h->gd, src, dst, h->key, h->rank, count, h->n, h->stream);
+    launch_key_rank(h->gd, src, h->key, h->rank, h->count, h->n, h->stream);
+    launch_exclusive_scan(h->count, h->gd.Nc + 1, h->scan_aux, h->stream);
+    launch_permute(h->gd, src, dst, h->key, h->rank, h->count, h->n, h->stream);
     h->cur ^= 1;
     h->launches += 6;
-    if (h->variant == MPM_VARIANT_SORTED) {
-        launch_force_payload(h->gd, dst, h->S[h->cur], h->n, h->stream);
-        launch_build_groups(h->gd, count, h->goff, h->scan_aux, h->groups, h->n_groups, h->stream);
-        h->launches += 6;
-    }
-}
-
-// one step of Algorithm 1 with the SORTED kernel family (see mpm_kernels_sorted.cu)
-void step_sorted(mpm_handle *h)
-{
-    const GridDesc &gd = h->gd;
-    cudaStream_t s = h->stream;
-    const PArr &p = h->pbuf[h->cur];
-    const PArr &q = h->pbuf[h->cur ^ 1];
-    int *off_old = h->off[h->ocur], *off_new = h->off[h->ocur ^ 1];
-    const SortedMap map{ h->groups, h->n_groups, nullptr };
-    (void)off_old;
-    {
-        Timed t(h, MPM_K_MISC);
-        launch_begin_step(h->sc, gd.h, s);                                                // dt (eq. 25/29)
-        launch_grid_clear(gd, h->g, s);                                                   // l.2
-        cudaMemsetAsync(off_new, 0, sizeof(int) * (size_t)(gd.Nc + 1), s);                // per-cell counters of l.12
-    }
-    { Timed t(h, MPM_K_P2G1); launch_p2g1_sorted(gd, p, h->S[h->cur], h->g, map, h->max_groups, s); }              // l.3
-    { Timed t(h, MPM_K_NODE1); launch_node1(gd, h->g, h->sc, s); }                                                 // l.4-5
-    { Timed t(h, MPM_K_G2P_P2G2);
-      launch_g2p_p2g2_sorted(gd, p, h->g, h->g.na, h->sc, map, off_new, h->dest, h->max_groups, s); }              // l.6-8
-    { Timed t(h, MPM_K_NODE2); launch_node2(gd, h->g, s); }                                                        // l.9
-    { Timed t(h, MPM_K_SORT); launch_exclusive_scan(off_new, gd.Nc + 1, h->scan_aux, s); }                         // l.12 offsets
-    { Timed t(h, MPM_K_UPDATE);
-      launch_update_sorted(gd, p, q, h->g.na, h->g.nb, h->sc, map, off_new, h->dest, h->S[h->cur ^ 1], h->max_groups, s); }  // l.10-12
-    { Timed t(h, MPM_K_MISC); launch_end_step(h->sc, gd.h, s); }                                                   // l.13-14
-    { Timed t(h, MPM_K_SORT);
-      launch_build_groups(gd, off_new, h->goff, h->scan_aux, h->groups, h->n_groups, s); }                         // next step's groups
-    h->cur ^= 1;
-    h->ocur ^= 1;
-    h->launches += 16;
 }
 
 // one step of Algorithm 1 with the TILED kernel family (see mpm_kernels_tiled.cu): l.3 of this step was done by the
@@ -373,11 +345,11 @@ void step_tiled(mpm_handle *h, bool last_of_call)
     cudaStream_t s = h->stream;
     const PArr &p = h->pbuf[h->cur];
     const PArr &q = h->pbuf[h->cur ^ 1];
-    const SortedMap map{ h->groups, h->n_groups, h->goff };
+    const SortedMap map{ h->groups, h->n_groups };
     const GArr gc = tiled_acc(h, h->acur), gnx = tiled_acc(h, h->acur ^ 1);
     {
         Timed t(h, MPM_K_MISC);
-        launch_begin_step(h->sc, gd.h, s);                                                // dt (eq. 25/29)
+        launch_begin_step(h->sc, gd.h, true, s);                                          // dt (eq. 25/29)
         // l.2 for the next step: its accumulator set (m, mv, f for l.3, mv2 for l.8; last read by the previous step's
         // update kernel) is cleared on the second stream while this step's gather kernel runs
         cudaEventRecord(h->ev_fork, s);
@@ -451,7 +423,11 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev <= 0)
         return fail(nullptr, MPM_E_CUDA, "mpm_create: no CUDA device (this library has no CPU fallback)");
     if (cfg->device < 0 || cfg->device >= ndev) return fail(nullptr, MPM_E_ARG, "mpm_create: bad device ordinal");
-    if (cudaSetDevice(cfg->device) != cudaSuccess) return fail(nullptr, MPM_E_CUDA, "mpm_create: cudaSetDevice failed");
+    DeviceGuard guard(cfg->device);
+    {
+        int now = -1;
+        if (cudaGetDevice(&now) != cudaSuccess || now != cfg->device) return fail(nullptr, MPM_E_CUDA, "mpm_create: cudaSetDevice failed");
+    }
 
     mpm_handle *h = new (std::nothrow) mpm_handle();
     if (!h) return fail(nullptr, MPM_E_OOM, "mpm_create: host allocation failed");
@@ -468,11 +444,11 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
     h->profiling = false;
     for (int k = 0; k < MPM_K_COUNT; ++k) { h->kernel_ms[k] = 0.0; h->kernel_calls[k] = 0; }
     h->d_flag = nullptr; h->key = h->rank = h->count = h->scan_aux = nullptr; h->sc = nullptr;
-    h->off[0] = h->off[1] = nullptr; h->ocur = 0; h->goff = h->n_groups = nullptr; h->groups = nullptr;
+    h->off[0] = nullptr; h->n_groups = nullptr; h->groups = nullptr;
     h->items = nullptr; h->n_items = nullptr; h->max_items = 0;
     h->rg_m = nullptr; for (int a = 0; a < 3; ++a) h->rg_mv[a] = h->rg_f[a] = h->rg_mv2[a] = nullptr;
     h->groups_alt = h->items_alt = nullptr; h->n_groups_alt = h->n_items_alt = nullptr; h->map_state = nullptr;
-    h->S[0] = h->S[1] = nullptr; h->dest = nullptr; h->max_groups = 0; h->coff = nullptr; h->slots = 0;
+    h->dest = nullptr; h->max_groups = 0; h->coff = nullptr; h->slots = 0;
     std::memset(h->pbuf, 0, sizeof(h->pbuf));
     std::memset(&h->g, 0, sizeof(h->g));
     for (int a = 0; a < 3; ++a) h->d_normal[a] = nullptr;
@@ -516,12 +492,14 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
 
     h->variant = cfg->variant == MPM_VARIANT_AUTO ? (cfg->sort_every == 1 ? MPM_VARIANT_TILED : MPM_VARIANT_ATOMIC)
                                                    : cfg->variant;
-    if (h->variant != MPM_VARIANT_ATOMIC && h->variant != MPM_VARIANT_SORTED && h->variant != MPM_VARIANT_TILED) {
+    if (h->variant != MPM_VARIANT_ATOMIC && h->variant != MPM_VARIANT_TILED) {
         discard(h);
-        return fail(nullptr, MPM_E_ARG, "mpm_create: unknown kernel variant");
+        return fail(nullptr, MPM_E_ARG, cfg->variant == MPM_VARIANT_SORTED_RETIRED
+                                            ? "mpm_create: the SORTED kernel family was retired (superseded by TILED)"
+                                            : "mpm_create: unknown kernel variant");
     }
     const bool tiled = h->variant == MPM_VARIANT_TILED;
-    const bool sorted = h->variant == MPM_VARIANT_SORTED || tiled;
+    const bool sorted = tiled;
     if (cfg->grid_accum != MPM_ACCUM_FP64 && !(cfg->grid_accum == MPM_ACCUM_FP32 && tiled)) {
         discard(h);
         return fail(nullptr, MPM_E_ARG, "mpm_create: grid_accum must be MPM_ACCUM_FP64, or MPM_ACCUM_FP32 with the TILED family");
@@ -543,7 +521,7 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
     if (sorted) {   // the group records pack the cell coordinates into one int
         const int lim = gd.dim == 3 ? 1024 : 65535;
         for (int a = 0; a < gd.dim; ++a)
-            if (gd.nc[a] > lim) { discard(h); return fail(nullptr, MPM_E_ARG, "mpm_create: SORTED family needs n[a] <= 1024 (3D) / 65535 (2D)"); }
+            if (gd.nc[a] > lim) { discard(h); return fail(nullptr, MPM_E_ARG, "mpm_create: TILED family needs n[a] <= 1024 (3D) / 65535 (2D)"); }
     }
 
     // grid arrays
@@ -565,11 +543,8 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
             ok = dev_alloc_t(h, &h->acc_mv[1][a], (size_t)gd.Nn) && dev_alloc_t(h, &h->acc_f[1][a], (size_t)gd.Nn) &&
                  dev_alloc_t(h, &h->acc_mv2[1][a], (size_t)gd.Nn);
     }
-    if (ok && sorted && !tiled)   // node-major node velocities; the TILED kernels form them per tile in shared memory
-        ok = dev_alloc_t(h, &h->g.na, (size_t)gd.Nn * 2 * gd.dim) && dev_alloc_t(h, &h->g.nb, (size_t)gd.Nn * gd.dim);
     if (ok && sorted)
-        ok = dev_alloc_t(h, &h->off[0], (size_t)gd.Nkeys + 1) && dev_alloc_t(h, &h->off[1], (size_t)gd.Nkeys + 1) &&
-             dev_alloc_t(h, &h->goff, (size_t)gd.Nkeys + 1) && dev_alloc_t(h, &h->n_groups, 1) && dev_alloc_t(h, &h->n_items, 1);
+        ok = dev_alloc_t(h, &h->off[0], (size_t)gd.Nkeys + 1) && dev_alloc_t(h, &h->n_groups, 1) && dev_alloc_t(h, &h->n_items, 1);
     if (ok && tiled) {
         unsigned char *st = nullptr;
         ok = dev_alloc_t(h, &h->n_groups_alt, 1) && dev_alloc_t(h, &h->n_items_alt, 1) && dev_alloc_t(h, &st, cell_map_state_bytes(gd));
@@ -602,8 +577,6 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
         for (int j = 0; j < 6 && e == cudaSuccess; ++j)
             if (arrs[j]) e = cudaMemsetAsync(arrs[j], 0, sizeof(double) * (size_t)gd.Nn, h->stream);
     }
-    if (sorted && !tiled && e == cudaSuccess) e = cudaMemsetAsync(h->g.na, 0, sizeof(double) * (size_t)gd.Nn * 2 * gd.dim, h->stream);
-    if (sorted && !tiled && e == cudaSuccess) e = cudaMemsetAsync(h->g.nb, 0, sizeof(double) * (size_t)gd.Nn * gd.dim, h->stream);
     if (sorted && e == cudaSuccess) e = cudaMemsetAsync(h->n_groups, 0, sizeof(int), h->stream);
     if (sorted && e == cudaSuccess) e = cudaMemsetAsync(h->n_items, 0, sizeof(int), h->stream);
     if (tiled && e == cudaSuccess) e = cudaMemsetAsync(h->acc_m[1], 0, sizeof(double) * (size_t)gd.Nn, h->stream);
@@ -625,6 +598,7 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
 void mpm_destroy(mpm_handle *h)
 {
     if (!h) return;
+    DeviceGuard guard(h->cfg.device);
     drain_spans(h);
     cudaStreamSynchronize(h->stream);
     for (cudaEvent_t e : h->event_pool) cudaEventDestroy(e);
@@ -640,6 +614,7 @@ int mpm_load_particles(mpm_handle *h, int64_t n, const double *const *x, const d
                        const double *rho, const double *e, const double *q, int ptr_location)
 {
     if (!h) return MPM_E_ARG;
+    DeviceGuard guard(h->cfg.device);
     if (n < 0 || n >= (1ll << 31) - 1 || !x || !v || !mass || !rho || !e)
         return fail(h, MPM_E_ARG, "mpm_load_particles: bad argument");
     if (ptr_location != MPM_HOST && ptr_location != MPM_DEVICE) return fail(h, MPM_E_ARG, "mpm_load_particles: bad ptr_location");
@@ -704,6 +679,7 @@ __global__ void k_set_mode(DevScalars *sc, double dt_fixed, double alpha)
 int mpm_step(mpm_handle *h, double dt, double cfl, int32_t nsteps, double *dt_last)
 {
     if (!h) return MPM_E_ARG;
+    DeviceGuard guard(h->cfg.device);
     if (!h->pbuf[0].m) return fail(h, MPM_E_STATE, "mpm_step: no particles loaded");
     if (nsteps < 0 || (!(dt > 0.0) && !(cfl > 0.0))) return fail(h, MPM_E_ARG, "mpm_step: need nsteps >= 0 and dt > 0 or cfl > 0");
     const GridDesc &gd = h->gd;
@@ -712,13 +688,13 @@ int mpm_step(mpm_handle *h, double dt, double cfl, int32_t nsteps, double *dt_la
     h->launches += 1;
     for (int it = 0; it < nsteps; ++it) {
         if (h->variant != MPM_VARIANT_ATOMIC) {
-            if (h->n > 0) { if (h->variant == MPM_VARIANT_TILED) step_tiled(h, it == nsteps - 1); else step_sorted(h); }
-            else { launch_begin_step(h->sc, gd.h, s); launch_grid_clear(gd, h->g, s); launch_end_step(h->sc, gd.h, s); h->launches += 2; }
+            if (h->n > 0) step_tiled(h, it == nsteps - 1);
+            else { launch_begin_step(h->sc, gd.h, false, s); launch_grid_clear(gd, h->g, s); launch_end_step(h->sc, gd.h, s); h->launches += 2; }
             h->steps_done += 1;
             continue;
         }
         const PArr &p = h->pbuf[h->cur];
-        { Timed t(h, MPM_K_MISC); launch_begin_step(h->sc, gd.h, s); launch_grid_clear(gd, h->g, s); }   // dt (eq. 25/29); l.2
+        { Timed t(h, MPM_K_MISC); launch_begin_step(h->sc, gd.h, h->n > 0, s); launch_grid_clear(gd, h->g, s); }   // dt (eq. 25/29); l.2
         { Timed t(h, MPM_K_P2G1); launch_p2g1_atomic(gd, p, h->g, h->n, s); }                  // l.3
         { Timed t(h, MPM_K_NODE1); launch_node1(gd, h->g, h->sc, s); }                         // l.4-5
         { Timed t(h, MPM_K_G2P_P2G2); launch_g2p_p2g2_atomic(gd, p, h->g, h->sc, h->n, s); }   // l.6-8
@@ -736,6 +712,7 @@ int mpm_step(mpm_handle *h, double dt, double cfl, int32_t nsteps, double *dt_la
         MPM_CUDA(h, cudaStreamSynchronize(s));
         *dt_last = host.dt;
         if (host.n_nonfinite) return fail(h, MPM_E_NONFINITE, "mpm_step: non-finite particle state encountered");
+        if (host.n_bad_dt) return fail(h, MPM_E_NONFINITE, "mpm_step: no positive finite CFL time step (v_max + c_max is zero or not finite)");
     }
     return MPM_OK;
 }
@@ -743,6 +720,7 @@ int mpm_step(mpm_handle *h, double dt, double cfl, int32_t nsteps, double *dt_la
 int mpm_read_particles(mpm_handle *h, uint32_t field_mask, double *const *out, int order, int ptr_location)
 {
     if (!h || !out) return MPM_E_ARG;
+    DeviceGuard guard(h->cfg.device);
     if (!h->pbuf[0].m) return fail(h, MPM_E_STATE, "mpm_read_particles: no particles loaded");
     if (ptr_location != MPM_HOST && ptr_location != MPM_DEVICE) return fail(h, MPM_E_ARG, "mpm_read_particles: bad ptr_location");
     const PArr &p = h->pbuf[h->cur];
@@ -757,7 +735,7 @@ int mpm_read_particles(mpm_handle *h, uint32_t field_mask, double *const *out, i
     if (field_mask & MPM_P_E) { src.push_back(p.e); tmp.push_back(scratch.e); }
     if (field_mask & MPM_P_Q) { src.push_back(p.q); tmp.push_back(scratch.q); }
     const bool tiled = h->variant == MPM_VARIANT_TILED && h->n > 0;
-    const SortedMap map{ h->groups, h->n_groups, h->goff };
+    const SortedMap map{ h->groups, h->n_groups };
     if (tiled && order != 0) {   // storage order without the unused slots: compact offsets = scan of the per-key counts
         if (!h->coff && !dev_alloc_t(h, &h->coff, (size_t)h->gd.Nkeys + 1)) return fail(h, MPM_E_OOM, "mpm_read_particles: out of device memory");
         launch_exclusive_scan_from(h->count, h->coff, h->gd.Nkeys + 1, h->scan_aux, false, h->stream);
@@ -785,6 +763,7 @@ int mpm_read_particles(mpm_handle *h, uint32_t field_mask, double *const *out, i
 int mpm_read_grid(mpm_handle *h, int field, double *out, int ptr_location)
 {
     if (!h || !out) return MPM_E_ARG;
+    DeviceGuard guard(h->cfg.device);
     if (ptr_location != MPM_HOST && ptr_location != MPM_DEVICE) return fail(h, MPM_E_ARG, "mpm_read_grid: bad ptr_location");
     const GridDesc &gd = h->gd;
     const size_t Nn = (size_t)gd.Nn;
@@ -853,11 +832,12 @@ int mpm_read_grid(mpm_handle *h, int field, double *out, int ptr_location)
 int mpm_get_stats(mpm_handle *h, mpm_stats *out)
 {
     if (!h || !out) return MPM_E_ARG;
+    DeviceGuard guard(h->cfg.device);
     std::memset(out, 0, sizeof(*out));
     DevScalars host;
     if (h->pbuf[0].m) {
         if (h->variant == MPM_VARIANT_TILED && h->n > 0)
-            launch_stats_reduce_groups(h->gd, h->pbuf[h->cur], h->sc, SortedMap{ h->groups, h->n_groups, h->goff }, h->max_groups, h->stream);
+            launch_stats_reduce_groups(h->gd, h->pbuf[h->cur], h->sc, SortedMap{ h->groups, h->n_groups }, h->max_groups, h->stream);
         else
             launch_stats_reduce(h->gd, h->pbuf[h->cur], h->sc, h->n, h->stream);
         h->launches += 2;
@@ -868,6 +848,8 @@ int mpm_get_stats(mpm_handle *h, mpm_stats *out)
     out->vmax = host.vmax; out->cmax = host.cmax;
     out->n_recycled = (int64_t)host.n_recycled; out->n_clamped = (int64_t)host.n_clamped;
     out->n_negjac = (int64_t)host.n_negjac; out->n_nonfinite = (int64_t)host.n_nonfinite;
+    out->n_cell_changes = (int64_t)host.n_cell_changes; out->n_out_of_cell = (int64_t)host.n_out_of_cell;
+    out->n_bad_dt = (int64_t)host.n_bad_dt;
     out->sum_mass = host.sum_mass; out->sum_energy = host.sum_energy;
     for (int a = 0; a < 3; ++a) { out->sum_momentum[a] = host.sum_mom[a]; out->nn[a] = h->gd.nn[a]; }
     out->num_particles = h->n; out->num_nodes = h->gd.Nn;
@@ -880,6 +862,7 @@ int mpm_get_stats(mpm_handle *h, mpm_stats *out)
 int mpm_set_profiling(mpm_handle *h, int on)
 {
     if (!h) return MPM_E_ARG;
+    DeviceGuard guard(h->cfg.device);
     drain_spans(h);
     if (on) for (int k = 0; k < MPM_K_COUNT; ++k) { h->kernel_ms[k] = 0.0; h->kernel_calls[k] = 0; }
     h->profiling = on != 0;

@@ -88,14 +88,12 @@ struct PArr {
     int *id;   // persistent id = load index
 };
 
-// node SoA.  vbar = mv'/m, acc = f/m, v2 = mv2/m are the node velocities the gathers read (ratio := 0 where m = 0, A5):
-// component-major (vbar, acc, v2; ATOMIC family) or node-major (na[node][2 dim] = vbar, acc; nb[node][dim] = v2; SORTED
-// family, so that one corner's channels come in with 16-byte loads).  The unused set is NULL.
+// node SoA.  vbar = mv'/m, acc = f/m, v2 = mv2/m are the node velocities the gathers of the ATOMIC family read (ratio := 0
+// where m = 0, A5), component-major; NULL in the TILED family, which forms them per tile node in shared memory.
 struct GArr {
     double *m;
     double *mv[3], *f[3], *mv2[3];
     double *vbar[3], *acc[3], *v2[3];
-    double *na, *nb;
     const unsigned char *flag;   // 1 = obstacle node, NULL when there is no obstacle
     const double *normal[3];
 };
@@ -111,6 +109,10 @@ struct DevScalars {
     unsigned long long vmax_bits, cmax_bits;   // running maxima (non-negative doubles compared as integers)
     long long step;
     unsigned long long n_recycled, n_clamped, n_negjac, n_nonfinite;
+    // cumulative: particles that changed cell in a step (l.12), particles found outside their group's cell by a tile
+    // kernel (must stay 0: the TILED family's weights rely on the exact sort), steps whose CFL dt was not a positive
+    // finite number (v_max + c_max = 0 or non-finite: dt := 0 for that step)
+    unsigned long long n_cell_changes, n_out_of_cell, n_bad_dt;
     double sum_mass, sum_mom[3], sum_energy;   // filled by the stats reduction on demand
 };
 
@@ -199,7 +201,6 @@ __device__ __forceinline__ void atomic_max_nonneg(unsigned long long *addr, doub
 struct SortedMap {
     const int4 *groups;     // [n_groups]
     const int *n_groups;    // device scalar
-    const int *goff;        // TILED: first group of every key, [Nkeys + 1] (the groups of tile t are goff[t TC] .. goff[(t+1) TC])
 };
 
 // ---------------------------------------------------------------------------------------------- launchers
@@ -210,18 +211,6 @@ void launch_g2p_p2g2_atomic(const GridDesc &gd, const PArr &p, const GArr &g, co
                             cudaStream_t s);
 void launch_update_atomic(const GridDesc &gd, const PArr &p, const GArr &g, DevScalars *sc, long long n,
                           cudaStream_t s);
-
-// SORTED family (cell-sorted particles, lane groups, butterfly reductions, fused re-ordering) -- mpm_kernels_sorted.cu
-void launch_force_payload(const GridDesc &gd, const PArr &p, double *S, long long n, cudaStream_t s);
-void launch_build_groups(const GridDesc &gd, const int *off, int *gcount_goff, int *scan_aux, int4 *groups, int *n_groups,
-                         cudaStream_t s);
-void launch_p2g1_sorted(const GridDesc &gd, const PArr &p, const double *S, const GArr &g, const SortedMap &map,
-                        long long max_groups, cudaStream_t s);
-void launch_g2p_p2g2_sorted(const GridDesc &gd, const PArr &p, const GArr &g, const double *na, const DevScalars *sc,
-                            const SortedMap &map, int *count, unsigned long long *dest, long long max_groups, cudaStream_t s);
-void launch_update_sorted(const GridDesc &gd, const PArr &p, const PArr &q, const double *na, const double *nb, DevScalars *sc,
-                          const SortedMap &map, const int *off_new, const unsigned long long *dest, double *S_out,
-                          long long max_groups, cudaStream_t s);
 
 // TILED family (tile-major cell order, even-aligned cell slots, tile nodes in shared memory) -- mpm_kernels_tiled.cu
 // Alg. 1 l.12 bookkeeping in one kernel: per-key counts -> even-aligned slot offsets off[Nkeys + 1], group records, work
@@ -262,7 +251,7 @@ void launch_node1(const GridDesc &gd, const GArr &g, const DevScalars *sc, cudaS
 void launch_node2(const GridDesc &gd, const GArr &g, cudaStream_t s);
 
 // time loop scalars -- mpm_kernels_grid.cu
-void launch_begin_step(DevScalars *sc, double h, cudaStream_t s);
+void launch_begin_step(DevScalars *sc, double h, bool have_particles, cudaStream_t s);
 void launch_end_step(DevScalars *sc, double h, cudaStream_t s);
 void launch_initial_cfl(const GridDesc &gd, const PArr &p, DevScalars *sc, long long n, cudaStream_t s);
 void launch_stats_reduce(const GridDesc &gd, const PArr &p, DevScalars *sc, long long n, cudaStream_t s);

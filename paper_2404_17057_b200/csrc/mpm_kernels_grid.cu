@@ -44,10 +44,7 @@ __global__ void __launch_bounds__(kBlock) k_node1(GridDesc gd, GArr g, const Dev
         g.f[a][i] = f[a];
         const double vb = (m != 0.0) ? mvp / m : 0.0;
         const double ac = (m != 0.0) ? f[a] / m : 0.0;
-        if (g.na) {
-            g.na[i * (2 * DIM) + a] = vb;
-            g.na[i * (2 * DIM) + DIM + a] = ac;
-        } else if (g.vbar[a]) {
+        if (g.vbar[a]) {
             g.vbar[a][i] = vb;
             g.acc[a][i] = ac;
         }
@@ -71,13 +68,24 @@ __global__ void __launch_bounds__(kBlock) k_node2(GridDesc gd, GArr g)
     for (int a = 0; a < DIM; ++a) {
         g.mv2[a][i] = mv[a];
         const double v2 = (m != 0.0) ? mv[a] / m : 0.0;
-        if (g.nb) g.nb[i * DIM + a] = v2; else if (g.v2[a]) g.v2[a][i] = v2;
+        if (g.v2[a]) g.v2[a][i] = v2;
     }
 }
 
-__global__ void k_begin_step(DevScalars *sc, double h)
+// dt of the step (eq. 25/29).  A state with v_max + c_max = 0 (cold gas at rest) or a non-finite
+// maximum has no CFL step: dt := 0 for this step (nothing moves, nothing becomes NaN) and the event is counted; mpm_step
+// reports it as MPM_E_NONFINITE when the caller asks for dt_last, mpm_get_stats shows the counter.
+__global__ void k_begin_step(DevScalars *sc, double h, int have_particles)
 {
-    sc->dt = (sc->dt_fixed > 0.0) ? sc->dt_fixed : sc->alpha * h / (sc->vmax + sc->cmax);
+    double dt = sc->dt_fixed;
+    if (!(dt > 0.0)) {
+        dt = sc->alpha * h / (sc->vmax + sc->cmax);
+        if (!(dt > 0.0) || !isfinite(dt)) {
+            dt = 0.0;
+            if (have_particles) sc->n_bad_dt += 1ull;
+        }
+    }
+    sc->dt = dt;
     sc->vmax_bits = 0ull;
     sc->cmax_bits = 0ull;
 }
@@ -86,7 +94,8 @@ __global__ void k_end_step(DevScalars *sc, double h)
 {
     sc->vmax = __longlong_as_double((long long)sc->vmax_bits);
     sc->cmax = __longlong_as_double((long long)sc->cmax_bits);
-    sc->dt_next = sc->alpha * h / (sc->vmax + sc->cmax);
+    const double dtn = sc->alpha * h / (sc->vmax + sc->cmax);
+    sc->dt_next = (dtn > 0.0 && isfinite(dtn)) ? dtn : 0.0;
     sc->t += sc->dt;
     sc->step += 1;
 }
@@ -187,7 +196,7 @@ void launch_node2(const GridDesc &gd, const GArr &g, cudaStream_t s)
     else k_node2<3><<<grid_for(gd.Nn), kBlock, 0, s>>>(gd, g);
 }
 
-void launch_begin_step(DevScalars *sc, double h, cudaStream_t s) { k_begin_step<<<1, 1, 0, s>>>(sc, h); }
+void launch_begin_step(DevScalars *sc, double h, bool have_particles, cudaStream_t s) { k_begin_step<<<1, 1, 0, s>>>(sc, h, have_particles ? 1 : 0); }
 void launch_end_step(DevScalars *sc, double h, cudaStream_t s) { k_end_step<<<1, 1, 0, s>>>(sc, h); }
 
 void launch_initial_cfl(const GridDesc &gd, const PArr &p, DevScalars *sc, long long n, cudaStream_t s)

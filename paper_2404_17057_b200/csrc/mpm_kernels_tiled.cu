@@ -1,5 +1,5 @@
-// mpm_kernels_tiled.cu -- TILED kernel family: the SORTED family's lane groups (one cell per group of 2^d / 2 lanes, two
-// particles per lane, butterfly reductions, per-group staging of corner node values, fused re-ordering) with
+// mpm_kernels_tiled.cu -- TILED kernel family: lane groups (one cell per group of 2^d / 2 lanes, two particles per lane,
+// butterfly reductions, fused re-ordering: mpm_lane_groups.cuh) with
 //
 //   * tile-major cell keys (TileGeo: 8 x 8 x 4 cells in 3D, 16 x 16 in 2D): the particles of one tile are one contiguous
 //     run of the cell-sorted order (the grid-to-particle connectivity of PAPER.md:745-748, per tile).  One thread block
@@ -15,7 +15,7 @@
 //     The force payload S = (P+Q) M / rho never goes to memory.  Node accumulators m, mv, f are double-buffered.
 //
 // Shared-memory accumulator tiles with fp64 atomicAdd were measured and dropped (git history: CAS loops stall the
-// 16 resident warps; a global RED is asynchronous): scatters use global fp64 reductions as in the SORTED family.
+// 16 resident warps; a global RED is asynchronous): scatters use global fp64 reductions.
 #include "mpm_lane_groups.cuh"
 #include "mpm_node_bc.cuh"
 
@@ -106,7 +106,7 @@ __device__ __forceinline__ bool warp_one_cell(int cell, int cnt)
 }
 
 // Group totals of the P2G#1 channels (m, mv, f) from per-lane payloads and butterfly-order weights, reduced into the node
-// accumulators g.m, g.mv, g.f with one global fp64 reduction per corner and channel (see mpm_kernels_sorted.cu):
+// accumulators g.m, g.mv, g.f with one global fp64 reduction per corner and channel:
 //   pay[i] = { M, M V_a, S } of the lane's particle i, w[i][r] = weight of corner r ^ l (0 for a particle that is not
 //   part of the group reduction).
 template <int DIM, bool ACC32>
@@ -344,6 +344,17 @@ __device__ __forceinline__ void weights_1d(const GridDesc &gd, const double X[DI
     }
 }
 
+// Is a local coordinate vector inside the closed unit cell [0, 1]^d (1 included: a particle on the upper domain face,
+// A6)?  Exact, on the integer pipe: a double in [0, 1] has a bit pattern <= that of 1.0 (sign clear, order-preserving).
+template <int DIM>
+__device__ __forceinline__ bool in_unit_cell(const double xi[DIM])
+{
+    bool in = true;
+#pragma unroll
+    for (int a = 0; a < DIM; ++a) in = in && ((unsigned long long)__double_as_longlong(xi[a]) <= 0x3FF0000000000000ull);
+    return in;
+}
+
 // phi-weighted gather of the staged tile for the TWO particles of a lane (each corner is read once for both):
 //   out[i][ch] = sum_b phi_b(X_i) n_b[ch]  (eq. 17), ch < 2 DIM (Vbar, A) without WITH_D, ch < DIM (Vbar) with it;
 //   with WITH_D also Dh[i] = h * sum_b sum_a v2_a(b) d_a phi_b(X_i), v2 = channels [DIM, 2 DIM)  (eq. 19, trace; the
@@ -461,12 +472,16 @@ template <int DIM, bool ACC32>
 __global__ void __launch_bounds__(kTB, kTBMinG) k_g2p_p2g2_tiled(GridDesc gd, PArr p, GArr g,
                                                                 const DevScalars *__restrict__ sc, SortedMap map,
                                                                 const int4 *__restrict__ items, const int *__restrict__ n_items,
-                                                                int *__restrict__ count, unsigned long long *__restrict__ dest)
+                                                                int *__restrict__ count, unsigned long long *__restrict__ dest,
+                                                                unsigned long long *__restrict__ n_cell_changes)
 {
     using TG = TileGeo<DIM>;
     constexpr int NB = 1 << DIM, LG = Geo<DIM>::LG, GPB = kTB / LG, CH = 2 * DIM, NF = 2 * DIM + 1;
     __shared__ __align__(16) double s_tile[TG::NN * CH];
     __shared__ __align__(16) double2 s_pf[NF][kTB];      // x[d], v[d], m of the thread's two particles
+    __shared__ int s_moved;
+    if (threadIdx.x == 0) s_moved = 0;
+    int n_moved = 0;
     if ((int)blockIdx.x >= *n_items) return;
     const int4 item = __ldg(items + blockIdx.x);      // {tile, first group, groups, -}
     if (item.z == 0) return;                          // a tile without particles
@@ -558,6 +573,7 @@ __global__ void __launch_bounds__(kTB, kTBMinG) k_g2p_p2g2_tiled(GridDesc gd, PA
         }
         // ranks among the particles that end up in the same cell (arrival order of the atomics, A17): issue the atomics
         const bool stay[2] = { valid[0] && key[0] == grp.cell, valid[1] && key[1] == grp.cell };
+        n_moved += (int)(valid[0] && !stay[0]) + (int)(valid[1] && !stay[1]);
         const unsigned gmask = (1u << LG) - 1u;
         const unsigned b0 = __ballot_sync(kFull, stay[0]), b1 = __ballot_sync(kFull, stay[1]);
         const unsigned g0 = (b0 >> sh) & gmask, g1 = (b1 >> sh) & gmask;
@@ -609,6 +625,11 @@ __global__ void __launch_bounds__(kTB, kTBMinG) k_g2p_p2g2_tiled(GridDesc gd, PA
         grp = nxt;
         nxt = nn;
     }
+    // particles that changed cell in this step (mpm_stats.n_cell_changes): one atomic per block
+    n_moved = __reduce_add_sync(kFull, n_moved);
+    if (lane == 0 && n_moved) atomicAdd(&s_moved, n_moved);
+    __syncthreads();
+    if (threadIdx.x == 0 && s_moved) atomicAdd(n_cell_changes, (unsigned long long)s_moved);
 }
 
 // ------------------------------------------------------------------------------------------------ Alg. 1 l.10-13 + l.3 of the next step
@@ -685,7 +706,7 @@ __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr
     stage_tile<DIM, CH, true, ACC32>(gd, org, g, dt, s_tile);
     __syncthreads();
     double vloc = 0.0, cloc = 0.0;
-    int n_rec = 0, n_clamp = 0, n_neg = 0, n_nonfin = 0;
+    int n_rec = 0, n_clamp = 0, n_neg = 0, n_nonfin = 0, n_ooc = 0;
     const double gm1 = gd.gamma - 1.0;
     for (int p0 = 0; p0 < item.z; p0 += GPB, gl += GPB) {
         int c[DIM];
@@ -713,7 +734,10 @@ __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr
         issue_x(nxt);                                 // the slots have been read: refill them for the next pass
         double W[2][DIM][2], xi[2][DIM], out[2][2 * DIM], Dh[2];
 #pragma unroll
-        for (int i = 0; i < 2; ++i) weights_1d<DIM>(gd, X[i], c, xi[i], W[i]);
+        for (int i = 0; i < 2; ++i) {
+            weights_1d<DIM>(gd, X[i], c, xi[i], W[i]);
+            n_ooc += (int)(valid[i] && !in_unit_cell<DIM>(xi[i]));      // the exact-sort invariant (must never count)
+        }
         gather_tile<DIM, CH, true>(s_tile + j0 * CH, W, out, Dh);
         // the fields that are only needed from here on stay in shared memory during the gather (register budget)
         cp_async_wait_but_one();                      // ... they have landed (the next X may still be in flight)
@@ -763,10 +787,11 @@ __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr
             double rhon = r / jac;
             if (valid[i]) {
                 if (jac <= 0.0) n_neg++;
-                if (!isfinite(En) || !isfinite(rhon)) n_nonfin++;
                 double vv = 0.0, vb2 = 0.0;
 #pragma unroll
                 for (int a = 0; a < DIM; ++a) { vv = fma(Vo[i][a], Vo[i][a], vv); vb2 = fma(out[i][a], out[i][a], vb2); }
+                // E', rho', V' and Vbar (hence X' = X + dt Vbar) all finite?
+                if (!isfinite(En) || !isfinite(rhon) || !isfinite(vv + vb2)) n_nonfin++;
                 vloc = fmax(vloc, fmax(vv, vb2));                // squared; the root is taken once at the end
                 cloc = fmax(cloc, gd.gamma * gm1 * En);          // c_s^2 = gamma P'/rho' (the root is monotone: taken at the end)
             }
@@ -828,6 +853,7 @@ __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr
             double xin[DIM];
 #pragma unroll
             for (int a = 0; a < DIM; ++a) xin[a] = __dmul_rn(Xo[i][a], gd.inv_h) - (double)c[a];
+            n_ooc += (int)(stay[i] && !in_unit_cell<DIM>(xin));      // both kernels must agree on X' bit for bit
             swizzled_weights<DIM>(xin, l, wn[i]);
             pay[i][0] = stay[i] ? Mo[i] : 0.0;
             pay[i][DIM + 1] = stay[i] ? Sn[i] : 0.0;
@@ -843,12 +869,14 @@ __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr
     cloc = warp_max_nonneg(cloc > 0.0 ? sqrt(cloc) : 0.0);
     if (lane == 0) { s_v[warp] = vloc; s_c[warp] = cloc; }
     const int rec_sum = __reduce_add_sync(kFull, n_rec), neg_sum = __reduce_add_sync(kFull, n_neg),
-              nf_sum = __reduce_add_sync(kFull, n_nonfin), clamp_sum = __reduce_add_sync(kFull, n_clamp);
+              nf_sum = __reduce_add_sync(kFull, n_nonfin), clamp_sum = __reduce_add_sync(kFull, n_clamp),
+              ooc_sum = __reduce_add_sync(kFull, n_ooc);
     if (lane == 0) {
         if (rec_sum) atomicAdd(&sc->n_recycled, (unsigned long long)rec_sum);
         if (neg_sum) atomicAdd(&sc->n_negjac, (unsigned long long)neg_sum);
         if (nf_sum) atomicAdd(&sc->n_nonfinite, (unsigned long long)nf_sum);
         if (clamp_sum) atomicAdd(&sc->n_clamped, (unsigned long long)clamp_sum);
+        if (ooc_sum) atomicAdd(&sc->n_out_of_cell, (unsigned long long)ooc_sum);
     }
     __syncthreads();
     if (threadIdx.x == 0) {
@@ -1135,7 +1163,9 @@ void launch_g2p_p2g2_tiled(const GridDesc &gd, const PArr &p, const GArr &g, con
                            unsigned long long *dest, cudaStream_t s)
 {
     if (max_items <= 0) return;
-#define MPM_LAUNCH_G2P(D, A) k_g2p_p2g2_tiled<D, A><<<(unsigned)max_items, kTB, 0, s>>>(gd, p, g, sc, map, items, n_items, count, dest)
+#define MPM_LAUNCH_G2P(D, A) \
+    k_g2p_p2g2_tiled<D, A><<<(unsigned)max_items, kTB, 0, s>>>(gd, p, g, sc, map, items, n_items, count, dest, \
+                                                               const_cast<unsigned long long *>(&sc->n_cell_changes))
     if (gd.dim == 2) { if (gd.acc32) MPM_LAUNCH_G2P(2, true); else MPM_LAUNCH_G2P(2, false); }
     else { if (gd.acc32) MPM_LAUNCH_G2P(3, true); else MPM_LAUNCH_G2P(3, false); }
 #undef MPM_LAUNCH_G2P
@@ -1147,14 +1177,7 @@ void launch_update_tiled(const GridDesc &gd, const PArr &p, const PArr &q, const
 {
     if (max_items <= 0) return;
     const int sq = store_q ? 1 : 0;
-    static bool attr_set = false;      // more than 48 KB of dynamic shared memory needs the opt-in, once per process
-    if (!attr_set) {
-        cudaFuncSetAttribute(k_update_tiled<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UpdSmem<2>::BYTES);
-        cudaFuncSetAttribute(k_update_tiled<3, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UpdSmem<3>::BYTES);
-        cudaFuncSetAttribute(k_update_tiled<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UpdSmem<2>::BYTES);
-        cudaFuncSetAttribute(k_update_tiled<3, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)UpdSmem<3>::BYTES);
-        attr_set = true;
-    }
+    static_assert(UpdSmem<2>::BYTES <= 48 * 1024 && UpdSmem<3>::BYTES <= 48 * 1024, "dynamic shared memory beyond 48 KB needs a per-device opt-in");
 #define MPM_LAUNCH_UPD(D, A) \
     k_update_tiled<D, A><<<(unsigned)max_items, kTB, UpdSmem<D>::BYTES, s>>>(gd, p, q, g, sc, map, items, n_items, off_new, dest, g_next, sq)
     if (gd.dim == 2) { if (gd.acc32) MPM_LAUNCH_UPD(2, true); else MPM_LAUNCH_UPD(2, false); }

@@ -1,4 +1,4 @@
-// mpm_lane_groups.cuh -- device helpers shared by the SORTED and TILED kernel families: lane-group geometry, the
+// mpm_lane_groups.cuh -- device helpers of the TILED kernel family: lane-group geometry, the
 // transposed butterfly reduction, corner weights in natural / butterfly order, slow paths for a particle whose cell
 // is not its group's cell, and the particle move of Alg. 1 l.11.
 #pragma once
