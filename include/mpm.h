@@ -32,7 +32,7 @@
 extern "C" {
 #endif
 
-#define MPM_ABI_VERSION 2   /* 2: mpm_stats grew three counters; the SORTED kernel family was retired */
+#define MPM_ABI_VERSION 2   /* 2: mpm_stats grew three counters, mpm_config two fields; the SORTED kernel family was retired */
 
 #if defined(__GNUC__)
 #define MPM_API __attribute__((visibility("default")))
@@ -67,6 +67,10 @@ enum { MPM_VARIANT_AUTO = 0, MPM_VARIANT_ATOMIC = 1, MPM_VARIANT_SORTED_RETIRED 
  * = the fp32 grid-accumulation variant of the clustered stress workload: the scatters reduce in fp32 and the sums are
  * kept in fp32, all particle arithmetic stays fp64.  TILED family only (MPM_E_ARG otherwise). */
 enum { MPM_ACCUM_FP64 = 0, MPM_ACCUM_FP32 = 1 };
+/* how the TILED kernels bring the next pass's particle fields into shared memory: CP_ASYNC (default) = per-thread
+ * 16-byte cp.async; BULK = one bulk asynchronous copy (cp.async.bulk, the non-tensor form of TMA) per field, warp and pass,
+ * tracked by an mbarrier (a tile's particles are one contiguous run of slots).  Same results bit for bit.  TILED only. */
+enum { MPM_STREAM_CP_ASYNC = 0, MPM_STREAM_BULK = 1 };
 /* particle fields (bit mask for mpm_read_particles; output pointers are consumed in this order, a vector field
  * takes `dim` pointers) */
 enum { MPM_P_X = 1, MPM_P_V = 2, MPM_P_M = 4, MPM_P_RHO = 8, MPM_P_E = 16, MPM_P_Q = 32 };
@@ -101,6 +105,8 @@ typedef struct mpm_config {
     int32_t variant;          /* MPM_VARIANT_* */
     int32_t device;           /* CUDA device ordinal */
     int32_t grid_accum;       /* MPM_ACCUM_* (this field was `reserved`, 0, in ABI version 1) */
+    int32_t particle_stream;  /* MPM_STREAM_* (ABI version 2) */
+    int32_t reserved2;        /* must be 0 */
     void *stream;             /* cudaStream_t; NULL = the legacy default stream */
     mpm_alloc_fn alloc;       /* NULL = cudaMalloc */
     mpm_free_fn free;         /* NULL = cudaFree */

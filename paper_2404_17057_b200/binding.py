@@ -18,6 +18,7 @@ BC_PERIODIC, BC_REFLECT, BC_INFLOW, BC_OUTFLOW = 0, 1, 2, 3
 VISC_PRINTED, VISC_STANDARD = 0, 1
 VARIANT_AUTO, VARIANT_ATOMIC, VARIANT_SORTED_RETIRED, VARIANT_TILED = 0, 1, 2, 3
 ACCUM_FP64, ACCUM_FP32 = 0, 1
+STREAM_CP_ASYNC, STREAM_BULK = 0, 1
 P_X, P_V, P_M, P_RHO, P_E, P_Q = 1, 2, 4, 8, 16, 32
 G_MASS, G_MOMENTUM, G_FORCE, G_MOMENTUM2, G_NORMAL, G_FLAG = 0, 1, 2, 3, 4, 5
 
@@ -39,6 +40,7 @@ class Config(C.Structure):
         ("obstacle_mask", C.c_void_p), ("node_normals", C.c_void_p),
         ("recycle_seed", C.c_uint64), ("ppc_inflow", C.c_double),
         ("sort_every", C.c_int32), ("variant", C.c_int32), ("device", C.c_int32), ("grid_accum", C.c_int32),
+        ("particle_stream", C.c_int32), ("reserved2", C.c_int32),
         ("stream", C.c_void_p), ("alloc", ALLOC_FN), ("free", FREE_FN), ("alloc_user", C.c_void_p),
     ]
 
@@ -101,9 +103,10 @@ class MpmError(RuntimeError):
 
 class Solver:
     """mpm_handle wrapper.  `cfg` is the dict of inputs.py workloads (`w["cfg"]`); extra keyword arguments
-    (sort_every, variant, device, grid_accum) select the execution options of mpm_config."""
+    (sort_every, variant, device, grid_accum, particle_stream) select the execution options of mpm_config."""
 
-    def __init__(self, cfg, sort_every=0, variant=VARIANT_AUTO, device=0, use_torch_allocator=True, grid_accum=0):
+    def __init__(self, cfg, sort_every=0, variant=VARIANT_AUTO, device=0, use_torch_allocator=True, grid_accum=0,
+                 particle_stream=STREAM_CP_ASYNC):
         import torch
         self._lib = load()
         self._torch = torch
@@ -139,6 +142,7 @@ class Solver:
         c.recycle_seed = int(cfg.get("recycle_seed", 0)); c.ppc_inflow = float(cfg.get("ppc_inflow", 1.0))
         c.sort_every = int(sort_every); c.variant = int(variant); c.device = int(device)
         c.grid_accum = int(grid_accum)
+        c.particle_stream = int(particle_stream)
         with torch.cuda.device(self.device):
             self.stream = torch.cuda.current_stream()
         c.stream = self.stream.cuda_stream

@@ -504,8 +504,13 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
         discard(h);
         return fail(nullptr, MPM_E_ARG, "mpm_create: grid_accum must be MPM_ACCUM_FP64, or MPM_ACCUM_FP32 with the TILED family");
     }
+    if ((cfg->particle_stream != MPM_STREAM_CP_ASYNC && !(cfg->particle_stream == MPM_STREAM_BULK && tiled)) || cfg->reserved2 != 0) {
+        discard(h);
+        return fail(nullptr, MPM_E_ARG, "mpm_create: particle_stream must be MPM_STREAM_CP_ASYNC, or MPM_STREAM_BULK with the TILED family; reserved2 must be 0");
+    }
     gd.tiled = tiled ? 1 : 0;
     gd.acc32 = cfg->grid_accum == MPM_ACCUM_FP32 ? 1 : 0;
+    gd.bulk_stream = cfg->particle_stream == MPM_STREAM_BULK ? 1 : 0;
     gd.Nkeys = gd.Nc;
     if (tiled) {    // tile-major key space (TileGeo): whole tiles, so it can be larger than the number of cells
         long long nt = 1;

@@ -40,6 +40,9 @@ struct GridDesc {
     double um;
     // TILED: node accumulators m, mv, f, mv2 are fp32 (mpm_config.grid_accum = MPM_ACCUM_FP32)
     int acc32;
+    // TILED: particle fields are streamed with bulk asynchronous copies + mbarriers instead of per-thread cp.async
+    // (mpm_config.particle_stream = MPM_STREAM_BULK)
+    int bulk_stream;
 };
 
 // TILED family: the grid is cut into tiles of T0 x T1 (x T2) cells; the cell key is (tile index, cell inside the

@@ -38,7 +38,20 @@ __device__ __forceinline__ void st2(double *p, long long k, double a, double b)
     *reinterpret_cast<double2 *>(p + k) = make_double2(a, b);
 }
 
-// cp.async: 16 / 8 bytes from global memory straight into shared memory, L2 only (streamed particle data)
+// ------------------------------------------------------------------------------------------------ particle streams
+// The particle fields of the NEXT pass are copied into shared memory while the current pass computes.  Two mechanisms,
+// selected by the kernels' BULK template parameter (mpm_config.particle_stream):
+//   BULK = false (default): per-thread cp.async (SASS LDGSTS), 16 bytes per lane and field = the lane's two particles,
+//     tracked by commit groups;
+//   BULK = true: the particles of a tile are ONE contiguous run of slots (tile-major cell order), and so are the particles
+//     the 32 / LG groups of a warp work on in one pass: <= 64 slots.  Their fields come in with bulk asynchronous copies
+//     (cp.async.bulk.shared::cluster.global, the non-tensor form of TMA: SASS UBLKCP), one per field and pass, issued by
+//     lane 0 of the warp and tracked by an mbarrier (expect_tx / complete_tx); the lanes read their two particles from
+//     the warp's window.  This takes the copies off the LSU / L1TEX path and replaces 32 address computations per field
+//     by one.  Measured (profiles/r02_particle_stream.md): no faster than cp.async on config 4 and 2 % slower on config
+//     5 (a one-lane issue sequence costs as many issue slots as a full-warp LDGSTS, and an mbarrier wait more than a
+//     commit-group wait), hence not the default.
+// Both use the same shared-memory layout, [warp][field][kWin slots]: cp.async lanes own slots 2 lane, 2 lane + 1.
 __device__ __forceinline__ void cp_async16(void *smem, const void *gmem)
 {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem) : "memory");
@@ -48,9 +61,50 @@ __device__ __forceinline__ void cp_async8(void *smem, const void *gmem)
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem) : "memory");
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 // all committed groups but the most recent one have landed
 __device__ __forceinline__ void cp_async_wait_but_one() { asm volatile("cp.async.wait_group 1;" ::: "memory"); }
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+// one arrival that also announces `bytes` of bulk copies to come (0 = none: the phase completes at once)
+__device__ __forceinline__ void mbar_arrive_expect_tx(unsigned long long *bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "MPM_WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra MPM_DONE_%=;\n"
+        "bra MPM_WAIT_%=;\n"
+        "MPM_DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+// bytes: a multiple of 16; smem and gmem 16-byte aligned
+__device__ __forceinline__ void bulk_g2s(void *smem, const void *gmem, unsigned bytes, unsigned long long *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(smem)), "l"(gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+// Window of slots [w0, w0 + wn) that holds the particles of the warp's groups in one pass, widened to multiples of 4 slots
+// (16-byte alignment of the 4-byte id stream); wn = 0 for a warp without particles in this pass.  At most kWin slots.
+constexpr int kWin = 2 * 32 + 4;
+template <bool BULK>
+__device__ __forceinline__ void warp_window(int first, int cnt, int &w0, int &wn)
+{
+    if (!BULK) { w0 = 0; wn = 0; return; }
+    const int lo = __reduce_min_sync(0xffffffffu, cnt > 0 ? first : 0x7fffffff) & ~3;
+    const int hi = (__reduce_max_sync(0xffffffffu, cnt > 0 ? first + ((cnt + 1) & ~1) : 0) + 3) & ~3;
+    w0 = lo;
+    wn = hi > lo ? hi - lo : 0;
+}
 
 // Node accumulators m, mv, f, mv2: fp64 (default) or, with ACC32, fp32 values in the same allocations (the fp32
 // grid-accumulation variant of BASELINE.json config 5: particle arithmetic stays fp64, the sums on the grid and the
@@ -466,9 +520,9 @@ __device__ __forceinline__ void coop_p2g1(const GridDesc &gd, const GArr &gn, un
 // cell after the move of l.11 and its rank inside that cell, for the fused re-ordering (l.12): the particles of a group
 // that stay in their cell take consecutive ranks from ONE atomic per group (ballot + popc), only the others pay one
 // atomic each; the atomics are issued before the scatter and their results consumed after it.
-// The particle fields of the NEXT pass are copied into the thread's own shared-memory slots with cp.async while the
-// current pass computes (PfSlots).  V' overwrites V in place (the slots are this thread's own).
-template <int DIM, bool ACC32>
+// The particle fields of the NEXT pass are copied into shared memory while the current pass computes (see "particle
+// streams" above).  V' overwrites V in place.
+template <int DIM, bool ACC32, bool BULK>
 __global__ void __launch_bounds__(kTB, kTBMinG) k_g2p_p2g2_tiled(GridDesc gd, PArr p, GArr g,
                                                                 const DevScalars *__restrict__ sc, SortedMap map,
                                                                 const int4 *__restrict__ items, const int *__restrict__ n_items,
@@ -478,7 +532,8 @@ __global__ void __launch_bounds__(kTB, kTBMinG) k_g2p_p2g2_tiled(GridDesc gd, PA
     using TG = TileGeo<DIM>;
     constexpr int NB = 1 << DIM, LG = Geo<DIM>::LG, GPB = kTB / LG, CH = 2 * DIM, NF = 2 * DIM + 1;
     __shared__ __align__(16) double s_tile[TG::NN * CH];
-    __shared__ __align__(16) double2 s_pf[NF][kTB];      // x[d], v[d], m of the thread's two particles
+    __shared__ __align__(16) double s_pf[kTB / 32][NF][kWin];      // per warp: x[d], v[d], m of the pass's slot window
+    __shared__ __align__(8) unsigned long long s_bar[kTB / 32][2];  // per warp: X copies / V, M copies
     __shared__ int s_moved;
     if (threadIdx.x == 0) s_moved = 0;
     int n_moved = 0;
@@ -490,33 +545,61 @@ __global__ void __launch_bounds__(kTB, kTBMinG) k_g2p_p2g2_tiled(GridDesc gd, PA
     int gl = threadIdx.x / LG;
     Group grp = fetch_group(map.groups, (long long)item.y + gl, g_end);
     Group nxt = fetch_group(map.groups, (long long)item.y + gl + GPB, g_end);
-    // two copy groups per pass: X (needed first, refilled as soon as it has been read: a whole pass of lead time) and V, M
-    auto issue_x = [&](const Group &gr) {
-        if (2 * l < gr.cnt) {
-            const long long k0 = (long long)gr.first + 2 * l;
+    // two copy groups per pass: X (needed first, refilled as soon as it has been read: a whole pass of lead time) and V, M;
+    // w0 = first slot of the warp's window of the pass being issued (returned for the reads)
+    const int warp = threadIdx.x >> 5;
+    if (BULK) {
+        if (lane == 0) { mbar_init(&s_bar[warp][0], 1); mbar_init(&s_bar[warp][1], 1); mbar_fence_init(); }
+        __syncwarp();
+    }
+    auto issue_x = [&](const Group &gr, int w0, int wn) {
+        if (!BULK) {
+            if (2 * l < gr.cnt) {
+                const long long k0 = (long long)gr.first + 2 * l;
 #pragma unroll
-            for (int a = 0; a < DIM; ++a) cp_async16(&s_pf[a][threadIdx.x], p.x[a] + k0);
-        }
-        cp_async_commit();
-    };
-    auto issue_vm = [&](const Group &gr) {
-        if (2 * l < gr.cnt) {
-            const long long k0 = (long long)gr.first + 2 * l;
+                for (int a = 0; a < DIM; ++a) cp_async16(&s_pf[warp][a][2 * lane], p.x[a] + k0);
+            }
+            cp_async_commit();
+        } else if (lane == 0) {
+            mbar_arrive_expect_tx(&s_bar[warp][0], (unsigned)(DIM * wn * 8));
+            if (wn > 0) {
 #pragma unroll
-            for (int a = 0; a < DIM; ++a) cp_async16(&s_pf[DIM + a][threadIdx.x], p.v[a] + k0);
-            if (!gd.uniform_mass) cp_async16(&s_pf[2 * DIM][threadIdx.x], p.m + k0);
+                for (int a = 0; a < DIM; ++a) bulk_g2s(&s_pf[warp][a][0], p.x[a] + w0, (unsigned)(wn * 8), &s_bar[warp][0]);
+            }
         }
-        cp_async_commit();
     };
-    issue_x(grp);
-    issue_vm(grp);
+    auto issue_vm = [&](const Group &gr, int w0, int wn) {
+        if (!BULK) {
+            if (2 * l < gr.cnt) {
+                const long long k0 = (long long)gr.first + 2 * l;
+#pragma unroll
+                for (int a = 0; a < DIM; ++a) cp_async16(&s_pf[warp][DIM + a][2 * lane], p.v[a] + k0);
+                if (!gd.uniform_mass) cp_async16(&s_pf[warp][2 * DIM][2 * lane], p.m + k0);
+            }
+            cp_async_commit();
+        } else if (lane == 0) {
+            const int nf = gd.uniform_mass ? DIM : DIM + 1;
+            mbar_arrive_expect_tx(&s_bar[warp][1], (unsigned)(nf * wn * 8));
+            if (wn > 0) {
+#pragma unroll
+                for (int a = 0; a < DIM; ++a) bulk_g2s(&s_pf[warp][DIM + a][0], p.v[a] + w0, (unsigned)(wn * 8), &s_bar[warp][1]);
+                if (!gd.uniform_mass) bulk_g2s(&s_pf[warp][2 * DIM][0], p.m + w0, (unsigned)(wn * 8), &s_bar[warp][1]);
+            }
+        }
+    };
+    int w0, wn, w0n, wnn;
+    warp_window<BULK>(grp.first, grp.cnt, w0, wn);
+    warp_window<BULK>(nxt.first, nxt.cnt, w0n, wnn);
+    issue_x(grp, w0, wn);
+    issue_vm(grp, w0, wn);
     int org[DIM];
     tile_origin<DIM>(gd, item.x, org);
     const double dt = sc->dt;
     const long long step = sc->step;
     stage_tile<DIM, CH, false, ACC32>(gd, org, g, dt, s_tile);
     __syncthreads();
-    for (int p0 = 0; p0 < item.z; p0 += GPB, gl += GPB) {
+    unsigned parity = 0;
+    for (int p0 = 0; p0 < item.z; p0 += GPB, gl += GPB, parity ^= 1u) {
         int c[DIM];
         unpack_coords<DIM>(grp.cpack, c);
         const int local = grp.cell & (TG::TC - 1);      // grp.cell = tile-major key
@@ -524,29 +607,34 @@ __global__ void __launch_bounds__(kTB, kTBMinG) k_g2p_p2g2_tiled(GridDesc gd, PA
         const bool valid[2] = { 2 * l < grp.cnt, 2 * l + 1 < grp.cnt };
         const long long k0 = (long long)grp.first + 2 * l;
         double X[2][DIM], V[2][DIM], M[2];
-        cp_async_wait_but_one();                      // this pass's X has landed (its V, M may still be in flight)
+        const int o = !BULK ? 2 * lane : valid[0] ? (int)(k0 - w0) : 0;      // the lane's two particles inside the warp's window
+        if (BULK) mbar_wait(&s_bar[warp][0], parity); // this pass's X has landed (its V, M may still be in flight)
+        else cp_async_wait_but_one();
 #pragma unroll
         for (int a = 0; a < DIM; ++a) {
-            const double2 tx = s_pf[a][threadIdx.x];
+            const double2 tx = *reinterpret_cast<const double2 *>(&s_pf[warp][a][o]);
             X[0][a] = valid[0] ? tx.x : 0.0; X[1][a] = valid[1] ? tx.y : 0.0;
         }
-        issue_x(nxt);                                 // the slots have been read: refill them for the next pass
+        if (BULK) __syncwarp();
+        issue_x(nxt, w0n, wnn);                       // the window has been read: refill it for the next pass
         const Group nn = fetch_group(map.groups, (long long)item.y + gl + 2 * GPB, g_end);
         double W[2][DIM][2], xi[2][DIM], out[2][2 * DIM], Dh[2];
 #pragma unroll
         for (int i = 0; i < 2; ++i) weights_1d<DIM>(gd, X[i], c, xi[i], W[i]);
         gather_tile<DIM, CH, false>(s_tile + j0 * CH, W, out, Dh);
-        cp_async_wait_but_one();                      // this pass's V, M have landed (the next X may still be in flight)
+        if (BULK) mbar_wait(&s_bar[warp][1], parity); // this pass's V, M have landed (the next X may still be in flight)
+        else cp_async_wait_but_one();
 #pragma unroll
         for (int a = 0; a < DIM; ++a) {
-            const double2 tv = s_pf[DIM + a][threadIdx.x];
+            const double2 tv = *reinterpret_cast<const double2 *>(&s_pf[warp][DIM + a][o]);
             V[0][a] = valid[0] ? tv.x : 0.0; V[1][a] = valid[1] ? tv.y : 0.0;
         }
         {
-            const double2 tm = gd.uniform_mass ? make_double2(gd.um, gd.um) : s_pf[2 * DIM][threadIdx.x];
+            const double2 tm = gd.uniform_mass ? make_double2(gd.um, gd.um) : *reinterpret_cast<const double2 *>(&s_pf[warp][2 * DIM][o]);
             M[0] = valid[0] ? tm.x : 0.0; M[1] = valid[1] ? tm.y : 0.0;
         }
-        issue_vm(nxt);
+        if (BULK) __syncwarp();
+        issue_vm(nxt, w0n, wnn);
         double MV[2][DIM];
         int key[2];
 #pragma unroll
@@ -624,6 +712,9 @@ __global__ void __launch_bounds__(kTB, kTBMinG) k_g2p_p2g2_tiled(GridDesc gd, PA
         else if (valid[0]) dest[k0] = dk0;
         grp = nxt;
         nxt = nn;
+        w0 = w0n;
+        wn = wnn;
+        warp_window<BULK>(nxt.first, nxt.cnt, w0n, wnn);
     }
     // particles that changed cell in this step (mpm_stats.n_cell_changes): one atomic per block
     n_moved = __reduce_add_sync(kFull, n_moved);
@@ -638,20 +729,23 @@ __global__ void __launch_bounds__(kTB, kTBMinG) k_g2p_p2g2_tiled(GridDesc gd, PA
 // X' = X + dt Vbar; the particle is written to its cell-sorted slot of the OTHER buffer (l.12).  Then
 // P2G#1 of the NEXT step at X' into the node accumulators `gn` (the other buffer of m, mv, f): a
 // particle that stays in its cell joins the group's butterfly, the others are scattered by the whole warp (coop_p2g1).
-// Particle fields of the next pass arrive through cp.async in the thread's own shared-memory slots, as in the gather kernel.
+// Particle fields of the next pass arrive in shared memory as in the gather kernel (cp.async or bulk copies).
 template <int DIM>
 struct UpdSmem {
     using TG = TileGeo<DIM>;
     static constexpr int CH = 2 * DIM;                      // doubles per staged node: vbar, v2
     static constexpr int NF = 2 * DIM + 3;                  // x[d], v[d], m, rho, e
+    static constexpr int NW = kTB / 32;                     // warps: each has its own slot window of kWin slots per field
     static constexpr size_t TILE = sizeof(double) * TG::NN * CH;
-    static constexpr size_t PF = sizeof(double2) * NF * kTB;
-    static constexpr size_t DEST = sizeof(ulonglong2) * kTB;
-    static constexpr size_t ID = sizeof(int2) * kTB;
-    static constexpr size_t BYTES = TILE + PF + DEST + ID;
+    static constexpr size_t PF = sizeof(double) * NW * NF * kWin;
+    static constexpr size_t DEST = sizeof(unsigned long long) * NW * kWin;
+    static constexpr size_t ID = sizeof(int) * NW * kWin;
+    static constexpr size_t BAR = sizeof(unsigned long long) * NW * 2;
+    static constexpr size_t BYTES = TILE + PF + DEST + ID + BAR;
+    static_assert(TILE % 16 == 0 && PF % 16 == 0 && DEST % 16 == 0 && ID % 16 == 0, "16-byte aligned sections");
 };
 
-template <int DIM, bool ACC32>
+template <int DIM, bool ACC32, bool BULK>
 __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr p, PArr q, GArr g, DevScalars *sc, SortedMap map,
                                                               const int4 *__restrict__ items, const int *__restrict__ n_items,
                                                               const int *__restrict__ off_new,
@@ -662,9 +756,10 @@ __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr
     constexpr int NB = 1 << DIM, LG = Geo<DIM>::LG, GPB = kTB / LG, CH = SM::CH;
     extern __shared__ __align__(16) unsigned char s_raw[];
     double *s_tile = reinterpret_cast<double *>(s_raw);
-    double2 (*s_pf)[kTB] = reinterpret_cast<double2 (*)[kTB]>(s_raw + SM::TILE);
-    ulonglong2 *s_dest = reinterpret_cast<ulonglong2 *>(s_raw + SM::TILE + SM::PF);
-    int2 *s_id = reinterpret_cast<int2 *>(s_raw + SM::TILE + SM::PF + SM::DEST);
+    double (*s_pf)[SM::NF][kWin] = reinterpret_cast<double (*)[SM::NF][kWin]>(s_raw + SM::TILE);
+    unsigned long long (*s_dest)[kWin] = reinterpret_cast<unsigned long long (*)[kWin]>(s_raw + SM::TILE + SM::PF);
+    int (*s_id)[kWin] = reinterpret_cast<int (*)[kWin]>(s_raw + SM::TILE + SM::PF + SM::DEST);
+    unsigned long long (*s_bar)[2] = reinterpret_cast<unsigned long long (*)[2]>(s_raw + SM::TILE + SM::PF + SM::DEST + SM::ID);
     __shared__ double s_v[kTB / 32], s_c[kTB / 32];
     if ((int)blockIdx.x >= *n_items) return;
     const int4 item = __ldg(items + blockIdx.x);
@@ -676,29 +771,58 @@ __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr
     Group nxt = fetch_group(map.groups, (long long)item.y + gl + GPB, g_end);
     // two copy groups per pass: X and the destination record (needed first, refilled as soon as they have been read: a
     // whole pass of lead time) and the fields that are only needed after the gather
-    auto issue_x = [&](const Group &gr) {
-        if (2 * l < gr.cnt) {
-            const long long k0 = (long long)gr.first + 2 * l;
+    if (BULK) {
+        if (lane == 0) { mbar_init(&s_bar[warp][0], 1); mbar_init(&s_bar[warp][1], 1); mbar_fence_init(); }
+        __syncwarp();
+    }
+    auto issue_x = [&](const Group &gr, int w0, int wn) {
+        if (!BULK) {
+            if (2 * l < gr.cnt) {
+                const long long k0 = (long long)gr.first + 2 * l;
 #pragma unroll
-            for (int a = 0; a < DIM; ++a) cp_async16(&s_pf[a][threadIdx.x], p.x[a] + k0);
-            cp_async16(&s_dest[threadIdx.x], dest + k0);
-        }
-        cp_async_commit();
-    };
-    auto issue_rest = [&](const Group &gr) {
-        if (2 * l < gr.cnt) {
-            const long long k0 = (long long)gr.first + 2 * l;
+                for (int a = 0; a < DIM; ++a) cp_async16(&s_pf[warp][a][2 * lane], p.x[a] + k0);
+                cp_async16(&s_dest[warp][2 * lane], dest + k0);
+            }
+            cp_async_commit();
+        } else if (lane == 0) {
+            mbar_arrive_expect_tx(&s_bar[warp][0], (unsigned)((DIM + 1) * wn * 8));
+            if (wn > 0) {
 #pragma unroll
-            for (int a = 0; a < DIM; ++a) cp_async16(&s_pf[DIM + a][threadIdx.x], p.v[a] + k0);
-            if (!gd.uniform_mass) cp_async16(&s_pf[2 * DIM][threadIdx.x], p.m + k0);
-            cp_async16(&s_pf[2 * DIM + 1][threadIdx.x], p.rho + k0);
-            cp_async16(&s_pf[2 * DIM + 2][threadIdx.x], p.e + k0);
-            cp_async8(&s_id[threadIdx.x], p.id + k0);
+                for (int a = 0; a < DIM; ++a) bulk_g2s(&s_pf[warp][a][0], p.x[a] + w0, (unsigned)(wn * 8), &s_bar[warp][0]);
+                bulk_g2s(&s_dest[warp][0], dest + w0, (unsigned)(wn * 8), &s_bar[warp][0]);
+            }
         }
-        cp_async_commit();
     };
-    issue_x(grp);
-    issue_rest(grp);
+    auto issue_rest = [&](const Group &gr, int w0, int wn) {
+        if (!BULK) {
+            if (2 * l < gr.cnt) {
+                const long long k0 = (long long)gr.first + 2 * l;
+#pragma unroll
+                for (int a = 0; a < DIM; ++a) cp_async16(&s_pf[warp][DIM + a][2 * lane], p.v[a] + k0);
+                if (!gd.uniform_mass) cp_async16(&s_pf[warp][2 * DIM][2 * lane], p.m + k0);
+                cp_async16(&s_pf[warp][2 * DIM + 1][2 * lane], p.rho + k0);
+                cp_async16(&s_pf[warp][2 * DIM + 2][2 * lane], p.e + k0);
+                cp_async8(&s_id[warp][2 * lane], p.id + k0);
+            }
+            cp_async_commit();
+        } else if (lane == 0) {
+            const int nf = gd.uniform_mass ? DIM + 2 : DIM + 3;
+            mbar_arrive_expect_tx(&s_bar[warp][1], (unsigned)(nf * wn * 8 + wn * 4));
+            if (wn > 0) {
+#pragma unroll
+                for (int a = 0; a < DIM; ++a) bulk_g2s(&s_pf[warp][DIM + a][0], p.v[a] + w0, (unsigned)(wn * 8), &s_bar[warp][1]);
+                if (!gd.uniform_mass) bulk_g2s(&s_pf[warp][2 * DIM][0], p.m + w0, (unsigned)(wn * 8), &s_bar[warp][1]);
+                bulk_g2s(&s_pf[warp][2 * DIM + 1][0], p.rho + w0, (unsigned)(wn * 8), &s_bar[warp][1]);
+                bulk_g2s(&s_pf[warp][2 * DIM + 2][0], p.e + w0, (unsigned)(wn * 8), &s_bar[warp][1]);
+                bulk_g2s(&s_id[warp][0], p.id + w0, (unsigned)(wn * 4), &s_bar[warp][1]);
+            }
+        }
+    };
+    int w0, wn, w0n, wnn;
+    warp_window<BULK>(grp.first, grp.cnt, w0, wn);
+    warp_window<BULK>(nxt.first, nxt.cnt, w0n, wnn);
+    issue_x(grp, w0, wn);
+    issue_rest(grp, w0, wn);
     int org[DIM];
     tile_origin<DIM>(gd, item.x, org);
     const double dt = sc->dt;
@@ -708,7 +832,8 @@ __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr
     double vloc = 0.0, cloc = 0.0;
     int n_rec = 0, n_clamp = 0, n_neg = 0, n_nonfin = 0, n_ooc = 0;
     const double gm1 = gd.gamma - 1.0;
-    for (int p0 = 0; p0 < item.z; p0 += GPB, gl += GPB) {
+    unsigned parity = 0;
+    for (int p0 = 0; p0 < item.z; p0 += GPB, gl += GPB, parity ^= 1u) {
         int c[DIM];
         unpack_coords<DIM>(grp.cpack, c);
         const int local = grp.cell & (TG::TC - 1);
@@ -717,10 +842,12 @@ __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr
         double X[2][DIM];
         int key[2];
         long long dst[2] = { -1, -1 };
-        cp_async_wait_but_one();                      // this pass's X and destination records have landed
+        const int o = !BULK ? 2 * lane : valid[0] ? grp.first + 2 * l - w0 : 0;      // the lane's two particles inside the warp's window
+        if (BULK) mbar_wait(&s_bar[warp][0], parity); // this pass's X and destination records have landed
+        else cp_async_wait_but_one();
         {   // l.12: slot of the particle in the other buffer = offset of its new cell + its rank there; the offset load
             // is issued first so that it overlaps the gather
-            const ulonglong2 td = s_dest[threadIdx.x];
+            const ulonglong2 td = *reinterpret_cast<const ulonglong2 *>(&s_dest[warp][o]);
             key[0] = valid[0] ? (int)(td.x >> 32) : -1;
             key[1] = valid[1] ? (int)(td.y >> 32) : -1;
             if (valid[0]) dst[0] = (long long)__ldg(off_new + key[0]) + (long long)(unsigned)(td.x & 0xffffffffull);
@@ -728,10 +855,11 @@ __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr
         }
 #pragma unroll
         for (int a = 0; a < DIM; ++a) {
-            const double2 tx = s_pf[a][threadIdx.x];
+            const double2 tx = *reinterpret_cast<const double2 *>(&s_pf[warp][a][o]);
             X[0][a] = valid[0] ? tx.x : 0.0; X[1][a] = valid[1] ? tx.y : 0.0;
         }
-        issue_x(nxt);                                 // the slots have been read: refill them for the next pass
+        if (BULK) __syncwarp();
+        issue_x(nxt, w0n, wnn);                       // the window has been read: refill it for the next pass
         double W[2][DIM][2], xi[2][DIM], out[2][2 * DIM], Dh[2];
 #pragma unroll
         for (int i = 0; i < 2; ++i) {
@@ -740,24 +868,27 @@ __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr
         }
         gather_tile<DIM, CH, true>(s_tile + j0 * CH, W, out, Dh);
         // the fields that are only needed from here on stay in shared memory during the gather (register budget)
-        cp_async_wait_but_one();                      // ... they have landed (the next X may still be in flight)
+        if (BULK) mbar_wait(&s_bar[warp][1], parity); // ... they have landed (the next X may still be in flight)
+        else cp_async_wait_but_one();
         double V[2][DIM], M[2], rho[2], E[2];
         int id[2];
 #pragma unroll
         for (int a = 0; a < DIM; ++a) {
-            const double2 tv = s_pf[DIM + a][threadIdx.x];
+            const double2 tv = *reinterpret_cast<const double2 *>(&s_pf[warp][DIM + a][o]);
             V[0][a] = valid[0] ? tv.x : 0.0; V[1][a] = valid[1] ? tv.y : 0.0;
         }
         {
-            const double2 tm = gd.uniform_mass ? make_double2(gd.um, gd.um) : s_pf[2 * DIM][threadIdx.x];
-            const double2 tr = s_pf[2 * DIM + 1][threadIdx.x], te = s_pf[2 * DIM + 2][threadIdx.x];
+            const double2 tm = gd.uniform_mass ? make_double2(gd.um, gd.um) : *reinterpret_cast<const double2 *>(&s_pf[warp][2 * DIM][o]);
+            const double2 tr = *reinterpret_cast<const double2 *>(&s_pf[warp][2 * DIM + 1][o]),
+                          te = *reinterpret_cast<const double2 *>(&s_pf[warp][2 * DIM + 2][o]);
             M[0] = valid[0] ? tm.x : 0.0; M[1] = valid[1] ? tm.y : 0.0;
             rho[0] = valid[0] ? tr.x : 1.0; rho[1] = valid[1] ? tr.y : 1.0;
             E[0] = valid[0] ? te.x : 0.0; E[1] = valid[1] ? te.y : 0.0;
-            const int2 ti = s_id[threadIdx.x];
+            const int2 ti = *reinterpret_cast<const int2 *>(&s_id[warp][o]);
             id[0] = ti.x; id[1] = ti.y;
         }
-        issue_rest(nxt);
+        if (BULK) __syncwarp();
+        issue_rest(nxt, w0n, wnn);
         const Group nn = fetch_group(map.groups, (long long)item.y + gl + 2 * GPB, g_end);
         // per particle: the new state (what goes to memory), S' for the next step's force, and whether it stays in the
         // group's cell.  Straight-line code for both particles of the lane (an unused slot computes on M = 0, rho = 1,
@@ -847,22 +978,25 @@ __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr
             const unsigned mm = __ballot_sync(kFull, valid[i] && !stay[i]);
             if (mm) coop_p2g1<DIM, ACC32>(gd, gn, mm, Xo[i], Vo[i], Mo[i], Sn[i], lane);
         }
-        double pay[2][DIM + 2], wn[2][NB];      // the others join the group's butterfly: payload M, M V', S', weights at X'
+        double pay[2][DIM + 2], wnew[2][NB];      // the others join the group's butterfly: payload M, M V', S', weights at X'
 #pragma unroll
         for (int i = 0; i < 2; ++i) {
             double xin[DIM];
 #pragma unroll
             for (int a = 0; a < DIM; ++a) xin[a] = __dmul_rn(Xo[i][a], gd.inv_h) - (double)c[a];
             n_ooc += (int)(stay[i] && !in_unit_cell<DIM>(xin));      // both kernels must agree on X' bit for bit
-            swizzled_weights<DIM>(xin, l, wn[i]);
+            swizzled_weights<DIM>(xin, l, wnew[i]);
             pay[i][0] = stay[i] ? Mo[i] : 0.0;
             pay[i][DIM + 1] = stay[i] ? Sn[i] : 0.0;
 #pragma unroll
             for (int a = 0; a < DIM; ++a) pay[i][1 + a] = stay[i] ? Mo[i] * Vo[i][a] : 0.0;
         }
-        scatter_p2g1_group<DIM, ACC32>(gd, gn, c, l, grp.cnt > 0, pay, wn, warp_one_cell(grp.cell, grp.cnt));
+        scatter_p2g1_group<DIM, ACC32>(gd, gn, c, l, grp.cnt > 0, pay, wnew, warp_one_cell(grp.cell, grp.cnt));
         grp = nxt;
         nxt = nn;
+        w0 = w0n;
+        wn = wnn;
+        warp_window<BULK>(nxt.first, nxt.cnt, w0n, wnn);
     }
     // block maxima -> at most one atomicMax per block (max is order-free, so this is exact)
     vloc = warp_max_nonneg(sqrt(vloc));
@@ -1163,11 +1297,13 @@ void launch_g2p_p2g2_tiled(const GridDesc &gd, const PArr &p, const GArr &g, con
                            unsigned long long *dest, cudaStream_t s)
 {
     if (max_items <= 0) return;
-#define MPM_LAUNCH_G2P(D, A) \
-    k_g2p_p2g2_tiled<D, A><<<(unsigned)max_items, kTB, 0, s>>>(gd, p, g, sc, map, items, n_items, count, dest, \
-                                                               const_cast<unsigned long long *>(&sc->n_cell_changes))
-    if (gd.dim == 2) { if (gd.acc32) MPM_LAUNCH_G2P(2, true); else MPM_LAUNCH_G2P(2, false); }
-    else { if (gd.acc32) MPM_LAUNCH_G2P(3, true); else MPM_LAUNCH_G2P(3, false); }
+#define MPM_LAUNCH_G2P(D, A, B) \
+    k_g2p_p2g2_tiled<D, A, B><<<(unsigned)max_items, kTB, 0, s>>>(gd, p, g, sc, map, items, n_items, count, dest, \
+                                                                  const_cast<unsigned long long *>(&sc->n_cell_changes))
+#define MPM_LAUNCH_G2P_A(D, A) do { if (gd.bulk_stream) MPM_LAUNCH_G2P(D, A, true); else MPM_LAUNCH_G2P(D, A, false); } while (0)
+    if (gd.dim == 2) { if (gd.acc32) MPM_LAUNCH_G2P_A(2, true); else MPM_LAUNCH_G2P_A(2, false); }
+    else { if (gd.acc32) MPM_LAUNCH_G2P_A(3, true); else MPM_LAUNCH_G2P_A(3, false); }
+#undef MPM_LAUNCH_G2P_A
 #undef MPM_LAUNCH_G2P
 }
 
@@ -1178,10 +1314,12 @@ void launch_update_tiled(const GridDesc &gd, const PArr &p, const PArr &q, const
     if (max_items <= 0) return;
     const int sq = store_q ? 1 : 0;
     static_assert(UpdSmem<2>::BYTES <= 48 * 1024 && UpdSmem<3>::BYTES <= 48 * 1024, "dynamic shared memory beyond 48 KB needs a per-device opt-in");
-#define MPM_LAUNCH_UPD(D, A) \
-    k_update_tiled<D, A><<<(unsigned)max_items, kTB, UpdSmem<D>::BYTES, s>>>(gd, p, q, g, sc, map, items, n_items, off_new, dest, g_next, sq)
-    if (gd.dim == 2) { if (gd.acc32) MPM_LAUNCH_UPD(2, true); else MPM_LAUNCH_UPD(2, false); }
-    else { if (gd.acc32) MPM_LAUNCH_UPD(3, true); else MPM_LAUNCH_UPD(3, false); }
+#define MPM_LAUNCH_UPD(D, A, B) \
+    k_update_tiled<D, A, B><<<(unsigned)max_items, kTB, UpdSmem<D>::BYTES, s>>>(gd, p, q, g, sc, map, items, n_items, off_new, dest, g_next, sq)
+#define MPM_LAUNCH_UPD_A(D, A) do { if (gd.bulk_stream) MPM_LAUNCH_UPD(D, A, true); else MPM_LAUNCH_UPD(D, A, false); } while (0)
+    if (gd.dim == 2) { if (gd.acc32) MPM_LAUNCH_UPD_A(2, true); else MPM_LAUNCH_UPD_A(2, false); }
+    else { if (gd.acc32) MPM_LAUNCH_UPD_A(3, true); else MPM_LAUNCH_UPD_A(3, false); }
+#undef MPM_LAUNCH_UPD_A
 #undef MPM_LAUNCH_UPD
 }
 
