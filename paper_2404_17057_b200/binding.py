@@ -10,7 +10,8 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libmpm_b200.so")
+# MPM_B200_LIB: another build of the same sources (tests: the checked build libmpm_b200_checked.so)
+LIB_PATH = os.environ.get("MPM_B200_LIB") or os.path.join(_HERE, "libmpm_b200.so")
 
 OK, E_ARG, E_CUDA, E_OOM, E_STATE, E_NONFINITE = 0, -1, -2, -3, -4, -5
 HOST, DEVICE = 0, 1

@@ -295,6 +295,7 @@ int alloc_particles(mpm_handle *h, long long n)
         cudaMemsetAsync(h->dest, 0, 8 * N, h->stream);
     }
     h->n = n; h->cap = n; h->cur = 0;
+    h->gd.slots = h->slots; h->gd.max_groups = h->max_groups; h->gd.max_items = h->max_items;
     return MPM_OK;
 }
 

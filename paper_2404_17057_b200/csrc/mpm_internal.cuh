@@ -9,6 +9,16 @@
 
 #include "../../include/mpm.h"
 
+// Checked build (nvcc -DMPM_CHECKED=1, libmpm_b200_checked.so): every index the tile kernels form -- particle slots, node
+// indices, cell keys, window offsets, group and item records -- is tested against its bound and the kernel traps on a
+// violation (the next CUDA call then fails loudly).  compute-sanitizer is not available on the GPU pool, so this build
+// run through the parity tests is the memory-safety evidence (tests/test_gpu_parity.py::test_checked_build).
+#if defined(MPM_CHECKED) && MPM_CHECKED
+#define MPM_CHECK(cond) do { if (!(cond)) __trap(); } while (0)
+#else
+#define MPM_CHECK(cond) ((void)0)
+#endif
+
 namespace mpm {
 
 // ---------------------------------------------------------------------------------------------- descriptors
@@ -43,6 +53,8 @@ struct GridDesc {
     // TILED: particle fields are streamed with bulk asynchronous copies + mbarriers instead of per-thread cp.async
     // (mpm_config.particle_stream = MPM_STREAM_BULK)
     int bulk_stream;
+    // TILED: allocated slots per particle array and capacities of the group / item lists (bounds of the checked build)
+    long long slots, max_groups, max_items;
 };
 
 // TILED family: the grid is cut into tiles of T0 x T1 (x T2) cells; the cell key is (tile index, cell inside the

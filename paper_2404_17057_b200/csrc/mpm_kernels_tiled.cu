@@ -29,12 +29,19 @@ namespace {
 
 using namespace lg;
 
+#if defined(MPM_CHECKED) && MPM_CHECKED
+// bounds of the checked build, set by the launchers before every launch (one handle at a time per process in that build)
+__device__ long long g_checked_nodes = 0, g_checked_slots = 0;
+#endif
+
 __device__ __forceinline__ double2 ld2(const double *__restrict__ p, long long k, bool ok)
 {
+    MPM_CHECK(!ok || (k >= 0 && k + 1 < g_checked_slots && (k & 1) == 0));
     return ok ? __ldg(reinterpret_cast<const double2 *>(p + k)) : make_double2(0.0, 0.0);
 }
 __device__ __forceinline__ void st2(double *p, long long k, double a, double b)
 {
+    MPM_CHECK(k >= 0 && k + 1 < g_checked_slots && (k & 1) == 0);
     *reinterpret_cast<double2 *>(p + k) = make_double2(a, b);
 }
 
@@ -112,12 +119,14 @@ __device__ __forceinline__ void warp_window(int first, int cnt, int &w0, int &wn
 template <bool ACC32>
 __device__ __forceinline__ void acc_add(double *arr, long long i, double v)
 {
+    MPM_CHECK(i >= 0 && i < g_checked_nodes);
     if (ACC32) atomicAdd(reinterpret_cast<float *>(arr) + i, (float)v);
     else atomicAdd(arr + i, v);
 }
 template <bool ACC32>
 __device__ __forceinline__ double acc_ld(const double *arr, long long i)
 {
+    MPM_CHECK(i >= 0 && i < g_checked_nodes);
     if (ACC32) return (double)__ldg(reinterpret_cast<const float *>(arr) + i);
     return __ldg(arr + i);
 }
@@ -608,6 +617,8 @@ __global__ void __launch_bounds__(kTB, kTBMinG) k_g2p_p2g2_tiled(GridDesc gd, PA
         const long long k0 = (long long)grp.first + 2 * l;
         double X[2][DIM], V[2][DIM], M[2];
         const int o = !BULK ? 2 * lane : valid[0] ? (int)(k0 - w0) : 0;      // the lane's two particles inside the warp's window
+        MPM_CHECK(o >= 0 && o + 2 <= kWin && (o & 1) == 0 && j0 >= 0 && j0 + corner_off<DIM>(NB - 1) < TG::NN);
+        MPM_CHECK(!valid[0] || (k0 >= 0 && k0 + 1 < gd.slots && grp.cell >= 0 && grp.cell < gd.Nkeys && (grp.cell >> TG::LTC) == item.x));
         if (BULK) mbar_wait(&s_bar[warp][0], parity); // this pass's X has landed (its V, M may still be in flight)
         else cp_async_wait_but_one();
 #pragma unroll
@@ -660,6 +671,7 @@ __global__ void __launch_bounds__(kTB, kTBMinG) k_g2p_p2g2_tiled(GridDesc gd, PA
             else if (valid[0]) p.v[a][k0] = V[0][a];
         }
         // ranks among the particles that end up in the same cell (arrival order of the atomics, A17): issue the atomics
+        MPM_CHECK((!valid[0] || (key[0] >= 0 && key[0] < gd.Nkeys)) && (!valid[1] || (key[1] >= 0 && key[1] < gd.Nkeys)));
         const bool stay[2] = { valid[0] && key[0] == grp.cell, valid[1] && key[1] == grp.cell };
         n_moved += (int)(valid[0] && !stay[0]) + (int)(valid[1] && !stay[1]);
         const unsigned gmask = (1u << LG) - 1u;
@@ -843,6 +855,8 @@ __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr
         int key[2];
         long long dst[2] = { -1, -1 };
         const int o = !BULK ? 2 * lane : valid[0] ? grp.first + 2 * l - w0 : 0;      // the lane's two particles inside the warp's window
+        MPM_CHECK(o >= 0 && o + 2 <= kWin && (o & 1) == 0 && j0 >= 0 && j0 + corner_off<DIM>(NB - 1) < TG::NN);
+        MPM_CHECK(!valid[0] || (grp.first >= 0 && (long long)grp.first + 2 * l + 1 < gd.slots && (grp.cell >> TG::LTC) == item.x));
         if (BULK) mbar_wait(&s_bar[warp][0], parity); // this pass's X and destination records have landed
         else cp_async_wait_but_one();
         {   // l.12: slot of the particle in the other buffer = offset of its new cell + its rank there; the offset load
@@ -850,8 +864,12 @@ __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr
             const ulonglong2 td = *reinterpret_cast<const ulonglong2 *>(&s_dest[warp][o]);
             key[0] = valid[0] ? (int)(td.x >> 32) : -1;
             key[1] = valid[1] ? (int)(td.y >> 32) : -1;
+            MPM_CHECK((!valid[0] || (key[0] >= 0 && key[0] < gd.Nkeys)) && (!valid[1] || (key[1] >= 0 && key[1] < gd.Nkeys)));
             if (valid[0]) dst[0] = (long long)__ldg(off_new + key[0]) + (long long)(unsigned)(td.x & 0xffffffffull);
             if (valid[1]) dst[1] = (long long)__ldg(off_new + key[1]) + (long long)(unsigned)(td.y & 0xffffffffull);
+            // the destination slot lies inside the new cell's slot range
+            MPM_CHECK(!valid[0] || (dst[0] >= 0 && dst[0] < __ldg(off_new + key[0] + 1) && dst[0] < gd.slots));
+            MPM_CHECK(!valid[1] || (dst[1] >= 0 && dst[1] < __ldg(off_new + key[1] + 1) && dst[1] < gd.slots));
         }
 #pragma unroll
         for (int a = 0; a < DIM; ++a) {
@@ -1128,7 +1146,10 @@ __global__ void __launch_bounds__(kMapBlock) k_cell_map_tiled(GridDesc gd, const
                 int cc[DIM];
                 tiled_cell_of_key<DIM>(gd, key, cc);
                 const int cpack = (DIM == 3) ? (cc[0] | (cc[1] << 10) | (cc[DIM - 1] << 20)) : (cc[0] | (cc[1] << 16));
-                for (int first = 0; first < c[j]; first += CAP, ++g) groups[g] = make_int4(slot + first, min(CAP, c[j] - first), key, cpack);
+                for (int first = 0; first < c[j]; first += CAP, ++g) {
+                    MPM_CHECK(g >= 0 && g < gd.max_groups && (long long)slot + c[j] <= gd.slots);
+                    groups[g] = make_int4(slot + first, min(CAP, c[j] - first), key, cpack);
+                }
             }
             slot += (c[j] + 1) & ~1;
         }
@@ -1143,7 +1164,10 @@ __global__ void __launch_bounds__(kMapBlock) k_cell_map_tiled(GridDesc gd, const
             if (ng > per_item) {
                 const int more = (ng - 1) / per_item;
                 int at = ntiles + atomicAdd(&state->extra, more);
-                for (int done = per_item; done < ng; done += per_item) items[at++] = make_int4(tile, gfirst + done, min(per_item, ng - done), 0);
+                for (int done = per_item; done < ng; done += per_item) {
+                    MPM_CHECK(at >= 0 && at < gd.max_items);
+                    items[at++] = make_int4(tile, gfirst + done, min(per_item, ng - done), 0);
+                }
             }
         }
     }
@@ -1244,6 +1268,17 @@ inline unsigned persistent_blocks(long long max_groups, int groups_per_block, Ke
 
 }  // namespace
 
+// checked build: publish the array bounds the raw access helpers test against
+static void set_checked_bounds(const GridDesc &gd, cudaStream_t s)
+{
+#if defined(MPM_CHECKED) && MPM_CHECKED
+    cudaMemcpyToSymbolAsync(g_checked_nodes, &gd.Nn, sizeof(long long), 0, cudaMemcpyHostToDevice, s);
+    cudaMemcpyToSymbolAsync(g_checked_slots, &gd.slots, sizeof(long long), 0, cudaMemcpyHostToDevice, s);
+#else
+    (void)gd; (void)s;
+#endif
+}
+
 size_t cell_map_state_bytes(const GridDesc &gd)
 {
     const long long n_blocks = (gd.Nkeys + kMapKeys - 1) / kMapKeys;
@@ -1267,6 +1302,7 @@ void launch_cell_map_tiled(const GridDesc &gd, const int *count, int *off, int4 
 void launch_p2g1_tiled(const GridDesc &gd, const PArr &p, const GArr &g, const SortedMap &map, long long max_groups, cudaStream_t s)
 {
     if (max_groups <= 0) return;
+    set_checked_bounds(gd, s);
 #define MPM_LAUNCH_P2G1(D, A) \
     k_p2g1_tiled<D, A><<<persistent_blocks(max_groups, Geo<D>::GPB, k_p2g1_tiled<D, A>), kBlock, 0, s>>>(gd, p, g, map)
     if (gd.dim == 2) { if (gd.acc32) MPM_LAUNCH_P2G1(2, true); else MPM_LAUNCH_P2G1(2, false); }
@@ -1297,6 +1333,7 @@ void launch_g2p_p2g2_tiled(const GridDesc &gd, const PArr &p, const GArr &g, con
                            unsigned long long *dest, cudaStream_t s)
 {
     if (max_items <= 0) return;
+    set_checked_bounds(gd, s);
 #define MPM_LAUNCH_G2P(D, A, B) \
     k_g2p_p2g2_tiled<D, A, B><<<(unsigned)max_items, kTB, 0, s>>>(gd, p, g, sc, map, items, n_items, count, dest, \
                                                                   const_cast<unsigned long long *>(&sc->n_cell_changes))
@@ -1312,6 +1349,7 @@ void launch_update_tiled(const GridDesc &gd, const PArr &p, const PArr &q, const
                          const unsigned long long *dest, const GArr &g_next, bool store_q, cudaStream_t s)
 {
     if (max_items <= 0) return;
+    set_checked_bounds(gd, s);
     const int sq = store_q ? 1 : 0;
     static_assert(UpdSmem<2>::BYTES <= 48 * 1024 && UpdSmem<3>::BYTES <= 48 * 1024, "dynamic shared memory beyond 48 KB needs a per-device opt-in");
 #define MPM_LAUNCH_UPD(D, A, B) \

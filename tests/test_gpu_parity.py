@@ -450,3 +450,23 @@ def test_cold_gas_at_rest_has_no_cfl_step(mpm, variant):
     h = mpm.Solver(cfg, sort_every=1 if variant == 3 else 0, variant=variant)
     h.load_particles(x, v, np.full(n, 1e-3), np.ones(n), np.zeros(n))
     assert h.step(1e-3, 0.3, 3) == 1e-3 and h.stats().n_bad_dt == 0
+
+
+def test_checked_build(mpm):
+    """Memory-safety evidence without compute-sanitizer (closed on the GPU pool): the same sources compiled with
+    -DMPM_CHECKED=1 test every particle slot, node index, cell key, window offset, group and item record against its bound
+    and trap on a violation.  The TILED parity tests (all workloads: ragged grids, odd counts, dense cells, recycling,
+    obstacles, both particle streams, fp32 accumulation, the at-size cases) are repeated against that build in a child
+    process; a trap would fail every CUDA call after it."""
+    import os
+    import subprocess
+    import sys
+    from paper_2404_17057_b200 import build
+    lib = build.build(checked=True)
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    sel = ("(test_one_step_grid_parity and mode2) or (test_many_step_particle_parity and mode2) or bulk_particle_stream "
+           "or fp32_grid_accumulation_variant or test_edge_cases or (test_parity_at_size and (clumps64 or cylinder1024))")
+    r = subprocess.run([sys.executable, "-m", "pytest", os.path.join(root, "tests", "test_gpu_parity.py"), "-x", "-q",
+                        "-p", "no:cacheprovider", "-k", sel], env=dict(os.environ, MPM_B200_LIB=lib),
+                       capture_output=True, text=True, cwd=root)
+    assert r.returncode == 0 and " passed" in r.stdout, r.stdout[-3000:] + r.stderr[-2000:]
