@@ -108,6 +108,70 @@ void oracle_shape(const oracle_t *o, const double *X, long long *node, double *p
     }
 }
 
+/* ---------------------------------------------------------------- quadratic B-spline basis (A20)
+ * PAPER.md:721, :735-739 name quadratic B-splines [60, 19] as the next basis.  The standard MPM quadratic B-spline centred on
+ * the grid nodes:  N(u) = 3/4 - u^2 (|u| < 1/2),  (3/2 - |u|)^2 / 2 (1/2 <= |u| < 3/2),  0 otherwise,  u = (x - x_i)/h;
+ * phi_i(X) = prod_a N((X_a - x_{i,a})/h).  A particle sees 3 nodes per axis: b, b+1, b+2 with b = floor(X/h - 1/2);
+ * with f = X/h - b in [1/2, 3/2):  w(0) = (3/2 - f)^2/2,  w(1) = 3/4 - (f - 1)^2,  w(2) = (f - 1/2)^2/2  and slopes
+ * dN/dx:  -(3/2 - f)/h,  -2 (f - 1)/h,  (f - 1/2)/h.  Periodic axes only: node index modulo n. */
+typedef struct {
+    int n;                 /* 3^d */
+    long long node[27];
+    double phi[27];
+    double grad[27][3];
+} support_t;
+
+static void support_quadratic(const oracle_t *o, const double *X, long long stride, support_t *s)
+{
+    int base[3] = { 0, 0, 0 }, ns[3] = { 1, 1, 1 };
+    double w[3][3] = { { 1, 0, 0 }, { 1, 0, 0 }, { 1, 0, 0 } }, g[3][3] = { { 0, 0, 0 }, { 0, 0, 0 }, { 0, 0, 0 } };
+    for (int a = 0; a < o->d; ++a) {
+        double sx = X[a * stride] * o->inv_h;
+        int b = (int)floor(sx - 0.5);
+        double f = sx - (double)b;
+        base[a] = b; ns[a] = 3;
+        w[a][0] = 0.5 * (1.5 - f) * (1.5 - f);
+        w[a][1] = 0.75 - (f - 1.0) * (f - 1.0);
+        w[a][2] = 0.5 * (f - 0.5) * (f - 0.5);
+        g[a][0] = -(1.5 - f) * o->inv_h;
+        g[a][1] = -2.0 * (f - 1.0) * o->inv_h;
+        g[a][2] = (f - 0.5) * o->inv_h;
+    }
+    int q = 0;
+    for (int iz = 0; iz < ns[2]; ++iz)
+        for (int iy = 0; iy < ns[1]; ++iy)
+            for (int ix = 0; ix < ns[0]; ++ix, ++q) {
+                int j[3] = { ix, iy, iz }, i[3] = { 0, 0, 0 };
+                for (int a = 0; a < o->d; ++a) {
+                    int t = (base[a] + j[a]) % o->nc[a];
+                    i[a] = t < 0 ? t + o->nc[a] : t;
+                }
+                s->node[q] = node_index(o, i);
+                double phi = 1.0;
+                for (int a = 0; a < o->d; ++a) phi *= w[a][j[a]];
+                s->phi[q] = phi;
+                for (int a = 0; a < 3; ++a) s->grad[q][a] = 0.0;
+                for (int a = 0; a < o->d; ++a) {
+                    double t = g[a][j[a]];
+                    for (int a2 = 0; a2 < o->d; ++a2)
+                        if (a2 != a) t *= w[a2][j[a2]];
+                    s->grad[q][a] = t;
+                }
+            }
+    s->n = q;
+}
+
+void oracle_shape_quadratic(const oracle_t *o, const double *X, long long *node, double *phi, double *grad)
+{
+    support_t s;
+    support_quadratic(o, X, 1, &s);
+    for (int q = 0; q < s.n; ++q) {
+        node[q] = s.node[q];
+        phi[q] = s.phi[q];
+        for (int a = 0; a < o->d; ++a) grad[q * o->d + a] = s.grad[q][a];
+    }
+}
+
 /* counter-based uniform in [0,1): the splitmix64 finaliser (Steele, Lea & Flood 2014) applied to
  * a counter built from (seed, id, step, j).  Restated independently in the CUDA path (A8). */
 static unsigned long long mix64(unsigned long long z)
@@ -247,6 +311,11 @@ oracle_t *oracle_create(const oracle_config *cfg)
         o->Nn *= o->nn[a];
         o->Nc *= o->nc[a];
     }
+    if (cfg->basis != ORC_BASIS_Q1) {      /* A20: quadratic B-splines on fully periodic grids of >= 3 cells per axis */
+        int ok = cfg->basis == ORC_BASIS_QUADRATIC && !cfg->obstacle_mask;
+        for (int a = 0; a < o->d; ++a) ok = ok && o->per[a] && o->nc[a] >= 3;
+        if (!ok) { free(o); return NULL; }
+    }
     if (cfg->obstacle_mask) {
         o->mask = (unsigned char *)malloc((size_t)o->Nc);
         memcpy(o->mask, cfg->obstacle_mask, (size_t)o->Nc);
@@ -348,9 +417,22 @@ void oracle_p2g1(oracle_t *o)
     const int nb = 1 << o->d;
     for (long long k = 0; k < n; ++k) {
         int c[3]; double w[3][2], g[3][2];
-        particle_cell(o, &o->X[k], n, c, w, g);
         double P = (o->cfg.gamma - 1.0) * o->rho[k] * o->E[k];
         double S = (P + o->Q[k]) * o->M[k] / o->rho[k];
+        if (o->cfg.basis == ORC_BASIS_QUADRATIC) {   /* the same three sums over the 3^d nodes of the B-spline support */
+            support_t s;
+            support_quadratic(o, &o->X[k], n, &s);
+            for (int q = 0; q < s.n; ++q) {
+                long long i = s.node[q];
+                o->m[i] += o->M[k] * s.phi[q];
+                for (int a = 0; a < o->d; ++a) {
+                    o->mv[a * Nn + i] += o->M[k] * o->V[a * n + k] * s.phi[q];
+                    o->f[a * Nn + i] += S * s.grad[q][a];
+                }
+            }
+            continue;
+        }
+        particle_cell(o, &o->X[k], n, c, w, g);
         for (int ib = 0; ib < nb; ++ib) {
             int b[3] = { ib & 1, (ib >> 1) & 1, (ib >> 2) & 1 };
             double phi, grad[3];
@@ -429,8 +511,22 @@ void oracle_g2p_velocity(oracle_t *o, double dt)
     const int nb = 1 << o->d;
     for (long long k = 0; k < n; ++k) {
         int c[3]; double w[3][2], g[3][2];
-        particle_cell(o, &o->X[k], n, c, w, g);
         double vb[3] = { 0, 0, 0 }, ac[3] = { 0, 0, 0 };
+        if (o->cfg.basis == ORC_BASIS_QUADRATIC) {
+            support_t s;
+            support_quadratic(o, &o->X[k], n, &s);
+            for (int q = 0; q < s.n; ++q) {
+                long long i = s.node[q];
+                double mi = o->m[i];
+                for (int a = 0; a < o->d; ++a) {
+                    double vel = (mi != 0.0) ? o->mv[a * Nn + i] / mi : 0.0;
+                    double acc = (mi != 0.0) ? o->f[a * Nn + i] / mi : 0.0;
+                    vb[a] += s.phi[q] * vel;
+                    ac[a] += s.phi[q] * acc;
+                }
+            }
+        } else {
+        particle_cell(o, &o->X[k], n, c, w, g);
         for (int ib = 0; ib < nb; ++ib) {
             int b[3] = { ib & 1, (ib >> 1) & 1, (ib >> 2) & 1 };
             double phi, grad[3];
@@ -443,6 +539,7 @@ void oracle_g2p_velocity(oracle_t *o, double dt)
                 vb[a] += phi * vel;
                 ac[a] += phi * acc;
             }
+        }
         }
         for (int a = 0; a < o->d; ++a) {
             o->Vbar[a * n + k] = vb[a];
@@ -460,6 +557,13 @@ void oracle_p2g2(oracle_t *o)
     memset(o->mv2, 0, sizeof(double) * (size_t)(o->d * Nn));
     for (long long k = 0; k < n; ++k) {
         int c[3]; double w[3][2], g[3][2];
+        if (o->cfg.basis == ORC_BASIS_QUADRATIC) {
+            support_t s;
+            support_quadratic(o, &o->X[k], n, &s);
+            for (int q = 0; q < s.n; ++q)
+                for (int a = 0; a < o->d; ++a) o->mv2[a * Nn + s.node[q]] += o->M[k] * o->V[a * n + k] * s.phi[q];
+            continue;
+        }
         particle_cell(o, &o->X[k], n, c, w, g);
         for (int ib = 0; ib < nb; ++ib) {
             int b[3] = { ib & 1, (ib >> 1) & 1, (ib >> 2) & 1 };
@@ -488,8 +592,19 @@ void oracle_particle_update(oracle_t *o, double dt)
     long long nonfinite = 0;
     for (long long k = 0; k < n; ++k) {
         int c[3]; double w[3][2], g[3][2];
-        particle_cell(o, &o->X[k], n, c, w, g);
         double D = 0.0;
+        if (o->cfg.basis == ORC_BASIS_QUADRATIC) {
+            support_t s;
+            support_quadratic(o, &o->X[k], n, &s);
+            for (int q = 0; q < s.n; ++q) {
+                double mi = o->m[s.node[q]];
+                for (int a = 0; a < o->d; ++a) {
+                    double vel = (mi != 0.0) ? o->mv2[a * Nn + s.node[q]] / mi : 0.0;
+                    D += vel * s.grad[q][a];
+                }
+            }
+        } else {
+        particle_cell(o, &o->X[k], n, c, w, g);
         for (int ib = 0; ib < nb; ++ib) {
             int b[3] = { ib & 1, (ib >> 1) & 1, (ib >> 2) & 1 };
             double phi, grad[3];
@@ -500,6 +615,7 @@ void oracle_particle_update(oracle_t *o, double dt)
                 double vel = (mi != 0.0) ? o->mv2[a * Nn + i] / mi : 0.0;
                 D += vel * grad[a];
             }
+        }
         }
         o->D[k] = D;
         double rho = o->rho[k], E = o->E[k];

@@ -32,6 +32,12 @@ enum { ORC_BC_PERIODIC = 0, ORC_BC_REFLECT = 1, ORC_BC_INFLOW = 2, ORC_BC_OUTFLO
 /* artificial-viscosity form (reading A3): eq. (4) as printed, or the textbook vNR+Landshoff */
 enum { ORC_VISC_PRINTED = 0, ORC_VISC_STANDARD = 1 };
 
+/* shape functions: the paper's Q1 hats, or the quadratic B-splines it names as the next basis
+ * (the standard MPM quadratic B-spline of its refs. [60, 19]).  The quadratic basis is offered on
+ * fully periodic grids only: the paper does not say how a spline whose support leaves the grid is to be modified at a
+ * wall (reading A20). */
+enum { ORC_BASIS_Q1 = 0, ORC_BASIS_QUADRATIC = 1 };
+
 /* grid fields for oracle_read_grid (content = whatever the last sub-step left there) */
 enum { ORC_G_MASS = 0, ORC_G_MOM = 1, ORC_G_FORCE = 2, ORC_G_MOM2 = 3, ORC_G_NORMAL = 4, ORC_G_FLAG = 5 };
 /* particle fields for oracle_read_particles */
@@ -51,6 +57,7 @@ typedef struct {
     const double *node_normals;         /* [dim][N_n] component-major, NULL = derive (A7) (copied) */
     unsigned long long recycle_seed;    /* A8 */
     double ppc_inflow;                  /* A8: recycled mass = rho_in h^d / ppc_inflow */
+    int basis;                          /* ORC_BASIS_* (A20) */
 } oracle_config;
 
 typedef struct {
@@ -77,6 +84,9 @@ int oracle_load_particles(oracle_t *o, long long n, const double *x, const doubl
 
 /* Q1 shape functions at a point (3D by :729-733): node[2^d], phi[2^d], grad[2^d*d] */
 void oracle_shape(const oracle_t *o, const double *X, long long *node, double *phi, double *grad);
+
+/* quadratic B-spline shape functions at a point: node[3^d], phi[3^d], grad[3^d*d] (x fastest) */
+void oracle_shape_quadratic(const oracle_t *o, const double *X, long long *node, double *phi, double *grad);
 
 /* counter-based generator of reading A8, exported so that the tests can pin it to the published
  * splitmix64 test vector: oracle_mix64(z) = output function applied to state z + golden gamma */

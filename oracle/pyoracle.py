@@ -14,6 +14,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 
 BC_PERIODIC, BC_REFLECT, BC_INFLOW, BC_OUTFLOW = 0, 1, 2, 3
 VISC_PRINTED, VISC_STANDARD = 0, 1
+BASIS_Q1, BASIS_QUADRATIC = 0, 1
 G_MASS, G_MOM, G_FORCE, G_MOM2, G_NORMAL, G_FLAG = 0, 1, 2, 3, 4, 5
 P_X, P_V, P_M, P_RHO, P_E, P_Q, P_VBAR, P_ACC, P_DIV = range(9)
 
@@ -25,7 +26,7 @@ class _Config(C.Structure):
         ("bc", (C.c_int * 2) * 3),
         ("inflow_rho", C.c_double), ("inflow_p", C.c_double), ("inflow_v", C.c_double * 3),
         ("obstacle_mask", C.c_void_p), ("node_normals", C.c_void_p),
-        ("recycle_seed", C.c_ulonglong), ("ppc_inflow", C.c_double),
+        ("recycle_seed", C.c_ulonglong), ("ppc_inflow", C.c_double), ("basis", C.c_int),
     ]
 
 
@@ -59,6 +60,7 @@ def _load():
     lib.oracle_num_particles.argtypes = [vp]
     lib.oracle_load_particles.argtypes = [vp, C.c_longlong, vp, vp, vp, vp, vp, vp]
     lib.oracle_shape.argtypes = [vp, vp, vp, vp, vp]
+    lib.oracle_shape_quadratic.argtypes = [vp, vp, vp, vp, vp]
     for name in ("oracle_grid_reset", "oracle_p2g1", "oracle_grid_bc", "oracle_p2g2", "oracle_grid_bc2"):
         getattr(lib, name).argtypes = [vp]
         getattr(lib, name).restype = None
@@ -93,7 +95,7 @@ def recycle_uniform(seed, pid, step, j):
 class Oracle:
     """Thin handle around oracle_t.  `cfg` is a dict with the keys of oracle_config
     (dim, n, dx, gamma, c0, c1, visc_form, bc, inflow_rho, inflow_p, inflow_v, obstacle_mask,
-    node_normals, recycle_seed, ppc_inflow); missing keys take the documented defaults."""
+    node_normals, recycle_seed, ppc_inflow, basis); missing keys take the documented defaults."""
 
     def __init__(self, cfg):
         lib = _load()
@@ -131,6 +133,7 @@ class Oracle:
             c.node_normals = normals.ctypes.data
         c.recycle_seed = int(cfg.get("recycle_seed", 0))
         c.ppc_inflow = float(cfg.get("ppc_inflow", 1.0))
+        c.basis = int(cfg.get("basis", BASIS_Q1))
         self.dim = d
         self._h = lib.oracle_create(C.byref(c))
         if not self._h:
@@ -167,6 +170,15 @@ class Oracle:
         phi = np.zeros(nb)
         grad = np.zeros((nb, self.dim))
         self._lib.oracle_shape(self._h, X.ctypes.data, node.ctypes.data, phi.ctypes.data, grad.ctypes.data)
+        return node, phi, grad
+
+    def shape_quadratic(self, X):
+        X = _f64(X)
+        nb = 3 ** self.dim
+        node = np.zeros(nb, dtype=np.int64)
+        phi = np.zeros(nb)
+        grad = np.zeros((nb, self.dim))
+        self._lib.oracle_shape_quadratic(self._h, X.ctypes.data, node.ctypes.data, phi.ctypes.data, grad.ctypes.data)
         return node, phi, grad
 
     # ---- Algorithm 1, line by line
