@@ -363,6 +363,15 @@ static double sound_speed(const oracle_t *o, double rho, double e)
 int oracle_load_particles(oracle_t *o, long long n, const double *x, const double *v,
                           const double *mass, const double *rho, const double *e, const double *q)
 {
+    return oracle_load_particles_ex(o, n, x, v, mass, rho, e, q, NULL, 0);
+}
+
+/* ids: persistent ids chosen by the caller (NULL = the load index); keep_time: time, step, maxima and counters survive
+ * (a slab of a decomposed domain replacing its particle set, tests/slab_oracle_engine.py) */
+int oracle_load_particles_ex(oracle_t *o, long long n, const double *x, const double *v,
+                             const double *mass, const double *rho, const double *e, const double *q,
+                             const long long *ids, int keep_time)
+{
     if (!o || n < 0) return -1;
     free_particles(o);
     o->Np = n;
@@ -383,7 +392,8 @@ int oracle_load_particles(oracle_t *o, long long n, const double *x, const doubl
     memcpy(o->rho, rho, sizeof(double) * (size_t)n);
     memcpy(o->E, e, sizeof(double) * (size_t)n);
     if (q) memcpy(o->Q, q, sizeof(double) * (size_t)n);
-    for (long long k = 0; k < n; ++k) o->id[k] = k;
+    for (long long k = 0; k < n; ++k) o->id[k] = ids ? ids[k] : k;
+    if (keep_time) return 0;
     memset(&o->st, 0, sizeof(o->st));
     /* first CFL reduction from the loaded state, ||V|| only (A13) */
     double vmax = 0.0, cmax = 0.0;
@@ -674,8 +684,12 @@ void oracle_advect(oracle_t *o, double dt)
                 } else {
                     double u1 = recycle_uniform(cfg->recycle_seed, id, o->st.step, j++);
                     double u2 = recycle_uniform(cfg->recycle_seed, id, o->st.step, j++);
-                    int cell = (int)floor(u1 * (double)o->nc[a]);
-                    if (cell > o->nc[a] - 1) cell = o->nc[a] - 1;
+                    /* a slab of a larger domain (last axis): the inflow face is the global one, the cell index slab-local */
+                    int slab = cfg->slab_global_n > 0 && a == o->d - 1;
+                    int na = slab ? cfg->slab_global_n : o->nc[a];
+                    int cell = (int)floor(u1 * (double)na);
+                    if (cell > na - 1) cell = na - 1;
+                    if (slab) cell -= cfg->slab_offset;
                     Xn[a] = ((double)cell + u2) * o->h;
                 }
                 o->V[a * n + k] = cfg->inflow_v[a];
@@ -689,9 +703,9 @@ void oracle_advect(oracle_t *o, double dt)
             o->st.n_recycled++;
         }
         for (int a = 0; a < o->d; ++a) {
-            if (!o->per[a]) {
-                if (Xn[a] < 0.0) { Xn[a] = 0.0; o->st.n_clamped++; }
-                if (Xn[a] > o->L[a]) { Xn[a] = o->L[a]; o->st.n_clamped++; }
+            if (!o->per[a]) {   /* an OPEN face is an interface to a neighbouring slab: the particle leaves, unclamped */
+                if (Xn[a] < 0.0 && cfg->bc[a][0] != ORC_BC_OPEN) { Xn[a] = 0.0; o->st.n_clamped++; }
+                if (Xn[a] > o->L[a] && cfg->bc[a][1] != ORC_BC_OPEN) { Xn[a] = o->L[a]; o->st.n_clamped++; }
             }
             o->X[a * n + k] = Xn[a];
         }
@@ -721,6 +735,14 @@ void oracle_cfl(oracle_t *o, double alpha)
     o->st.dt_next = alpha * o->h / (vmax + cmax);
 }
 
+/* l.13 time advance for a caller that drives Algorithm 1 line by line (oracle_step does the same inline) */
+void oracle_advance_time(oracle_t *o, double dt)
+{
+    o->st.t += dt;
+    o->st.dt_last = dt;
+    o->st.step += 1;
+}
+
 int oracle_step(oracle_t *o, double dt_fixed, double alpha, int nsteps, double *dt_last)
 {
     if (!o) return -1;
@@ -741,6 +763,27 @@ int oracle_step(oracle_t *o, double dt_fixed, double alpha, int nsteps, double *
         o->st.step += 1;
     }
     if (dt_last) *dt_last = o->st.dt_last;
+    return 0;
+}
+
+/* Node plane `side` (0 low, 1 high) of the last axis of a slab: which = 0: m, mv[d], f[d]; 1: mv2[d].  op 0: buf <- plane,
+ * op 1: plane += buf (the halo sum-exchange of a decomposed domain).  buf: [channels][plane nodes]. */
+int oracle_halo(oracle_t *o, int which, int side, int op, double *buf)
+{
+    if (!o || !buf || (which != 0 && which != 1) || (side != 0 && side != 1) || (op != 0 && op != 1)) return -1;
+    const int last = o->d - 1;
+    const long long plane = o->Nn / o->nn[last], at = side ? (long long)(o->nn[last] - 1) * plane : 0;
+    double *ch[7]; int nch = 0;
+    if (which == 0) {
+        ch[nch++] = o->m;
+        for (int a = 0; a < o->d; ++a) ch[nch++] = o->mv + a * o->Nn;
+        for (int a = 0; a < o->d; ++a) ch[nch++] = o->f + a * o->Nn;
+    } else for (int a = 0; a < o->d; ++a) ch[nch++] = o->mv2 + a * o->Nn;
+    for (int c = 0; c < nch; ++c)
+        for (long long j = 0; j < plane; ++j) {
+            if (op == 0) buf[c * plane + j] = ch[c][at + j];
+            else ch[c][at + j] += buf[c * plane + j];
+        }
     return 0;
 }
 

@@ -28,7 +28,8 @@ extern "C" {
 #endif
 
 /* boundary-condition codes per face, bc[axis][side] (side 0 = low, 1 = high) */
-enum { ORC_BC_PERIODIC = 0, ORC_BC_REFLECT = 1, ORC_BC_INFLOW = 2, ORC_BC_OUTFLOW = 3 };
+enum { ORC_BC_PERIODIC = 0, ORC_BC_REFLECT = 1, ORC_BC_INFLOW = 2, ORC_BC_OUTFLOW = 3,
+       ORC_BC_OPEN = 4 /* interface to a neighbouring slab of a decomposed domain: no nodal condition, no clamp */ };
 /* artificial-viscosity form (reading A3): eq. (4) as printed, or the textbook vNR+Landshoff */
 enum { ORC_VISC_PRINTED = 0, ORC_VISC_STANDARD = 1 };
 
@@ -58,6 +59,8 @@ typedef struct {
     unsigned long long recycle_seed;    /* A8 */
     double ppc_inflow;                  /* A8: recycled mass = rho_in h^d / ppc_inflow */
     int basis;                          /* ORC_BASIS_* (A20) */
+    int slab_global_n, slab_offset;     /* > 0: this grid is cells [offset, offset + n[last]) of slab_global_n along the last
+                                           axis (recycled particles are placed on the GLOBAL inflow face) */
 } oracle_config;
 
 typedef struct {
@@ -81,6 +84,12 @@ long long oracle_num_particles(const oracle_t *o);
  * Also performs the first CFL reduction from the loaded state (A13). */
 int oracle_load_particles(oracle_t *o, long long n, const double *x, const double *v,
                           const double *mass, const double *rho, const double *e, const double *q);
+
+int oracle_load_particles_ex(oracle_t *o, long long n, const double *x, const double *v,
+                             const double *mass, const double *rho, const double *e, const double *q,
+                             const long long *ids, int keep_time);
+int oracle_halo(oracle_t *o, int which, int side, int op, double *buf);
+void oracle_advance_time(oracle_t *o, double dt);
 
 /* Q1 shape functions at a point (3D by :729-733): node[2^d], phi[2^d], grad[2^d*d] */
 void oracle_shape(const oracle_t *o, const double *X, long long *node, double *phi, double *grad);

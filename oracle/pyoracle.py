@@ -12,7 +12,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 
-BC_PERIODIC, BC_REFLECT, BC_INFLOW, BC_OUTFLOW = 0, 1, 2, 3
+BC_PERIODIC, BC_REFLECT, BC_INFLOW, BC_OUTFLOW, BC_OPEN = 0, 1, 2, 3, 4
 VISC_PRINTED, VISC_STANDARD = 0, 1
 BASIS_Q1, BASIS_QUADRATIC = 0, 1
 G_MASS, G_MOM, G_FORCE, G_MOM2, G_NORMAL, G_FLAG = 0, 1, 2, 3, 4, 5
@@ -27,6 +27,7 @@ class _Config(C.Structure):
         ("inflow_rho", C.c_double), ("inflow_p", C.c_double), ("inflow_v", C.c_double * 3),
         ("obstacle_mask", C.c_void_p), ("node_normals", C.c_void_p),
         ("recycle_seed", C.c_ulonglong), ("ppc_inflow", C.c_double), ("basis", C.c_int),
+        ("slab_global_n", C.c_int), ("slab_offset", C.c_int),
     ]
 
 
@@ -59,13 +60,15 @@ def _load():
     lib.oracle_num_particles.restype = C.c_longlong
     lib.oracle_num_particles.argtypes = [vp]
     lib.oracle_load_particles.argtypes = [vp, C.c_longlong, vp, vp, vp, vp, vp, vp]
+    lib.oracle_load_particles_ex.argtypes = [vp, C.c_longlong, vp, vp, vp, vp, vp, vp, vp, C.c_int]
+    lib.oracle_halo.argtypes = [vp, C.c_int, C.c_int, C.c_int, vp]
     lib.oracle_shape.argtypes = [vp, vp, vp, vp, vp]
     lib.oracle_shape_quadratic.argtypes = [vp, vp, vp, vp, vp]
     for name in ("oracle_grid_reset", "oracle_p2g1", "oracle_grid_bc", "oracle_p2g2", "oracle_grid_bc2"):
         getattr(lib, name).argtypes = [vp]
         getattr(lib, name).restype = None
     for name in ("oracle_grid_advance", "oracle_g2p_velocity", "oracle_particle_update", "oracle_advect",
-                 "oracle_cfl"):
+                 "oracle_cfl", "oracle_advance_time"):
         getattr(lib, name).argtypes = [vp, C.c_double]
         getattr(lib, name).restype = None
     lib.oracle_mix64.restype = C.c_ulonglong
@@ -134,6 +137,7 @@ class Oracle:
         c.recycle_seed = int(cfg.get("recycle_seed", 0))
         c.ppc_inflow = float(cfg.get("ppc_inflow", 1.0))
         c.basis = int(cfg.get("basis", BASIS_Q1))
+        c.slab_global_n = int(cfg.get("slab_global_n", 0)); c.slab_offset = int(cfg.get("slab_offset", 0))
         self.dim = d
         self._h = lib.oracle_create(C.byref(c))
         if not self._h:
@@ -152,16 +156,23 @@ class Oracle:
         self.close()
 
     # ---- particles
-    def load_particles(self, x, v, mass, rho, e, q=None):
+    def load_particles(self, x, v, mass, rho, e, q=None, ids=None, keep_time=False):
         x, v, mass, rho, e = _f64(x), _f64(v), _f64(mass), _f64(rho), _f64(e)
         n = mass.shape[0]
         assert x.shape == (self.dim, n) and v.shape == (self.dim, n)
         qq = _f64(q) if q is not None else None
-        rc = self._lib.oracle_load_particles(self._h, n, x.ctypes.data, v.ctypes.data, mass.ctypes.data,
-                                             rho.ctypes.data, e.ctypes.data,
-                                             qq.ctypes.data if qq is not None else None)
+        ii = np.ascontiguousarray(ids, dtype=np.int64) if ids is not None else None
+        rc = self._lib.oracle_load_particles_ex(self._h, n, x.ctypes.data, v.ctypes.data, mass.ctypes.data,
+                                                rho.ctypes.data, e.ctypes.data,
+                                                qq.ctypes.data if qq is not None else None,
+                                                ii.ctypes.data if ii is not None else None, 1 if keep_time else 0)
         assert rc == 0
         self.n = n
+
+    def halo(self, which, side, op, buf):
+        """buf: C-contiguous float64 [channels, plane nodes]; op 0 = export into buf, 1 = add buf to the plane"""
+        assert buf.dtype == np.float64 and buf.flags["C_CONTIGUOUS"]
+        assert self._lib.oracle_halo(self._h, int(which), int(side), int(op), buf.ctypes.data) == 0
 
     def shape(self, X):
         X = _f64(X)
@@ -192,6 +203,7 @@ class Oracle:
     def particle_update(self, dt): self._lib.oracle_particle_update(self._h, float(dt))
     def advect(self, dt): self._lib.oracle_advect(self._h, float(dt))
     def cfl(self, alpha): self._lib.oracle_cfl(self._h, float(alpha))
+    def advance_time(self, dt): self._lib.oracle_advance_time(self._h, float(dt))
 
     def step(self, dt=0.0, cfl=0.3, nsteps=1):
         out = C.c_double(0.0)
