@@ -222,7 +222,8 @@ def run_ours(args):
         dim = w["cfg"]["dim"]
         n_p = int(w["mass"].shape[0])
         g = mpm.Solver(w["cfg"], sort_every=1, variant=variant, device=local, grid_accum=accum,
-                       particle_stream=mpm.STREAM_BULK if args.stream == "bulk" else mpm.STREAM_CP_ASYNC)
+                       particle_stream=mpm.STREAM_BULK if args.stream == "bulk" else mpm.STREAM_CP_ASYNC,
+                       p2g_mode=args.p2g_mode)
         n_n = g.num_nodes
         g.load_particles(w["x"], w["v"], w["mass"], w["rho"], w["e"])
         g.step(0.0, w["cfl"], warmup, sync=False)
@@ -278,7 +279,7 @@ def run_ours(args):
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64" if args.grid_accum == "fp64" else "f64 particles, f32 grid accumulation (separate variant)", "data": "synthetic",
         "config": {"workload": w["name"], "grid_accum": args.grid_accum, "particles_per_gpu": n_p, "nodes": n_n, "dim": dim,
-                   "kernel_family": args.variant, "particle_stream": args.stream, "parallelism": f"replicas x{world}",
+                   "kernel_family": args.variant, "particle_stream": args.stream, "p2g_mode": args.p2g_mode, "parallelism": f"replicas x{world}",
                    "l2": "inputs (%.1f GB particle state) exceed the 126 MB L2; no flush" % (n_p * (2 * dim + 5) * 8 / 1e9),
                    "movers_per_step": r["movers"],
                    "window": "steps %d-%d after the load" % (args.warmup + 1, args.warmup + args.steps)},
@@ -353,6 +354,9 @@ def main():
                     help="fp32: the fp32 grid-accumulation variant of config 5 (tiled family), reported separately")
     ap.add_argument("--stream", default="cp_async", choices=["cp_async", "bulk"],
                     help="particle stream of the tile kernels: per-thread cp.async (default) or bulk copies (TMA) + mbarriers")
+    ap.add_argument("--p2g-mode", type=int, default=0, choices=[0, 1, 2, 3],
+                    help="0 = global reductions (default); bit 0 / bit 1: atomics-free shared-memory accumulation by cell "
+                         "colour in the gather / update kernel (include/mpm.h MPM_P2G_*)")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")

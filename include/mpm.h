@@ -48,8 +48,10 @@ enum { MPM_HOST = 0, MPM_DEVICE = 1 };
  * PERIODIC must be set on both sides of an axis.  REFLECT: v.n = 0 (eq. 30), normal components of
  * nodal momentum and force zeroed.  INFLOW: Dirichlet, nodal momentum = m v_in, force = 0.
  * OUTFLOW: nodal momentum untouched, normal force zeroed; particles that pass the face are recycled at the
- * first INFLOW face with the inflow state. */
-enum { MPM_BC_PERIODIC = 0, MPM_BC_REFLECT = 1, MPM_BC_INFLOW = 2, MPM_BC_OUTFLOW = 3 };
+ * first INFLOW face with the inflow state.
+ * OPEN: an interface to a neighbouring sub-domain (slab decomposition over several GPUs): no nodal
+ * condition, particles that pass it keep their position (no clamp) and are handed to the neighbour by the caller. */
+enum { MPM_BC_PERIODIC = 0, MPM_BC_REFLECT = 1, MPM_BC_INFLOW = 2, MPM_BC_OUTFLOW = 3, MPM_BC_OPEN = 4 };
 /* artificial viscosity q of eq. (4): as printed, or the textbook rho (c0 h^2 D^2 - c1 h c_s D) */
 enum { MPM_VISC_PRINTED = 0, MPM_VISC_STANDARD = 1 };
 /* kernel family.  AUTO = TILED when sort_every == 1, else ATOMIC.
@@ -71,9 +73,21 @@ enum { MPM_ACCUM_FP64 = 0, MPM_ACCUM_FP32 = 1 };
  * 16-byte cp.async; BULK = one bulk asynchronous copy (cp.async.bulk, the non-tensor form of TMA) per field, warp and pass,
  * tracked by an mbarrier (a tile's particles are one contiguous run of slots).  Same results bit for bit.  TILED only. */
 enum { MPM_STREAM_CP_ASYNC = 0, MPM_STREAM_BULK = 1 };
+/* how the TILED kernels add a group's node totals to the grid.  RED (default): one global fp64 reduction per corner and
+ * channel.  COLOUR_*: the atomics-free accumulation by cell colouring the paper proposes -- the cells of a
+ * tile are numbered colour-major, a pass's groups add into a shared-memory accumulator tile with plain additions, one
+ * colour at a time, and the tile is flushed with one reduction per node; bit 0: the second P2G (gather kernel, mv2), bit 1:
+ * the first P2G (update kernel, m, mv, f).  Same results up to summation order.  TILED, fp64 accumulation, cp.async stream. */
+enum { MPM_P2G_RED = 0, MPM_P2G_COLOUR_G2P = 1, MPM_P2G_COLOUR_UPDATE = 2, MPM_P2G_COLOUR_BOTH = 3 };
+/* shape functions.  Q1 (default): the paper's bi/tri-linear hats.  QUADRATIC: the quadratic B-splines the paper
+ * names as the next basis, N(u) = 3/4 - u^2 (|u| < 1/2), (3/2 - |u|)^2 / 2 (1/2 <= |u| < 3/2), centred
+ * on the nodes, 3^dim nodes per particle; all axes must be PERIODIC with at least 3 cells (the paper gives no wall
+ * treatment for a spline whose support leaves the grid) and the kernel family is ATOMIC (any sort_every). */
+enum { MPM_BASIS_Q1 = 0, MPM_BASIS_QUADRATIC = 1 };
 /* particle fields (bit mask for mpm_read_particles; output pointers are consumed in this order, a vector field
  * takes `dim` pointers) */
-enum { MPM_P_X = 1, MPM_P_V = 2, MPM_P_M = 4, MPM_P_RHO = 8, MPM_P_E = 16, MPM_P_Q = 32 };
+enum { MPM_P_X = 1, MPM_P_V = 2, MPM_P_M = 4, MPM_P_RHO = 8, MPM_P_E = 16, MPM_P_Q = 32,
+       MPM_P_ID = 64 /* the persistent particle id, as a double (exact below 2^53); last in the pointer order */ };
 /* grid fields for mpm_read_grid, as left by the LAST completed step (Algorithm 1):
  *   MASS       m_i                         after l.3   (1 component)
  *   MOMENTUM   (mv)'_i = mv_i + dt f_i     after l.5   (dim components)
@@ -106,11 +120,15 @@ typedef struct mpm_config {
     int32_t device;           /* CUDA device ordinal */
     int32_t grid_accum;       /* MPM_ACCUM_* (this field was `reserved`, 0, in ABI version 1) */
     int32_t particle_stream;  /* MPM_STREAM_* (ABI version 2) */
-    int32_t reserved2;        /* must be 0 */
+    int32_t p2g_mode;         /* MPM_P2G_* (ABI version 2) */
     void *stream;             /* cudaStream_t; NULL = the legacy default stream */
     mpm_alloc_fn alloc;       /* NULL = cudaMalloc */
     mpm_free_fn free;         /* NULL = cudaFree */
     void *alloc_user;
+    int32_t basis;            /* MPM_BASIS_* (ABI version 2) */
+    int32_t slab_global_n;    /* > 0: this grid is one slab of a domain with slab_global_n cells along the LAST axis ... */
+    int32_t slab_offset;      /* ... and starts at that cell of it (recycled particles are placed on the global inflow face) */
+    int32_t reserved3;        /* must be 0 */
 } mpm_config;
 
 /* kernel classes for the optional per-kernel timers (mpm_set_profiling) */
@@ -162,6 +180,34 @@ MPM_API int mpm_read_particles(mpm_handle *h, uint32_t field_mask, double *const
 
 /* Read one grid field (MPM_G_*) of the last completed step: out[ncomp][N_n], HOST or DEVICE. */
 MPM_API int mpm_read_grid(mpm_handle *h, int field, double *out, int ptr_location);
+
+/* ---- slab decomposition over several GPUs.  One handle per slab of cells along
+ * the last axis, interfaces flagged MPM_BC_OPEN.  A step is then driven in two phases with a halo SUM-exchange of the shared
+ * node plane before each (paper_2404_17057_b200/slab.py does this over torch.distributed):
+ *     exchange(MPM_HALO_P2G1)  ->  mpm_step_phase(GATHER, dt)  ->  exchange(MPM_HALO_P2G2)  ->  mpm_step_phase(UPDATE)
+ *     ->  all-reduce(max) of vmax, cmax for the next dt  ->  hand over the particles that left the slab
+ *     (mpm_read_particles / mpm_load_particles_ex), which also redoes the first P2G of the next step.
+ * mpm_step_phase(GATHER): Algorithm 1 l.4-8 with the given dt (> 0; the caller forms the global CFL step);
+ * mpm_step_phase(UPDATE): l.9-13.  Both asynchronous on the stream. */
+enum { MPM_PHASE_GATHER = 0, MPM_PHASE_UPDATE = 1 };
+MPM_API int mpm_step_phase(mpm_handle *h, int phase, double dt);
+
+/* Node plane `side` (0 = low, 1 = high) of the last axis.  which: MPM_HALO_P2G1 = raw sums m, mv[dim], f[dim] of the first P2G
+ * (1 + 2 dim channels), MPM_HALO_P2G2 = mv2[dim] of the second.  op MPM_HALO_EXPORT: buf <- plane; MPM_HALO_ADD: plane += buf.
+ * buf: [channels][nodes of the plane] doubles, HOST or DEVICE per ptr_location.  Asynchronous on the stream for DEVICE. */
+enum { MPM_HALO_P2G1 = 0, MPM_HALO_P2G2 = 1 };
+enum { MPM_HALO_EXPORT = 0, MPM_HALO_ADD = 1 };
+MPM_API int mpm_halo(mpm_handle *h, int which, int side, int op, double *buf, int ptr_location);
+
+/* mpm_load_particles with two options.  ids (HOST or DEVICE like the other arrays; NULL = the load index): persistent
+ * ids chosen by the caller, 0 <= id < 2^31 -- a slab passes the GLOBAL ids, which the recycling generator (reading A8) is
+ * keyed on; with caller-chosen ids mpm_read_particles offers storage order only (order = 1; MPM_P_ID tells which is which).
+ * flags: MPM_LOAD_KEEP_TIME = replace the particle set WITHOUT resetting time, step, CFL maxima and counters (the particles
+ * that stay in a slab plus the arrivals); the re-ordering and the first P2G of the next step are redone. */
+enum { MPM_LOAD_KEEP_TIME = 1 };
+MPM_API int mpm_load_particles_ex(mpm_handle *h, int64_t n, const double *const *x, const double *const *v,
+                          const double *mass, const double *rho, const double *e, const double *q, const int64_t *ids,
+                          int ptr_location, int flags);
 
 /* Time, step, dt, CFL maxima, counters, conserved sums (computed on the device on demand).  out: HOST. */
 MPM_API int mpm_get_stats(mpm_handle *h, mpm_stats *out);

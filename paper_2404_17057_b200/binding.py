@@ -15,18 +15,24 @@ LIB_PATH = os.environ.get("MPM_B200_LIB") or os.path.join(_HERE, "libmpm_b200.so
 
 OK, E_ARG, E_CUDA, E_OOM, E_STATE, E_NONFINITE = 0, -1, -2, -3, -4, -5
 HOST, DEVICE = 0, 1
-BC_PERIODIC, BC_REFLECT, BC_INFLOW, BC_OUTFLOW = 0, 1, 2, 3
+BC_PERIODIC, BC_REFLECT, BC_INFLOW, BC_OUTFLOW, BC_OPEN = 0, 1, 2, 3, 4
+PHASE_GATHER, PHASE_UPDATE = 0, 1
+HALO_P2G1, HALO_P2G2 = 0, 1
+HALO_EXPORT, HALO_ADD = 0, 1
 VISC_PRINTED, VISC_STANDARD = 0, 1
 VARIANT_AUTO, VARIANT_ATOMIC, VARIANT_SORTED_RETIRED, VARIANT_TILED = 0, 1, 2, 3
 ACCUM_FP64, ACCUM_FP32 = 0, 1
 STREAM_CP_ASYNC, STREAM_BULK = 0, 1
-P_X, P_V, P_M, P_RHO, P_E, P_Q = 1, 2, 4, 8, 16, 32
+BASIS_Q1, BASIS_QUADRATIC = 0, 1
+P2G_RED, P2G_COLOUR_G2P, P2G_COLOUR_UPDATE, P2G_COLOUR_BOTH = 0, 1, 2, 3
+P_X, P_V, P_M, P_RHO, P_E, P_Q, P_ID = 1, 2, 4, 8, 16, 32, 64
+LOAD_KEEP_TIME = 1
 G_MASS, G_MOMENTUM, G_FORCE, G_MOMENTUM2, G_NORMAL, G_FLAG = 0, 1, 2, 3, 4, 5
 
 K_P2G1, K_NODE1, K_G2P_P2G2, K_NODE2, K_UPDATE, K_SORT, K_MISC = range(7)
 KERNEL_NAMES = ["p2g1", "node1", "g2p_p2g2", "node2", "update", "sort", "misc"]
 
-EXPORTS = ["mpm_set_profiling", "mpm_abi_version", "mpm_create", "mpm_load_particles", "mpm_step", "mpm_read_particles",
+EXPORTS = ["mpm_step_phase", "mpm_halo", "mpm_load_particles_ex", "mpm_set_profiling", "mpm_abi_version", "mpm_create", "mpm_load_particles", "mpm_step", "mpm_read_particles",
            "mpm_read_grid", "mpm_get_stats", "mpm_last_error", "mpm_destroy"]
 
 ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p, C.c_void_p)
@@ -41,8 +47,9 @@ class Config(C.Structure):
         ("obstacle_mask", C.c_void_p), ("node_normals", C.c_void_p),
         ("recycle_seed", C.c_uint64), ("ppc_inflow", C.c_double),
         ("sort_every", C.c_int32), ("variant", C.c_int32), ("device", C.c_int32), ("grid_accum", C.c_int32),
-        ("particle_stream", C.c_int32), ("reserved2", C.c_int32),
+        ("particle_stream", C.c_int32), ("p2g_mode", C.c_int32),
         ("stream", C.c_void_p), ("alloc", ALLOC_FN), ("free", FREE_FN), ("alloc_user", C.c_void_p),
+        ("basis", C.c_int32), ("slab_global_n", C.c_int32), ("slab_offset", C.c_int32), ("reserved3", C.c_int32),
     ]
 
 
@@ -75,6 +82,9 @@ def load_library():
     lib.mpm_create.argtypes = [C.POINTER(Config), C.POINTER(vp)]
     lib.mpm_load_particles.argtypes = [vp, C.c_int64, vp, vp, vp, vp, vp, vp, C.c_int]
     lib.mpm_step.argtypes = [vp, C.c_double, C.c_double, C.c_int32, C.POINTER(C.c_double)]
+    lib.mpm_load_particles_ex.argtypes = [vp, C.c_int64, vp, vp, vp, vp, vp, vp, vp, C.c_int, C.c_int]
+    lib.mpm_step_phase.argtypes = [vp, C.c_int, C.c_double]
+    lib.mpm_halo.argtypes = [vp, C.c_int, C.c_int, C.c_int, vp, C.c_int]
     lib.mpm_read_particles.argtypes = [vp, C.c_uint32, vp, C.c_int, C.c_int]
     lib.mpm_read_grid.argtypes = [vp, C.c_int, vp, C.c_int]
     lib.mpm_get_stats.argtypes = [vp, C.POINTER(Stats)]
@@ -107,7 +117,7 @@ class Solver:
     (sort_every, variant, device, grid_accum, particle_stream) select the execution options of mpm_config."""
 
     def __init__(self, cfg, sort_every=0, variant=VARIANT_AUTO, device=0, use_torch_allocator=True, grid_accum=0,
-                 particle_stream=STREAM_CP_ASYNC):
+                 particle_stream=STREAM_CP_ASYNC, p2g_mode=P2G_RED):
         import torch
         self._lib = load()
         self._torch = torch
@@ -144,6 +154,9 @@ class Solver:
         c.sort_every = int(sort_every); c.variant = int(variant); c.device = int(device)
         c.grid_accum = int(grid_accum)
         c.particle_stream = int(particle_stream)
+        c.p2g_mode = int(p2g_mode)
+        c.basis = int(cfg.get("basis", BASIS_Q1))
+        c.slab_global_n = int(cfg.get("slab_global_n", 0)); c.slab_offset = int(cfg.get("slab_offset", 0))
         with torch.cuda.device(self.device):
             self.stream = torch.cuda.current_stream()
         c.stream = self.stream.cuda_stream
@@ -197,8 +210,10 @@ class Solver:
         return a.data_ptr()          # torch tensor (host pinned or device)
 
     # ------------------------------------------------------------------ the C-ABI calls
-    def load_particles(self, x, v, mass, rho, e, q=None, location=HOST):
-        """x, v: [dim, N]; mass, rho, e, q: [N].  numpy arrays / pinned torch tensors (HOST) or CUDA tensors (DEVICE)."""
+    def load_particles(self, x, v, mass, rho, e, q=None, location=HOST, ids=None, keep_time=False):
+        """x, v: [dim, N]; mass, rho, e, q: [N].  numpy arrays / pinned torch tensors (HOST) or CUDA tensors (DEVICE).
+        ids (int64, same location) / keep_time: mpm_load_particles_ex (caller-chosen persistent ids; time, step and
+        counters kept)."""
         d = self.dim
         n = int(mass.shape[0])
         if location == HOST:
@@ -207,9 +222,24 @@ class Solver:
             q = cv(q) if q is not None else None
         xp = (C.c_void_p * d)(*[self._ptr(x[a]) for a in range(d)])
         vp = (C.c_void_p * d)(*[self._ptr(v[a]) for a in range(d)])
-        self._check(self._lib.mpm_load_particles(self._h, n, xp, vp, self._ptr(mass), self._ptr(rho), self._ptr(e),
-                                                 self._ptr(q) if q is not None else None, location))
+        if ids is None and not keep_time:
+            self._check(self._lib.mpm_load_particles(self._h, n, xp, vp, self._ptr(mass), self._ptr(rho), self._ptr(e),
+                                                     self._ptr(q) if q is not None else None, location))
+        else:
+            if ids is not None and isinstance(ids, np.ndarray):
+                ids = np.ascontiguousarray(ids, dtype=np.int64)
+            self._check(self._lib.mpm_load_particles_ex(self._h, n, xp, vp, self._ptr(mass), self._ptr(rho), self._ptr(e),
+                                                        self._ptr(q) if q is not None else None,
+                                                        self._ptr(ids) if ids is not None else None, location,
+                                                        LOAD_KEEP_TIME if keep_time else 0))
         self.n = n
+
+    def step_phase(self, phase, dt=0.0):
+        self._check(self._lib.mpm_step_phase(self._h, int(phase), float(dt)))
+
+    def halo(self, which, side, op, buf, location=DEVICE):
+        """buf: [channels, plane nodes] float64, contiguous (CUDA tensor for DEVICE, numpy / pinned tensor for HOST)."""
+        self._check(self._lib.mpm_halo(self._h, int(which), int(side), int(op), self._ptr(buf), location))
 
     def step(self, dt=0.0, cfl=0.3, nsteps=1, sync=True):
         if sync:
@@ -223,7 +253,7 @@ class Solver:
         """Returns a dict name -> array ([dim, N] for X and V).  `out` may supply preallocated buffers
         (numpy / pinned torch for HOST, CUDA tensors for DEVICE) under the same names."""
         d, n = self.dim, self.n
-        names = [("x", P_X, d), ("v", P_V, d), ("mass", P_M, 1), ("rho", P_RHO, 1), ("e", P_E, 1), ("q", P_Q, 1)]
+        names = [("x", P_X, d), ("v", P_V, d), ("mass", P_M, 1), ("rho", P_RHO, 1), ("e", P_E, 1), ("q", P_Q, 1), ("id", P_ID, 1)]
         res, ptrs = {}, []
         for name, bit, nc in names:
             if not mask & bit:

@@ -54,6 +54,9 @@ struct mpm_handle {
     DevScalars *sc;
     long long launches;
     long long steps_done;
+    double *id_wide;      // scratch of mpm_read_particles(MPM_P_ID): ids as doubles, 2 x id_wide_slots
+    long long id_wide_slots;
+    bool external_ids;    // the caller chose the persistent ids (mpm_load_particles_ex): no read-back in id order
     std::vector<void *> allocations;
     std::string err;
     // optional per-kernel-class timers (CUDA events on the launching stream)
@@ -340,12 +343,12 @@ void reorder(mpm_handle *h)
 
 // one step of Algorithm 1 with the TILED kernel family (see mpm_kernels_tiled.cu): l.3 of this step was done by the
 // previous step's update kernel (or by the load), l.3 of the next step is done by this step's update kernel
-void step_tiled(mpm_handle *h, bool last_of_call)
+// first half: dt, reset of the next accumulators, l.4-8 (gather kernel)
+void step_tiled_gather(mpm_handle *h)
 {
     const GridDesc &gd = h->gd;
     cudaStream_t s = h->stream;
     const PArr &p = h->pbuf[h->cur];
-    const PArr &q = h->pbuf[h->cur ^ 1];
     const SortedMap map{ h->groups, h->n_groups };
     const GArr gc = tiled_acc(h, h->acur), gnx = tiled_acc(h, h->acur ^ 1);
     {
@@ -364,6 +367,18 @@ void step_tiled(mpm_handle *h, bool last_of_call)
     // kernels evaluate them per tile node while staging the tile (stage_tile)
     { Timed t(h, MPM_K_G2P_P2G2);
       launch_g2p_p2g2_tiled(gd, p, gc, h->sc, map, h->items, h->n_items, h->max_items, h->count, h->dest, s); }          // l.4-8
+    h->launches += 2;      // kernels only (begin_step, gather); the memsets are not counted
+}
+
+// second half: cell map, l.9-13 and l.3 of the next step (update kernel), time advance
+void step_tiled_update(mpm_handle *h, bool last_of_call)
+{
+    const GridDesc &gd = h->gd;
+    cudaStream_t s = h->stream;
+    const PArr &p = h->pbuf[h->cur];
+    const PArr &q = h->pbuf[h->cur ^ 1];
+    const SortedMap map{ h->groups, h->n_groups };
+    const GArr gc = tiled_acc(h, h->acur), gnx = tiled_acc(h, h->acur ^ 1);
     { Timed t(h, MPM_K_SORT);                                                         // l.12: offsets, next step's groups and work items
       launch_cell_map_tiled(gd, h->count, h->off[0], h->groups_alt, h->n_groups_alt, h->items_alt, h->n_items_alt, h->map_state, s); }
     cudaStreamWaitEvent(s, h->ev_join, 0);
@@ -375,7 +390,13 @@ void step_tiled(mpm_handle *h, bool last_of_call)
     h->cur ^= 1;
     h->acur ^= 1;
     h->grid_final = false;
-    h->launches += 5;      // kernels only (begin_step, gather, cell map, update, end_step); the memsets are not counted
+    h->launches += 3;      // kernels only (cell map, update, end_step)
+}
+
+void step_tiled(mpm_handle *h, bool last_of_call)
+{
+    step_tiled_gather(h);
+    step_tiled_update(h, last_of_call);
 }
 
 int copy_in(mpm_handle *h, double *dst, const double *src, long long n, int loc)
@@ -441,7 +462,7 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
         discard(h);
         return fail(nullptr, MPM_E_CUDA, "mpm_create: cannot create the second stream");
     }
-    h->cur = 0; h->n = h->cap = 0; h->launches = 0; h->steps_done = 0;
+    h->cur = 0; h->n = h->cap = 0; h->launches = 0; h->steps_done = 0; h->external_ids = false; h->id_wide = nullptr; h->id_wide_slots = 0;
     h->profiling = false;
     for (int k = 0; k < MPM_K_COUNT; ++k) { h->kernel_ms[k] = 0.0; h->kernel_calls[k] = 0; }
     h->d_flag = nullptr; h->key = h->rank = h->count = h->scan_aux = nullptr; h->sc = nullptr;
@@ -491,8 +512,9 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
     gd.recycle_seed = cfg->recycle_seed;
     gd.has_obstacle = cfg->obstacle_mask != nullptr;
 
-    h->variant = cfg->variant == MPM_VARIANT_AUTO ? (cfg->sort_every == 1 ? MPM_VARIANT_TILED : MPM_VARIANT_ATOMIC)
-                                                   : cfg->variant;
+    h->variant = cfg->variant == MPM_VARIANT_AUTO
+                     ? (cfg->sort_every == 1 && cfg->basis == MPM_BASIS_Q1 ? MPM_VARIANT_TILED : MPM_VARIANT_ATOMIC)
+                     : cfg->variant;
     if (h->variant != MPM_VARIANT_ATOMIC && h->variant != MPM_VARIANT_TILED) {
         discard(h);
         return fail(nullptr, MPM_E_ARG, cfg->variant == MPM_VARIANT_SORTED_RETIRED
@@ -505,13 +527,40 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
         discard(h);
         return fail(nullptr, MPM_E_ARG, "mpm_create: grid_accum must be MPM_ACCUM_FP64, or MPM_ACCUM_FP32 with the TILED family");
     }
-    if ((cfg->particle_stream != MPM_STREAM_CP_ASYNC && !(cfg->particle_stream == MPM_STREAM_BULK && tiled)) || cfg->reserved2 != 0) {
+    if (cfg->particle_stream != MPM_STREAM_CP_ASYNC && !(cfg->particle_stream == MPM_STREAM_BULK && tiled)) {
         discard(h);
-        return fail(nullptr, MPM_E_ARG, "mpm_create: particle_stream must be MPM_STREAM_CP_ASYNC, or MPM_STREAM_BULK with the TILED family; reserved2 must be 0");
+        return fail(nullptr, MPM_E_ARG, "mpm_create: particle_stream must be MPM_STREAM_CP_ASYNC, or MPM_STREAM_BULK with the TILED family");
     }
+    if (cfg->p2g_mode != MPM_P2G_RED &&
+        !(cfg->p2g_mode > 0 && cfg->p2g_mode <= MPM_P2G_COLOUR_BOTH && tiled && cfg->grid_accum == MPM_ACCUM_FP64 &&
+          cfg->particle_stream == MPM_STREAM_CP_ASYNC)) {
+        discard(h);
+        return fail(nullptr, MPM_E_ARG, "mpm_create: p2g_mode MPM_P2G_COLOUR_* needs the TILED family, fp64 accumulation and the cp.async stream");
+    }
+    if (cfg->basis != MPM_BASIS_Q1 || cfg->reserved3 != 0) {
+        bool ok = cfg->basis == MPM_BASIS_QUADRATIC && cfg->reserved3 == 0 && !tiled && !cfg->obstacle_mask;
+        for (int a = 0; a < gd.dim; ++a) ok = ok && gd.per[a] && gd.nc[a] >= 3;
+        if (!ok) {
+            discard(h);
+            return fail(nullptr, MPM_E_ARG, "mpm_create: MPM_BASIS_QUADRATIC needs the ATOMIC family and a fully periodic grid of >= 3 cells per axis without obstacle; reserved3 must be 0");
+        }
+    }
+    gd.quadratic = cfg->basis == MPM_BASIS_QUADRATIC ? 1 : 0;
+    if (cfg->slab_global_n < 0 || cfg->slab_offset < 0 ||
+        (cfg->slab_global_n > 0 && cfg->slab_offset + gd.nc[gd.dim - 1] > cfg->slab_global_n)) {
+        discard(h);
+        return fail(nullptr, MPM_E_ARG, "mpm_create: slab_offset + n[last] must not exceed slab_global_n");
+    }
+    gd.slab_global_n = cfg->slab_global_n; gd.slab_offset = cfg->slab_offset;
+    gd.has_open = 0;
+    for (int a = 0; a < gd.dim; ++a)
+        for (int sd = 0; sd < 2; ++sd)
+            if (cfg->bc[a][sd] == MPM_BC_OPEN) gd.has_open = 1;
     gd.tiled = tiled ? 1 : 0;
     gd.acc32 = cfg->grid_accum == MPM_ACCUM_FP32 ? 1 : 0;
     gd.bulk_stream = cfg->particle_stream == MPM_STREAM_BULK ? 1 : 0;
+    gd.p2g_mode = cfg->p2g_mode;
+    gd.colour_major = cfg->p2g_mode != MPM_P2G_RED ? 1 : 0;
     gd.Nkeys = gd.Nc;
     if (tiled) {    // tile-major key space (TileGeo): whole tiles, so it can be larger than the number of cells
         long long nt = 1;
@@ -616,11 +665,48 @@ void mpm_destroy(mpm_handle *h)
     delete h;
 }
 
+namespace {
+int load_impl(mpm_handle *h, int64_t n, const double *const *x, const double *const *v, const double *mass,
+              const double *rho, const double *e, const double *q, const int64_t *ids, int ptr_location, bool keep_time);
+
+// id[k] = (int)ids64[k]; out[k] = (double)id[k]
+__global__ void k_ids_from_i64(int *__restrict__ id, const long long *__restrict__ ids64, long long n, int *bad)
+{
+    for (long long k = (long long)blockIdx.x * 256 + threadIdx.x; k < n; k += (long long)gridDim.x * 256) {
+        const long long v = ids64[k];
+        if (v < 0 || v >= (1ll << 31)) atomicOr(bad, 1);
+        id[k] = (int)v;
+    }
+}
+__global__ void k_ids_to_double(const int *__restrict__ id, double *__restrict__ out, long long n)
+{
+    for (long long k = (long long)blockIdx.x * 256 + threadIdx.x; k < n; k += (long long)gridDim.x * 256) out[k] = (double)id[k];
+}
+}
+
 int mpm_load_particles(mpm_handle *h, int64_t n, const double *const *x, const double *const *v, const double *mass,
                        const double *rho, const double *e, const double *q, int ptr_location)
 {
     if (!h) return MPM_E_ARG;
     DeviceGuard guard(h->cfg.device);
+    return load_impl(h, n, x, v, mass, rho, e, q, nullptr, ptr_location, false);
+}
+
+int mpm_load_particles_ex(mpm_handle *h, int64_t n, const double *const *x, const double *const *v, const double *mass,
+                          const double *rho, const double *e, const double *q, const int64_t *ids, int ptr_location, int flags)
+{
+    if (!h) return MPM_E_ARG;
+    DeviceGuard guard(h->cfg.device);
+    if (flags & ~MPM_LOAD_KEEP_TIME) return fail(h, MPM_E_ARG, "mpm_load_particles_ex: unknown flag");
+    const bool keep = (flags & MPM_LOAD_KEEP_TIME) != 0;
+    if (keep && !h->pbuf[0].m) return fail(h, MPM_E_STATE, "mpm_load_particles_ex: MPM_LOAD_KEEP_TIME needs a loaded particle set");
+    return load_impl(h, n, x, v, mass, rho, e, q, ids, ptr_location, keep);
+}
+
+namespace {
+int load_impl(mpm_handle *h, int64_t n, const double *const *x, const double *const *v, const double *mass,
+              const double *rho, const double *e, const double *q, const int64_t *ids, int ptr_location, bool keep_time)
+{
     if (n < 0 || n >= (1ll << 31) - 1 || !x || !v || !mass || !rho || !e)
         return fail(h, MPM_E_ARG, "mpm_load_particles: bad argument");
     if (ptr_location != MPM_HOST && ptr_location != MPM_DEVICE) return fail(h, MPM_E_ARG, "mpm_load_particles: bad ptr_location");
@@ -658,11 +744,33 @@ int mpm_load_particles(mpm_handle *h, int64_t n, const double *const *x, const d
         if (!probe.differs && inflow_ok) { h->gd.uniform_mass = 1; h->gd.um = probe.first; }
         h->launches += 1;
     }
-    launch_iota(p.id, n, h->stream);
-    MPM_CUDA(h, cudaMemsetAsync(h->sc, 0, sizeof(DevScalars), h->stream));
-    launch_initial_cfl(h->gd, p, h->sc, n, h->stream);
+    h->external_ids = ids != nullptr;
+    if (ids && n > 0) {      // caller-chosen persistent ids: staged in the (free) destination-record array, narrowed to 32 bits
+        if (!h->dest) return fail(h, MPM_E_STATE, "mpm_load_particles_ex: caller-chosen ids are offered by the TILED family");
+        long long *stage = reinterpret_cast<long long *>(h->dest);
+        MPM_CUDA(h, cudaMemcpyAsync(stage, ids, sizeof(long long) * (size_t)n,
+                                    ptr_location == MPM_DEVICE ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, h->stream));
+        int bad = 0;
+        MPM_CUDA(h, cudaMemsetAsync(h->n_items_alt, 0, sizeof(int), h->stream));
+        k_ids_from_i64<<<148 * 4, 256, 0, h->stream>>>(p.id, stage, n, h->n_items_alt);
+        MPM_CUDA(h, cudaMemcpyAsync(&bad, h->n_items_alt, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+        MPM_CUDA(h, cudaStreamSynchronize(h->stream));
+        if (bad) return fail(h, MPM_E_ARG, "mpm_load_particles_ex: ids must lie in [0, 2^31)");
+    } else launch_iota(p.id, n, h->stream);
+    if (h->variant == MPM_VARIANT_TILED && n == 0) {
+        // an empty slab still takes part in the halo exchanges: its accumulators must read zero
+        h->acur = 0;
+        h->grid_final = false;
+        const GArr g0 = tiled_acc(h, 0);
+        launch_grid_clear(h->gd, g0, h->stream);
+        for (int a = 0; a < h->gd.dim; ++a) cudaMemsetAsync(g0.mv2[a], 0, sizeof(double) * (size_t)h->gd.Nn, h->stream);
+    }
+    if (!keep_time) {
+        MPM_CUDA(h, cudaMemsetAsync(h->sc, 0, sizeof(DevScalars), h->stream));
+        launch_initial_cfl(h->gd, p, h->sc, n, h->stream);
+        h->steps_done = 0;
+    }
     h->launches += 3;
-    h->steps_done = 0;
     if ((h->cfg.sort_every > 0 || h->variant != MPM_VARIANT_ATOMIC) && n > 0) reorder(h);
     if (h->gd.uniform_mass) {      // every slot of both buffers holds the mass: nothing moves it any more
         launch_fill(h->pbuf[0].m, h->slots, h->gd.um, h->stream);
@@ -673,6 +781,7 @@ int mpm_load_particles(mpm_handle *h, int64_t n, const double *const *x, const d
     if (ptr_location == MPM_HOST) MPM_CUDA(h, cudaStreamSynchronize(h->stream));   // caller may reuse its buffers
     return MPM_OK;
 }
+}  // namespace
 
 namespace {
 __global__ void k_set_mode(DevScalars *sc, double dt_fixed, double alpha)
@@ -723,6 +832,76 @@ int mpm_step(mpm_handle *h, double dt, double cfl, int32_t nsteps, double *dt_la
     return MPM_OK;
 }
 
+int mpm_step_phase(mpm_handle *h, int phase, double dt)
+{
+    if (!h) return MPM_E_ARG;
+    DeviceGuard guard(h->cfg.device);
+    if (!h->pbuf[0].m) return fail(h, MPM_E_STATE, "mpm_step_phase: no particles loaded");
+    if (h->variant != MPM_VARIANT_TILED) return fail(h, MPM_E_STATE, "mpm_step_phase: the phase interface is offered by the TILED family");
+    if (phase == MPM_PHASE_GATHER) {
+        if (!(dt > 0.0)) return fail(h, MPM_E_ARG, "mpm_step_phase(GATHER): dt must be > 0 (the caller forms the global CFL step)");
+        k_set_mode<<<1, 1, 0, h->stream>>>(h->sc, dt, 0.0);
+        h->launches += 1;
+        if (h->n > 0) step_tiled_gather(h);
+        else {      // an empty slab: nothing to gather, but its mv2 plane is exported next
+            launch_begin_step(h->sc, h->gd.h, false, h->stream);
+            const GArr gc = tiled_acc(h, h->acur);
+            for (int a = 0; a < h->gd.dim; ++a) cudaMemsetAsync(gc.mv2[a], 0, sizeof(double) * (size_t)h->gd.Nn, h->stream);
+            h->launches += 1;
+        }
+    } else if (phase == MPM_PHASE_UPDATE) {
+        if (h->n > 0) step_tiled_update(h, true);
+        else {
+            launch_grid_clear(h->gd, tiled_acc(h, h->acur ^ 1), h->stream);
+            h->acur ^= 1;
+            launch_end_step(h->sc, h->gd.h, h->stream);
+            h->launches += 1;
+        }
+        h->steps_done += 1;
+    } else return fail(h, MPM_E_ARG, "mpm_step_phase: unknown phase");
+    MPM_CUDA(h, cudaGetLastError());
+    return MPM_OK;
+}
+
+int mpm_halo(mpm_handle *h, int which, int side, int op, double *buf, int ptr_location)
+{
+    if (!h || !buf) return MPM_E_ARG;
+    DeviceGuard guard(h->cfg.device);
+    if (h->variant != MPM_VARIANT_TILED || h->gd.acc32) return fail(h, MPM_E_STATE, "mpm_halo: TILED family with fp64 accumulation only");
+    if ((which != MPM_HALO_P2G1 && which != MPM_HALO_P2G2) || (side != 0 && side != 1) || (op != MPM_HALO_EXPORT && op != MPM_HALO_ADD) ||
+        (ptr_location != MPM_HOST && ptr_location != MPM_DEVICE))
+        return fail(h, MPM_E_ARG, "mpm_halo: bad argument");
+    const GridDesc &gd = h->gd;
+    const int last = gd.dim - 1;
+    const long long plane = gd.Nn / gd.nn[last];                              // the last axis is the slowest: a plane is contiguous
+    const long long at = side ? (long long)(gd.nn[last] - 1) * plane : 0;
+    const GArr g = tiled_acc(h, h->acur);                                       // the set the next GATHER phase reads / has written
+    std::vector<double *> ch;
+    if (which == MPM_HALO_P2G1) {
+        ch.push_back(g.m);
+        for (int a = 0; a < gd.dim; ++a) ch.push_back(g.mv[a]);
+        for (int a = 0; a < gd.dim; ++a) ch.push_back(g.f[a]);
+    } else for (int a = 0; a < gd.dim; ++a) ch.push_back(g.mv2[a]);
+    double *stage = nullptr;
+    if (op == MPM_HALO_ADD && ptr_location == MPM_HOST) {                       // host data are staged in the inactive particle buffer
+        stage = h->pbuf[h->cur ^ 1].x[0];
+        if ((long long)ch.size() * plane > h->slots) return fail(h, MPM_E_STATE, "mpm_halo: plane larger than the staging buffer");
+        MPM_CUDA(h, cudaMemcpyAsync(stage, buf, sizeof(double) * ch.size() * (size_t)plane, cudaMemcpyHostToDevice, h->stream));
+    }
+    for (size_t c = 0; c < ch.size(); ++c) {
+        double *node = ch[c] + at, *user = buf + c * plane;
+        if (op == MPM_HALO_EXPORT) {
+            int rc = copy_out(h, user, node, plane, ptr_location);
+            if (rc != MPM_OK) return rc;
+        } else launch_add_into(node, stage ? stage + c * plane : user, plane, h->stream);
+    }
+    h->launches += op == MPM_HALO_ADD ? (long long)ch.size() : 0;
+    h->grid_final = false;
+    MPM_CUDA(h, cudaGetLastError());
+    if (ptr_location == MPM_HOST) MPM_CUDA(h, cudaStreamSynchronize(h->stream));
+    return MPM_OK;
+}
+
 int mpm_read_particles(mpm_handle *h, uint32_t field_mask, double *const *out, int order, int ptr_location)
 {
     if (!h || !out) return MPM_E_ARG;
@@ -740,6 +919,21 @@ int mpm_read_particles(mpm_handle *h, uint32_t field_mask, double *const *out, i
     if (field_mask & MPM_P_RHO) { src.push_back(p.rho); tmp.push_back(scratch.rho); }
     if (field_mask & MPM_P_E) { src.push_back(p.e); tmp.push_back(scratch.e); }
     if (field_mask & MPM_P_Q) { src.push_back(p.q); tmp.push_back(scratch.q); }
+    if (h->external_ids && order == 0)
+        return fail(h, MPM_E_STATE, "mpm_read_particles: caller-chosen ids: read in storage order (order = 1) with MPM_P_ID");
+    if (field_mask & MPM_P_ID) {      // ids widened to fp64 in a scratch pair of their own (allocated on first use)
+        const size_t N = (size_t)(h->slots > 0 ? h->slots : 1);
+        if (h->id_wide_slots < (long long)N) {
+            dev_free(h, h->id_wide);
+            h->id_wide = nullptr;
+            if (!dev_alloc_t(h, &h->id_wide, 2 * N)) return fail(h, MPM_E_OOM, "mpm_read_particles: out of device memory");
+            h->id_wide_slots = (long long)N;
+        }
+        k_ids_to_double<<<148 * 4, 256, 0, h->stream>>>(p.id, h->id_wide, (long long)N);
+        h->launches += 1;
+        src.push_back(h->id_wide);
+        tmp.push_back(h->id_wide + N);
+    }
     const bool tiled = h->variant == MPM_VARIANT_TILED && h->n > 0;
     const SortedMap map{ h->groups, h->n_groups };
     if (tiled && order != 0) {   // storage order without the unused slots: compact offsets = scan of the per-key counts

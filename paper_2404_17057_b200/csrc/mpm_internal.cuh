@@ -53,13 +53,22 @@ struct GridDesc {
     // TILED: particle fields are streamed with bulk asynchronous copies + mbarriers instead of per-thread cp.async
     // (mpm_config.particle_stream = MPM_STREAM_BULK)
     int bulk_stream;
+    // TILED: which scatters accumulate in a shared-memory tile by cell colour (mpm_config.p2g_mode, MPM_P2G_* bits)
+    int p2g_mode;
+    // slab decomposition: this grid is cells [slab_offset, slab_offset + nc[dim-1]) of slab_global_n along the last axis
+    // (0 = not a slab); only the recycling position needs to know
+    int slab_global_n, slab_offset;
+    int has_open;       // some face is MPM_BC_OPEN (particles beyond it are out of their cell until the caller hands them over)
+    int quadratic;      // ATOMIC family: quadratic B-spline basis instead of Q1 (mpm_config.basis), periodic grids only
+    int colour_major;   // layout of the cell numbering inside a tile (TileGeo): 1 when p2g_mode != 0
     // TILED: allocated slots per particle array and capacities of the group / item lists (bounds of the checked build)
     long long slots, max_groups, max_items;
 };
 
 // TILED family: the grid is cut into tiles of T0 x T1 (x T2) cells; the cell key is (tile index, cell inside the
-// tile), both x fastest, so that the particles of one tile are contiguous in the cell-sorted order (PAPER.md:745-748
-// applied per tile) and one thread block can keep the tile's (T+1)^d nodes in shared memory.
+// tile): tiles x fastest, cells inside a tile x fastest or colour-major (see below), so that the particles of one tile are contiguous
+// in the cell-sorted order (PAPER.md:745-748 applied per tile) and one thread block can keep the tile's (T+1)^d nodes in
+// shared memory.
 template <int DIM>
 struct TileGeo {
     static constexpr int LT0 = (DIM == 3) ? 3 : 4;
@@ -70,19 +79,56 @@ struct TileGeo {
     static constexpr int TC = 1 << LTC;                      // cells per tile
     static constexpr int N0 = T0 + 1, N1 = T1 + 1, N2 = (DIM == 3) ? T2 + 1 : 1;
     static constexpr int NN = N0 * N1 * N2;                  // nodes per tile
+    // Numbering of the cells inside a tile (the low LTC bits of the cell key), two layouts:
+    //   natural (default): x fastest, then y, then z;
+    //   colour-major (cm, used when a scatter accumulates by cell colour, mpm_config.p2g_mode): colour = parities of the
+    //     tile-local cell coordinates (the 2^d colouring the paper proposes for an atomics-free P2G: cells
+    //     of one colour share no node), then the position among the cells of that colour, x fastest.  Consecutive keys --
+    //     and hence the groups a block works on in one pass -- then belong to one colour: their corner nodes are disjoint.
+    static constexpr int NCOL = 1 << DIM;                    // colours
+    static constexpr int LCC = LTC - DIM;                    // log2(cells per colour)
+    __host__ __device__ static constexpr int local_of(int lx, int ly, int lz, bool cm)
+    {
+        return cm ? ((((lx & 1) | ((ly & 1) << 1) | ((DIM == 3 ? (lz & 1) : 0) << 2)) << LCC) |
+                     (lx >> 1) | ((ly >> 1) << (LT0 - 1)) | ((DIM == 3 ? (lz >> 1) : 0) << (LT0 + LT1 - 2)))
+                  : (lx | (ly << LT0) | ((DIM == 3 ? lz : 0) << (LT0 + LT1)));
+    }
+    __host__ __device__ static constexpr int colour_of(int local) { return local >> LCC; }      // colour-major layout only
+    __host__ __device__ static constexpr int lx_of(int local, bool cm)
+    {
+        return cm ? ((((local & ((1 << (LT0 - 1)) - 1))) << 1) | ((local >> LCC) & 1)) : (local & (T0 - 1));
+    }
+    __host__ __device__ static constexpr int ly_of(int local, bool cm)
+    {
+        return cm ? ((((local >> (LT0 - 1)) & ((1 << (LT1 - 1)) - 1)) << 1) | ((local >> (LCC + 1)) & 1)) : ((local >> LT0) & (T1 - 1));
+    }
+    __host__ __device__ static constexpr int lz_of(int local, bool cm)
+    {
+        return DIM != 3 ? 0
+               : cm ? ((((local >> (LT0 + LT1 - 2)) & ((1 << (LT2 > 0 ? LT2 - 1 : 0)) - 1)) << 1) | ((local >> (LCC + 2)) & 1))
+                    : (local >> (LT0 + LT1));
+    }
+    // tile-local node index of the cell's corner 0
+    __host__ __device__ static constexpr int node0_of(int local, bool cm)
+    {
+        return lx_of(local, cm) + N0 * (ly_of(local, cm) + N1 * lz_of(local, cm));
+    }
 };
 
+// cm: colour-major numbering inside the tile (a compile-time constant in the tile kernels, gd.colour_major elsewhere)
 template <int DIM>
-__host__ __device__ __forceinline__ int tiled_key_of_cell(const GridDesc &gd, const int c[DIM])
+__host__ __device__ __forceinline__ int tiled_key_of_cell(const GridDesc &gd, const int c[DIM], bool cm)
 {
     using TG = TileGeo<DIM>;
     int tile = (c[0] >> TG::LT0) + gd.ntile[0] * (c[1] >> TG::LT1);
-    int local = (c[0] & (TG::T0 - 1)) | ((c[1] & (TG::T1 - 1)) << TG::LT0);
-    if (DIM == 3) {
-        tile += gd.ntile[0] * gd.ntile[1] * (c[DIM - 1] >> TG::LT2);
-        local |= (c[DIM - 1] & (TG::T2 - 1)) << (TG::LT0 + TG::LT1);
-    }
+    if (DIM == 3) tile += gd.ntile[0] * gd.ntile[1] * (c[DIM - 1] >> TG::LT2);
+    const int local = TG::local_of(c[0] & (TG::T0 - 1), c[1] & (TG::T1 - 1), DIM == 3 ? (c[DIM - 1] & (TG::T2 - 1)) : 0, cm);
     return (tile << TG::LTC) | local;
+}
+template <int DIM>
+__host__ __device__ __forceinline__ int tiled_key_of_cell(const GridDesc &gd, const int c[DIM])
+{
+    return tiled_key_of_cell<DIM>(gd, c, gd.colour_major != 0);
 }
 
 template <int DIM>
@@ -90,9 +136,10 @@ __host__ __device__ __forceinline__ void tiled_cell_of_key(const GridDesc &gd, i
 {
     using TG = TileGeo<DIM>;
     const int tile = key >> TG::LTC, local = key & (TG::TC - 1);
-    c[0] = ((tile % gd.ntile[0]) << TG::LT0) | (local & (TG::T0 - 1));
-    c[1] = (((tile / gd.ntile[0]) % gd.ntile[1]) << TG::LT1) | ((local >> TG::LT0) & (TG::T1 - 1));
-    if (DIM == 3) c[DIM - 1] = ((tile / (gd.ntile[0] * gd.ntile[1])) << TG::LT2) | (local >> (TG::LT0 + TG::LT1));
+    const bool cm = gd.colour_major != 0;
+    c[0] = ((tile % gd.ntile[0]) << TG::LT0) | TG::lx_of(local, cm);
+    c[1] = (((tile / gd.ntile[0]) % gd.ntile[1]) << TG::LT1) | TG::ly_of(local, cm);
+    if (DIM == 3) c[DIM - 1] = ((tile / (gd.ntile[0] * gd.ntile[1])) << TG::LT2) | TG::lz_of(local, cm);
 }
 
 // particle SoA.  P, Vbar, A, grad V are transient and never stored.
@@ -241,6 +288,8 @@ void launch_mass_differs(const double *m, long long n, int *flag, cudaStream_t s
 void launch_fill(double *m, long long n, double value, cudaStream_t s);
 // dst[i] = (double)((const float *)src)[i]: fp32 accumulators widened for mpm_read_grid
 void launch_widen(const double *src_as_float, double *dst, long long n, cudaStream_t s);
+// dst[i] += src[i], i < n (halo sum-exchange of a node plane)
+void launch_add_into(double *dst, const double *src, long long n, cudaStream_t s);
 long long max_items_tiled(const GridDesc &gd, long long max_groups);   // upper bound of the item count (launch size)
 // g: the node accumulators m, mv, f of this step (raw P2G#1) and mv2; the kernels apply l.4-5 / l.9 while staging a tile
 void launch_g2p_p2g2_tiled(const GridDesc &gd, const PArr &p, const GArr &g, const DevScalars *sc,

@@ -5,6 +5,10 @@
 // (Alg. 1 l.3), one gather+scatter kernel for l.6-8, one gather+update kernel for l.10-11 and the CFL maxima.
 // It works for ANY particle order, so it serves the shuffled runs of config 2 and is the parity cross-check
 // of the TILED family.
+//
+// The kernels are written over a tensor-product SUPPORT of NS nodes per axis: NS = 2 is the paper's Q1 hat basis
+// (PAPER.md:254), NS = 3 the quadratic B-spline basis it names as the next one (mpm_config.basis =
+// MPM_BASIS_QUADRATIC, periodic grids only: reading A20).  Everything else of Algorithm 1 is the same code.
 #include "mpm_internal.cuh"
 
 namespace mpm {
@@ -20,9 +24,76 @@ __device__ __forceinline__ void load_vec(double *const arr[3], long long k, doub
     for (int a = 0; a < DIM; ++a) out[a] = arr[a][k];
 }
 
+// 1D weights and slopes of the NS^d nodes a particle sees, and the index of the first one per axis.
+//   NS = 2 (Q1, A6, A19): base = cell c, w = (1 - xi, xi), slopes (-1/h, +1/h);
+//   NS = 3 (quadratic B-spline N(u) = 3/4 - u^2 for |u| < 1/2, (3/2 - |u|)^2 / 2 for 1/2 <= |u| < 3/2):
+//          base = floor(X/h - 1/2) (may be -1: periodic wrap), f = X/h - base in [1/2, 3/2),
+//          w = ((3/2 - f)^2 / 2, 3/4 - (f - 1)^2, (f - 1/2)^2 / 2), slopes (-(3/2 - f), -2 (f - 1), f - 1/2) / h.
+template <int DIM, int NS>
+struct Support {
+    int base[DIM];
+    double w[DIM][NS], g[DIM][NS];
+    static constexpr int NODES = (NS == 2) ? (1 << DIM) : (DIM == 2 ? 9 : 27);
+
+    __device__ __forceinline__ void at(const GridDesc &gd, const double X[DIM])
+    {
+#pragma unroll
+        for (int a = 0; a < DIM; ++a) {
+            if (NS == 2) {
+                double xi;
+                cell_1d(X[a], gd.inv_h, gd.nc[a], base[a], xi);
+                w[a][0] = 1.0 - xi; w[a][1] = xi;
+                g[a][0] = -gd.inv_h; g[a][1] = gd.inv_h;
+            } else {
+                const double s = __dmul_rn(X[a], gd.inv_h);
+                const int b = (int)floor(s - 0.5);
+                const double f = s - (double)b;
+                base[a] = b;
+                w[a][0] = 0.5 * (1.5 - f) * (1.5 - f);
+                w[a][1] = 0.75 - (f - 1.0) * (f - 1.0);
+                w[a][NS - 1] = 0.5 * (f - 0.5) * (f - 0.5);
+                g[a][0] = -(1.5 - f) * gd.inv_h;
+                g[a][1] = -2.0 * (f - 1.0) * gd.inv_h;
+                g[a][NS - 1] = (f - 0.5) * gd.inv_h;
+            }
+        }
+    }
+    // position of node q (x fastest) inside the support along axis a
+    __device__ __forceinline__ static constexpr int j_of(int q, int a) { return a == 0 ? q % NS : a == 1 ? (q / NS) % NS : q / (NS * NS); }
+    // global node index (periodic: node n == node 0, A11; the quadratic support wraps on both sides)
+    __device__ __forceinline__ long long node(const GridDesc &gd, int q) const
+    {
+        long long idx = 0, stride = 1;
+#pragma unroll
+        for (int a = 0; a < DIM; ++a) {
+            int i = base[a] + j_of(q, a);
+            if (NS == 2) { if (gd.per[a] && i == gd.nc[a]) i = 0; }
+            else { if (i < 0) i += gd.nc[a]; else if (i >= gd.nc[a]) i -= gd.nc[a]; }
+            idx += stride * (long long)i;
+            stride *= (long long)gd.nn[a];
+        }
+        return idx;
+    }
+    __device__ __forceinline__ double phi(int q) const
+    {
+        double v = 1.0;
+#pragma unroll
+        for (int a = 0; a < DIM; ++a) v *= w[a][j_of(q, a)];
+        return v;
+    }
+    __device__ __forceinline__ double dphi(int q, int a) const
+    {
+        double v = g[a][j_of(q, a)];
+#pragma unroll
+        for (int a2 = 0; a2 < DIM; ++a2)
+            if (a2 != a) v *= w[a2][j_of(q, a2)];
+        return v;
+    }
+};
+
 // ------------------------------------------------------------------------------------------------ Alg. 1 l.3
 // m_i += M phi, mv_i += M V phi, f_i += (P+Q)(M/rho) grad phi  (eqs. 13, 14, 16, 18)
-template <int DIM>
+template <int DIM, int NS>
 __global__ void __launch_bounds__(kBlock) k_p2g1_atomic(GridDesc gd, PArr p, GArr g, long long n)
 {
     long long k = (long long)blockIdx.x * kBlock + threadIdx.x;
@@ -31,20 +102,19 @@ __global__ void __launch_bounds__(kBlock) k_p2g1_atomic(GridDesc gd, PArr p, GAr
     load_vec<DIM>(p.x, k, X);
     load_vec<DIM>(p.v, k, V);
     const double M = p.m[k], rho = p.rho[k], E = p.e[k], Q = p.q[k];
-    int c[DIM];
-    double xi[DIM];
-    particle_cell<DIM>(gd, X, c, xi);
+    Support<DIM, NS> sp;
+    sp.at(gd, X);
     const double P = (gd.gamma - 1.0) * rho * E;   // eq. (3)
     const double S = (P + Q) * M / rho;            // eq. (13)
 #pragma unroll
-    for (int ib = 0; ib < (1 << DIM); ++ib) {
-        const long long i = corner_node<DIM>(gd, c, ib);
-        const double phi = corner_phi<DIM>(xi, ib);
+    for (int ib = 0; ib < Support<DIM, NS>::NODES; ++ib) {
+        const long long i = sp.node(gd, ib);
+        const double phi = sp.phi(ib);
         atomicAdd(&g.m[i], M * phi);
 #pragma unroll
         for (int a = 0; a < DIM; ++a) {
             atomicAdd(&g.mv[a][i], M * V[a] * phi);
-            atomicAdd(&g.f[a][i], S * corner_dphi<DIM>(xi, ib, a, gd.inv_h));
+            atomicAdd(&g.f[a][i], S * sp.dphi(ib, a));
         }
     }
 }
@@ -52,7 +122,7 @@ __global__ void __launch_bounds__(kBlock) k_p2g1_atomic(GridDesc gd, PArr p, GAr
 // ------------------------------------------------------------------------------------------------ Alg. 1 l.6-8
 // A = G2P(f/m); V' = V + dt A; mv2_i += M V' phi at the same weights.
 // Vbar = G2P(mv'/m) is not needed here: it is gathered again, from the same node field, where it is used (l.11).
-template <int DIM>
+template <int DIM, int NS>
 __global__ void __launch_bounds__(kBlock) k_g2p_p2g2_atomic(GridDesc gd, PArr p, GArr g, const DevScalars *sc, long long n)
 {
     long long k = (long long)blockIdx.x * kBlock + threadIdx.x;
@@ -62,18 +132,18 @@ __global__ void __launch_bounds__(kBlock) k_g2p_p2g2_atomic(GridDesc gd, PArr p,
     load_vec<DIM>(p.x, k, X);
     load_vec<DIM>(p.v, k, V);
     const double M = p.m[k];
-    int c[DIM];
-    double xi[DIM];
-    particle_cell<DIM>(gd, X, c, xi);
-    long long node[1 << DIM];
-    double phi[1 << DIM];
+    constexpr int NODES = Support<DIM, NS>::NODES;
+    Support<DIM, NS> sp;
+    sp.at(gd, X);
+    long long node[NODES];
+    double phi[NODES];
     double A[DIM];
 #pragma unroll
     for (int a = 0; a < DIM; ++a) A[a] = 0.0;
 #pragma unroll
-    for (int ib = 0; ib < (1 << DIM); ++ib) {
-        node[ib] = corner_node<DIM>(gd, c, ib);
-        phi[ib] = corner_phi<DIM>(xi, ib);
+    for (int ib = 0; ib < NODES; ++ib) {
+        node[ib] = sp.node(gd, ib);
+        phi[ib] = sp.phi(ib);
 #pragma unroll
         for (int a = 0; a < DIM; ++a) A[a] += phi[ib] * g.acc[a][node[ib]];
     }
@@ -83,7 +153,7 @@ __global__ void __launch_bounds__(kBlock) k_g2p_p2g2_atomic(GridDesc gd, PArr p,
         p.v[a][k] = V[a];
     }
 #pragma unroll
-    for (int ib = 0; ib < (1 << DIM); ++ib)
+    for (int ib = 0; ib < NODES; ++ib)
 #pragma unroll
         for (int a = 0; a < DIM; ++a) atomicAdd(&g.mv2[a][node[ib]], M * V[a] * phi[ib]);
 }
@@ -92,7 +162,7 @@ __global__ void __launch_bounds__(kBlock) k_g2p_p2g2_atomic(GridDesc gd, PArr p,
 // D = trace G2PD(mv2/m); E, rho, Q update (eq. 4); Vbar = G2P(mv'/m);
 // CFL maxima over |V'|, |Vbar|, c_s (A12); X' = X + dt Vbar, wrap / recycle / clamp (PAPER.md:372-376,
 // :548-554; A8, A11).
-template <int DIM>
+template <int DIM, int NS>
 __global__ void __launch_bounds__(kBlock) k_update_atomic(GridDesc gd, PArr p, GArr g, DevScalars *sc, long long n)
 {
     __shared__ double s_v[kBlock / 32], s_c[kBlock / 32];
@@ -106,19 +176,18 @@ __global__ void __launch_bounds__(kBlock) k_update_atomic(GridDesc gd, PArr p, G
         load_vec<DIM>(p.x, k, X);
         load_vec<DIM>(p.v, k, V);
         double rho = p.rho[k], E = p.e[k], Q;
-        int c[DIM];
-        double xi[DIM];
-        particle_cell<DIM>(gd, X, c, xi);
+        Support<DIM, NS> sp;
+        sp.at(gd, X);
         double D = 0.0, Vb[DIM];
 #pragma unroll
         for (int a = 0; a < DIM; ++a) Vb[a] = 0.0;
 #pragma unroll
-        for (int ib = 0; ib < (1 << DIM); ++ib) {
-            const long long i = corner_node<DIM>(gd, c, ib);
-            const double phi = corner_phi<DIM>(xi, ib);
+        for (int ib = 0; ib < Support<DIM, NS>::NODES; ++ib) {
+            const long long i = sp.node(gd, ib);
+            const double phi = sp.phi(ib);
 #pragma unroll
             for (int a = 0; a < DIM; ++a) {
-                D += g.v2[a][i] * corner_dphi<DIM>(xi, ib, a, gd.inv_h);
+                D += g.v2[a][i] * sp.dphi(ib, a);
                 Vb[a] += phi * g.vbar[a][i];
             }
         }
@@ -178,8 +247,10 @@ __global__ void __launch_bounds__(kBlock) k_update_atomic(GridDesc gd, PArr p, G
                 } else {
                     const double u1 = recycle_uniform(gd.recycle_seed, id, step, j++);
                     const double u2 = recycle_uniform(gd.recycle_seed, id, step, j++);
-                    int cell = (int)floor(u1 * (double)gd.nc[a]);
-                    cell = min(cell, gd.nc[a] - 1);
+                    const bool slab = gd.slab_global_n > 0 && a == DIM - 1;      // see lg::move_particle
+                    const int na = slab ? gd.slab_global_n : gd.nc[a];
+                    int cell = (int)floor(u1 * (double)na);
+                    cell = min(cell, na - 1) - (slab ? gd.slab_offset : 0);
                     Xn[a] = ((double)cell + u2) * gd.h;
                 }
                 V[a] = gd.inflow_v[a];
@@ -198,8 +269,8 @@ __global__ void __launch_bounds__(kBlock) k_update_atomic(GridDesc gd, PArr p, G
 #pragma unroll
         for (int a = 0; a < DIM; ++a) {
             if (!gd.per[a]) {
-                if (Xn[a] < 0.0) { Xn[a] = 0.0; n_clamp++; }
-                if (Xn[a] > gd.L[a]) { Xn[a] = gd.L[a]; n_clamp++; }
+                if (Xn[a] < 0.0 && gd.bc[a][0] != MPM_BC_OPEN) { Xn[a] = 0.0; n_clamp++; }
+                if (Xn[a] > gd.L[a] && gd.bc[a][1] != MPM_BC_OPEN) { Xn[a] = gd.L[a]; n_clamp++; }
             }
             p.x[a][k] = Xn[a];
         }
@@ -249,23 +320,32 @@ inline unsigned grid_for(long long n) { return (unsigned)((n + kBlock - 1) / kBl
 void launch_p2g1_atomic(const GridDesc &gd, const PArr &p, const GArr &g, long long n, cudaStream_t s)
 {
     if (n <= 0) return;
-    if (gd.dim == 2) k_p2g1_atomic<2><<<grid_for(n), kBlock, 0, s>>>(gd, p, g, n);
-    else k_p2g1_atomic<3><<<grid_for(n), kBlock, 0, s>>>(gd, p, g, n);
+    if (gd.quadratic) {
+        if (gd.dim == 2) k_p2g1_atomic<2, 3><<<grid_for(n), kBlock, 0, s>>>(gd, p, g, n);
+        else k_p2g1_atomic<3, 3><<<grid_for(n), kBlock, 0, s>>>(gd, p, g, n);
+    } else if (gd.dim == 2) k_p2g1_atomic<2, 2><<<grid_for(n), kBlock, 0, s>>>(gd, p, g, n);
+    else k_p2g1_atomic<3, 2><<<grid_for(n), kBlock, 0, s>>>(gd, p, g, n);
 }
 
 void launch_g2p_p2g2_atomic(const GridDesc &gd, const PArr &p, const GArr &g, const DevScalars *sc, long long n,
                             cudaStream_t s)
 {
     if (n <= 0) return;
-    if (gd.dim == 2) k_g2p_p2g2_atomic<2><<<grid_for(n), kBlock, 0, s>>>(gd, p, g, sc, n);
-    else k_g2p_p2g2_atomic<3><<<grid_for(n), kBlock, 0, s>>>(gd, p, g, sc, n);
+    if (gd.quadratic) {
+        if (gd.dim == 2) k_g2p_p2g2_atomic<2, 3><<<grid_for(n), kBlock, 0, s>>>(gd, p, g, sc, n);
+        else k_g2p_p2g2_atomic<3, 3><<<grid_for(n), kBlock, 0, s>>>(gd, p, g, sc, n);
+    } else if (gd.dim == 2) k_g2p_p2g2_atomic<2, 2><<<grid_for(n), kBlock, 0, s>>>(gd, p, g, sc, n);
+    else k_g2p_p2g2_atomic<3, 2><<<grid_for(n), kBlock, 0, s>>>(gd, p, g, sc, n);
 }
 
 void launch_update_atomic(const GridDesc &gd, const PArr &p, const GArr &g, DevScalars *sc, long long n, cudaStream_t s)
 {
     if (n <= 0) return;
-    if (gd.dim == 2) k_update_atomic<2><<<grid_for(n), kBlock, 0, s>>>(gd, p, g, sc, n);
-    else k_update_atomic<3><<<grid_for(n), kBlock, 0, s>>>(gd, p, g, sc, n);
+    if (gd.quadratic) {
+        if (gd.dim == 2) k_update_atomic<2, 3><<<grid_for(n), kBlock, 0, s>>>(gd, p, g, sc, n);
+        else k_update_atomic<3, 3><<<grid_for(n), kBlock, 0, s>>>(gd, p, g, sc, n);
+    } else if (gd.dim == 2) k_update_atomic<2, 2><<<grid_for(n), kBlock, 0, s>>>(gd, p, g, sc, n);
+    else k_update_atomic<3, 2><<<grid_for(n), kBlock, 0, s>>>(gd, p, g, sc, n);
 }
 
 }  // namespace mpm

@@ -131,7 +131,7 @@ __device__ __forceinline__ double acc_ld(const double *arr, long long i)
     return __ldg(arr + i);
 }
 
-template <int DIM>
+template <int DIM, bool CM>
 __device__ __forceinline__ int tiled_key_of_position(const GridDesc &gd, const double X[DIM])
 {
     int c[DIM];
@@ -140,7 +140,7 @@ __device__ __forceinline__ int tiled_key_of_position(const GridDesc &gd, const d
         double xi;
         cell_1d(X[a], gd.inv_h, gd.nc[a], c[a], xi);
     }
-    return tiled_key_of_cell<DIM>(gd, c);
+    return tiled_key_of_cell<DIM>(gd, c, CM);
 }
 
 // A dense cell fills whole warps with its groups.  Then the groups' corner totals are added up across the warp first
@@ -172,9 +172,11 @@ __device__ __forceinline__ bool warp_one_cell(int cell, int cnt)
 // accumulators g.m, g.mv, g.f with one global fp64 reduction per corner and channel:
 //   pay[i] = { M, M V_a, S } of the lane's particle i, w[i][r] = weight of corner r ^ l (0 for a particle that is not
 //   part of the group reduction).
-template <int DIM, bool ACC32>
-__device__ __forceinline__ void scatter_p2g1_group(const GridDesc &gd, const GArr &g, const int c[DIM], int l, bool any,
-                                                   const double pay[2][DIM + 2], const double w[2][1 << DIM], bool one_cell = false)
+// p2g1_group_totals leaves in out[ch][q], ch = 0 (m), 1 .. DIM (mv), DIM + 1 .. 2 DIM (f), the group's totals for the
+// corners b_q = l + q LG and returns whether this lane's group has to add them to the grid at all.
+template <int DIM>
+__device__ __forceinline__ bool p2g1_group_totals(const GridDesc &gd, int l, bool any, const double pay[2][DIM + 2],
+                                                  const double w[2][1 << DIM], bool one_cell, double out[2 * DIM + 1][2])
 {
     constexpr int NB = 1 << DIM, LG = Geo<DIM>::LG;
     double tot[DIM + 2][2];
@@ -202,17 +204,90 @@ __device__ __forceinline__ void scatter_p2g1_group(const GridDesc &gd, const GAr
             F[a][q] = ((b >> a) & 1) ? pair : -pair;
         }
     }
-    if (any) {
 #pragma unroll
-        for (int q = 0; q < 2; ++q) {
-            const int node = corner_node_i<DIM>(gd, c, l + q * LG);
-            acc_add<ACC32>(g.m, node, tot[0][q]);
+    for (int q = 0; q < 2; ++q) {
+        out[0][q] = tot[0][q];
 #pragma unroll
-            for (int a = 0; a < DIM; ++a) {
-                acc_add<ACC32>(g.mv[a], node, tot[1 + a][q]);
-                acc_add<ACC32>(g.f[a], node, F[a][q]);
-            }
+        for (int a = 0; a < DIM; ++a) { out[1 + a][q] = tot[1 + a][q]; out[1 + DIM + a][q] = F[a][q]; }
+    }
+    return any;
+}
+
+// ... added to the node accumulators with one global fp64 reduction per corner and channel
+template <int DIM, bool ACC32>
+__device__ __forceinline__ void p2g1_commit_global(const GridDesc &gd, const GArr &g, const int c[DIM], int l, const double tot[2 * DIM + 1][2])
+{
+    constexpr int LG = Geo<DIM>::LG;
+#pragma unroll
+    for (int q = 0; q < 2; ++q) {
+        const int node = corner_node_i<DIM>(gd, c, l + q * LG);
+        acc_add<ACC32>(g.m, node, tot[0][q]);
+#pragma unroll
+        for (int a = 0; a < DIM; ++a) {
+            acc_add<ACC32>(g.mv[a], node, tot[1 + a][q]);
+            acc_add<ACC32>(g.f[a], node, tot[1 + DIM + a][q]);
         }
+    }
+}
+
+template <int DIM, bool ACC32>
+__device__ __forceinline__ void scatter_p2g1_group(const GridDesc &gd, const GArr &g, const int c[DIM], int l, bool any,
+                                                   const double pay[2][DIM + 2], const double w[2][1 << DIM], bool one_cell = false)
+{
+    double tot[2 * DIM + 1][2];
+    if (p2g1_group_totals<DIM>(gd, l, any, pay, w, one_cell, tot)) p2g1_commit_global<DIM, ACC32>(gd, g, c, l, tot);
+}
+
+// ------------------------------------------------------------------------------------------------ atomics-free tile accumulation
+// The paper's proposal for a P2G without atomics: sort the particles by cell, colour the cells so that
+// cells of one colour share no node, and process one colour at a time.  Here: the tile-local cell numbering is colour-major
+// (TileGeo), so the groups a block works on in one pass belong to at most two consecutive colours in the common case.
+// With COLOUR the group totals of a pass are added into a shared-memory accumulator tile with PLAIN read-modify-writes
+// (no atomic of any kind): first the groups of the pass's first colour, after a block barrier those of its last colour.
+// Groups of one colour in one pass are different cells, hence touch disjoint nodes.  Not eligible, and sent to the grid
+// with global reductions as in the default path: groups of a cell that has more than one group (more than 2^d particles:
+// the cell map flags them), groups of a third colour in a sparse pass, and particles that change cell.  The accumulator tile
+// is flushed once per block with one global reduction per non-zero node value (neighbouring tiles and the ineligible
+// groups add to the same nodes, so the flush cannot be a plain store).
+template <int DIM>
+__device__ __forceinline__ constexpr int corner_off(int b);
+
+template <int DIM>
+struct PassColours {
+    int lo, hi;      // colours of the first and of the last group of the pass (block-uniform)
+};
+
+template <int DIM>
+__device__ __forceinline__ PassColours<DIM> pass_colours(const int4 *__restrict__ groups, int g_first, int g_end, int gpb)
+{
+    using TG = TileGeo<DIM>;
+    PassColours<DIM> pc{ 0, 0 };
+    const int g_last = min(g_first + gpb, g_end) - 1;
+    if (g_first <= g_last) {
+        pc.lo = TG::colour_of(__ldg(&groups[g_first].z) & (TG::TC - 1));
+        pc.hi = TG::colour_of(__ldg(&groups[g_last].z) & (TG::TC - 1));
+    }
+    return pc;
+}
+
+// phase in which this lane's group adds its totals to the shared accumulator tile: 0, 1, or -1 = not eligible
+template <int DIM>
+__device__ __forceinline__ int colour_phase(const PassColours<DIM> &pc, const Group &grp)
+{
+    if (grp.cnt == 0 || grp.multi) return -1;
+    const int col = TileGeo<DIM>::colour_of(grp.cell & (TileGeo<DIM>::TC - 1));
+    return col == pc.lo ? 0 : col == pc.hi ? 1 : -1;
+}
+
+// s_acc[node][NCH] += tot[ch][q] for the lane's two corners (plain additions: see above)
+template <int DIM, int NCH>
+__device__ __forceinline__ void tile_accumulate(double *s_acc, int j0, int l, const double tot[NCH][2])
+{
+#pragma unroll
+    for (int q = 0; q < 2; ++q) {
+        double *dst = s_acc + (j0 + corner_off<DIM>(l + q * Geo<DIM>::LG)) * NCH;
+#pragma unroll
+        for (int ch = 0; ch < NCH; ++ch) dst[ch] += tot[ch][q];
     }
 }
 
@@ -281,6 +356,15 @@ __global__ void __launch_bounds__(kBlock, MPM_MINB) k_p2g1_tiled(GridDesc gd, PA
 constexpr int kTB = MPM_TB;              // threads per block of the tile kernels
 constexpr int kTBMinG = MPM_TBMIN_G;     // resident blocks per SM the gather kernel is compiled for (128 registers)
 constexpr int kTBMinU = MPM_TBMIN_U;     // ... and the update kernel (128 registers, no spills)
+#ifndef MPM_TBMIN_G2
+#define MPM_TBMIN_G2 6
+#endif
+#ifndef MPM_TBMIN_U2
+#define MPM_TBMIN_U2 4
+#endif
+// 2D: half the state per particle.  Measured on config 3 (profiles/r02_experiments.md): the gather kernel gains 14 % at 6 blocks
+// per SM (80 registers, no spill); the update kernel spills below 128 registers and loses, so it stays at 4
+constexpr int kTBMinG2 = MPM_TBMIN_G2, kTBMinU2 = MPM_TBMIN_U2;
 
 template <int DIM>
 struct Chunk {
@@ -531,20 +615,23 @@ __device__ __forceinline__ void coop_p2g1(const GridDesc &gd, const GArr &gn, un
 // atomic each; the atomics are issued before the scatter and their results consumed after it.
 // The particle fields of the NEXT pass are copied into shared memory while the current pass computes (see "particle
 // streams" above).  V' overwrites V in place.
-template <int DIM, bool ACC32, bool BULK>
-__global__ void __launch_bounds__(kTB, kTBMinG) k_g2p_p2g2_tiled(GridDesc gd, PArr p, GArr g,
+template <int DIM, bool ACC32, bool BULK, bool COLOUR, bool CM>
+__global__ void __launch_bounds__(kTB, DIM == 2 ? kTBMinG2 : kTBMinG) k_g2p_p2g2_tiled(GridDesc gd, PArr p, GArr g,
                                                                 const DevScalars *__restrict__ sc, SortedMap map,
                                                                 const int4 *__restrict__ items, const int *__restrict__ n_items,
                                                                 int *__restrict__ count, unsigned long long *__restrict__ dest,
                                                                 unsigned long long *__restrict__ n_cell_changes)
 {
+    static_assert(CM || !COLOUR, "accumulation by colour needs the colour-major cell numbering");
     using TG = TileGeo<DIM>;
     constexpr int NB = 1 << DIM, LG = Geo<DIM>::LG, GPB = kTB / LG, CH = 2 * DIM, NF = 2 * DIM + 1;
     __shared__ __align__(16) double s_tile[TG::NN * CH];
     __shared__ __align__(16) double s_pf[kTB / 32][NF][kWin];      // per warp: x[d], v[d], m of the pass's slot window
     __shared__ __align__(8) unsigned long long s_bar[kTB / 32][2];  // per warp: X copies / V, M copies
+    __shared__ __align__(16) double s_acc[COLOUR ? TG::NN * DIM : 1];   // COLOUR: accumulator tile of mv2
     __shared__ int s_moved;
     if (threadIdx.x == 0) s_moved = 0;
+    if (COLOUR) for (int j = threadIdx.x; j < TG::NN * DIM; j += kTB) s_acc[j] = 0.0;
     int n_moved = 0;
     if ((int)blockIdx.x >= *n_items) return;
     const int4 item = __ldg(items + blockIdx.x);      // {tile, first group, groups, -}
@@ -608,11 +695,13 @@ __global__ void __launch_bounds__(kTB, kTBMinG) k_g2p_p2g2_tiled(GridDesc gd, PA
     stage_tile<DIM, CH, false, ACC32>(gd, org, g, dt, s_tile);
     __syncthreads();
     unsigned parity = 0;
+    PassColours<DIM> pc{ 0, 0 }, pcn{ 0, 0 };
+    if (COLOUR) { pc = pass_colours<DIM>(map.groups, item.y, g_end, GPB); pcn = pass_colours<DIM>(map.groups, item.y + GPB, g_end, GPB); }
     for (int p0 = 0; p0 < item.z; p0 += GPB, gl += GPB, parity ^= 1u) {
         int c[DIM];
         unpack_coords<DIM>(grp.cpack, c);
         const int local = grp.cell & (TG::TC - 1);      // grp.cell = tile-major key
-        const int j0 = (local & (TG::T0 - 1)) + TG::N0 * (((local >> TG::LT0) & (TG::T1 - 1)) + TG::N1 * (local >> (TG::LT0 + TG::LT1)));
+        const int j0 = TG::node0_of(local, CM);
         const bool valid[2] = { 2 * l < grp.cnt, 2 * l + 1 < grp.cnt };
         const long long k0 = (long long)grp.first + 2 * l;
         double X[2][DIM], V[2][DIM], M[2];
@@ -662,7 +751,7 @@ __global__ void __launch_bounds__(kTB, kTBMinG) k_g2p_p2g2_tiled(GridDesc gd, PA
                 int nclamp;
                 move_particle<DIM>(gd, X[i], out[i], dt, gd.in_axis >= 0 ? (long long)p.id[k0 + i] : 0, step, Xn, recycled, nclamp);
             }
-            key[i] = valid[i] ? tiled_key_of_position<DIM>(gd, Xn) : -1;
+            key[i] = valid[i] ? tiled_key_of_position<DIM, CM>(gd, Xn) : -1;
         }
         // V' replaces V in memory (the update kernel reads it back instead of gathering A again)
 #pragma unroll
@@ -703,7 +792,18 @@ __global__ void __launch_bounds__(kTB, kTBMinG) k_g2p_p2g2_tiled(GridDesc gd, PA
                 tot[a][0] = v[0];
                 tot[a][1] = v[LG];
             }
-            if (fold_warp_one_cell<DIM, DIM>(tot, lane, one_cell, grp.cnt > 0)) {
+            const bool issue = fold_warp_one_cell<DIM, DIM>(tot, lane, one_cell, grp.cnt > 0);
+            int phase = -1;
+            if (COLOUR) {      // eligible groups add into the shared accumulator tile, one colour at a time
+                phase = colour_phase<DIM>(pc, grp);
+                __syncthreads();                                   // the previous pass's additions are complete
+                if (phase == 0 && issue) tile_accumulate<DIM, DIM>(s_acc, j0, l, tot);
+                if (pc.hi != pc.lo) {
+                    __syncthreads();
+                    if (phase == 1 && issue) tile_accumulate<DIM, DIM>(s_acc, j0, l, tot);
+                }
+            }
+            if (phase < 0 && issue) {
 #pragma unroll
                 for (int q = 0; q < 2; ++q) {
                     const int node = corner_node_i<DIM>(gd, c, l + q * LG);
@@ -727,6 +827,20 @@ __global__ void __launch_bounds__(kTB, kTBMinG) k_g2p_p2g2_tiled(GridDesc gd, PA
         w0 = w0n;
         wn = wnn;
         warp_window<BULK>(nxt.first, nxt.cnt, w0n, wnn);
+        if (COLOUR) { pc = pcn; pcn = pass_colours<DIM>(map.groups, item.y + p0 + 2 * GPB, g_end, GPB); }
+    }
+    if (COLOUR) {      // flush the accumulator tile: one global reduction per non-zero node value
+        __syncthreads();
+        for (int j = threadIdx.x; j < TG::NN; j += kTB) {
+            int idx[DIM];
+            const int node = tile_node_global<DIM>(gd, org, j, idx);
+            if (node < 0) continue;
+#pragma unroll
+            for (int a = 0; a < DIM; ++a) {
+                const double v = s_acc[j * DIM + a];
+                if (v != 0.0) acc_add<ACC32>(g.mv2[a], node, v);
+            }
+        }
     }
     // particles that changed cell in this step (mpm_stats.n_cell_changes): one atomic per block
     n_moved = __reduce_add_sync(kFull, n_moved);
@@ -754,11 +868,13 @@ struct UpdSmem {
     static constexpr size_t ID = sizeof(int) * NW * kWin;
     static constexpr size_t BAR = sizeof(unsigned long long) * NW * 2;
     static constexpr size_t BYTES = TILE + PF + DEST + ID + BAR;
+    static constexpr int NACC = 2 * DIM + 1;                // COLOUR: accumulator tile of m, mv, f behind the rest
+    static constexpr size_t ACC = sizeof(double) * TG::NN * NACC;
     static_assert(TILE % 16 == 0 && PF % 16 == 0 && DEST % 16 == 0 && ID % 16 == 0, "16-byte aligned sections");
 };
 
-template <int DIM, bool ACC32, bool BULK>
-__global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr p, PArr q, GArr g, DevScalars *sc, SortedMap map,
+template <int DIM, bool ACC32, bool BULK, bool COLOUR, bool CM>
+__global__ void __launch_bounds__(kTB, COLOUR ? 3 : DIM == 2 ? kTBMinU2 : kTBMinU) k_update_tiled(GridDesc gd, PArr p, PArr q, GArr g, DevScalars *sc, SortedMap map,
                                                               const int4 *__restrict__ items, const int *__restrict__ n_items,
                                                               const int *__restrict__ off_new,
                                                               const unsigned long long *__restrict__ dest, GArr gn, int store_q)
@@ -772,6 +888,7 @@ __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr
     unsigned long long (*s_dest)[kWin] = reinterpret_cast<unsigned long long (*)[kWin]>(s_raw + SM::TILE + SM::PF);
     int (*s_id)[kWin] = reinterpret_cast<int (*)[kWin]>(s_raw + SM::TILE + SM::PF + SM::DEST);
     unsigned long long (*s_bar)[2] = reinterpret_cast<unsigned long long (*)[2]>(s_raw + SM::TILE + SM::PF + SM::DEST + SM::ID);
+    double *s_acc = reinterpret_cast<double *>(s_raw + SM::BYTES);      // COLOUR only
     __shared__ double s_v[kTB / 32], s_c[kTB / 32];
     if ((int)blockIdx.x >= *n_items) return;
     const int4 item = __ldg(items + blockIdx.x);
@@ -840,16 +957,22 @@ __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr
     const double dt = sc->dt;
     const long long step = sc->step;
     stage_tile<DIM, CH, true, ACC32>(gd, org, g, dt, s_tile);
+    if (COLOUR) for (int j = threadIdx.x; j < TG::NN * SM::NACC; j += kTB) s_acc[j] = 0.0;
+    PassColours<DIM> pc{ 0, 0 }, pcn{ 0, 0 };
+    if (COLOUR) { pc = pass_colours<DIM>(map.groups, item.y, g_end, GPB); pcn = pass_colours<DIM>(map.groups, item.y + GPB, g_end, GPB); }
     __syncthreads();
     double vloc = 0.0, cloc = 0.0;
-    int n_rec = 0, n_clamp = 0, n_neg = 0, n_nonfin = 0, n_ooc = 0;
+    // per-thread event counters of the block's <= 16 passes x 2 particles, packed into one register: recycled (bits 0-5),
+    // clamped coordinates (6-12, <= 3 per particle), 1 + dt D <= 0 (13-18), non-finite (19-24), out of cell (25-30)
+    unsigned events = 0u;
+    static_assert(Chunk<DIM>::PASSES * 2 <= 32, "event counters are 6 bits wide");
     const double gm1 = gd.gamma - 1.0;
     unsigned parity = 0;
     for (int p0 = 0; p0 < item.z; p0 += GPB, gl += GPB, parity ^= 1u) {
         int c[DIM];
         unpack_coords<DIM>(grp.cpack, c);
         const int local = grp.cell & (TG::TC - 1);
-        const int j0 = (local & (TG::T0 - 1)) + TG::N0 * (((local >> TG::LT0) & (TG::T1 - 1)) + TG::N1 * (local >> (TG::LT0 + TG::LT1)));
+        const int j0 = TG::node0_of(local, CM);
         const bool valid[2] = { 2 * l < grp.cnt, 2 * l + 1 < grp.cnt };
         double X[2][DIM];
         int key[2];
@@ -882,7 +1005,7 @@ __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr
 #pragma unroll
         for (int i = 0; i < 2; ++i) {
             weights_1d<DIM>(gd, X[i], c, xi[i], W[i]);
-            n_ooc += (int)(valid[i] && !in_unit_cell<DIM>(xi[i]));      // the exact-sort invariant (must never count)
+            events += (unsigned)(valid[i] && !in_unit_cell<DIM>(xi[i])) << 25;      // the exact-sort invariant (must never count)
         }
         gather_tile<DIM, CH, true>(s_tile + j0 * CH, W, out, Dh);
         // the fields that are only needed from here on stay in shared memory during the gather (register budget)
@@ -935,12 +1058,12 @@ __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr
             const double jac = fma(dt, D, 1.0);
             double rhon = r / jac;
             if (valid[i]) {
-                if (jac <= 0.0) n_neg++;
+                events += (unsigned)(jac <= 0.0) << 13;
                 double vv = 0.0, vb2 = 0.0;
 #pragma unroll
                 for (int a = 0; a < DIM; ++a) { vv = fma(Vo[i][a], Vo[i][a], vv); vb2 = fma(out[i][a], out[i][a], vb2); }
                 // E', rho', V' and Vbar (hence X' = X + dt Vbar) all finite?
-                if (!isfinite(En) || !isfinite(rhon) || !isfinite(vv + vb2)) n_nonfin++;
+                events += (unsigned)(!isfinite(En) || !isfinite(rhon) || !isfinite(vv + vb2)) << 19;
                 vloc = fmax(vloc, fmax(vv, vb2));                // squared; the root is taken once at the end
                 cloc = fmax(cloc, gd.gamma * gm1 * En);          // c_s^2 = gamma P'/rho' (the root is monotone: taken at the end)
             }
@@ -949,12 +1072,12 @@ __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr
                 bool recycled;
                 int nclamp;
                 move_particle<DIM>(gd, X[i], out[i], dt, (long long)id[i], step, Xo[i], recycled, nclamp);
-                n_clamp += nclamp;
+                events += (unsigned)nclamp << 6;
                 if (recycled) {
 #pragma unroll
                     for (int a = 0; a < DIM; ++a) Vo[i][a] = gd.inflow_v[a];
                     rhon = gd.inflow_rho; En = gd.inflow_e; Q = 0.0; Q_over_rho = 0.0; Mn = gd.inflow_mass;
-                    n_rec++;
+                    events += 1u;
                 }
             }
             Mo[i] = Mn; Ro[i] = rhon; Eo[i] = En; Qo[i] = Q;
@@ -1002,27 +1125,62 @@ __global__ void __launch_bounds__(kTB, kTBMinU) k_update_tiled(GridDesc gd, PArr
             double xin[DIM];
 #pragma unroll
             for (int a = 0; a < DIM; ++a) xin[a] = __dmul_rn(Xo[i][a], gd.inv_h) - (double)c[a];
-            n_ooc += (int)(stay[i] && !in_unit_cell<DIM>(xin));      // both kernels must agree on X' bit for bit
+            events += (unsigned)(stay[i] && !gd.has_open && !in_unit_cell<DIM>(xin)) << 25;      // both kernels must agree on X' bit for bit
             swizzled_weights<DIM>(xin, l, wnew[i]);
             pay[i][0] = stay[i] ? Mo[i] : 0.0;
             pay[i][DIM + 1] = stay[i] ? Sn[i] : 0.0;
 #pragma unroll
             for (int a = 0; a < DIM; ++a) pay[i][1 + a] = stay[i] ? Mo[i] * Vo[i][a] : 0.0;
         }
-        scatter_p2g1_group<DIM, ACC32>(gd, gn, c, l, grp.cnt > 0, pay, wnew, warp_one_cell(grp.cell, grp.cnt));
+        {
+            double tot[SM::NACC][2];
+            const bool issue = p2g1_group_totals<DIM>(gd, l, grp.cnt > 0, pay, wnew, warp_one_cell(grp.cell, grp.cnt), tot);
+            int phase = -1;
+            if (COLOUR) {      // eligible groups add into the shared accumulator tile, one colour at a time
+                phase = colour_phase<DIM>(pc, grp);
+                __syncthreads();                                   // the previous pass's additions are complete
+                if (phase == 0 && issue) tile_accumulate<DIM, SM::NACC>(s_acc, j0, l, tot);
+                if (pc.hi != pc.lo) {
+                    __syncthreads();
+                    if (phase == 1 && issue) tile_accumulate<DIM, SM::NACC>(s_acc, j0, l, tot);
+                }
+            }
+            if (phase < 0 && issue) p2g1_commit_global<DIM, ACC32>(gd, gn, c, l, tot);
+        }
         grp = nxt;
         nxt = nn;
         w0 = w0n;
         wn = wnn;
         warp_window<BULK>(nxt.first, nxt.cnt, w0n, wnn);
+        if (COLOUR) { pc = pcn; pcn = pass_colours<DIM>(map.groups, item.y + p0 + 2 * GPB, g_end, GPB); }
+    }
+    if (COLOUR) {      // flush the accumulator tile: one global reduction per non-zero node value
+        __syncthreads();
+        for (int j = threadIdx.x; j < TG::NN; j += kTB) {
+            int idx[DIM];
+            const int node = tile_node_global<DIM>(gd, org, j, idx);
+            if (node < 0) continue;
+            const double *src = s_acc + j * SM::NACC;
+            if (src[0] != 0.0) acc_add<ACC32>(gn.m, node, src[0]);
+#pragma unroll
+            for (int a = 0; a < DIM; ++a) {
+                if (src[1 + a] != 0.0) acc_add<ACC32>(gn.mv[a], node, src[1 + a]);
+                if (src[1 + DIM + a] != 0.0) acc_add<ACC32>(gn.f[a], node, src[1 + DIM + a]);
+            }
+        }
     }
     // block maxima -> at most one atomicMax per block (max is order-free, so this is exact)
     vloc = warp_max_nonneg(sqrt(vloc));
     cloc = warp_max_nonneg(cloc > 0.0 ? sqrt(cloc) : 0.0);
     if (lane == 0) { s_v[warp] = vloc; s_c[warp] = cloc; }
-    const int rec_sum = __reduce_add_sync(kFull, n_rec), neg_sum = __reduce_add_sync(kFull, n_neg),
-              nf_sum = __reduce_add_sync(kFull, n_nonfin), clamp_sum = __reduce_add_sync(kFull, n_clamp),
-              ooc_sum = __reduce_add_sync(kFull, n_ooc);
+    int rec_sum = 0, neg_sum = 0, nf_sum = 0, clamp_sum = 0, ooc_sum = 0;
+    if (__any_sync(kFull, events != 0u)) {      // rare
+        rec_sum = __reduce_add_sync(kFull, (int)(events & 63u));
+        clamp_sum = __reduce_add_sync(kFull, (int)((events >> 6) & 127u));
+        neg_sum = __reduce_add_sync(kFull, (int)((events >> 13) & 63u));
+        nf_sum = __reduce_add_sync(kFull, (int)((events >> 19) & 63u));
+        ooc_sum = __reduce_add_sync(kFull, (int)((events >> 25) & 63u));
+    }
     if (lane == 0) {
         if (rec_sum) atomicAdd(&sc->n_recycled, (unsigned long long)rec_sum);
         if (neg_sum) atomicAdd(&sc->n_negjac, (unsigned long long)neg_sum);
@@ -1148,7 +1306,7 @@ __global__ void __launch_bounds__(kMapBlock) k_cell_map_tiled(GridDesc gd, const
                 const int cpack = (DIM == 3) ? (cc[0] | (cc[1] << 10) | (cc[DIM - 1] << 20)) : (cc[0] | (cc[1] << 16));
                 for (int first = 0; first < c[j]; first += CAP, ++g) {
                     MPM_CHECK(g >= 0 && g < gd.max_groups && (long long)slot + c[j] <= gd.slots);
-                    groups[g] = make_int4(slot + first, min(CAP, c[j] - first), key, cpack);
+                    groups[g] = make_int4(slot + first, min(CAP, c[j] - first) | (c[j] > CAP ? 0x100 : 0), key, cpack);
                 }
             }
             slot += (c[j] + 1) & ~1;
@@ -1191,7 +1349,7 @@ __global__ void __launch_bounds__(kBlock) k_gather_by_id_groups(const double *sr
     const int n_groups = *map.n_groups;
     for (long long gq = (long long)blockIdx.x * kBlock + threadIdx.x; gq < n_groups; gq += (long long)gridDim.x * kBlock) {
         const int4 r = map.groups[gq];
-        for (int j = 0; j < r.y; ++j) {
+        for (int j = 0; j < (r.y & 0xff); ++j) {
             const long long k = (long long)r.x + j;
             const long long d = coff ? (long long)coff[r.z] + (k - off[r.z]) : (long long)id[k];
             dst[d] = src[k];
@@ -1207,7 +1365,7 @@ __global__ void __launch_bounds__(kBlock) k_stats_reduce_groups(PArr p, DevScala
     const int n_groups = *map.n_groups;
     for (long long gq = (long long)blockIdx.x * kBlock + threadIdx.x; gq < n_groups; gq += (long long)gridDim.x * kBlock) {
         const int4 r = map.groups[gq];
-        for (int j = 0; j < r.y; ++j) {
+        for (int j = 0; j < (r.y & 0xff); ++j) {
             const long long k = (long long)r.x + j;
             const double M = p.m[k];
             double v2 = 0.0;
@@ -1334,11 +1492,15 @@ void launch_g2p_p2g2_tiled(const GridDesc &gd, const PArr &p, const GArr &g, con
 {
     if (max_items <= 0) return;
     set_checked_bounds(gd, s);
-#define MPM_LAUNCH_G2P(D, A, B) \
-    k_g2p_p2g2_tiled<D, A, B><<<(unsigned)max_items, kTB, 0, s>>>(gd, p, g, sc, map, items, n_items, count, dest, \
-                                                                  const_cast<unsigned long long *>(&sc->n_cell_changes))
-#define MPM_LAUNCH_G2P_A(D, A) do { if (gd.bulk_stream) MPM_LAUNCH_G2P(D, A, true); else MPM_LAUNCH_G2P(D, A, false); } while (0)
-    if (gd.dim == 2) { if (gd.acc32) MPM_LAUNCH_G2P_A(2, true); else MPM_LAUNCH_G2P_A(2, false); }
+#define MPM_LAUNCH_G2P(D, A, B, C, CM) \
+    k_g2p_p2g2_tiled<D, A, B, C, CM><<<(unsigned)max_items, kTB, 0, s>>>(gd, p, g, sc, map, items, n_items, count, dest, \
+                                                                         const_cast<unsigned long long *>(&sc->n_cell_changes))
+#define MPM_LAUNCH_G2P_A(D, A) do { if (gd.bulk_stream) MPM_LAUNCH_G2P(D, A, true, false, false); else MPM_LAUNCH_G2P(D, A, false, false, false); } while (0)
+    if (gd.p2g_mode & MPM_P2G_COLOUR_G2P) {      // fp64 accumulation and the cp.async stream only (mpm_create checks)
+        if (gd.dim == 2) MPM_LAUNCH_G2P(2, false, false, true, true); else MPM_LAUNCH_G2P(3, false, false, true, true);
+    } else if (gd.colour_major) {                // the update kernel accumulates by colour: same cell numbering here
+        if (gd.dim == 2) MPM_LAUNCH_G2P(2, false, false, false, true); else MPM_LAUNCH_G2P(3, false, false, false, true);
+    } else if (gd.dim == 2) { if (gd.acc32) MPM_LAUNCH_G2P_A(2, true); else MPM_LAUNCH_G2P_A(2, false); }
     else { if (gd.acc32) MPM_LAUNCH_G2P_A(3, true); else MPM_LAUNCH_G2P_A(3, false); }
 #undef MPM_LAUNCH_G2P_A
 #undef MPM_LAUNCH_G2P
@@ -1352,10 +1514,23 @@ void launch_update_tiled(const GridDesc &gd, const PArr &p, const PArr &q, const
     set_checked_bounds(gd, s);
     const int sq = store_q ? 1 : 0;
     static_assert(UpdSmem<2>::BYTES <= 48 * 1024 && UpdSmem<3>::BYTES <= 48 * 1024, "dynamic shared memory beyond 48 KB needs a per-device opt-in");
-#define MPM_LAUNCH_UPD(D, A, B) \
-    k_update_tiled<D, A, B><<<(unsigned)max_items, kTB, UpdSmem<D>::BYTES, s>>>(gd, p, q, g, sc, map, items, n_items, off_new, dest, g_next, sq)
-#define MPM_LAUNCH_UPD_A(D, A) do { if (gd.bulk_stream) MPM_LAUNCH_UPD(D, A, true); else MPM_LAUNCH_UPD(D, A, false); } while (0)
-    if (gd.dim == 2) { if (gd.acc32) MPM_LAUNCH_UPD_A(2, true); else MPM_LAUNCH_UPD_A(2, false); }
+    static_assert(UpdSmem<2>::BYTES % 16 == 0 && UpdSmem<3>::BYTES % 16 == 0, "the accumulator tile starts 16-byte aligned");
+#define MPM_LAUNCH_UPD(D, A, B, C, CM, BYTES) \
+    k_update_tiled<D, A, B, C, CM><<<(unsigned)max_items, kTB, BYTES, s>>>(gd, p, q, g, sc, map, items, n_items, off_new, dest, g_next, sq)
+#define MPM_LAUNCH_UPD_A(D, A) do { if (gd.bulk_stream) MPM_LAUNCH_UPD(D, A, true, false, false, UpdSmem<D>::BYTES); else MPM_LAUNCH_UPD(D, A, false, false, false, UpdSmem<D>::BYTES); } while (0)
+    if (gd.p2g_mode & MPM_P2G_COLOUR_UPDATE) {   // fp64 accumulation and the cp.async stream only (mpm_create checks)
+        // more than 48 KB of dynamic shared memory needs the opt-in; the attribute is per device, so it is set at every
+        // launch (a host-side call without a synchronisation)
+        if (gd.dim == 2) {
+            cudaFuncSetAttribute(k_update_tiled<2, false, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(UpdSmem<2>::BYTES + UpdSmem<2>::ACC));
+            MPM_LAUNCH_UPD(2, false, false, true, true, UpdSmem<2>::BYTES + UpdSmem<2>::ACC);
+        } else {
+            cudaFuncSetAttribute(k_update_tiled<3, false, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(UpdSmem<3>::BYTES + UpdSmem<3>::ACC));
+            MPM_LAUNCH_UPD(3, false, false, true, true, UpdSmem<3>::BYTES + UpdSmem<3>::ACC);
+        }
+    } else if (gd.colour_major) {                // the gather kernel accumulates by colour: same cell numbering here
+        if (gd.dim == 2) MPM_LAUNCH_UPD(2, false, false, false, true, UpdSmem<2>::BYTES); else MPM_LAUNCH_UPD(3, false, false, false, true, UpdSmem<3>::BYTES);
+    } else if (gd.dim == 2) { if (gd.acc32) MPM_LAUNCH_UPD_A(2, true); else MPM_LAUNCH_UPD_A(2, false); }
     else { if (gd.acc32) MPM_LAUNCH_UPD_A(3, true); else MPM_LAUNCH_UPD_A(3, false); }
 #undef MPM_LAUNCH_UPD_A
 #undef MPM_LAUNCH_UPD
@@ -1365,6 +1540,14 @@ void launch_update_tiled(const GridDesc &gd, const PArr &p, const PArr &q, const
 __global__ void __launch_bounds__(256) k_widen(const float *__restrict__ src, double *__restrict__ dst, long long n)
 {
     for (long long i = (long long)blockIdx.x * 256 + threadIdx.x; i < n; i += (long long)gridDim.x * 256) dst[i] = (double)src[i];
+}
+__global__ void __launch_bounds__(256) k_add_into(double *__restrict__ dst, const double *__restrict__ src, long long n)
+{
+    for (long long i = (long long)blockIdx.x * 256 + threadIdx.x; i < n; i += (long long)gridDim.x * 256) dst[i] += src[i];
+}
+void launch_add_into(double *dst, const double *src, long long n, cudaStream_t s)
+{
+    if (n > 0) k_add_into<<<(unsigned)((n + 255) / 256 < 148 * 8 ? (n + 255) / 256 : 148 * 8), 256, 0, s>>>(dst, src, n);
 }
 void launch_widen(const double *src_as_float, double *dst, long long n, cudaStream_t s)
 {

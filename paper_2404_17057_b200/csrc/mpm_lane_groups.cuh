@@ -42,16 +42,17 @@ __device__ __forceinline__ void butterfly(double v[1 << DIM])
 struct Group {
     int first;     // first particle of the group
     int cnt;       // particles in the group (<= 2^d), 0 = idle
-    int cell;      // linear cell index
+    int cell;      // cell key
     int cpack;     // packed cell coordinates (3D: 10 bits each, 2D: 16 bits each)
+    int multi;     // the cell has more than one group (more than 2^d particles)
 };
 
 __device__ __forceinline__ Group fetch_group(const int4 *__restrict__ groups, long long gidx, int n_groups)
 {
-    Group g{ 0, 0, 0, 0 };
+    Group g{ 0, 0, 0, 0, 0 };
     if (gidx < (long long)n_groups) {
-        const int4 r = __ldg(groups + gidx);
-        g.first = r.x; g.cnt = r.y; g.cell = r.z; g.cpack = r.w;
+        const int4 r = __ldg(groups + gidx);      // {first slot, count | multi << 8, key, packed coordinates}
+        g.first = r.x; g.cnt = r.y & 0xff; g.multi = r.y >> 8; g.cell = r.z; g.cpack = r.w;
     }
     return g;
 }
@@ -231,8 +232,11 @@ __device__ __forceinline__ void move_particle(const GridDesc &gd, const double X
             const int jb = 1 + 2 * (a - (a > gd.in_axis ? 1 : 0));
             const double u1 = recycle_uniform(gd.recycle_seed, id, step, jb);
             const double u2 = recycle_uniform(gd.recycle_seed, id, step, jb + 1);
-            int cell = (int)floor(u1 * (double)gd.nc[a]);
-            cell = min(cell, gd.nc[a] - 1);
+            // a slab of a larger domain (last axis): the inflow face is the GLOBAL one, the cell index is made slab-local
+            const bool slab = gd.slab_global_n > 0 && a == DIM - 1;
+            const int na = slab ? gd.slab_global_n : gd.nc[a];
+            int cell = (int)floor(u1 * (double)na);
+            cell = min(cell, na - 1) - (slab ? gd.slab_offset : 0);
             const double x_face = (gd.in_side == 0) ? off : __dsub_rn(gd.L[a], off);
             const double x_other = ((double)cell + u2) * gd.h;
             Xn[a] = (a == gd.in_axis) ? x_face : x_other;
@@ -241,9 +245,9 @@ __device__ __forceinline__ void move_particle(const GridDesc &gd, const double X
     nclamp = 0;
 #pragma unroll
     for (int a = 0; a < DIM; ++a) {
-        if (!gd.per[a]) {
-            if (Xn[a] < 0.0) { Xn[a] = 0.0; nclamp++; }
-            if (Xn[a] > gd.L[a]) { Xn[a] = gd.L[a]; nclamp++; }
+        if (!gd.per[a]) {      // an OPEN face is an interface to the neighbouring slab: the particle leaves, unclamped
+            if (Xn[a] < 0.0 && gd.bc[a][0] != MPM_BC_OPEN) { Xn[a] = 0.0; nclamp++; }
+            if (Xn[a] > gd.L[a] && gd.bc[a][1] != MPM_BC_OPEN) { Xn[a] = gd.L[a]; nclamp++; }
         }
     }
 }

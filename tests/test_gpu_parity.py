@@ -322,6 +322,90 @@ def test_bulk_particle_stream_matches_cp_async_bit_for_bit(po, mpm, name):
         mpm.Solver(w["cfg"], sort_every=0, variant=mpm.VARIANT_ATOMIC, particle_stream=mpm.STREAM_BULK)
 
 
+@pytest.mark.parametrize("p2g_mode", [1, 2, 3])
+@pytest.mark.parametrize("name", ["sod", "box", "box_shuffled", "cylinder", "sedov", "clumps", "clumps_dense", "sphere3d"])
+def test_colour_accumulation_matches_oracle(po, mpm, name, p2g_mode):
+    """mpm_config.p2g_mode = MPM_P2G_COLOUR_*: the atomics-free accumulation by cell colouring in the
+    gather kernel (bit 0), the update kernel (bit 1) or both.  Only the summation order changes (reading A17): same
+    one-step grid parity (1e-12) and many-step particle parity (1e-9) against the oracle as the default path."""
+    w = small_workloads()[name]()
+    o = po.Oracle(w["cfg"])
+    o.load_particles(w["x"], w["v"], w["mass"], w["rho"], w["e"])
+    g = mpm.Solver(w["cfg"], sort_every=1, variant=mpm.VARIANT_TILED, p2g_mode=p2g_mode)
+    g.load_particles(w["x"], w["v"], w["mass"], w["rho"], w["e"])
+    o.step(0.0, w["cfl"], 2)       # two steps: the second one starts from the update kernel's fused P2G#1
+    g.step(0.0, w["cfl"], 2)
+    fscale = _force_scale(w)
+    for fo, fg, scale in ((po.G_MASS, mpm.G_MASS, None), (po.G_MOM, mpm.G_MOMENTUM, None),
+                          (po.G_MOM2, mpm.G_MOMENTUM2, None), (po.G_FORCE, mpm.G_FORCE, fscale)):
+        a, b = o.grid(fo), g.read_grid(fg)
+        sc = scale if scale is not None else np.abs(a).max()
+        assert np.abs(a - b).max() <= 4 * GRID_TOL * sc, (name, fo, np.abs(a - b).max(), sc)
+    nsteps = min(STEPS[name], 40)
+    o.step(0.0, w["cfl"], nsteps - 2)
+    g.step(0.0, w["cfl"], nsteps - 2)
+    so, sg = o.stats(), g.stats()
+    assert sg.n_out_of_cell == 0 and sg.n_nonfinite == 0 and sg.n_recycled == so.n_recycled
+    p = g.read_particles()
+    for key, fo in (("rho", po.P_RHO), ("e", po.P_E), ("x", po.P_X)):
+        a = o.particles(fo)
+        assert np.abs(a - p[key]).sum() <= PART_TOL * np.abs(a).sum(), (name, p2g_mode, key)
+    v = o.particles(po.P_V)
+    assert np.abs(v - p["v"]).sum() <= PART_TOL * np.sqrt((v ** 2).sum(axis=0)).sum() * w["cfg"]["dim"], name
+    with pytest.raises(mpm.MpmError):
+        mpm.Solver(w["cfg"], sort_every=1, variant=mpm.VARIANT_TILED, p2g_mode=p2g_mode, grid_accum=mpm.ACCUM_FP32)
+
+
+@pytest.mark.parametrize("sort_every", [0, 1, 4])
+@pytest.mark.parametrize("name", ["box", "box_shuffled", "clumps", "clumps_dense"])
+def test_quadratic_bspline_basis_matches_oracle(po, mpm, name, sort_every):
+    """mpm_config.basis = MPM_BASIS_QUADRATIC (reading A20): the ATOMIC
+    kernels over the 3^d-node B-spline support against the oracle's quadratic code path on the periodic workloads:
+    grid fields after one step (1e-12), particle fields after 30-50 steps (1e-9)."""
+    w = small_workloads()[name]()
+    cfg = dict(w["cfg"], basis=1)
+    o = po.Oracle(cfg)
+    o.load_particles(w["x"], w["v"], w["mass"], w["rho"], w["e"])
+    g = mpm.Solver(cfg, sort_every=sort_every)            # AUTO -> ATOMIC for this basis
+    g.load_particles(w["x"], w["v"], w["mass"], w["rho"], w["e"])
+    assert g.stats().variant == mpm.VARIANT_ATOMIC
+    assert o.step(0.0, w["cfl"], 1) == g.step(0.0, w["cfl"], 1)
+    fscale = _force_scale(w)
+    for fo, fg, scale in ((po.G_MASS, mpm.G_MASS, None), (po.G_MOM, mpm.G_MOMENTUM, None),
+                          (po.G_MOM2, mpm.G_MOMENTUM2, None), (po.G_FORCE, mpm.G_FORCE, fscale)):
+        a, b = o.grid(fo), g.read_grid(fg)
+        sc = scale if scale is not None else np.abs(a).max()
+        assert np.abs(a - b).max() <= GRID_TOL * sc, (name, fo, np.abs(a - b).max(), sc)
+    nsteps = min(STEPS[name], 50)
+    o.step(0.0, w["cfl"], nsteps - 1)
+    g.step(0.0, w["cfl"], nsteps - 1)
+    so, sg = o.stats(), g.stats()
+    assert so.step == sg.step and abs(so.t - sg.t) <= 1e-10 * so.t and sg.n_nonfinite == 0 and so.n_negjac == sg.n_negjac
+    p = g.read_particles()
+    for key, fo in (("rho", po.P_RHO), ("e", po.P_E)):
+        a = o.particles(fo)
+        assert np.abs(a - p[key]).sum() <= PART_TOL * np.abs(a).sum(), (name, key)
+    v = o.particles(po.P_V)
+    assert np.abs(v - p["v"]).sum() <= PART_TOL * np.sqrt((v ** 2).sum(axis=0)).sum() * cfg["dim"], name
+    # the quadratic result is NOT the Q1 result (the basis really changed)
+    q1 = po.Oracle(w["cfg"])
+    q1.load_particles(w["x"], w["v"], w["mass"], w["rho"], w["e"])
+    q1.step(0.0, w["cfl"], 1)
+    o1 = po.Oracle(cfg)
+    o1.load_particles(w["x"], w["v"], w["mass"], w["rho"], w["e"])
+    o1.step(0.0, w["cfl"], 1)
+    assert np.abs(q1.particles(po.P_RHO) - o1.particles(po.P_RHO)).max() > 1e-6
+
+
+def test_quadratic_bspline_basis_needs_periodic_atomic(mpm):
+    cfg = dict(dim=2, n=[8, 8], dx=0.125, gamma=1.4, bc=[[0, 0], [0, 0]], basis=1)
+    with pytest.raises(mpm.MpmError):
+        mpm.Solver(cfg, sort_every=1, variant=mpm.VARIANT_TILED)
+    with pytest.raises(mpm.MpmError):
+        mpm.Solver(dict(cfg, bc=[[1, 1], [0, 0]]), sort_every=0)
+    assert mpm.Solver(cfg, sort_every=1).stats().variant == mpm.VARIANT_ATOMIC
+
+
 def test_fp32_grid_accumulation_needs_tiled(mpm):
     cfg = dict(dim=2, n=[8, 8], dx=0.125, gamma=1.4, bc=[[0, 0], [0, 0]])
     with pytest.raises(mpm.MpmError):
