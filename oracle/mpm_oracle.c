@@ -787,6 +787,34 @@ int oracle_halo(oracle_t *o, int which, int side, int op, double *buf)
     return 0;
 }
 
+/* Diagnostic only (reading A18; the "interpolated on the grid" curve of Fig. 5): mass-weighted nodal mean
+ * of a particle field, out_i = sum_k M_k a_k phi_i(X_k) / sum_k M_k phi_i(X_k) with a = rho (which 0) or E (which 1), 0 where
+ * the node has no mass.  Q1 basis.  Not part of Algorithm 1; touches none of its arrays. */
+int oracle_grid_diagnostic(const oracle_t *o, int which, double *out)
+{
+    if (!o || !out || (which != 0 && which != 1) || o->cfg.basis != ORC_BASIS_Q1) return -1;
+    const long long n = o->Np, Nn = o->Nn;
+    const int nb = 1 << o->d;
+    double *den = (double *)calloc((size_t)Nn, sizeof(double));
+    for (long long i = 0; i < Nn; ++i) out[i] = 0.0;
+    for (long long k = 0; k < n; ++k) {
+        int c[3]; double w[3][2], g[3][2];
+        particle_cell(o, &o->X[k], n, c, w, g);
+        double a = which == 0 ? o->rho[k] : o->E[k];
+        for (int ib = 0; ib < nb; ++ib) {
+            int b[3] = { ib & 1, (ib >> 1) & 1, (ib >> 2) & 1 };
+            double phi, grad[3];
+            long long i = corner_node(o, c, b);
+            corner_weights(o, w, g, b, &phi, grad);
+            out[i] += o->M[k] * a * phi;
+            den[i] += o->M[k] * phi;
+        }
+    }
+    for (long long i = 0; i < Nn; ++i) out[i] = (den[i] != 0.0) ? out[i] / den[i] : 0.0;
+    free(den);
+    return 0;
+}
+
 /* ---------------------------------------------------------------- read-back */
 
 int oracle_read_particles(const oracle_t *o, int field, double *out)

@@ -117,6 +117,8 @@ void oracle_cfl(oracle_t *o, double alpha);          /* l.13 */
 /* dt > 0: fixed step; dt <= 0: dt = alpha*h/(vmax+cmax) from the latest reduction (eq. 25/29) */
 int oracle_step(oracle_t *o, double dt, double alpha, int nsteps, double *dt_last);
 
+/* diagnostic nodal mean of rho (which 0) or E (which 1), reading A18: out[N_n] */
+int oracle_grid_diagnostic(const oracle_t *o, int which, double *out);
 int oracle_read_particles(const oracle_t *o, int field, double *out); /* [ncomp][n] */
 int oracle_read_grid(const oracle_t *o, int field, double *out);      /* [ncomp][N_n] */
 void oracle_get_stats(const oracle_t *o, oracle_stats *s);

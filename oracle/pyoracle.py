@@ -78,6 +78,7 @@ def _load():
     lib.oracle_step.argtypes = [vp, C.c_double, C.c_double, C.c_int, dp]
     lib.oracle_read_particles.argtypes = [vp, C.c_int, vp]
     lib.oracle_read_grid.argtypes = [vp, C.c_int, vp]
+    lib.oracle_grid_diagnostic.argtypes = [vp, C.c_int, vp]
     lib.oracle_get_stats.argtypes = [vp, C.POINTER(Stats)]
     _lib = lib
     return lib
@@ -225,6 +226,12 @@ class Oracle:
         rc = self._lib.oracle_read_grid(self._h, int(field), out.ctypes.data)
         assert rc == 0
         return out if nc > 1 else out[0]
+
+    def grid_diagnostic(self, which):
+        """mass-weighted nodal mean of rho (0) or E (1), reading A18"""
+        out = np.zeros(self.num_nodes)
+        assert self._lib.oracle_grid_diagnostic(self._h, int(which), out.ctypes.data) == 0
+        return out
 
     def stats(self):
         s = Stats()

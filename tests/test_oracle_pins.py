@@ -291,6 +291,26 @@ def test_viscosity_density_scaling_tells_the_two_forms_apart(po):
             assert np.abs(e2 - e1).max() > 1e-9 and np.abs(el2 - el1).max() > 1e-9
 
 
+@pytest.mark.parametrize("dim,periodic", [(2, True), (3, False)])
+def test_grid_diagnostic_density_and_energy(po, dim, periodic):
+    """Reading A18: rho_i = sum_k M rho phi_i / sum_k M phi_i, same for E, against the global hat
+    functions over all (particle, node) pairs; a uniform particle field is reproduced exactly wherever there is mass."""
+    n = [6, 5, 4][:dim]
+    cfg = _cfg(dim, n, 0.2, [[0, 0]] * dim if periodic else [[1, 1]] * dim)
+    o = po.Oracle(cfg)
+    rng = np.random.default_rng(17)
+    x, v, mass, rho, e, q = _random_particles(rng, dim, n, 0.2, 120)
+    o.load_particles(x, v, mass, rho, e, q)
+    phi, _ = _global_hats(o, cfg, x)
+    den = phi @ mass
+    for which, a in ((0, rho), (1, e)):
+        want = np.where(den > 0, (phi @ (mass * a)) / np.where(den > 0, den, 1.0), 0.0)
+        np.testing.assert_allclose(o.grid_diagnostic(which), want, rtol=1e-13, atol=1e-15)
+    o.load_particles(x, v, mass, np.full_like(rho, 1.7), e, q)
+    got = o.grid_diagnostic(0)
+    np.testing.assert_allclose(got[den > 0], 1.7, rtol=1e-14)
+
+
 # --------------------------------------------------------------------------- conservation
 
 def _periodic_box(po, dim, seed=3, N=600):
