@@ -94,8 +94,13 @@ enum { MPM_P_X = 1, MPM_P_V = 2, MPM_P_M = 4, MPM_P_RHO = 8, MPM_P_E = 16, MPM_P
  *   FORCE      f_i after BC/obstacle       after l.4   (dim)
  *   MOMENTUM2  second momentum P2G, after BC   l.9     (dim)
  *   NORMAL     obstacle normals n_i (static)           (dim)
- *   FLAG       1.0 at obstacle nodes, else 0 (static)  (1)  */
-enum { MPM_G_MASS = 0, MPM_G_MOMENTUM = 1, MPM_G_FORCE = 2, MPM_G_MOMENTUM2 = 3, MPM_G_NORMAL = 4, MPM_G_FLAG = 5 };
+ *   FLAG       1.0 at obstacle nodes, else 0 (static)  (1)
+ * diagnostics of the CURRENT particle state, computed on demand, off the hot path (reading A18; the density "interpolated
+ * on the grid" of Fig. 5), Q1 basis:
+ *   RHO_GRID   sum_k M_k rho_k phi_i(X_k) / sum_k M_k phi_i(X_k), 0 where the node has no mass   (1)
+ *   E_GRID     the same mass-weighted nodal mean of E                                            (1)  */
+enum { MPM_G_MASS = 0, MPM_G_MOMENTUM = 1, MPM_G_FORCE = 2, MPM_G_MOMENTUM2 = 3, MPM_G_NORMAL = 4, MPM_G_FLAG = 5,
+       MPM_G_RHO_GRID = 6, MPM_G_E_GRID = 7 };
 
 /* device allocator callbacks (e.g. torch's caching allocator).  `stream` is the cudaStream_t of the handle. */
 typedef void *(*mpm_alloc_fn)(size_t bytes, void *stream, void *user);
@@ -154,6 +159,7 @@ typedef struct mpm_stats {
     int64_t n_out_of_cell;    /* cumulative: particles a TILED kernel found outside their group's cell (debug counter of
                                  the exact-sort invariant; must be 0) */
     int64_t n_bad_dt;         /* cumulative: CFL steps with v_max + c_max = 0 or non-finite; such a step runs with dt = 0 */
+    int64_t n_left_slab;      /* cumulative: particles that ended a step beyond an MPM_BC_OPEN face (slab decomposition) */
 } mpm_stats;
 
 typedef struct mpm_handle mpm_handle;
@@ -198,6 +204,11 @@ MPM_API int mpm_step_phase(mpm_handle *h, int phase, double dt);
 enum { MPM_HALO_P2G1 = 0, MPM_HALO_P2G2 = 1 };
 enum { MPM_HALO_EXPORT = 0, MPM_HALO_ADD = 1 };
 MPM_API int mpm_halo(mpm_handle *h, int which, int side, int op, double *buf, int ptr_location);
+
+/* The scalars a slab driver needs after every step, without the reductions of mpm_get_stats: out[0] = v_max, out[1] = c_max of
+ * the last CFL reduction, out[2] = cumulative count of particles that ended a step beyond an MPM_BC_OPEN face, out[3] = t.
+ * out: HOST.  Synchronises the stream. */
+MPM_API int mpm_peek(mpm_handle *h, double out[4]);
 
 /* mpm_load_particles with two options.  ids (HOST or DEVICE like the other arrays; NULL = the load index): persistent
  * ids chosen by the caller, 0 <= id < 2^31 -- a slab passes the GLOBAL ids, which the recycling generator (reading A8) is

@@ -27,12 +27,12 @@ BASIS_Q1, BASIS_QUADRATIC = 0, 1
 P2G_RED, P2G_COLOUR_G2P, P2G_COLOUR_UPDATE, P2G_COLOUR_BOTH = 0, 1, 2, 3
 P_X, P_V, P_M, P_RHO, P_E, P_Q, P_ID = 1, 2, 4, 8, 16, 32, 64
 LOAD_KEEP_TIME = 1
-G_MASS, G_MOMENTUM, G_FORCE, G_MOMENTUM2, G_NORMAL, G_FLAG = 0, 1, 2, 3, 4, 5
+G_MASS, G_MOMENTUM, G_FORCE, G_MOMENTUM2, G_NORMAL, G_FLAG, G_RHO_GRID, G_E_GRID = 0, 1, 2, 3, 4, 5, 6, 7
 
 K_P2G1, K_NODE1, K_G2P_P2G2, K_NODE2, K_UPDATE, K_SORT, K_MISC = range(7)
 KERNEL_NAMES = ["p2g1", "node1", "g2p_p2g2", "node2", "update", "sort", "misc"]
 
-EXPORTS = ["mpm_step_phase", "mpm_halo", "mpm_load_particles_ex", "mpm_set_profiling", "mpm_abi_version", "mpm_create", "mpm_load_particles", "mpm_step", "mpm_read_particles",
+EXPORTS = ["mpm_peek", "mpm_step_phase", "mpm_halo", "mpm_load_particles_ex", "mpm_set_profiling", "mpm_abi_version", "mpm_create", "mpm_load_particles", "mpm_step", "mpm_read_particles",
            "mpm_read_grid", "mpm_get_stats", "mpm_last_error", "mpm_destroy"]
 
 ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p, C.c_void_p)
@@ -61,7 +61,7 @@ class Stats(C.Structure):
         ("sum_mass", C.c_double), ("sum_momentum", C.c_double * 3), ("sum_energy", C.c_double),
         ("num_particles", C.c_int64), ("num_nodes", C.c_int64), ("nn", C.c_int32 * 3), ("variant", C.c_int32),
         ("launches", C.c_int64), ("kernel_ms", C.c_double * 8), ("kernel_calls", C.c_int64 * 8),
-        ("n_cell_changes", C.c_int64), ("n_out_of_cell", C.c_int64), ("n_bad_dt", C.c_int64),
+        ("n_cell_changes", C.c_int64), ("n_out_of_cell", C.c_int64), ("n_bad_dt", C.c_int64), ("n_left_slab", C.c_int64),
     ]
 
 
@@ -84,6 +84,7 @@ def load_library():
     lib.mpm_step.argtypes = [vp, C.c_double, C.c_double, C.c_int32, C.POINTER(C.c_double)]
     lib.mpm_load_particles_ex.argtypes = [vp, C.c_int64, vp, vp, vp, vp, vp, vp, vp, C.c_int, C.c_int]
     lib.mpm_step_phase.argtypes = [vp, C.c_int, C.c_double]
+    lib.mpm_peek.argtypes = [vp, C.POINTER(C.c_double * 4)]
     lib.mpm_halo.argtypes = [vp, C.c_int, C.c_int, C.c_int, vp, C.c_int]
     lib.mpm_read_particles.argtypes = [vp, C.c_uint32, vp, C.c_int, C.c_int]
     lib.mpm_read_grid.argtypes = [vp, C.c_int, vp, C.c_int]
@@ -236,6 +237,12 @@ class Solver:
 
     def step_phase(self, phase, dt=0.0):
         self._check(self._lib.mpm_step_phase(self._h, int(phase), float(dt)))
+
+    def peek(self):
+        """(v_max, c_max, particles that left through OPEN faces so far, t) without the reductions of stats()"""
+        out = (C.c_double * 4)()
+        self._check(self._lib.mpm_peek(self._h, C.byref(out)))
+        return out[0], out[1], int(out[2]), out[3]
 
     def halo(self, which, side, op, buf, location=DEVICE):
         """buf: [channels, plane nodes] float64, contiguous (CUDA tensor for DEVICE, numpy / pinned tensor for HOST)."""

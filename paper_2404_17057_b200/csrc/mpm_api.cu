@@ -863,6 +863,17 @@ int mpm_step_phase(mpm_handle *h, int phase, double dt)
     return MPM_OK;
 }
 
+int mpm_peek(mpm_handle *h, double out[4])
+{
+    if (!h || !out) return MPM_E_ARG;
+    DeviceGuard guard(h->cfg.device);
+    DevScalars host;
+    MPM_CUDA(h, cudaMemcpyAsync(&host, h->sc, sizeof(host), cudaMemcpyDeviceToHost, h->stream));
+    MPM_CUDA(h, cudaStreamSynchronize(h->stream));
+    out[0] = host.vmax; out[1] = host.cmax; out[2] = (double)host.n_left_slab; out[3] = host.t;
+    return MPM_OK;
+}
+
 int mpm_halo(mpm_handle *h, int which, int side, int op, double *buf, int ptr_location)
 {
     if (!h || !buf) return MPM_E_ARG;
@@ -968,6 +979,24 @@ int mpm_read_grid(mpm_handle *h, int field, double *out, int ptr_location)
     const GridDesc &gd = h->gd;
     const size_t Nn = (size_t)gd.Nn;
     int rc = MPM_OK;
+    if (field == MPM_G_RHO_GRID || field == MPM_G_E_GRID) {      // diagnostics of the current particle state (A18), off the hot path
+        if (!h->pbuf[0].m) return fail(h, MPM_E_STATE, "mpm_read_grid: no particles loaded");
+        if (gd.quadratic) return fail(h, MPM_E_ARG, "mpm_read_grid: RHO_GRID / E_GRID are offered for the Q1 basis");
+        double *num = nullptr;
+        if (!dev_alloc_t(h, &num, 2 * Nn)) return fail(h, MPM_E_OOM, "mpm_read_grid: out of device memory");
+        MPM_CUDA(h, cudaMemsetAsync(num, 0, sizeof(double) * 2 * Nn, h->stream));
+        const PArr &p = h->pbuf[h->cur];
+        const bool tiled = h->variant == MPM_VARIANT_TILED;
+        launch_grid_diagnostic(gd, p, field == MPM_G_RHO_GRID ? p.rho : p.e, num, num + Nn, h->n,
+                               SortedMap{ tiled && h->n > 0 ? h->groups : nullptr, h->n_groups }, h->max_groups, h->stream);
+        h->launches += 2;
+        rc = copy_out(h, out, num, gd.Nn, ptr_location);
+        cudaError_t e = cudaStreamSynchronize(h->stream);
+        dev_free(h, num);
+        if (rc != MPM_OK) return rc;
+        MPM_CUDA(h, e);
+        return MPM_OK;
+    }
     // TILED: the last completed step used the accumulator set that is no longer current
     GArr gl = (h->variant == MPM_VARIANT_TILED) ? tiled_acc(h, h->steps_done > 0 ? h->acur ^ 1 : h->acur) : h->g;
     if (gd.acc32) {
@@ -1049,7 +1078,7 @@ int mpm_get_stats(mpm_handle *h, mpm_stats *out)
     out->n_recycled = (int64_t)host.n_recycled; out->n_clamped = (int64_t)host.n_clamped;
     out->n_negjac = (int64_t)host.n_negjac; out->n_nonfinite = (int64_t)host.n_nonfinite;
     out->n_cell_changes = (int64_t)host.n_cell_changes; out->n_out_of_cell = (int64_t)host.n_out_of_cell;
-    out->n_bad_dt = (int64_t)host.n_bad_dt;
+    out->n_bad_dt = (int64_t)host.n_bad_dt; out->n_left_slab = (int64_t)host.n_left_slab;
     out->sum_mass = host.sum_mass; out->sum_energy = host.sum_energy;
     for (int a = 0; a < 3; ++a) { out->sum_momentum[a] = host.sum_mom[a]; out->nn[a] = h->gd.nn[a]; }
     out->num_particles = h->n; out->num_nodes = h->gd.Nn;

@@ -175,6 +175,7 @@ struct DevScalars {
     // kernel (must stay 0: the TILED family's weights rely on the exact sort), steps whose CFL dt was not a positive
     // finite number (v_max + c_max = 0 or non-finite: dt := 0 for that step)
     unsigned long long n_cell_changes, n_out_of_cell, n_bad_dt;
+    unsigned long long n_left_slab;   // cumulative: particles that ended a step beyond an MPM_BC_OPEN face (to be handed over)
     double sum_mass, sum_mom[3], sum_energy;   // filled by the stats reduction on demand
 };
 
@@ -307,6 +308,11 @@ void launch_gather_by_id_groups(const double *src, const int *id, double *dst, c
                                 const int *coff, const int *off, cudaStream_t s);
 void launch_stats_reduce_groups(const GridDesc &gd, const PArr &p, DevScalars *sc, const SortedMap &map, long long max_groups,
                                 cudaStream_t s);
+
+// diagnostics (mpm_read_grid RHO_GRID / E_GRID, reading A18): num[i] = sum_k M a phi_i, den[i] = sum_k M phi_i with a = rho or E,
+// then num[i] = num[i] / den[i] (0 where den = 0).  num, den: zeroed by the caller.  map.groups == NULL: particles 0 .. n-1.
+void launch_grid_diagnostic(const GridDesc &gd, const PArr &p, const double *field, double *num, double *den, long long n,
+                            const SortedMap &map, long long max_groups, cudaStream_t s);
 
 // node kernels -- mpm_kernels_grid.cu
 void launch_grid_clear(const GridDesc &gd, const GArr &g, cudaStream_t s);

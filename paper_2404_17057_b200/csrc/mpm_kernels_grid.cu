@@ -170,9 +170,60 @@ __global__ void k_stats_clear(DevScalars *sc)
     sc->sum_mom[0] = sc->sum_mom[1] = sc->sum_mom[2] = 0.0;
 }
 
+// diagnostics, off the hot path: one thread per particle (ATOMIC layout) or per group record (TILED layout)
+template <int DIM>
+__device__ __forceinline__ void diag_scatter(const GridDesc &gd, const PArr &p, const double *field, double *num, double *den, long long k)
+{
+    double X[DIM], xi[DIM];
+    int c[DIM];
+#pragma unroll
+    for (int a = 0; a < DIM; ++a) X[a] = p.x[a][k];
+    particle_cell<DIM>(gd, X, c, xi);
+    const double M = p.m[k], a = field[k];
+#pragma unroll
+    for (int ib = 0; ib < (1 << DIM); ++ib) {
+        const long long i = corner_node<DIM>(gd, c, ib);
+        const double phi = corner_phi<DIM>(xi, ib);
+        atomicAdd(&num[i], M * a * phi);
+        atomicAdd(&den[i], M * phi);
+    }
+}
+template <int DIM>
+__global__ void __launch_bounds__(kBlock) k_grid_diagnostic(GridDesc gd, PArr p, const double *field, double *num, double *den,
+                                                            long long n, SortedMap map)
+{
+    if (map.groups) {
+        const int n_groups = *map.n_groups;
+        for (long long gq = (long long)blockIdx.x * kBlock + threadIdx.x; gq < n_groups; gq += (long long)gridDim.x * kBlock) {
+            const int4 r = map.groups[gq];
+            for (int j = 0; j < (r.y & 0xff); ++j) diag_scatter<DIM>(gd, p, field, num, den, (long long)r.x + j);
+        }
+    } else {
+        for (long long k = (long long)blockIdx.x * kBlock + threadIdx.x; k < n; k += (long long)gridDim.x * kBlock)
+            diag_scatter<DIM>(gd, p, field, num, den, k);
+    }
+}
+__global__ void __launch_bounds__(kBlock) k_safe_quotient(double *num, const double *den, long long n)
+{
+    for (long long i = (long long)blockIdx.x * kBlock + threadIdx.x; i < n; i += (long long)gridDim.x * kBlock)
+        num[i] = (den[i] != 0.0) ? num[i] / den[i] : 0.0;
+}
+
 inline unsigned grid_for(long long n) { return (unsigned)((n + kBlock - 1) / kBlock); }
 
 }  // namespace
+
+void launch_grid_diagnostic(const GridDesc &gd, const PArr &p, const double *field, double *num, double *den, long long n,
+                            const SortedMap &map, long long max_groups, cudaStream_t s)
+{
+    const long long work = map.groups ? max_groups : n;
+    if (work > 0) {
+        const unsigned blocks = (unsigned)((work + kBlock - 1) / kBlock < 148 * 16 ? (work + kBlock - 1) / kBlock : 148 * 16);
+        if (gd.dim == 2) k_grid_diagnostic<2><<<blocks, kBlock, 0, s>>>(gd, p, field, num, den, n, map);
+        else k_grid_diagnostic<3><<<blocks, kBlock, 0, s>>>(gd, p, field, num, den, n, map);
+    }
+    k_safe_quotient<<<148 * 4, kBlock, 0, s>>>(num, den, gd.Nn);
+}
 
 void launch_grid_clear(const GridDesc &gd, const GArr &g, cudaStream_t s)
 {

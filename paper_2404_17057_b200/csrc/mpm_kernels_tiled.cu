@@ -616,7 +616,7 @@ __device__ __forceinline__ void coop_p2g1(const GridDesc &gd, const GArr &gn, un
 // The particle fields of the NEXT pass are copied into shared memory while the current pass computes (see "particle
 // streams" above).  V' overwrites V in place.
 template <int DIM, bool ACC32, bool BULK, bool COLOUR, bool CM>
-__global__ void __launch_bounds__(kTB, DIM == 2 ? kTBMinG2 : kTBMinG) k_g2p_p2g2_tiled(GridDesc gd, PArr p, GArr g,
+__global__ void __launch_bounds__(kTB, (DIM == 2 && !COLOUR) ? kTBMinG2 : kTBMinG) k_g2p_p2g2_tiled(GridDesc gd, PArr p, GArr g,
                                                                 const DevScalars *__restrict__ sc, SortedMap map,
                                                                 const int4 *__restrict__ items, const int *__restrict__ n_items,
                                                                 int *__restrict__ count, unsigned long long *__restrict__ dest,
@@ -965,6 +965,7 @@ __global__ void __launch_bounds__(kTB, COLOUR ? 3 : DIM == 2 ? kTBMinU2 : kTBMin
     // per-thread event counters of the block's <= 16 passes x 2 particles, packed into one register: recycled (bits 0-5),
     // clamped coordinates (6-12, <= 3 per particle), 1 + dt D <= 0 (13-18), non-finite (19-24), out of cell (25-30)
     unsigned events = 0u;
+    int n_left = 0;      // particles that ended beyond an OPEN face (slab interfaces only)
     static_assert(Chunk<DIM>::PASSES * 2 <= 32, "event counters are 6 bits wide");
     const double gm1 = gd.gamma - 1.0;
     unsigned parity = 0;
@@ -1016,15 +1017,15 @@ __global__ void __launch_bounds__(kTB, COLOUR ? 3 : DIM == 2 ? kTBMinU2 : kTBMin
 #pragma unroll
         for (int a = 0; a < DIM; ++a) {
             const double2 tv = *reinterpret_cast<const double2 *>(&s_pf[warp][DIM + a][o]);
-            V[0][a] = valid[0] ? tv.x : 0.0; V[1][a] = valid[1] ? tv.y : 0.0;
+            V[0][a] = tv.x; V[1][a] = tv.y;      // an unused slot computes on whatever it holds: masked where it could be seen
         }
         {
             const double2 tm = gd.uniform_mass ? make_double2(gd.um, gd.um) : *reinterpret_cast<const double2 *>(&s_pf[warp][2 * DIM][o]);
             const double2 tr = *reinterpret_cast<const double2 *>(&s_pf[warp][2 * DIM + 1][o]),
                           te = *reinterpret_cast<const double2 *>(&s_pf[warp][2 * DIM + 2][o]);
             M[0] = valid[0] ? tm.x : 0.0; M[1] = valid[1] ? tm.y : 0.0;
-            rho[0] = valid[0] ? tr.x : 1.0; rho[1] = valid[1] ? tr.y : 1.0;
-            E[0] = valid[0] ? te.x : 0.0; E[1] = valid[1] ? te.y : 0.0;
+            rho[0] = tr.x; rho[1] = tr.y;
+            E[0] = te.x; E[1] = te.y;
             const int2 ti = *reinterpret_cast<const int2 *>(&s_id[warp][o]);
             id[0] = ti.x; id[1] = ti.y;
         }
@@ -1032,8 +1033,9 @@ __global__ void __launch_bounds__(kTB, COLOUR ? 3 : DIM == 2 ? kTBMinU2 : kTBMin
         issue_rest(nxt, w0n, wnn);
         const Group nn = fetch_group(map.groups, (long long)item.y + gl + 2 * GPB, g_end);
         // per particle: the new state (what goes to memory), S' for the next step's force, and whether it stays in the
-        // group's cell.  Straight-line code for both particles of the lane (an unused slot computes on M = 0, rho = 1,
-        // E = 0, X = 0 and is masked where it could be seen: counters, maxima, stores, scatter payloads).
+        // group's cell.  Straight-line code for both particles of the lane (an unused slot computes on M = 0, X = 0 and
+        // whatever V, rho, E its slot holds -- possibly NaN -- and is masked by SELECTS, never by a multiplication with 0,
+        // wherever it could be seen: counters, maxima, stores, scatter payloads).
         double Xo[2][DIM], Vo[2][DIM], Mo[2], Ro[2], Eo[2], Qo[2], Sn[2];
         bool stay[2];
 #pragma unroll
@@ -1071,8 +1073,10 @@ __global__ void __launch_bounds__(kTB, COLOUR ? 3 : DIM == 2 ? kTBMinU2 : kTBMin
             if (!move_inside<DIM>(gd, X[i], out[i], dt, Xo[i]) && valid[i]) {      // next to a domain face (rare)
                 bool recycled;
                 int nclamp;
-                move_particle<DIM>(gd, X[i], out[i], dt, (long long)id[i], step, Xo[i], recycled, nclamp);
+                bool left = false;
+                move_particle<DIM>(gd, X[i], out[i], dt, (long long)id[i], step, Xo[i], recycled, nclamp, &left);
                 events += (unsigned)nclamp << 6;
+                n_left += (int)left;
                 if (recycled) {
 #pragma unroll
                     for (int a = 0; a < DIM; ++a) Vo[i][a] = gd.inflow_v[a];
@@ -1187,6 +1191,10 @@ __global__ void __launch_bounds__(kTB, COLOUR ? 3 : DIM == 2 ? kTBMinU2 : kTBMin
         if (nf_sum) atomicAdd(&sc->n_nonfinite, (unsigned long long)nf_sum);
         if (clamp_sum) atomicAdd(&sc->n_clamped, (unsigned long long)clamp_sum);
         if (ooc_sum) atomicAdd(&sc->n_out_of_cell, (unsigned long long)ooc_sum);
+    }
+    if (gd.has_open) {
+        const int left_sum = __reduce_add_sync(kFull, n_left);
+        if (lane == 0 && left_sum) atomicAdd(&sc->n_left_slab, (unsigned long long)left_sum);
     }
     __syncthreads();
     if (threadIdx.x == 0) {

@@ -205,7 +205,8 @@ __device__ __forceinline__ void slow_p2g2(const GridDesc &gd, const GArr &g, con
 // explicit (fma / __dmul_rn / __dsub_rn), so that both kernels get the same X' bit for bit from the same inputs.
 template <int DIM>
 __device__ __forceinline__ void move_particle(const GridDesc &gd, const double X[DIM], const double Vb[DIM], double dt,
-                                              long long id, long long step, double Xn[DIM], bool &recycled, int &nclamp)
+                                              long long id, long long step, double Xn[DIM], bool &recycled, int &nclamp,
+                                              bool *left_slab = nullptr)
 {
     bool recycle = false;
 #pragma unroll
@@ -246,8 +247,11 @@ __device__ __forceinline__ void move_particle(const GridDesc &gd, const double X
 #pragma unroll
     for (int a = 0; a < DIM; ++a) {
         if (!gd.per[a]) {      // an OPEN face is an interface to the neighbouring slab: the particle leaves, unclamped
-            if (Xn[a] < 0.0 && gd.bc[a][0] != MPM_BC_OPEN) { Xn[a] = 0.0; nclamp++; }
-            if (Xn[a] > gd.L[a] && gd.bc[a][1] != MPM_BC_OPEN) { Xn[a] = gd.L[a]; nclamp++; }
+            if (Xn[a] < 0.0) { if (gd.bc[a][0] != MPM_BC_OPEN) { Xn[a] = 0.0; nclamp++; } else if (left_slab) *left_slab = true; }
+            if (Xn[a] >= gd.L[a]) {
+                if (gd.bc[a][1] == MPM_BC_OPEN) { if (left_slab) *left_slab = true; }
+                else if (Xn[a] > gd.L[a]) { Xn[a] = gd.L[a]; nclamp++; }
+            }
         }
     }
 }

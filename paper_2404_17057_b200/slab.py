@@ -10,7 +10,7 @@ neighbouring slabs share exactly one node plane.  One time step:
     3. halo SUM-exchange of the shared plane's mv2                                  (l.8 is complete)
     4. UPDATE phase: l.9-13
     5. all-reduce(max) of v_max and c_max -> the next global dt = alpha h / (v_max + c_max)   (eq. 25/29)
-    6. particles that left their slab (<= 1 cell per step by the CFL condition; anywhere for a recycled
+    6. if any particle anywhere left its slab (a device-side counter, all-reduced with the maxima): particles that left their slab (<= 1 cell per step by the CFL condition; anywhere for a recycled
        particle) are handed to the slab that now contains them; every slab replaces its particle set, which re-orders it
        and redoes the first P2G of the next step (mpm_load_particles_ex with MPM_LOAD_KEEP_TIME and the global ids, on
        which the recycling generator of reading A8 is keyed).
@@ -182,8 +182,9 @@ class CudaSlabEngine:
         self.solver.step_phase(self.mpm.PHASE_UPDATE)
 
     def maxima(self):
-        st = self.solver.stats()
-        return st.vmax, st.cmax
+        """(v_max, c_max, cumulative number of particles that ended a step beyond an interface)"""
+        vmax, cmax, left, _ = self.solver.peek()
+        return vmax, cmax, left
 
     def stats(self):
         return self.solver.stats()
@@ -218,6 +219,7 @@ class SlabDomain:
         self.vmax = self.cmax = 0.0
         self.t, self.step_count, self.dt_last = 0.0, 0, 0.0
         self.n_migrated = 0
+        self._left_seen = {}
         # interfaces (lower slab, upper slab): the lower one's HIGH plane is the upper one's LOW plane
         self.interfaces = [(s, s + 1) for s in range(num_slabs - 1)]
         if self.periodic and num_slabs > 1:
@@ -254,11 +256,16 @@ class SlabDomain:
         self._reduce_maxima()
 
     def _reduce_maxima(self):
+        """global CFL maxima (eq. 25/29); returns whether any particle, anywhere, left its slab since the last hand-over"""
         vm = cm = 0.0
+        left = 0
         for s in self.local:
-            v, c = self.engines[s].maxima()
+            v, c, l = self.engines[s].maxima()
             vm, cm = max(vm, v), max(cm, c)
-        self.vmax, self.cmax = self.transport.allreduce_max([vm, cm])
+            left += l - self._left_seen.get(s, 0)
+            self._left_seen[s] = l
+        self.vmax, self.cmax, any_left = self.transport.allreduce_max([vm, cm, float(left > 0)])
+        return any_left > 0.0
 
     # -- halo SUM-exchange of the shared node planes; which = 0: m, mv, f of the first P2G, 1: mv2 of the second
     def _halo_exchange(self, which):
@@ -328,8 +335,8 @@ class SlabDomain:
             self._halo_exchange(1)
             for s in self.local:
                 self.engines[s].phase_update()
-            self._reduce_maxima()
-            self._migrate()
+            if self._reduce_maxima():      # nobody crossed an interface: the fused re-ordering and P2G#1 stand, nothing to do
+                self._migrate()
             self.t += step_dt
             self.dt_last = step_dt
             self.step_count += 1

@@ -536,6 +536,20 @@ def test_cold_gas_at_rest_has_no_cfl_step(mpm, variant):
     assert h.step(1e-3, 0.3, 3) == 1e-3 and h.stats().n_bad_dt == 0
 
 
+@pytest.mark.parametrize("mode", MODES)
+@pytest.mark.parametrize("name", ["sod", "cylinder", "clumps_dense"])
+def test_grid_diagnostics_match_oracle(po, mpm, name, mode):
+    """mpm_read_grid(MPM_G_RHO_GRID / MPM_G_E_GRID): the mass-weighted nodal means of rho and E (reading A18, the density
+    'interpolated on the grid' of Fig. 5) of the state after 5 steps against the oracle's, node by node."""
+    w = small_workloads()[name]()
+    o, g = _make(po, mpm, w, mode[0], mode[1])
+    o.step(0.0, w["cfl"], 5)
+    g.step(0.0, w["cfl"], 5)
+    for which, field in ((0, mpm.G_RHO_GRID), (1, mpm.G_E_GRID)):
+        a, b = o.grid_diagnostic(which), g.read_grid(field)
+        assert np.abs(a - b).max() <= 1e-11 * np.abs(a).max(), (name, which, np.abs(a - b).max())
+
+
 def test_checked_build(mpm):
     """Memory-safety evidence without compute-sanitizer (closed on the GPU pool): the same sources compiled with
     -DMPM_CHECKED=1 test every particle slot, node index, cell key, window offset, group and item record against its bound
