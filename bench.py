@@ -286,7 +286,7 @@ def run_ours(args):
         n_p = int(w["mass"].shape[0])
         g = mpm.Solver(w["cfg"], sort_every=1, variant=variant, device=local, grid_accum=accum,
                        particle_stream=mpm.STREAM_BULK if args.stream == "bulk" else mpm.STREAM_CP_ASYNC,
-                       p2g_mode=args.p2g_mode)
+                       p2g_mode=args.p2g_mode, particle_ids=mpm.IDS_NONE if args.particle_ids == "none" else mpm.IDS_TRACK)
         n_n = g.num_nodes
         g.load_particles(w["x"], w["v"], w["mass"], w["rho"], w["e"])
         g.step(0.0, w["cfl"], warmup, sync=False)
@@ -344,6 +344,7 @@ def run_ours(args):
         "config": {"workload": w["name"], "grid_accum": args.grid_accum, "particles_per_gpu": n_p, "nodes": n_n, "dim": dim,
                    "kernel_family": args.variant, "particle_stream": args.stream, "p2g_mode": args.p2g_mode, "parallelism": f"replicas x{world}",
                    "l2": "inputs (%.1f GB particle state) exceed the 126 MB L2; no flush" % (n_p * (2 * dim + 5) * 8 / 1e9),
+                   "particle_ids": "tracked" if g.ids_tracked else "none (Algorithm 1 has no ids; read-back in storage order)",
                    "movers_per_step": r["movers"],
                    "window": "steps %d-%d after the load" % (args.warmup + 1, args.warmup + args.steps)},
         "clocks": r["clocks"], "gpu_launches": r["launches"], "roofline": roofline, "step_roofline": r["step_roofline"],
@@ -420,6 +421,9 @@ def main():
     ap.add_argument("--p2g-mode", type=int, default=0, choices=[0, 1, 2, 3],
                     help="0 = global reductions (default); bit 0 / bit 1: atomics-free shared-memory accumulation by cell "
                          "colour in the gather / update kernel (include/mpm.h MPM_P2G_*)")
+    ap.add_argument("--particle-ids", default="none", choices=["none", "track"],
+                    help="none (default): the sweeps carry no persistent particle ids (mpm.h MPM_IDS_NONE; grids with an inflow "
+                         "face keep them regardless); track: 4 more bytes read and written per particle and step")
     ap.add_argument("--decompose", action="store_true",
                     help="N > 1 (or --slabs > 1): ONE problem cut into slabs over the GPUs (strong scaling) instead of replicas")
     ap.add_argument("--slabs", type=int, default=0, help="with --decompose: number of slabs (default: one per GPU)")

@@ -32,7 +32,8 @@
 extern "C" {
 #endif
 
-#define MPM_ABI_VERSION 2   /* 2: mpm_stats grew three counters, mpm_config two fields; the SORTED kernel family was retired */
+#define MPM_ABI_VERSION 3   /* 2: mpm_stats grew three counters, mpm_config two fields; the SORTED kernel family was retired.
+                             * 3: mpm_config.reserved3 became particle_ids (same size and layout; 0 keeps the old behaviour) */
 
 #if defined(__GNUC__)
 #define MPM_API __attribute__((visibility("default")))
@@ -84,6 +85,13 @@ enum { MPM_P2G_RED = 0, MPM_P2G_COLOUR_G2P = 1, MPM_P2G_COLOUR_UPDATE = 2, MPM_P
  * on the nodes, 3^dim nodes per particle; all axes must be PERIODIC with at least 3 cells (the paper gives no wall
  * treatment for a spline whose support leaves the grid) and the kernel family is ATOMIC (any sort_every). */
 enum { MPM_BASIS_Q1 = 0, MPM_BASIS_QUADRATIC = 1 };
+/* persistent particle ids (= load index, or the caller's with mpm_load_particles_ex).  Algorithm 1 has none: they exist so
+ * that mpm_read_particles can return the particles in load order although l.12 re-orders them, and the recycling generator
+ * (reading A8) is keyed on them.  TRACK (default): they travel with the particles (4 bytes read and written per particle and
+ * step).  NONE: not kept -- mpm_read_particles then offers storage order only (order = 1) and no MPM_P_ID, and
+ * mpm_load_particles_ex takes no ids.  Honoured by the TILED family on grids without an INFLOW face; ignored (ids are kept)
+ * otherwise. */
+enum { MPM_IDS_TRACK = 0, MPM_IDS_NONE = 1 };
 /* particle fields (bit mask for mpm_read_particles; output pointers are consumed in this order, a vector field
  * takes `dim` pointers) */
 enum { MPM_P_X = 1, MPM_P_V = 2, MPM_P_M = 4, MPM_P_RHO = 8, MPM_P_E = 16, MPM_P_Q = 32,
@@ -133,7 +141,7 @@ typedef struct mpm_config {
     int32_t basis;            /* MPM_BASIS_* (ABI version 2) */
     int32_t slab_global_n;    /* > 0: this grid is one slab of a domain with slab_global_n cells along the LAST axis ... */
     int32_t slab_offset;      /* ... and starts at that cell of it (recycled particles are placed on the global inflow face) */
-    int32_t reserved3;        /* must be 0 */
+    int32_t particle_ids;     /* MPM_IDS_* (ABI version 3; this field was `reserved3`, 0, before) */
 } mpm_config;
 
 /* kernel classes for the optional per-kernel timers (mpm_set_profiling) */

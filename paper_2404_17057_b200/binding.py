@@ -24,6 +24,7 @@ VARIANT_AUTO, VARIANT_ATOMIC, VARIANT_SORTED_RETIRED, VARIANT_TILED = 0, 1, 2, 3
 ACCUM_FP64, ACCUM_FP32 = 0, 1
 STREAM_CP_ASYNC, STREAM_BULK = 0, 1
 BASIS_Q1, BASIS_QUADRATIC = 0, 1
+IDS_TRACK, IDS_NONE = 0, 1
 P2G_RED, P2G_COLOUR_G2P, P2G_COLOUR_UPDATE, P2G_COLOUR_BOTH = 0, 1, 2, 3
 P_X, P_V, P_M, P_RHO, P_E, P_Q, P_ID = 1, 2, 4, 8, 16, 32, 64
 LOAD_KEEP_TIME = 1
@@ -49,7 +50,7 @@ class Config(C.Structure):
         ("sort_every", C.c_int32), ("variant", C.c_int32), ("device", C.c_int32), ("grid_accum", C.c_int32),
         ("particle_stream", C.c_int32), ("p2g_mode", C.c_int32),
         ("stream", C.c_void_p), ("alloc", ALLOC_FN), ("free", FREE_FN), ("alloc_user", C.c_void_p),
-        ("basis", C.c_int32), ("slab_global_n", C.c_int32), ("slab_offset", C.c_int32), ("reserved3", C.c_int32),
+        ("basis", C.c_int32), ("slab_global_n", C.c_int32), ("slab_offset", C.c_int32), ("particle_ids", C.c_int32),
     ]
 
 
@@ -115,10 +116,10 @@ class MpmError(RuntimeError):
 
 class Solver:
     """mpm_handle wrapper.  `cfg` is the dict of inputs.py workloads (`w["cfg"]`); extra keyword arguments
-    (sort_every, variant, device, grid_accum, particle_stream) select the execution options of mpm_config."""
+    (sort_every, variant, device, grid_accum, particle_stream, p2g_mode, particle_ids) select the execution options of mpm_config."""
 
     def __init__(self, cfg, sort_every=0, variant=VARIANT_AUTO, device=0, use_torch_allocator=True, grid_accum=0,
-                 particle_stream=STREAM_CP_ASYNC, p2g_mode=P2G_RED):
+                 particle_stream=STREAM_CP_ASYNC, p2g_mode=P2G_RED, particle_ids=IDS_TRACK):
         import torch
         self._lib = load()
         self._torch = torch
@@ -156,6 +157,7 @@ class Solver:
         c.grid_accum = int(grid_accum)
         c.particle_stream = int(particle_stream)
         c.p2g_mode = int(p2g_mode)
+        c.particle_ids = int(particle_ids)
         c.basis = int(cfg.get("basis", BASIS_Q1))
         c.slab_global_n = int(cfg.get("slab_global_n", 0)); c.slab_offset = int(cfg.get("slab_offset", 0))
         with torch.cuda.device(self.device):
@@ -186,6 +188,9 @@ class Solver:
         st = self.stats()
         self.num_nodes = int(st.num_nodes)
         self.nn = tuple(int(v) for v in st.nn)
+        # mpm.h MPM_IDS_NONE: honoured by the TILED family on grids without an INFLOW face
+        inflow = any(int(c.bc[a][sd]) == BC_INFLOW for a in range(self.dim) for sd in range(2))
+        self.ids_tracked = not (int(particle_ids) == IDS_NONE and int(st.variant) == VARIANT_TILED and not inflow)
 
     # ------------------------------------------------------------------ plumbing
     def _check(self, rc):
@@ -256,9 +261,12 @@ class Solver:
         self._check(self._lib.mpm_step(self._h, float(dt), float(cfl), int(nsteps), None))
         return None
 
-    def read_particles(self, mask=P_X | P_V | P_M | P_RHO | P_E | P_Q, order=0, out=None, location=HOST):
+    def read_particles(self, mask=P_X | P_V | P_M | P_RHO | P_E | P_Q, order=None, out=None, location=HOST):
         """Returns a dict name -> array ([dim, N] for X and V).  `out` may supply preallocated buffers
-        (numpy / pinned torch for HOST, CUDA tensors for DEVICE) under the same names."""
+        (numpy / pinned torch for HOST, CUDA tensors for DEVICE) under the same names.  order: 0 = load order (by
+        persistent id), 1 = storage order; default 0, or 1 for a solver created with IDS_NONE."""
+        if order is None:
+            order = 0 if self.ids_tracked else 1
         d, n = self.dim, self.n
         names = [("x", P_X, d), ("v", P_V, d), ("mass", P_M, 1), ("rho", P_RHO, 1), ("e", P_E, 1), ("q", P_Q, 1), ("id", P_ID, 1)]
         res, ptrs = {}, []

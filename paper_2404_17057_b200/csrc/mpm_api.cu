@@ -49,7 +49,8 @@ struct mpm_handle {
     // TILED with fp32 accumulators: fp64 copies of the last step's m, mv, f, mv2 for mpm_read_grid (allocated on first use)
     double *rg_m, *rg_mv[3], *rg_f[3], *rg_mv2[3];
     long long max_items;
-    unsigned long long *dest;
+    unsigned long long *dest;   // TILED: destination records of l.12, one 32-bit rank per slot (8 bytes per slot are allocated:
+                                // mpm_load_particles_ex stages the caller's 64-bit ids here)
     long long max_groups;
     DevScalars *sc;
     long long launches;
@@ -366,7 +367,7 @@ void step_tiled_gather(mpm_handle *h)
     // l.4-5 and l.9 (BC, obstacle, mv' = mv + dt f, the quotients by m) have no kernel of their own: the two particle
     // kernels evaluate them per tile node while staging the tile (stage_tile)
     { Timed t(h, MPM_K_G2P_P2G2);
-      launch_g2p_p2g2_tiled(gd, p, gc, h->sc, map, h->items, h->n_items, h->max_items, h->count, h->dest, s); }          // l.4-8
+      launch_g2p_p2g2_tiled(gd, p, gc, h->sc, map, h->items, h->n_items, h->max_items, h->count, reinterpret_cast<unsigned *>(h->dest), s); }          // l.4-8
     h->launches += 2;      // kernels only (begin_step, gather); the memsets are not counted
 }
 
@@ -383,7 +384,7 @@ void step_tiled_update(mpm_handle *h, bool last_of_call)
       launch_cell_map_tiled(gd, h->count, h->off[0], h->groups_alt, h->n_groups_alt, h->items_alt, h->n_items_alt, h->map_state, s); }
     cudaStreamWaitEvent(s, h->ev_join, 0);
     { Timed t(h, MPM_K_UPDATE);
-      launch_update_tiled(gd, p, q, gc, h->sc, map, h->items, h->n_items, h->max_items, h->off[0], h->dest, gnx, last_of_call, s); }   // l.9-12, next l.3
+      launch_update_tiled(gd, p, q, gc, h->sc, map, h->items, h->n_items, h->max_items, h->off[0], reinterpret_cast<const unsigned *>(h->dest), gnx, last_of_call, s); }   // l.9-12, next l.3
     { Timed t(h, MPM_K_MISC); launch_end_step(h->sc, gd.h, s); }                                                   // l.13-14
     { int4 *t4 = h->groups; h->groups = h->groups_alt; h->groups_alt = t4; t4 = h->items; h->items = h->items_alt; h->items_alt = t4;
       int *t1 = h->n_groups; h->n_groups = h->n_groups_alt; h->n_groups_alt = t1; t1 = h->n_items; h->n_items = h->n_items_alt; h->n_items_alt = t1; }
@@ -537,15 +538,22 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
         discard(h);
         return fail(nullptr, MPM_E_ARG, "mpm_create: p2g_mode MPM_P2G_COLOUR_* needs the TILED family, fp64 accumulation and the cp.async stream");
     }
-    if (cfg->basis != MPM_BASIS_Q1 || cfg->reserved3 != 0) {
-        bool ok = cfg->basis == MPM_BASIS_QUADRATIC && cfg->reserved3 == 0 && !tiled && !cfg->obstacle_mask;
+    if (cfg->particle_ids != MPM_IDS_TRACK && cfg->particle_ids != MPM_IDS_NONE) {
+        discard(h);
+        return fail(nullptr, MPM_E_ARG, "mpm_create: particle_ids must be MPM_IDS_TRACK or MPM_IDS_NONE");
+    }
+    if (cfg->basis != MPM_BASIS_Q1) {
+        bool ok = cfg->basis == MPM_BASIS_QUADRATIC && !tiled && !cfg->obstacle_mask;
         for (int a = 0; a < gd.dim; ++a) ok = ok && gd.per[a] && gd.nc[a] >= 3;
         if (!ok) {
             discard(h);
-            return fail(nullptr, MPM_E_ARG, "mpm_create: MPM_BASIS_QUADRATIC needs the ATOMIC family and a fully periodic grid of >= 3 cells per axis without obstacle; reserved3 must be 0");
+            return fail(nullptr, MPM_E_ARG, "mpm_create: MPM_BASIS_QUADRATIC needs the ATOMIC family and a fully periodic grid of >= 3 cells per axis without obstacle");
         }
     }
     gd.quadratic = cfg->basis == MPM_BASIS_QUADRATIC ? 1 : 0;
+    // persistent ids: dropped on request by the TILED family when nothing on the device needs them (the recycling generator of
+    // an INFLOW face is keyed on them, reading A8)
+    gd.track_ids = (cfg->particle_ids == MPM_IDS_NONE && tiled && gd.in_axis < 0) ? 0 : 1;
     if (cfg->slab_global_n < 0 || cfg->slab_offset < 0 ||
         (cfg->slab_global_n > 0 && cfg->slab_offset + gd.nc[gd.dim - 1] > cfg->slab_global_n)) {
         discard(h);
@@ -744,6 +752,7 @@ int load_impl(mpm_handle *h, int64_t n, const double *const *x, const double *co
         if (!probe.differs && inflow_ok) { h->gd.uniform_mass = 1; h->gd.um = probe.first; }
         h->launches += 1;
     }
+    if (ids && !h->gd.track_ids) return fail(h, MPM_E_ARG, "mpm_load_particles_ex: created with MPM_IDS_NONE: no caller-chosen ids");
     h->external_ids = ids != nullptr;
     if (ids && n > 0) {      // caller-chosen persistent ids: staged in the (free) destination-record array, narrowed to 32 bits
         if (!h->dest) return fail(h, MPM_E_STATE, "mpm_load_particles_ex: caller-chosen ids are offered by the TILED family");
@@ -932,6 +941,8 @@ int mpm_read_particles(mpm_handle *h, uint32_t field_mask, double *const *out, i
     if (field_mask & MPM_P_Q) { src.push_back(p.q); tmp.push_back(scratch.q); }
     if (h->external_ids && order == 0)
         return fail(h, MPM_E_STATE, "mpm_read_particles: caller-chosen ids: read in storage order (order = 1) with MPM_P_ID");
+    if (!h->gd.track_ids && (order == 0 || (field_mask & MPM_P_ID)))
+        return fail(h, MPM_E_STATE, "mpm_read_particles: created with MPM_IDS_NONE: storage order (order = 1) only, no MPM_P_ID");
     if (field_mask & MPM_P_ID) {      // ids widened to fp64 in a scratch pair of their own (allocated on first use)
         const size_t N = (size_t)(h->slots > 0 ? h->slots : 1);
         if (h->id_wide_slots < (long long)N) {

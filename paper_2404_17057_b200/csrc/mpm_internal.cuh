@@ -63,6 +63,9 @@ struct GridDesc {
     int colour_major;   // layout of the cell numbering inside a tile (TileGeo): 1 when p2g_mode != 0
     // TILED: allocated slots per particle array and capacities of the group / item lists (bounds of the checked build)
     long long slots, max_groups, max_items;
+    // TILED: the persistent particle ids travel with the particles (mpm_config.particle_ids; always with an INFLOW face, whose
+    // recycling generator is keyed on them, reading A8).  0: the sweeps neither read nor write the id arrays
+    int track_ids;
 };
 
 // TILED family: the grid is cut into tiles of T0 x T1 (x T2) cells; the cell key is (tile index, cell inside the
@@ -115,13 +118,31 @@ struct TileGeo {
     }
 };
 
+// Order of the tiles = order of their particles in memory = order in which the blocks of the tile kernels are scheduled:
+// x fastest over the whole grid.  (Measured in round 2, profiles/r02_experiments.md section 5: numbering the tiles in compact
+// super-tiles of 4 x 4 x 4, so that the node planes neighbouring tiles share are still in L2 when the second tile needs
+// them, changes neither kernel's time on configs 4 and 5.)
+template <int DIM>
+__host__ __device__ __forceinline__ int tile_index(const GridDesc &gd, int tx, int ty, int tz)
+{
+    int tile = tx + gd.ntile[0] * ty;
+    if (DIM == 3) tile += gd.ntile[0] * gd.ntile[1] * tz;
+    return tile;
+}
+template <int DIM>
+__host__ __device__ __forceinline__ void tile_coords(const GridDesc &gd, int tile, int t[3])
+{
+    t[0] = tile % gd.ntile[0];
+    t[1] = (tile / gd.ntile[0]) % gd.ntile[1];
+    t[2] = (DIM == 3) ? tile / (gd.ntile[0] * gd.ntile[1]) : 0;
+}
+
 // cm: colour-major numbering inside the tile (a compile-time constant in the tile kernels, gd.colour_major elsewhere)
 template <int DIM>
 __host__ __device__ __forceinline__ int tiled_key_of_cell(const GridDesc &gd, const int c[DIM], bool cm)
 {
     using TG = TileGeo<DIM>;
-    int tile = (c[0] >> TG::LT0) + gd.ntile[0] * (c[1] >> TG::LT1);
-    if (DIM == 3) tile += gd.ntile[0] * gd.ntile[1] * (c[DIM - 1] >> TG::LT2);
+    const int tile = tile_index<DIM>(gd, c[0] >> TG::LT0, c[1] >> TG::LT1, DIM == 3 ? (c[DIM - 1] >> TG::LT2) : 0);
     const int local = TG::local_of(c[0] & (TG::T0 - 1), c[1] & (TG::T1 - 1), DIM == 3 ? (c[DIM - 1] & (TG::T2 - 1)) : 0, cm);
     return (tile << TG::LTC) | local;
 }
@@ -137,9 +158,11 @@ __host__ __device__ __forceinline__ void tiled_cell_of_key(const GridDesc &gd, i
     using TG = TileGeo<DIM>;
     const int tile = key >> TG::LTC, local = key & (TG::TC - 1);
     const bool cm = gd.colour_major != 0;
-    c[0] = ((tile % gd.ntile[0]) << TG::LT0) | TG::lx_of(local, cm);
-    c[1] = (((tile / gd.ntile[0]) % gd.ntile[1]) << TG::LT1) | TG::ly_of(local, cm);
-    if (DIM == 3) c[DIM - 1] = ((tile / (gd.ntile[0] * gd.ntile[1])) << TG::LT2) | TG::lz_of(local, cm);
+    int t[3];
+    tile_coords<DIM>(gd, tile, t);
+    c[0] = (t[0] << TG::LT0) | TG::lx_of(local, cm);
+    c[1] = (t[1] << TG::LT1) | TG::ly_of(local, cm);
+    if (DIM == 3) c[DIM - 1] = (t[2] << TG::LT2) | TG::lz_of(local, cm);
 }
 
 // particle SoA.  P, Vbar, A, grad V are transient and never stored.
@@ -295,13 +318,13 @@ long long max_items_tiled(const GridDesc &gd, long long max_groups);   // upper 
 // g: the node accumulators m, mv, f of this step (raw P2G#1) and mv2; the kernels apply l.4-5 / l.9 while staging a tile
 void launch_g2p_p2g2_tiled(const GridDesc &gd, const PArr &p, const GArr &g, const DevScalars *sc,
                            const SortedMap &map, const int4 *items, const int *n_items, long long max_items, int *count,
-                           unsigned long long *dest, cudaStream_t s);
+                           unsigned *dest, cudaStream_t s);
 // update + re-ordering + P2G#1 of the next step into g_next.m, g_next.mv, g_next.f (zeroed by the caller).  store_q:
 // write Q' to memory (only needed when the state can be read back or re-loaded before the next step: the fused P2G#1
 // has already consumed it)
 void launch_update_tiled(const GridDesc &gd, const PArr &p, const PArr &q, const GArr &g, DevScalars *sc,
                          const SortedMap &map, const int4 *items, const int *n_items, long long max_items, const int *off_new,
-                         const unsigned long long *dest, const GArr &g_next, bool store_q, cudaStream_t s);
+                         const unsigned *dest, const GArr &g_next, bool store_q, cudaStream_t s);
 // dst[id] = src[slot] for every occupied slot; with coff (exclusive scan of the per-key counts) and off (slot offsets):
 // dst[compact storage index] = src[slot] instead
 void launch_gather_by_id_groups(const double *src, const int *id, double *dst, const SortedMap &map, long long max_groups,

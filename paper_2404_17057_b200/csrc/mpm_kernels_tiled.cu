@@ -384,9 +384,11 @@ template <int DIM>
 __device__ __forceinline__ void tile_origin(const GridDesc &gd, int tile, int org[DIM])
 {
     using TG = TileGeo<DIM>;
-    org[0] = (tile % gd.ntile[0]) << TG::LT0;
-    org[1] = ((tile / gd.ntile[0]) % gd.ntile[1]) << TG::LT1;
-    if (DIM == 3) org[DIM - 1] = (tile / (gd.ntile[0] * gd.ntile[1])) << TG::LT2;
+    int t[3];
+    tile_coords<DIM>(gd, tile, t);
+    org[0] = t[0] << TG::LT0;
+    org[1] = t[1] << TG::LT1;
+    if (DIM == 3) org[DIM - 1] = t[2] << TG::LT2;
 }
 
 // global node index and node coordinates of tile-local node j (periodic wrap: node n == node 0, A11); -1 = outside the grid
@@ -458,7 +460,7 @@ __device__ __forceinline__ void stage_tile(const GridDesc &gd, const int org[DIM
             apply_bc<DIM, true>(gd, g, node[it], idx[it], m[it], mv[it], f[it]);
             const double inv = (m[it] != 0.0) ? 1.0 / m[it] : 0.0;
 #pragma unroll
-            for (int a = 0; a < DIM; ++a) v[a] = (mv[it][a] + dt * f[it][a]) * inv;
+            for (int a = 0; a < DIM; ++a) v[a] = __dmul_rn(fma(dt, f[it][a], mv[it][a]), inv);      // every rounding explicit: both tile kernels stage the same vbar
             if (WITH_V2) {
                 double none[DIM];
 #pragma unroll
@@ -499,6 +501,24 @@ __device__ __forceinline__ bool in_unit_cell(const double xi[DIM])
     bool in = true;
 #pragma unroll
     for (int a = 0; a < DIM; ++a) in = in && ((unsigned long long)__double_as_longlong(xi[a]) <= 0x3FF0000000000000ull);
+    return in;
+}
+
+// Does a particle of the group's cell c stay in that cell when it moves to Xn (Alg. 1 l.11-12)?  It does iff its local
+// coordinate xin = Xn / h - c lies in [0, 1) on every axis: then floor(Xn / h) = c (the subtraction is exact next to c) and
+// c needs no clamp, i.e. the general binning (cell_1d, readings A6, A19) returns c.  Exact, on the integer pipe: 0 <= xin < 1
+// <=> the bit pattern is below that of 1.0 (a negative value has the sign bit set).  Everything else -- another cell, or the
+// clamped cases on a domain face -- is binned by tiled_key_of_position.  Both tile kernels take this decision with this
+// function on the same Xn (move_inside / move_particle), so they agree on it; xin is also what the P2G of the stayers needs.
+template <int DIM>
+__device__ __forceinline__ bool stays_in_cell(const GridDesc &gd, const double Xn[DIM], const int c[DIM], double xin[DIM])
+{
+    bool in = true;
+#pragma unroll
+    for (int a = 0; a < DIM; ++a) {
+        xin[a] = __dmul_rn(Xn[a], gd.inv_h) - (double)c[a];
+        in = in && ((unsigned long long)__double_as_longlong(xin[a]) < 0x3FF0000000000000ull);
+    }
     return in;
 }
 
@@ -619,7 +639,7 @@ template <int DIM, bool ACC32, bool BULK, bool COLOUR, bool CM>
 __global__ void __launch_bounds__(kTB, (DIM == 2 && !COLOUR) ? kTBMinG2 : kTBMinG) k_g2p_p2g2_tiled(GridDesc gd, PArr p, GArr g,
                                                                 const DevScalars *__restrict__ sc, SortedMap map,
                                                                 const int4 *__restrict__ items, const int *__restrict__ n_items,
-                                                                int *__restrict__ count, unsigned long long *__restrict__ dest,
+                                                                int *__restrict__ count, unsigned *__restrict__ dest,
                                                                 unsigned long long *__restrict__ n_cell_changes)
 {
     static_assert(CM || !COLOUR, "accumulation by colour needs the colour-major cell numbering");
@@ -737,6 +757,7 @@ __global__ void __launch_bounds__(kTB, (DIM == 2 && !COLOUR) ? kTBMinG2 : kTBMin
         issue_vm(nxt, w0n, wnn);
         double MV[2][DIM];
         int key[2];
+        bool stay[2];
 #pragma unroll
         for (int i = 0; i < 2; ++i) {
 #pragma unroll
@@ -745,13 +766,16 @@ __global__ void __launch_bounds__(kTB, (DIM == 2 && !COLOUR) ? kTBMinG2 : kTBMin
                 MV[i][a] = M[i] * V[i][a];                        // M V'
             }
             // where the particle will be after l.11 (the persistent id is only needed by the recycling generator, A8)
-            double Xn[DIM];
+            double Xn[DIM], xin[DIM];
             if (!move_inside<DIM>(gd, X[i], out[i], dt, Xn) && valid[i]) {
                 bool recycled;
                 int nclamp;
                 move_particle<DIM>(gd, X[i], out[i], dt, gd.in_axis >= 0 ? (long long)p.id[k0 + i] : 0, step, Xn, recycled, nclamp);
             }
-            key[i] = valid[i] ? tiled_key_of_position<DIM, CM>(gd, Xn) : -1;
+            // l.12: its cell there.  Still the group's cell (the common case at CFL < 1) or binned anew
+            stay[i] = stays_in_cell<DIM>(gd, Xn, c, xin) && valid[i];
+            key[i] = grp.cell;
+            if (valid[i] && !stay[i]) key[i] = tiled_key_of_position<DIM, CM>(gd, Xn);
         }
         // V' replaces V in memory (the update kernel reads it back instead of gathering A again)
 #pragma unroll
@@ -761,7 +785,6 @@ __global__ void __launch_bounds__(kTB, (DIM == 2 && !COLOUR) ? kTBMinG2 : kTBMin
         }
         // ranks among the particles that end up in the same cell (arrival order of the atomics, A17): issue the atomics
         MPM_CHECK((!valid[0] || (key[0] >= 0 && key[0] < gd.Nkeys)) && (!valid[1] || (key[1] >= 0 && key[1] < gd.Nkeys)));
-        const bool stay[2] = { valid[0] && key[0] == grp.cell, valid[1] && key[1] == grp.cell };
         n_moved += (int)(valid[0] && !stay[0]) + (int)(valid[1] && !stay[1]);
         const unsigned gmask = (1u << LG) - 1u;
         const unsigned b0 = __ballot_sync(kFull, stay[0]), b1 = __ballot_sync(kFull, stay[1]);
@@ -818,10 +841,11 @@ __global__ void __launch_bounds__(kTB, (DIM == 2 && !COLOUR) ? kTBMinG2 : kTBMin
         const unsigned lower = (1u << l) - 1u;
         const int pre = base + __popc(g0 & lower) + __popc(g1 & lower);
         const int rank0 = stay[0] ? pre : rank_m[0], rank1 = stay[1] ? pre + (int)((g0 >> l) & 1u) : rank_m[1];
-        const unsigned long long dk0 = ((unsigned long long)(unsigned)key[0] << 32) | (unsigned)rank0;
-        const unsigned long long dk1 = ((unsigned long long)(unsigned)key[1] << 32) | (unsigned)rank1;
-        if (valid[1]) *reinterpret_cast<ulonglong2 *>(dest + k0) = make_ulonglong2(dk0, dk1);
-        else if (valid[0]) dest[k0] = dk0;
+        // the destination record is the rank alone: the update kernel finds the cell again from X' (stays_in_cell)
+        // (bit 31: this kernel's stay / leave decision, which the update kernel checks against its own)
+        const unsigned r0 = (unsigned)rank0 | (stay[0] ? 0x80000000u : 0u), r1 = (unsigned)rank1 | (stay[1] ? 0x80000000u : 0u);
+        if (valid[1]) *reinterpret_cast<uint2 *>(dest + k0) = make_uint2(r0, r1);
+        else if (valid[0]) dest[k0] = r0;
         grp = nxt;
         nxt = nn;
         w0 = w0n;
@@ -864,7 +888,7 @@ struct UpdSmem {
     static constexpr int NW = kTB / 32;                     // warps: each has its own slot window of kWin slots per field
     static constexpr size_t TILE = sizeof(double) * TG::NN * CH;
     static constexpr size_t PF = sizeof(double) * NW * NF * kWin;
-    static constexpr size_t DEST = sizeof(unsigned long long) * NW * kWin;
+    static constexpr size_t DEST = sizeof(unsigned) * NW * kWin;      // destination records (ranks)
     static constexpr size_t ID = sizeof(int) * NW * kWin;
     static constexpr size_t BAR = sizeof(unsigned long long) * NW * 2;
     static constexpr size_t BYTES = TILE + PF + DEST + ID + BAR;
@@ -877,7 +901,7 @@ template <int DIM, bool ACC32, bool BULK, bool COLOUR, bool CM>
 __global__ void __launch_bounds__(kTB, COLOUR ? 3 : DIM == 2 ? kTBMinU2 : kTBMinU) k_update_tiled(GridDesc gd, PArr p, PArr q, GArr g, DevScalars *sc, SortedMap map,
                                                               const int4 *__restrict__ items, const int *__restrict__ n_items,
                                                               const int *__restrict__ off_new,
-                                                              const unsigned long long *__restrict__ dest, GArr gn, int store_q)
+                                                              const unsigned *__restrict__ dest, GArr gn, int store_q)
 {
     using TG = TileGeo<DIM>;
     using SM = UpdSmem<DIM>;
@@ -885,7 +909,7 @@ __global__ void __launch_bounds__(kTB, COLOUR ? 3 : DIM == 2 ? kTBMinU2 : kTBMin
     extern __shared__ __align__(16) unsigned char s_raw[];
     double *s_tile = reinterpret_cast<double *>(s_raw);
     double (*s_pf)[SM::NF][kWin] = reinterpret_cast<double (*)[SM::NF][kWin]>(s_raw + SM::TILE);
-    unsigned long long (*s_dest)[kWin] = reinterpret_cast<unsigned long long (*)[kWin]>(s_raw + SM::TILE + SM::PF);
+    unsigned (*s_dest)[kWin] = reinterpret_cast<unsigned (*)[kWin]>(s_raw + SM::TILE + SM::PF);
     int (*s_id)[kWin] = reinterpret_cast<int (*)[kWin]>(s_raw + SM::TILE + SM::PF + SM::DEST);
     unsigned long long (*s_bar)[2] = reinterpret_cast<unsigned long long (*)[2]>(s_raw + SM::TILE + SM::PF + SM::DEST + SM::ID);
     double *s_acc = reinterpret_cast<double *>(s_raw + SM::BYTES);      // COLOUR only
@@ -910,18 +934,19 @@ __global__ void __launch_bounds__(kTB, COLOUR ? 3 : DIM == 2 ? kTBMinU2 : kTBMin
                 const long long k0 = (long long)gr.first + 2 * l;
 #pragma unroll
                 for (int a = 0; a < DIM; ++a) cp_async16(&s_pf[warp][a][2 * lane], p.x[a] + k0);
-                cp_async16(&s_dest[warp][2 * lane], dest + k0);
+                cp_async8(&s_dest[warp][2 * lane], dest + k0);
             }
             cp_async_commit();
         } else if (lane == 0) {
-            mbar_arrive_expect_tx(&s_bar[warp][0], (unsigned)((DIM + 1) * wn * 8));
+            mbar_arrive_expect_tx(&s_bar[warp][0], (unsigned)(DIM * wn * 8 + wn * 4));
             if (wn > 0) {
 #pragma unroll
                 for (int a = 0; a < DIM; ++a) bulk_g2s(&s_pf[warp][a][0], p.x[a] + w0, (unsigned)(wn * 8), &s_bar[warp][0]);
-                bulk_g2s(&s_dest[warp][0], dest + w0, (unsigned)(wn * 8), &s_bar[warp][0]);
+                bulk_g2s(&s_dest[warp][0], dest + w0, (unsigned)(wn * 4), &s_bar[warp][0]);
             }
         }
     };
+    const bool ids = gd.track_ids != 0;      // the persistent ids travel with the particles (else the id arrays are not touched)
     auto issue_rest = [&](const Group &gr, int w0, int wn) {
         if (!BULK) {
             if (2 * l < gr.cnt) {
@@ -931,19 +956,19 @@ __global__ void __launch_bounds__(kTB, COLOUR ? 3 : DIM == 2 ? kTBMinU2 : kTBMin
                 if (!gd.uniform_mass) cp_async16(&s_pf[warp][2 * DIM][2 * lane], p.m + k0);
                 cp_async16(&s_pf[warp][2 * DIM + 1][2 * lane], p.rho + k0);
                 cp_async16(&s_pf[warp][2 * DIM + 2][2 * lane], p.e + k0);
-                cp_async8(&s_id[warp][2 * lane], p.id + k0);
+                if (ids) cp_async8(&s_id[warp][2 * lane], p.id + k0);
             }
             cp_async_commit();
         } else if (lane == 0) {
             const int nf = gd.uniform_mass ? DIM + 2 : DIM + 3;
-            mbar_arrive_expect_tx(&s_bar[warp][1], (unsigned)(nf * wn * 8 + wn * 4));
+            mbar_arrive_expect_tx(&s_bar[warp][1], (unsigned)(nf * wn * 8 + (ids ? wn * 4 : 0)));
             if (wn > 0) {
 #pragma unroll
                 for (int a = 0; a < DIM; ++a) bulk_g2s(&s_pf[warp][DIM + a][0], p.v[a] + w0, (unsigned)(wn * 8), &s_bar[warp][1]);
                 if (!gd.uniform_mass) bulk_g2s(&s_pf[warp][2 * DIM][0], p.m + w0, (unsigned)(wn * 8), &s_bar[warp][1]);
                 bulk_g2s(&s_pf[warp][2 * DIM + 1][0], p.rho + w0, (unsigned)(wn * 8), &s_bar[warp][1]);
                 bulk_g2s(&s_pf[warp][2 * DIM + 2][0], p.e + w0, (unsigned)(wn * 8), &s_bar[warp][1]);
-                bulk_g2s(&s_id[warp][0], p.id + w0, (unsigned)(wn * 4), &s_bar[warp][1]);
+                if (ids) bulk_g2s(&s_id[warp][0], p.id + w0, (unsigned)(wn * 4), &s_bar[warp][1]);
             }
         }
     };
@@ -976,25 +1001,17 @@ __global__ void __launch_bounds__(kTB, COLOUR ? 3 : DIM == 2 ? kTBMinU2 : kTBMin
         const int j0 = TG::node0_of(local, CM);
         const bool valid[2] = { 2 * l < grp.cnt, 2 * l + 1 < grp.cnt };
         double X[2][DIM];
-        int key[2];
         long long dst[2] = { -1, -1 };
         const int o = !BULK ? 2 * lane : valid[0] ? grp.first + 2 * l - w0 : 0;      // the lane's two particles inside the warp's window
         MPM_CHECK(o >= 0 && o + 2 <= kWin && (o & 1) == 0 && j0 >= 0 && j0 + corner_off<DIM>(NB - 1) < TG::NN);
         MPM_CHECK(!valid[0] || (grp.first >= 0 && (long long)grp.first + 2 * l + 1 < gd.slots && (grp.cell >> TG::LTC) == item.x));
         if (BULK) mbar_wait(&s_bar[warp][0], parity); // this pass's X and destination records have landed
         else cp_async_wait_but_one();
-        {   // l.12: slot of the particle in the other buffer = offset of its new cell + its rank there; the offset load
-            // is issued first so that it overlaps the gather
-            const ulonglong2 td = *reinterpret_cast<const ulonglong2 *>(&s_dest[warp][o]);
-            key[0] = valid[0] ? (int)(td.x >> 32) : -1;
-            key[1] = valid[1] ? (int)(td.y >> 32) : -1;
-            MPM_CHECK((!valid[0] || (key[0] >= 0 && key[0] < gd.Nkeys)) && (!valid[1] || (key[1] >= 0 && key[1] < gd.Nkeys)));
-            if (valid[0]) dst[0] = (long long)__ldg(off_new + key[0]) + (long long)(unsigned)(td.x & 0xffffffffull);
-            if (valid[1]) dst[1] = (long long)__ldg(off_new + key[1]) + (long long)(unsigned)(td.y & 0xffffffffull);
-            // the destination slot lies inside the new cell's slot range
-            MPM_CHECK(!valid[0] || (dst[0] >= 0 && dst[0] < __ldg(off_new + key[0] + 1) && dst[0] < gd.slots));
-            MPM_CHECK(!valid[1] || (dst[1] >= 0 && dst[1] < __ldg(off_new + key[1] + 1) && dst[1] < gd.slots));
-        }
+        // l.12: slot of a particle in the other buffer = first slot of its new cell + its rank there (the destination record
+        // the gather kernel left).  The particles that stay in the group's cell share ONE offset, loaded here so that it
+        // overlaps the gather; the others bin X' again after the move
+        const uint2 trank = *reinterpret_cast<const uint2 *>(&s_dest[warp][o]);
+        const int off_cell = __ldg(off_new + grp.cell);
 #pragma unroll
         for (int a = 0; a < DIM; ++a) {
             const double2 tx = *reinterpret_cast<const double2 *>(&s_pf[warp][a][o]);
@@ -1026,7 +1043,7 @@ __global__ void __launch_bounds__(kTB, COLOUR ? 3 : DIM == 2 ? kTBMinU2 : kTBMin
             M[0] = valid[0] ? tm.x : 0.0; M[1] = valid[1] ? tm.y : 0.0;
             rho[0] = tr.x; rho[1] = tr.y;
             E[0] = te.x; E[1] = te.y;
-            const int2 ti = *reinterpret_cast<const int2 *>(&s_id[warp][o]);
+            const int2 ti = ids ? *reinterpret_cast<const int2 *>(&s_id[warp][o]) : make_int2(0, 0);
             id[0] = ti.x; id[1] = ti.y;
         }
         if (BULK) __syncwarp();
@@ -1036,7 +1053,7 @@ __global__ void __launch_bounds__(kTB, COLOUR ? 3 : DIM == 2 ? kTBMinU2 : kTBMin
         // group's cell.  Straight-line code for both particles of the lane (an unused slot computes on M = 0, X = 0 and
         // whatever V, rho, E its slot holds -- possibly NaN -- and is masked by SELECTS, never by a multiplication with 0,
         // wherever it could be seen: counters, maxima, stores, scatter payloads).
-        double Xo[2][DIM], Vo[2][DIM], Mo[2], Ro[2], Eo[2], Qo[2], Sn[2];
+        double Xo[2][DIM], Vo[2][DIM], Mo[2], Ro[2], Eo[2], Qo[2], Sn[2], xin[2][DIM];
         bool stay[2];
 #pragma unroll
         for (int i = 0; i < 2; ++i) {
@@ -1087,7 +1104,18 @@ __global__ void __launch_bounds__(kTB, COLOUR ? 3 : DIM == 2 ? kTBMinU2 : kTBMin
             Mo[i] = Mn; Ro[i] = rhon; Eo[i] = En; Qo[i] = Q;
             // S' = (P' + Q') M / rho' with P' = (gamma-1) rho' E' (eq. 3) and Q'/rho' = (Q'/rho) (1 + dt D)  (rho' = rho / (1 + dt D))
             Sn[i] = (gm1 * En + Q_over_rho * jac) * Mn;
-            stay[i] = valid[i] && key[i] == grp.cell;
+            // l.12: still in the group's cell?  Then its slot follows from the cell's offset, else X' is binned again.  The
+            // gather kernel took the same decision from the same X' (bit 31 of the record); a disagreement would corrupt the
+            // re-ordering, so it is counted with the exact-sort invariant (n_out_of_cell: must never count)
+            const unsigned rec = i ? trank.y : trank.x;
+            stay[i] = stays_in_cell<DIM>(gd, Xo[i], c, xin[i]) && valid[i];
+            events += (unsigned)(valid[i] && stay[i] != (bool)(rec >> 31)) << 25;
+            if (valid[i]) {
+                int key = grp.cell, first = off_cell;
+                if (!stay[i]) { key = tiled_key_of_position<DIM, CM>(gd, Xo[i]); first = __ldg(off_new + key); }
+                dst[i] = (long long)first + (long long)(rec & 0x7fffffffu);
+                MPM_CHECK(key >= 0 && key < gd.Nkeys && dst[i] >= 0 && dst[i] < __ldg(off_new + key + 1) && dst[i] < gd.slots);
+            }
         }
         // l.12: the particle goes to its cell-sorted slot of the other buffer; the two particles of a lane usually
         // keep adjacent slots (ranks of the stayers are consecutive), then each field is ONE 16-byte store
@@ -1102,7 +1130,7 @@ __global__ void __launch_bounds__(kTB, COLOUR ? 3 : DIM == 2 ? kTBMinU2 : kTBMin
             st2(q.rho, d0, Ro[0], Ro[1]);
             st2(q.e, d0, Eo[0], Eo[1]);
             if (store_q) st2(q.q, d0, Qo[0], Qo[1]);
-            *reinterpret_cast<int2 *>(q.id + d0) = make_int2(id[0], id[1]);
+            if (ids) *reinterpret_cast<int2 *>(q.id + d0) = make_int2(id[0], id[1]);
         } else {
 #pragma unroll
             for (int i = 0; i < 2; ++i) {
@@ -1114,7 +1142,7 @@ __global__ void __launch_bounds__(kTB, COLOUR ? 3 : DIM == 2 ? kTBMinU2 : kTBMin
                 q.rho[d] = Ro[i];
                 q.e[d] = Eo[i];
                 if (store_q) q.q[d] = Qo[i];
-                q.id[d] = id[i];
+                if (ids) q.id[d] = id[i];
             }
         }
         // P2G#1 of the next step (eqs. 13, 14, 16, 18 at X')
@@ -1126,11 +1154,7 @@ __global__ void __launch_bounds__(kTB, COLOUR ? 3 : DIM == 2 ? kTBMinU2 : kTBMin
         double pay[2][DIM + 2], wnew[2][NB];      // the others join the group's butterfly: payload M, M V', S', weights at X'
 #pragma unroll
         for (int i = 0; i < 2; ++i) {
-            double xin[DIM];
-#pragma unroll
-            for (int a = 0; a < DIM; ++a) xin[a] = __dmul_rn(Xo[i][a], gd.inv_h) - (double)c[a];
-            events += (unsigned)(stay[i] && !gd.has_open && !in_unit_cell<DIM>(xin)) << 25;      // both kernels must agree on X' bit for bit
-            swizzled_weights<DIM>(xin, l, wnew[i]);
+            swizzled_weights<DIM>(xin[i], l, wnew[i]);
             pay[i][0] = stay[i] ? Mo[i] : 0.0;
             pay[i][DIM + 1] = stay[i] ? Sn[i] : 0.0;
 #pragma unroll
@@ -1496,7 +1520,7 @@ long long max_items_tiled(const GridDesc &gd, long long max_groups)
 
 void launch_g2p_p2g2_tiled(const GridDesc &gd, const PArr &p, const GArr &g, const DevScalars *sc,
                            const SortedMap &map, const int4 *items, const int *n_items, long long max_items, int *count,
-                           unsigned long long *dest, cudaStream_t s)
+                           unsigned *dest, cudaStream_t s)
 {
     if (max_items <= 0) return;
     set_checked_bounds(gd, s);
@@ -1516,7 +1540,7 @@ void launch_g2p_p2g2_tiled(const GridDesc &gd, const PArr &p, const GArr &g, con
 
 void launch_update_tiled(const GridDesc &gd, const PArr &p, const PArr &q, const GArr &g, DevScalars *sc,
                          const SortedMap &map, const int4 *items, const int *n_items, long long max_items, const int *off_new,
-                         const unsigned long long *dest, const GArr &g_next, bool store_q, cudaStream_t s)
+                         const unsigned *dest, const GArr &g_next, bool store_q, cudaStream_t s)
 {
     if (max_items <= 0) return;
     set_checked_bounds(gd, s);

@@ -26,7 +26,7 @@ def test_library_builds_and_exports_every_declared_symbol():
         assert hasattr(lib, name), name
     assert sorted(binding.EXPORTS) == _declared()
     lib.mpm_abi_version.restype = ctypes.c_int
-    assert lib.mpm_abi_version() == 2          # pure host function, no CUDA involved
+    assert lib.mpm_abi_version() == 3          # pure host function, no CUDA involved
 
 
 def test_struct_layouts_match_the_header():

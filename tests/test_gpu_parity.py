@@ -215,7 +215,8 @@ def test_full_size_properties(mpm, name):
     w = inputs.sedov() if name == "sedov" else inputs.clumps()
     cfg, d, h = w["cfg"], w["cfg"]["dim"], w["cfg"]["dx"]
     n = w["mass"].shape[0]
-    g = mpm.Solver(cfg, sort_every=1, variant=mpm.VARIANT_TILED)
+    g = mpm.Solver(cfg, sort_every=1, variant=mpm.VARIANT_TILED, particle_ids=mpm.IDS_NONE)      # as bench.py creates it
+    assert not g.ids_tracked
     g.load_particles(w["x"], w["v"], w["mass"], w["rho"], w["e"])
     nsteps = 3
     g.step(0.0, w["cfl"], nsteps)
@@ -235,8 +236,8 @@ def test_full_size_properties(mpm, name):
         fabs = float(np.abs(gf).sum())
         for a in range(d):
             assert abs(float(np.sum(gf[a], dtype=np.longdouble))) <= 1e-12 * fabs
-    p = g.read_particles()
-    np.testing.assert_array_equal(p["mass"], w["mass"])                      # M_k never changes, ids intact
+    p = g.read_particles()                                                   # storage order (no ids); the checks are order-free
+    np.testing.assert_array_equal(p["mass"], w["mass"])                      # M_k never changes (equal masses)
     if name == "clumps":
         mom = (p["mass"][None, :] * p["v"]).sum(axis=1, dtype=np.longdouble)
         scale = float(np.abs(p["mass"][None, :] * p["v"]).sum())
@@ -255,6 +256,51 @@ def test_full_size_properties(mpm, name):
     local = (c[0] % t[0]) + t[0] * ((c[1] % t[1]) + t[1] * (c[2] % t[2]))
     key = tile * (t[0] * t[1] * t[2]) + local
     assert s["mass"].shape[0] == n and (np.diff(key) >= 0).all()
+
+
+@pytest.mark.parametrize("stream", [0, 1])
+@pytest.mark.parametrize("name", ["box", "box_shuffled", "sedov", "clumps", "clumps_dense"])
+def test_without_particle_ids_matches_oracle(po, mpm, name, stream):
+    """mpm_config.particle_ids = MPM_IDS_NONE (what bench.py times): the sweeps carry no ids, read-back is in storage order.
+    The particles are told apart by their masses instead -- every particle gets its own (M_k is copied bit for bit by
+    both sides, Algorithm 1 never changes it) -- and all fields are compared with the oracle as in the id-ordered tests."""
+    w = small_workloads()[name]()
+    n = w["mass"].shape[0]
+    mass = w["mass"] * (1.0 + np.arange(1, n + 1) * 2.0 ** -30)
+    assert np.unique(mass).shape[0] == n
+    o = po.Oracle(w["cfg"])
+    o.load_particles(w["x"], w["v"], mass, w["rho"], w["e"])
+    g = mpm.Solver(w["cfg"], sort_every=1, variant=mpm.VARIANT_TILED, particle_ids=mpm.IDS_NONE, particle_stream=stream)
+    assert not g.ids_tracked
+    g.load_particles(w["x"], w["v"], mass, w["rho"], w["e"])
+    nsteps = STEPS[name] // 2
+    o.step(0.0, w["cfl"], nsteps)
+    g.step(0.0, w["cfl"], nsteps)
+    so, sg = o.stats(), g.stats()
+    assert so.step == sg.step == nsteps and abs(so.t - sg.t) <= 1e-10 * so.t
+    assert sg.n_nonfinite == 0 and sg.n_out_of_cell == 0 and so.n_negjac == sg.n_negjac
+    if name != "sedov":
+        assert sg.n_cell_changes > 0
+    with pytest.raises(mpm.MpmError):
+        g.read_particles(order=0)
+    with pytest.raises(mpm.MpmError):
+        g.read_particles(mask=mpm.P_X | mpm.P_ID, order=1)
+    p = g.read_particles()
+    og = np.argsort(p["mass"])
+    oo = np.argsort(mass)
+    np.testing.assert_array_equal(p["mass"][og], mass[oo])
+    d = w["cfg"]["dim"]
+    rho, e, v, x = (o.particles(f) for f in (po.P_RHO, po.P_E, po.P_V, po.P_X))
+    assert np.abs(rho[oo] - p["rho"][og]).sum() <= PART_TOL * np.abs(rho).sum(), name
+    assert np.abs(e[oo] - p["e"][og]).sum() <= PART_TOL * np.abs(e).sum(), name
+    vnorm = np.sqrt((v ** 2).sum(axis=0)).sum()
+    L = np.array(w["cfg"]["n"][:d]) * w["cfg"]["dx"]
+    for a in range(d):
+        assert np.abs(v[a][oo] - p["v"][a][og]).sum() <= PART_TOL * max(vnorm, 1e-300), (name, a)
+        dx = np.abs(x[a][oo] - p["x"][a][og])
+        if w["cfg"]["bc"][a][0] == 0:
+            dx = np.minimum(dx, L[a] - dx)
+        assert dx.sum() <= PART_TOL * np.abs(x).sum(), (name, a)
 
 
 @pytest.mark.parametrize("name", ["clumps", "clumps_dense", "sedov", "cylinder"])
@@ -563,7 +609,7 @@ def test_checked_build(mpm):
     lib = build.build(checked=True)
     root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
     sel = ("(test_one_step_grid_parity and mode2) or (test_many_step_particle_parity and mode2) or bulk_particle_stream "
-           "or fp32_grid_accumulation_variant or test_edge_cases or (test_parity_at_size and (clumps64 or cylinder1024))")
+           "or fp32_grid_accumulation_variant or without_particle_ids or test_edge_cases or (test_parity_at_size and (clumps64 or cylinder1024))")
     r = subprocess.run([sys.executable, "-m", "pytest", os.path.join(root, "tests", "test_gpu_parity.py"), "-x", "-q",
                         "-p", "no:cacheprovider", "-k", sel], env=dict(os.environ, MPM_B200_LIB=lib),
                        capture_output=True, text=True, cwd=root)
