@@ -70,6 +70,9 @@ __device__ __forceinline__ void cp_async8(void *smem, const void *gmem)
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 // all committed groups but the most recent one have landed
 __device__ __forceinline__ void cp_async_wait_but_one() { asm volatile("cp.async.wait_group 1;" ::: "memory"); }
+// all committed groups but the N most recent ones have landed
+template <int N>
+__device__ __forceinline__ void cp_async_wait_but() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 __device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(unsigned long long *bar, unsigned count)
 {
@@ -129,6 +132,26 @@ __device__ __forceinline__ double acc_ld(const double *arr, long long i)
     MPM_CHECK(i >= 0 && i < g_checked_nodes);
     if (ACC32) return (double)__ldg(reinterpret_cast<const float *>(arr) + i);
     return __ldg(arr + i);
+}
+
+// 1 / x to within about one unit in the last place for a finite x that is neither zero nor subnormal: the hardware
+// approximation (relative error 2^-23) refined by two Newton steps, 5 instructions in place of the ~25 of an IEEE division
+// (measured: profiles/r02_experiments.md section 6).  Used where the parity tolerance (1e-12) leaves room for the last bit:
+// rho' = rho / (1 + dt D) and the node quotients by m.  x = 0 gives inf like the division; a subnormal x is flushed to 0.
+#ifndef MPM_FAST_RCP
+#define MPM_FAST_RCP 1
+#endif
+__device__ __forceinline__ double rcp_newton(double x)
+{
+#if MPM_FAST_RCP
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    y = fma(y, fma(-x, y, 1.0), y);
+    y = fma(y, fma(-x, y, 1.0), y);
+    return y;
+#else
+    return 1.0 / x;
+#endif
 }
 
 template <int DIM, bool CM>
@@ -372,6 +395,45 @@ struct Chunk {
     static constexpr int GROUPS = PASSES * (kTB / Geo<DIM>::LG);
 };
 
+// The group records of a block's item are copied into shared memory once, at the start of the block (one 16-byte cp.async
+// per record: they are one contiguous run), and every pass reads its records from there.  ncu (profiles/r02_ncu_sedov256.md):
+// fetching them with a global load inside the pass cost 6 - 9 % of both sweeps' stall samples -- the unpacking right behind
+// the load, and shared-memory loads that waited on the scoreboard they shared with it.  STAGE = false (the COLOUR
+// instantiations, whose static shared memory is full): records come from global memory as before.
+template <int DIM, bool STAGE>
+__device__ __forceinline__ void stage_groups(int4 *s_grp, const int4 *__restrict__ groups, int first, int n)
+{
+    if (STAGE) {
+        for (int j = threadIdx.x; j < n; j += kTB) cp_async16(s_grp + j, groups + first + j);
+        cp_async_commit();
+    }
+}
+// record j of the item (j >= n: an idle group)
+template <bool STAGE>
+__device__ __forceinline__ Group item_group(const int4 *s_grp, const int4 *__restrict__ groups, int first, int j, int n)
+{
+    if (!STAGE) return fetch_group(groups, (long long)first + j, first + n);
+    Group g{ 0, 0, 0, 0, 0 };
+    if (j < n) {
+        MPM_CHECK(j >= 0);
+        const int4 r = s_grp[j];
+        g.first = r.x; g.cnt = r.y & 0xff; g.multi = r.y >> 8; g.cell = r.z; g.cpack = r.w;
+    }
+    return g;
+}
+// ... or, without the staging: the raw record is loaded from global memory in the middle of a pass and only unpacked at the
+// end of that pass, when it has had time to arrive (an all-zero record is an idle group)
+__device__ __forceinline__ int4 raw_group(const int4 *__restrict__ groups, long long gidx, int n_groups)
+{
+    return gidx < (long long)n_groups ? __ldg(groups + gidx) : make_int4(0, 0, 0, 0);
+}
+__device__ __forceinline__ Group unpack_group(const int4 &r)
+{
+    Group g;
+    g.first = r.x; g.cnt = r.y & 0xff; g.multi = r.y >> 8; g.cell = r.z; g.cpack = r.w;
+    return g;
+}
+
 // tile-local node index j = lx + N0 (ly + N1 lz) of corner b of the cell with tile-local node index j0
 template <int DIM>
 __device__ __forceinline__ constexpr int corner_off(int b)
@@ -458,7 +520,7 @@ __device__ __forceinline__ void stage_tile(const GridDesc &gd, const int org[DIM
         for (int q = 0; q < CH; ++q) v[q] = 0.0;
         if (node[it] >= 0) {
             apply_bc<DIM, true>(gd, g, node[it], idx[it], m[it], mv[it], f[it]);
-            const double inv = (m[it] != 0.0) ? 1.0 / m[it] : 0.0;
+            const double inv = (m[it] != 0.0) ? (fabs(m[it]) >= 1e-290 ? rcp_newton(m[it]) : 1.0 / m[it]) : 0.0;
 #pragma unroll
             for (int a = 0; a < DIM; ++a) v[a] = __dmul_rn(fma(dt, f[it][a], mv[it][a]), inv);      // every rounding explicit: both tile kernels stage the same vbar
             if (WITH_V2) {
@@ -649,6 +711,8 @@ __global__ void __launch_bounds__(kTB, (DIM == 2 && !COLOUR) ? kTBMinG2 : kTBMin
     __shared__ __align__(16) double s_pf[kTB / 32][NF][kWin];      // per warp: x[d], v[d], m of the pass's slot window
     __shared__ __align__(8) unsigned long long s_bar[kTB / 32][2];  // per warp: X copies / V, M copies
     __shared__ __align__(16) double s_acc[COLOUR ? TG::NN * DIM : 1];   // COLOUR: accumulator tile of mv2
+    constexpr bool SG = !COLOUR;                                        // group records staged in shared memory
+    __shared__ __align__(16) int4 s_grp[SG ? Chunk<DIM>::GROUPS : 1];
     __shared__ int s_moved;
     if (threadIdx.x == 0) s_moved = 0;
     if (COLOUR) for (int j = threadIdx.x; j < TG::NN * DIM; j += kTB) s_acc[j] = 0.0;
@@ -659,6 +723,8 @@ __global__ void __launch_bounds__(kTB, (DIM == 2 && !COLOUR) ? kTBMinG2 : kTBMin
     const int l = threadIdx.x % LG, lane = threadIdx.x & 31, sh = lane & ~(LG - 1);
     const int g_end = item.y + item.z;
     int gl = threadIdx.x / LG;
+    MPM_CHECK(item.z <= Chunk<DIM>::GROUPS);
+    stage_groups<DIM, SG>(s_grp, map.groups, item.y, item.z);      // the oldest copy group: complete before any later one
     Group grp = fetch_group(map.groups, (long long)item.y + gl, g_end);
     Group nxt = fetch_group(map.groups, (long long)item.y + gl + GPB, g_end);
     // two copy groups per pass: X (needed first, refilled as soon as it has been read: a whole pass of lead time) and V, M;
@@ -713,6 +779,7 @@ __global__ void __launch_bounds__(kTB, (DIM == 2 && !COLOUR) ? kTBMinG2 : kTBMin
     const double dt = sc->dt;
     const long long step = sc->step;
     stage_tile<DIM, CH, false, ACC32>(gd, org, g, dt, s_tile);
+    if (SG) { if (BULK) cp_async_wait_but<0>(); else cp_async_wait_but<2>(); }      // this thread's records have landed
     __syncthreads();
     unsigned parity = 0;
     PassColours<DIM> pc{ 0, 0 }, pcn{ 0, 0 };
@@ -737,7 +804,6 @@ __global__ void __launch_bounds__(kTB, (DIM == 2 && !COLOUR) ? kTBMinG2 : kTBMin
         }
         if (BULK) __syncwarp();
         issue_x(nxt, w0n, wnn);                       // the window has been read: refill it for the next pass
-        const Group nn = fetch_group(map.groups, (long long)item.y + gl + 2 * GPB, g_end);
         double W[2][DIM][2], xi[2][DIM], out[2][2 * DIM], Dh[2];
 #pragma unroll
         for (int i = 0; i < 2; ++i) weights_1d<DIM>(gd, X[i], c, xi[i], W[i]);
@@ -835,7 +901,7 @@ __global__ void __launch_bounds__(kTB, (DIM == 2 && !COLOUR) ? kTBMinG2 : kTBMin
                 }
             }
         }
-        // ... and only now use what they returned
+        // ... and only now use what they returned (consuming it one pass later instead was measured: neutral)
         if (one_cell) base = __shfl_sync(kFull, base, 0) + __popc(b0 & ((1u << sh) - 1u)) + __popc(b1 & ((1u << sh) - 1u));
         else base = __shfl_sync(kFull, base, sh);
         const unsigned lower = (1u << l) - 1u;
@@ -847,7 +913,7 @@ __global__ void __launch_bounds__(kTB, (DIM == 2 && !COLOUR) ? kTBMinG2 : kTBMin
         if (valid[1]) *reinterpret_cast<uint2 *>(dest + k0) = make_uint2(r0, r1);
         else if (valid[0]) dest[k0] = r0;
         grp = nxt;
-        nxt = nn;
+        nxt = item_group<SG>(s_grp, map.groups, item.y, gl + 2 * GPB, item.z);
         w0 = w0n;
         wn = wnn;
         warp_window<BULK>(nxt.first, nxt.cnt, w0n, wnn);
@@ -894,7 +960,7 @@ struct UpdSmem {
     static constexpr size_t BYTES = TILE + PF + DEST + ID + BAR;
     static constexpr int NACC = 2 * DIM + 1;                // COLOUR: accumulator tile of m, mv, f behind the rest
     static constexpr size_t ACC = sizeof(double) * TG::NN * NACC;
-    static_assert(TILE % 16 == 0 && PF % 16 == 0 && DEST % 16 == 0 && ID % 16 == 0, "16-byte aligned sections");
+    static_assert(TILE % 16 == 0 && PF % 16 == 0 && DEST % 16 == 0 && ID % 16 == 0 && BAR % 16 == 0, "16-byte aligned sections");
 };
 
 template <int DIM, bool ACC32, bool BULK, bool COLOUR, bool CM>
@@ -1048,7 +1114,9 @@ __global__ void __launch_bounds__(kTB, COLOUR ? 3 : DIM == 2 ? kTBMinU2 : kTBMin
         }
         if (BULK) __syncwarp();
         issue_rest(nxt, w0n, wnn);
-        const Group nn = fetch_group(map.groups, (long long)item.y + gl + 2 * GPB, g_end);
+        // the group record of the pass after the next: loaded here, unpacked at the end of this pass (staging the records in
+        // shared memory as the gather kernel does was measured slower here: 4 x 8 KB less L1 per SM)
+        const int4 nn_raw = raw_group(map.groups, (long long)item.y + gl + 2 * GPB, g_end);
         // per particle: the new state (what goes to memory), S' for the next step's force, and whether it stays in the
         // group's cell.  Straight-line code for both particles of the lane (an unused slot computes on M = 0, X = 0 and
         // whatever V, rho, E its slot holds -- possibly NaN -- and is masked by SELECTS, never by a multiplication with 0,
@@ -1075,7 +1143,7 @@ __global__ void __launch_bounds__(kTB, COLOUR ? 3 : DIM == 2 ? kTBMinU2 : kTBMin
             if (!(D < 0.0)) { Q = 0.0; Q_over_rho = 0.0; }      // eq. (4): only in compression
             double En = e0 - dt * (gm1 * e0 + Q_over_rho) * D;
             const double jac = fma(dt, D, 1.0);
-            double rhon = r / jac;
+            double rhon = r * rcp_newton(jac);      // rho' = rho / (1 + dt D); jac <= 0 is counted below
             if (valid[i]) {
                 events += (unsigned)(jac <= 0.0) << 13;
                 double vv = 0.0, vb2 = 0.0;
@@ -1176,7 +1244,7 @@ __global__ void __launch_bounds__(kTB, COLOUR ? 3 : DIM == 2 ? kTBMinU2 : kTBMin
             if (phase < 0 && issue) p2g1_commit_global<DIM, ACC32>(gd, gn, c, l, tot);
         }
         grp = nxt;
-        nxt = nn;
+        nxt = unpack_group(nn_raw);
         w0 = w0n;
         wn = wnn;
         warp_window<BULK>(nxt.first, nxt.cnt, w0n, wnn);
@@ -1545,21 +1613,16 @@ void launch_update_tiled(const GridDesc &gd, const PArr &p, const PArr &q, const
     if (max_items <= 0) return;
     set_checked_bounds(gd, s);
     const int sq = store_q ? 1 : 0;
-    static_assert(UpdSmem<2>::BYTES <= 48 * 1024 && UpdSmem<3>::BYTES <= 48 * 1024, "dynamic shared memory beyond 48 KB needs a per-device opt-in");
     static_assert(UpdSmem<2>::BYTES % 16 == 0 && UpdSmem<3>::BYTES % 16 == 0, "the accumulator tile starts 16-byte aligned");
-#define MPM_LAUNCH_UPD(D, A, B, C, CM, BYTES) \
-    k_update_tiled<D, A, B, C, CM><<<(unsigned)max_items, kTB, BYTES, s>>>(gd, p, q, g, sc, map, items, n_items, off_new, dest, g_next, sq)
+    // more than 48 KB of dynamic shared memory needs the opt-in; the attribute is per device, so it is set at every launch (a
+    // host-side call without a synchronisation)
+#define MPM_LAUNCH_UPD(D, A, B, C, CM, BYTES) do { \
+    if ((BYTES) > 48 * 1024) cudaFuncSetAttribute(k_update_tiled<D, A, B, C, CM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(BYTES)); \
+    k_update_tiled<D, A, B, C, CM><<<(unsigned)max_items, kTB, BYTES, s>>>(gd, p, q, g, sc, map, items, n_items, off_new, dest, g_next, sq); } while (0)
 #define MPM_LAUNCH_UPD_A(D, A) do { if (gd.bulk_stream) MPM_LAUNCH_UPD(D, A, true, false, false, UpdSmem<D>::BYTES); else MPM_LAUNCH_UPD(D, A, false, false, false, UpdSmem<D>::BYTES); } while (0)
     if (gd.p2g_mode & MPM_P2G_COLOUR_UPDATE) {   // fp64 accumulation and the cp.async stream only (mpm_create checks)
-        // more than 48 KB of dynamic shared memory needs the opt-in; the attribute is per device, so it is set at every
-        // launch (a host-side call without a synchronisation)
-        if (gd.dim == 2) {
-            cudaFuncSetAttribute(k_update_tiled<2, false, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(UpdSmem<2>::BYTES + UpdSmem<2>::ACC));
-            MPM_LAUNCH_UPD(2, false, false, true, true, UpdSmem<2>::BYTES + UpdSmem<2>::ACC);
-        } else {
-            cudaFuncSetAttribute(k_update_tiled<3, false, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(UpdSmem<3>::BYTES + UpdSmem<3>::ACC));
-            MPM_LAUNCH_UPD(3, false, false, true, true, UpdSmem<3>::BYTES + UpdSmem<3>::ACC);
-        }
+        if (gd.dim == 2) MPM_LAUNCH_UPD(2, false, false, true, true, UpdSmem<2>::BYTES + UpdSmem<2>::ACC);
+        else MPM_LAUNCH_UPD(3, false, false, true, true, UpdSmem<3>::BYTES + UpdSmem<3>::ACC);
     } else if (gd.colour_major) {                // the gather kernel accumulates by colour: same cell numbering here
         if (gd.dim == 2) MPM_LAUNCH_UPD(2, false, false, false, true, UpdSmem<2>::BYTES); else MPM_LAUNCH_UPD(3, false, false, false, true, UpdSmem<3>::BYTES);
     } else if (gd.dim == 2) { if (gd.acc32) MPM_LAUNCH_UPD_A(2, true); else MPM_LAUNCH_UPD_A(2, false); }
