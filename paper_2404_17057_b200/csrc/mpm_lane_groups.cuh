@@ -1,6 +1,6 @@
-// mpm_lane_groups.cuh -- device helpers of the TILED kernel family: lane-group geometry, the
-// transposed butterfly reduction, corner weights in natural / butterfly order, slow paths for a particle whose cell
-// is not its group's cell, and the particle move of Alg. 1 l.11.
+// mpm_lane_groups.cuh -- device helpers of the TILED kernel family: lane-group geometry, the transposed butterfly
+// reduction, corner weights in butterfly order, the P2G#1 of a particle whose cell is not its group's cell (after a load
+// only), and the particle move of Alg. 1 l.11.
 #pragma once
 #include "mpm_internal.cuh"
 
@@ -16,11 +16,6 @@ struct Geo {
     static constexpr int LG = NB / 2;              // lanes per group
     static constexpr int NG = 32 / LG;             // groups per warp
     static constexpr int GPB = kBlock / LG;        // groups per block and iteration
-    // shared staging of corner node values: [group][corner][channel]; the group stride is == 4 (mod 32) words so that
-    // the 16-byte broadcast reads of the groups of a warp fall into distinct banks
-    static constexpr int CH = (DIM == 3) ? 8 : 6;                       // doubles per corner (vbar, acc, dsum, pad)
-    static constexpr int GROUP_STRIDE = (DIM == 3) ? 66 : 34;           // doubles
-    static constexpr int WARP_DOUBLES = NG * GROUP_STRIDE;
 };
 
 __device__ __forceinline__ double shfl_xor_d(double v, int m) { return __shfl_xor_sync(kFull, v, m); }
@@ -93,14 +88,7 @@ __device__ __forceinline__ bool local_coords(const GridDesc &gd, const double X[
     return same;
 }
 
-// weights in natural corner order (gathers) ...
-template <int DIM>
-__device__ __forceinline__ void natural_weights(const double xi[DIM], double w[1 << DIM])
-{
-#pragma unroll
-    for (int b = 0; b < (1 << DIM); ++b) w[b] = corner_phi<DIM>(xi, b);
-}
-// ... and in butterfly order (scatters): register r of lane l holds the weight of corner r ^ l (l < LG)
+// corner weights in butterfly order (scatters): register r of lane l holds the weight of corner r ^ l (l < LG)
 template <int DIM>
 __device__ __forceinline__ void swizzled_weights(const double xi[DIM], int l, double w[1 << DIM])
 {
@@ -159,45 +147,6 @@ __device__ __forceinline__ void slow_p2g1(const GridDesc &gd, const GArr &g, con
     }
 }
 
-template <int DIM>
-__device__ __forceinline__ void slow_gather(const GridDesc &gd, const double *na, const double *nb, const double X[DIM],
-                                            double Vb[DIM], double A[DIM], double *D)
-{
-    int c[DIM];
-    double xi[DIM];
-    particle_cell<DIM>(gd, X, c, xi);
-    double d = 0.0;
-#pragma unroll
-    for (int a = 0; a < DIM; ++a) { Vb[a] = 0.0; A[a] = 0.0; }
-#pragma unroll 1
-    for (int ib = 0; ib < (1 << DIM); ++ib) {
-        const long long i = corner_node<DIM>(gd, c, ib);
-        const double phi = corner_phi<DIM>(xi, ib);
-#pragma unroll
-        for (int a = 0; a < DIM; ++a) {
-            Vb[a] += phi * na[i * (2 * DIM) + a];
-            A[a] += phi * na[i * (2 * DIM) + DIM + a];
-            if (nb) d += nb[i * DIM + a] * corner_dphi<DIM>(xi, ib, a, gd.inv_h);
-        }
-    }
-    if (D) *D = d;
-}
-
-template <int DIM>
-__device__ __forceinline__ void slow_p2g2(const GridDesc &gd, const GArr &g, const double X[DIM], const double MV[DIM])
-{
-    int c[DIM];
-    double xi[DIM];
-    particle_cell<DIM>(gd, X, c, xi);
-#pragma unroll 1
-    for (int ib = 0; ib < (1 << DIM); ++ib) {
-        const long long i = corner_node<DIM>(gd, c, ib);
-        const double phi = corner_phi<DIM>(xi, ib);
-#pragma unroll
-        for (int a = 0; a < DIM; ++a) atomicAdd(&g.mv2[a][i], MV[a] * phi);
-    }
-}
-
 // ---------------------------------------------------------------------------------------------- shared pieces
 
 // Alg. 1 l.11 for one particle: X' = X + dt Vbar, periodic wrap (A11), outflow detection, recycling position (A8),
@@ -252,49 +201,6 @@ __device__ __forceinline__ void move_particle(const GridDesc &gd, const double X
                 if (gd.bc[a][1] == MPM_BC_OPEN) { if (left_slab) *left_slab = true; }
                 else if (Xn[a] > gd.L[a]) { Xn[a] = gd.L[a]; nclamp++; }
             }
-        }
-    }
-}
-
-template <int DIM>
-__device__ __forceinline__ int cell_key(const GridDesc &gd, const double X[DIM])
-{
-    int key = 0, stride = 1;
-#pragma unroll
-    for (int a = 0; a < DIM; ++a) {
-        int c;
-        double xi;
-        cell_1d(X[a], gd.inv_h, gd.nc[a], c, xi);
-        key += stride * c;
-        stride *= gd.nc[a];
-    }
-    return key;
-}
-
-// lane l stages vbar, acc of one corner (node-major array na[node][2 DIM]) into shared memory
-template <int DIM>
-__device__ __forceinline__ void stage_na(const double *__restrict__ na, int node, double *s_corner)
-{
-    const double2 *src = reinterpret_cast<const double2 *>(na + (long long)node * (2 * DIM));
-    double2 *dst = reinterpret_cast<double2 *>(s_corner);
-#pragma unroll
-    for (int q = 0; q < DIM; ++q) dst[q] = __ldg(src + q);
-}
-
-// phi-weighted gather of the staged channels: out[c] = sum_b w[b] vals[b][c], c < 2*NPAIR
-template <int DIM, int NPAIR>
-__device__ __forceinline__ void gather_pairs(const double *s_group, const double w[1 << DIM], double out[2 * NPAIR])
-{
-#pragma unroll
-    for (int c = 0; c < 2 * NPAIR; ++c) out[c] = 0.0;
-#pragma unroll
-    for (int b = 0; b < (1 << DIM); ++b) {
-        const double2 *row = reinterpret_cast<const double2 *>(s_group + b * Geo<DIM>::CH);
-#pragma unroll
-        for (int q = 0; q < NPAIR; ++q) {
-            const double2 t = row[q];
-            out[2 * q] = fma(w[b], t.x, out[2 * q]);
-            out[2 * q + 1] = fma(w[b], t.y, out[2 * q + 1]);
         }
     }
 }
