@@ -67,8 +67,8 @@ enum { MPM_VISC_PRINTED = 0, MPM_VISC_STANDARD = 1 };
  * (2 was the SORTED family of ABI version 1, an intermediate of TILED; mpm_create now rejects it.) */
 enum { MPM_VARIANT_AUTO = 0, MPM_VARIANT_ATOMIC = 1, MPM_VARIANT_SORTED_RETIRED = 2, MPM_VARIANT_TILED = 3 };
 /* precision of the node sums m, mv, f, mv2 ("the code supports different choices"): FP64 (default), or FP32
- * = the fp32 grid-accumulation variant of the clustered stress workload: the scatters reduce in fp32 and the sums are
- * kept in fp32, all particle arithmetic stays fp64.  TILED family only (MPM_E_ARG otherwise). */
+ * = the fp32 grid-accumulation variant of the clustered stress workload: the scatters reduce in fp32 (vector reductions on
+ * node-major sums) and the sums are kept in fp32, all particle arithmetic stays fp64.  TILED family only (MPM_E_ARG otherwise). */
 enum { MPM_ACCUM_FP64 = 0, MPM_ACCUM_FP32 = 1 };
 /* how the TILED kernels bring the next pass's particle fields into shared memory: CP_ASYNC (default) = per-thread
  * 16-byte cp.async; BULK = one bulk asynchronous copy (cp.async.bulk, the non-tensor form of TMA) per field, warp and pass,

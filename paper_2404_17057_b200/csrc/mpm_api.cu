@@ -31,6 +31,9 @@ struct mpm_handle {
     // TILED: the node accumulators m, mv, f are double-buffered: the update kernel of step n already scatters P2G#1 of
     // step n+1 into the other set.  acc[acur] = the set the current / next mpm_step starts from (raw P2G#1).
     double *acc_m[2], *acc_mv[2][3], *acc_f[2][3], *acc_mv2[2][3];
+    // TILED with fp32 accumulation: the sums are node-major instead, nm[N_n][8] = { m, mv[3], f[3], - } and v2[N_n][4] = { mv2[3], - }
+    // (vector reductions, mpm_kernels_tiled.cu); the kernels find them behind g.m and g.mv2[0]
+    float *acc32_nm[2], *acc32_v2[2];
     // TILED: the next step's accumulator set is cleared on a second stream while the gather kernel runs
     cudaStream_t side;
     cudaEvent_t ev_fork, ev_join;
@@ -309,7 +312,23 @@ GArr tiled_acc(const mpm_handle *h, int which)
     GArr g = h->g;
     g.m = h->acc_m[which];
     for (int a = 0; a < 3; ++a) { g.mv[a] = h->acc_mv[which][a]; g.f[a] = h->acc_f[which][a]; g.mv2[a] = h->acc_mv2[which][a]; }
+    if (h->gd.acc32) {
+        g.m = reinterpret_cast<double *>(h->acc32_nm[which]);
+        g.mv2[0] = reinterpret_cast<double *>(h->acc32_v2[which]);
+    }
     return g;
+}
+
+// Alg. 1 l.2 for an accumulator set of the TILED family: m, mv, f (the targets of P2G#1) / mv2 (of P2G#2)
+void clear_p2g1(const mpm_handle *h, const GArr &g, cudaStream_t s)
+{
+    if (h->gd.acc32) cudaMemsetAsync(g.m, 0, sizeof(float) * 8 * (size_t)h->gd.Nn, s);
+    else launch_grid_clear(h->gd, g, s);
+}
+void clear_p2g2(const mpm_handle *h, const GArr &g, cudaStream_t s)
+{
+    if (h->gd.acc32) { cudaMemsetAsync(g.mv2[0], 0, sizeof(float) * 4 * (size_t)h->gd.Nn, s); return; }
+    for (int a = 0; a < h->gd.dim; ++a) cudaMemsetAsync(g.mv2[a], 0, sizeof(double) * (size_t)h->gd.Nn, s);
 }
 
 // cell-key counting sort of all particle arrays into the other buffer (Alg. 1 l.12).  TILED family: only after a
@@ -329,8 +348,8 @@ void reorder(mpm_handle *h)
         h->acur = 0;
         h->grid_final = false;
         GArr g0 = tiled_acc(h, 0);
-        launch_grid_clear(h->gd, g0, h->stream);
-        for (int a = 0; a < h->gd.dim; ++a) cudaMemsetAsync(g0.mv2[a], 0, sizeof(double) * (size_t)h->gd.Nn, h->stream);
+        clear_p2g1(h, g0, h->stream);
+        clear_p2g2(h, g0, h->stream);
         launch_p2g1_tiled(h->gd, dst, g0, SortedMap{ h->groups, h->n_groups }, h->max_groups, h->stream);
         h->launches += 6;
         return;
@@ -359,8 +378,8 @@ void step_tiled_gather(mpm_handle *h)
         // update kernel) is cleared on the second stream while this step's gather kernel runs
         cudaEventRecord(h->ev_fork, s);
         cudaStreamWaitEvent(h->side, h->ev_fork, 0);
-        launch_grid_clear(gd, gnx, h->side);
-        for (int a = 0; a < gd.dim; ++a) cudaMemsetAsync(gnx.mv2[a], 0, sizeof(double) * (size_t)gd.Nn, h->side);
+        clear_p2g1(h, gnx, h->side);
+        clear_p2g2(h, gnx, h->side);
         cudaEventRecord(h->ev_join, h->side);
         cudaMemsetAsync(h->count, 0, sizeof(int) * (size_t)(gd.Nkeys + 1), s);            // per-cell counters of l.12
     }
@@ -470,6 +489,7 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
     h->off[0] = nullptr; h->n_groups = nullptr; h->groups = nullptr;
     h->items = nullptr; h->n_items = nullptr; h->max_items = 0;
     h->rg_m = nullptr; for (int a = 0; a < 3; ++a) h->rg_mv[a] = h->rg_f[a] = h->rg_mv2[a] = nullptr;
+    h->acc32_nm[0] = h->acc32_nm[1] = h->acc32_v2[0] = h->acc32_v2[1] = nullptr;
     h->groups_alt = h->items_alt = nullptr; h->n_groups_alt = h->n_items_alt = nullptr; h->map_state = nullptr;
     h->dest = nullptr; h->max_groups = 0; h->coff = nullptr; h->slots = 0;
     std::memset(h->pbuf, 0, sizeof(h->pbuf));
@@ -606,6 +626,9 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
             ok = dev_alloc_t(h, &h->acc_mv[1][a], (size_t)gd.Nn) && dev_alloc_t(h, &h->acc_f[1][a], (size_t)gd.Nn) &&
                  dev_alloc_t(h, &h->acc_mv2[1][a], (size_t)gd.Nn);
     }
+    if (ok && tiled && gd.acc32)
+        for (int b = 0; b < 2 && ok; ++b)
+            ok = dev_alloc_t(h, &h->acc32_nm[b], 8 * (size_t)gd.Nn) && dev_alloc_t(h, &h->acc32_v2[b], 4 * (size_t)gd.Nn);
     if (ok && sorted)
         ok = dev_alloc_t(h, &h->off[0], (size_t)gd.Nkeys + 1) && dev_alloc_t(h, &h->n_groups, 1) && dev_alloc_t(h, &h->n_items, 1);
     if (ok && tiled) {
@@ -642,6 +665,10 @@ int mpm_create(const mpm_config *cfg, mpm_handle **out)
     }
     if (sorted && e == cudaSuccess) e = cudaMemsetAsync(h->n_groups, 0, sizeof(int), h->stream);
     if (sorted && e == cudaSuccess) e = cudaMemsetAsync(h->n_items, 0, sizeof(int), h->stream);
+    for (int b = 0; b < 2 && tiled && gd.acc32 && e == cudaSuccess; ++b) {
+        e = cudaMemsetAsync(h->acc32_nm[b], 0, sizeof(float) * 8 * (size_t)gd.Nn, h->stream);
+        if (e == cudaSuccess) e = cudaMemsetAsync(h->acc32_v2[b], 0, sizeof(float) * 4 * (size_t)gd.Nn, h->stream);
+    }
     if (tiled && e == cudaSuccess) e = cudaMemsetAsync(h->acc_m[1], 0, sizeof(double) * (size_t)gd.Nn, h->stream);
     for (int a = 0; a < gd.dim && tiled && e == cudaSuccess; ++a) {
         e = cudaMemsetAsync(h->acc_mv[1][a], 0, sizeof(double) * (size_t)gd.Nn, h->stream);
@@ -771,8 +798,8 @@ int load_impl(mpm_handle *h, int64_t n, const double *const *x, const double *co
         h->acur = 0;
         h->grid_final = false;
         const GArr g0 = tiled_acc(h, 0);
-        launch_grid_clear(h->gd, g0, h->stream);
-        for (int a = 0; a < h->gd.dim; ++a) cudaMemsetAsync(g0.mv2[a], 0, sizeof(double) * (size_t)h->gd.Nn, h->stream);
+        clear_p2g1(h, g0, h->stream);
+        clear_p2g2(h, g0, h->stream);
     }
     if (!keep_time) {
         MPM_CUDA(h, cudaMemsetAsync(h->sc, 0, sizeof(DevScalars), h->stream));
@@ -813,7 +840,13 @@ int mpm_step(mpm_handle *h, double dt, double cfl, int32_t nsteps, double *dt_la
     for (int it = 0; it < nsteps; ++it) {
         if (h->variant != MPM_VARIANT_ATOMIC) {
             if (h->n > 0) step_tiled(h, it == nsteps - 1);
-            else { launch_begin_step(h->sc, gd.h, false, s); launch_grid_clear(gd, h->g, s); launch_end_step(h->sc, gd.h, s); h->launches += 2; }
+            else {
+                launch_begin_step(h->sc, gd.h, false, s);
+                launch_grid_clear(gd, h->g, s);
+                if (gd.acc32) clear_p2g1(h, tiled_acc(h, 0), s);
+                launch_end_step(h->sc, gd.h, s);
+                h->launches += 2;
+            }
             h->steps_done += 1;
             continue;
         }
@@ -855,13 +888,13 @@ int mpm_step_phase(mpm_handle *h, int phase, double dt)
         else {      // an empty slab: nothing to gather, but its mv2 plane is exported next
             launch_begin_step(h->sc, h->gd.h, false, h->stream);
             const GArr gc = tiled_acc(h, h->acur);
-            for (int a = 0; a < h->gd.dim; ++a) cudaMemsetAsync(gc.mv2[a], 0, sizeof(double) * (size_t)h->gd.Nn, h->stream);
+            clear_p2g2(h, gc, h->stream);
             h->launches += 1;
         }
     } else if (phase == MPM_PHASE_UPDATE) {
         if (h->n > 0) step_tiled_update(h, true);
         else {
-            launch_grid_clear(h->gd, tiled_acc(h, h->acur ^ 1), h->stream);
+            clear_p2g1(h, tiled_acc(h, h->acur ^ 1), h->stream);
             h->acur ^= 1;
             launch_end_step(h->sc, h->gd.h, h->stream);
             h->launches += 1;
@@ -1023,15 +1056,10 @@ int mpm_read_grid(mpm_handle *h, int field, double *out, int ptr_location)
         gw.m = h->rg_m;
         for (int a = 0; a < gd.dim; ++a) { gw.mv[a] = h->rg_mv[a]; gw.f[a] = h->rg_f[a]; gw.mv2[a] = h->rg_mv2[a]; }
         if (!h->grid_final) {
-            launch_widen(gl.m, gw.m, gd.Nn, h->stream);
-            for (int a = 0; a < gd.dim; ++a) {
-                launch_widen(gl.mv[a], gw.mv[a], gd.Nn, h->stream);
-                launch_widen(gl.f[a], gw.f[a], gd.Nn, h->stream);
-                launch_widen(gl.mv2[a], gw.mv2[a], gd.Nn, h->stream);
-            }
+            launch_widen(gd, gl, gw, h->stream);      // node-major fp32 -> component-major fp64
             if (h->steps_done > 0) { launch_node1(gd, gw, h->sc, h->stream, false); launch_node2(gd, gw, h->stream); }
             h->grid_final = true;
-            h->launches += 3 + 3 * gd.dim;
+            h->launches += 3;
         }
         gl = gw;
     } else if (h->variant == MPM_VARIANT_TILED && !h->grid_final && h->steps_done > 0) {

@@ -119,7 +119,7 @@ struct TileGeo {
 };
 
 // Order of the tiles = order of their particles in memory = order in which the blocks of the tile kernels are scheduled:
-// x fastest over the whole grid.  (Measured in round 2, profiles/r02_experiments.md section 5: numbering the tiles in compact
+// x fastest over the whole grid.  (Measured in round 2, profiles/r02_experiments.md section 7: numbering the tiles in compact
 // super-tiles of 4 x 4 x 4, so that the node planes neighbouring tiles share are still in L2 when the second tile needs
 // them, changes neither kernel's time on configs 4 and 5.)
 template <int DIM>
@@ -310,8 +310,9 @@ void launch_p2g1_tiled(const GridDesc &gd, const PArr &p, const GArr &g, const S
 // flag[0] |= 1 if any of m[0..n) differs from m[0] bit for bit (flag zeroed by the caller); fill: m[0..n) = value
 void launch_mass_differs(const double *m, long long n, int *flag, cudaStream_t s);
 void launch_fill(double *m, long long n, double value, cudaStream_t s);
-// dst[i] = (double)((const float *)src)[i]: fp32 accumulators widened for mpm_read_grid
-void launch_widen(const double *src_as_float, double *dst, long long n, cudaStream_t s);
+// fp32 accumulators (node-major: src32.m = nm[N_n][8], src32.mv2[0] = v2[N_n][4]) widened into the component-major fp64 arrays of
+// dst64 for mpm_read_grid
+void launch_widen(const GridDesc &gd, const GArr &src32, const GArr &dst64, cudaStream_t s);
 // dst[i] += src[i], i < n (halo sum-exchange of a node plane)
 void launch_add_into(double *dst, const double *src, long long n, cudaStream_t s);
 long long max_items_tiled(const GridDesc &gd, long long max_groups);   // upper bound of the item count (launch size)

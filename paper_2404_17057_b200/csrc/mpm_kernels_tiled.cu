@@ -55,7 +55,7 @@ __device__ __forceinline__ void st2(double *p, long long k, double a, double b)
 //     (cp.async.bulk.shared::cluster.global, the non-tensor form of TMA: SASS UBLKCP), one per field and pass, issued by
 //     lane 0 of the warp and tracked by an mbarrier (expect_tx / complete_tx); the lanes read their two particles from
 //     the warp's window.  This takes the copies off the LSU / L1TEX path and replaces 32 address computations per field
-//     by one.  Measured (profiles/r02_particle_stream.md): no faster than cp.async on config 4 and 2 % slower on config
+//     by one.  Measured (profiles/r02_experiments.md sections 1 and 9): no faster than cp.async on config 4 and 2 % slower on config
 //     5 (a one-lane issue sequence costs as many issue slots as a full-warp LDGSTS, and an mbarrier wait more than a
 //     commit-group wait), hence not the default.
 // Both use the same shared-memory layout, [warp][field][kWin slots]: cp.async lanes own slots 2 lane, 2 lane + 1.
@@ -116,27 +116,65 @@ __device__ __forceinline__ void warp_window(int first, int cnt, int &w0, int &wn
     wn = hi > lo ? hi - lo : 0;
 }
 
-// Node accumulators m, mv, f, mv2: fp64 (default) or, with ACC32, fp32 values in the same allocations (the fp32
-// grid-accumulation variant of BASELINE.json config 5: particle arithmetic stays fp64, the sums on the grid and the
-// reductions that form them are fp32)
+// Node accumulators m, mv, f, mv2: fp64, component-major (default); or, with ACC32 (the fp32 grid-accumulation variant of
+// BASELINE.json config 5: particle arithmetic stays fp64, the sums on the grid and the reductions that form them are fp32),
+// fp32 and NODE-MAJOR: g.m points to float nm[N_n][8] = { m, mv_0, mv_1, mv_2, f_0, f_1, f_2, - } and g.mv2[0] to
+// float v2[N_n][4] = { mv2_0, mv2_1, mv2_2, - } (unused components stay zero), so that a corner's channels go to the grid with
+// TWO (one) vector reductions (red.global.add.v4.f32: SASS REDG.E.ADD.F32x4, sm_90+) instead of 1 + 2 d (d) scalar ones, and a
+// tile node is staged with two (three) 16-byte loads.  fp64 has no vector reduction.
 template <bool ACC32>
 __device__ __forceinline__ void acc_add(double *arr, long long i, double v)
 {
+    static_assert(!ACC32, "the fp32 accumulators are node-major: acc32_add_nm / acc32_add_v2");
     MPM_CHECK(i >= 0 && i < g_checked_nodes);
-    if (ACC32) atomicAdd(reinterpret_cast<float *>(arr) + i, (float)v);
-    else atomicAdd(arr + i, v);
+    atomicAdd(arr + i, v);
 }
 template <bool ACC32>
 __device__ __forceinline__ double acc_ld(const double *arr, long long i)
 {
+    static_assert(!ACC32, "the fp32 accumulators are node-major: acc32_ld");
     MPM_CHECK(i >= 0 && i < g_checked_nodes);
-    if (ACC32) return (double)__ldg(reinterpret_cast<const float *>(arr) + i);
     return __ldg(arr + i);
+}
+__device__ __forceinline__ void red_add_f32x4(float *p, float a, float b, float c, float d)
+{
+    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
+}
+// m, mv, f of one node += (ACC32 layout)
+template <int DIM>
+__device__ __forceinline__ void acc32_add_nm(const GArr &g, long long node, double m, const double mv[DIM], const double f[DIM])
+{
+    MPM_CHECK(node >= 0 && node < g_checked_nodes);
+    float *nm = reinterpret_cast<float *>(g.m) + 8 * node;
+    red_add_f32x4(nm, (float)m, (float)mv[0], (float)mv[1], DIM == 3 ? (float)mv[DIM - 1] : 0.f);
+    red_add_f32x4(nm + 4, (float)f[0], (float)f[1], DIM == 3 ? (float)f[DIM - 1] : 0.f, 0.f);
+}
+// mv2 of one node +=
+template <int DIM>
+__device__ __forceinline__ void acc32_add_v2(const GArr &g, long long node, const double v[DIM])
+{
+    MPM_CHECK(node >= 0 && node < g_checked_nodes);
+    red_add_f32x4(reinterpret_cast<float *>(g.mv2[0]) + 4 * node, (float)v[0], (float)v[1], DIM == 3 ? (float)v[DIM - 1] : 0.f, 0.f);
+}
+// all sums of one node, widened
+template <int DIM, bool WITH_V2>
+__device__ __forceinline__ void acc32_ld(const GArr &g, long long node, double &m, double mv[DIM], double f[DIM], double mv2[DIM])
+{
+    MPM_CHECK(node >= 0 && node < g_checked_nodes);
+    const float4 *nm = reinterpret_cast<const float4 *>(g.m) + 2 * node;
+    const float4 a = __ldg(nm), b = __ldg(nm + 1);
+    m = a.x;
+    mv[0] = a.y; mv[1] = a.z; if (DIM == 3) mv[DIM - 1] = a.w;
+    f[0] = b.x; f[1] = b.y; if (DIM == 3) f[DIM - 1] = b.z;
+    if (WITH_V2) {
+        const float4 c = __ldg(reinterpret_cast<const float4 *>(g.mv2[0]) + node);
+        mv2[0] = c.x; mv2[1] = c.y; if (DIM == 3) mv2[DIM - 1] = c.z;
+    }
 }
 
 // 1 / x to within about one unit in the last place for a finite x that is neither zero nor subnormal: the hardware
 // approximation (relative error 2^-23) refined by two Newton steps, 5 instructions in place of the ~25 of an IEEE division
-// (measured: profiles/r02_experiments.md section 6).  Used where the parity tolerance (1e-12) leaves room for the last bit:
+// (measured: profiles/r02_experiments.md section 8).  Used where the parity tolerance (1e-12) leaves room for the last bit:
 // rho' = rho / (1 + dt D) and the node quotients by m.  x = 0 gives inf like the division; a subnormal x is flushed to 0.
 #ifndef MPM_FAST_RCP
 #define MPM_FAST_RCP 1
@@ -244,11 +282,18 @@ __device__ __forceinline__ void p2g1_commit_global(const GridDesc &gd, const GAr
 #pragma unroll
     for (int q = 0; q < 2; ++q) {
         const int node = corner_node_i<DIM>(gd, c, l + q * LG);
-        acc_add<ACC32>(g.m, node, tot[0][q]);
+        if constexpr (ACC32) {
+            double mv[DIM], f[DIM];
 #pragma unroll
-        for (int a = 0; a < DIM; ++a) {
-            acc_add<ACC32>(g.mv[a], node, tot[1 + a][q]);
-            acc_add<ACC32>(g.f[a], node, tot[1 + DIM + a][q]);
+            for (int a = 0; a < DIM; ++a) { mv[a] = tot[1 + a][q]; f[a] = tot[1 + DIM + a][q]; }
+            acc32_add_nm<DIM>(g, node, tot[0][q], mv, f);
+        } else {
+            acc_add<false>(g.m, node, tot[0][q]);
+#pragma unroll
+            for (int a = 0; a < DIM; ++a) {
+                acc_add<false>(g.mv[a], node, tot[1 + a][q]);
+                acc_add<false>(g.f[a], node, tot[1 + DIM + a][q]);
+            }
         }
     }
 }
@@ -396,7 +441,7 @@ struct Chunk {
 };
 
 // The group records of a block's item are copied into shared memory once, at the start of the block (one 16-byte cp.async
-// per record: they are one contiguous run), and every pass reads its records from there.  ncu (profiles/r02_ncu_sedov256.md):
+// per record: they are one contiguous run), and every pass reads its records from there.  ncu (profiles/r02_ncu_final.md section 3):
 // fetching them with a global load inside the pass cost 6 - 9 % of both sweeps' stall samples -- the unpacking right behind
 // the load, and shared-memory loads that waited on the scoreboard they shared with it.  STAGE = false (the COLOUR
 // instantiations, whose static shared memory is full): records come from global memory as before.
@@ -502,12 +547,15 @@ __device__ __forceinline__ void stage_tile(const GridDesc &gd, const int org[DIM
 #pragma unroll
         for (int a = 0; a < DIM; ++a) { mv[it][a] = 0.0; f[it][a] = 0.0; mv2[it][a] = 0.0; }
         if (node[it] >= 0) {
-            m[it] = acc_ld<ACC32>(g.m, node[it]);
+            if constexpr (ACC32) acc32_ld<DIM, WITH_V2>(g, node[it], m[it], mv[it], f[it], mv2[it]);
+            else {
+                m[it] = acc_ld<false>(g.m, node[it]);
 #pragma unroll
-            for (int a = 0; a < DIM; ++a) { mv[it][a] = acc_ld<ACC32>(g.mv[a], node[it]); f[it][a] = acc_ld<ACC32>(g.f[a], node[it]); }
-            if (WITH_V2) {
+                for (int a = 0; a < DIM; ++a) { mv[it][a] = acc_ld<false>(g.mv[a], node[it]); f[it][a] = acc_ld<false>(g.f[a], node[it]); }
+                if (WITH_V2) {
 #pragma unroll
-                for (int a = 0; a < DIM; ++a) mv2[it][a] = acc_ld<ACC32>(g.mv2[a], node[it]);
+                    for (int a = 0; a < DIM; ++a) mv2[it][a] = acc_ld<false>(g.mv2[a], node[it]);
+                }
             }
         }
     }
@@ -678,11 +726,18 @@ __device__ __forceinline__ void coop_p2g1(const GridDesc &gd, const GArr &gn, un
             particle_cell<DIM>(gd, X, c, xi);
             const long long node = corner_node<DIM>(gd, c, b);
             const double Mphi = M * corner_phi<DIM>(xi, b);
-            acc_add<ACC32>(gn.m, node, Mphi);
+            if constexpr (ACC32) {
+                double mv[DIM], f[DIM];
 #pragma unroll
-            for (int a = 0; a < DIM; ++a) {
-                acc_add<ACC32>(gn.mv[a], node, V[a] * Mphi);
-                acc_add<ACC32>(gn.f[a], node, S * corner_dphi<DIM>(xi, b, a, gd.inv_h));
+                for (int a = 0; a < DIM; ++a) { mv[a] = V[a] * Mphi; f[a] = S * corner_dphi<DIM>(xi, b, a, gd.inv_h); }
+                acc32_add_nm<DIM>(gn, node, Mphi, mv, f);
+            } else {
+                acc_add<false>(gn.m, node, Mphi);
+#pragma unroll
+                for (int a = 0; a < DIM; ++a) {
+                    acc_add<false>(gn.mv[a], node, V[a] * Mphi);
+                    acc_add<false>(gn.f[a], node, S * corner_dphi<DIM>(xi, b, a, gd.inv_h));
+                }
             }
         }
     }
@@ -896,8 +951,15 @@ __global__ void __launch_bounds__(kTB, (DIM == 2 && !COLOUR) ? kTBMinG2 : kTBMin
 #pragma unroll
                 for (int q = 0; q < 2; ++q) {
                     const int node = corner_node_i<DIM>(gd, c, l + q * LG);
+                    if constexpr (ACC32) {
+                        double v[DIM];
 #pragma unroll
-                    for (int a = 0; a < DIM; ++a) acc_add<ACC32>(g.mv2[a], node, tot[a][q]);
+                        for (int a = 0; a < DIM; ++a) v[a] = tot[a][q];
+                        acc32_add_v2<DIM>(g, node, v);
+                    } else {
+#pragma unroll
+                        for (int a = 0; a < DIM; ++a) acc_add<false>(g.mv2[a], node, tot[a][q]);
+                    }
                 }
             }
         }
@@ -928,7 +990,7 @@ __global__ void __launch_bounds__(kTB, (DIM == 2 && !COLOUR) ? kTBMinG2 : kTBMin
 #pragma unroll
             for (int a = 0; a < DIM; ++a) {
                 const double v = s_acc[j * DIM + a];
-                if (v != 0.0) acc_add<ACC32>(g.mv2[a], node, v);
+                if (v != 0.0) acc_add<false>(g.mv2[a], node, v);      // COLOUR: fp64 accumulation only
             }
         }
     }
@@ -1257,11 +1319,11 @@ __global__ void __launch_bounds__(kTB, COLOUR ? 3 : DIM == 2 ? kTBMinU2 : kTBMin
             const int node = tile_node_global<DIM>(gd, org, j, idx);
             if (node < 0) continue;
             const double *src = s_acc + j * SM::NACC;
-            if (src[0] != 0.0) acc_add<ACC32>(gn.m, node, src[0]);
+            if (src[0] != 0.0) acc_add<false>(gn.m, node, src[0]);      // COLOUR: fp64 accumulation only
 #pragma unroll
             for (int a = 0; a < DIM; ++a) {
-                if (src[1 + a] != 0.0) acc_add<ACC32>(gn.mv[a], node, src[1 + a]);
-                if (src[1 + DIM + a] != 0.0) acc_add<ACC32>(gn.f[a], node, src[1 + DIM + a]);
+                if (src[1 + a] != 0.0) acc_add<false>(gn.mv[a], node, src[1 + a]);
+                if (src[1 + DIM + a] != 0.0) acc_add<false>(gn.f[a], node, src[1 + DIM + a]);
             }
         }
     }
@@ -1631,10 +1693,17 @@ void launch_update_tiled(const GridDesc &gd, const PArr &p, const PArr &q, const
 #undef MPM_LAUNCH_UPD
 }
 
-// dst[i] = (double)src[i], i < n (fp32 accumulators brought to fp64 for mpm_read_grid)
-__global__ void __launch_bounds__(256) k_widen(const float *__restrict__ src, double *__restrict__ dst, long long n)
+// fp32 accumulators (node-major nm[N_n][8], v2[N_n][4]) brought to component-major fp64 arrays for mpm_read_grid
+__global__ void __launch_bounds__(256) k_widen(const float4 *__restrict__ nm, const float4 *__restrict__ v2, GArr dst, int dim, long long n)
 {
-    for (long long i = (long long)blockIdx.x * 256 + threadIdx.x; i < n; i += (long long)gridDim.x * 256) dst[i] = (double)src[i];
+    for (long long i = (long long)blockIdx.x * 256 + threadIdx.x; i < n; i += (long long)gridDim.x * 256) {
+        const float4 a = nm[2 * i], b = nm[2 * i + 1], c = v2[i];
+        dst.m[i] = a.x;
+        dst.mv[0][i] = a.y; dst.mv[1][i] = a.z;
+        dst.f[0][i] = b.x; dst.f[1][i] = b.y;
+        dst.mv2[0][i] = c.x; dst.mv2[1][i] = c.y;
+        if (dim == 3) { dst.mv[2][i] = a.w; dst.f[2][i] = b.z; dst.mv2[2][i] = c.z; }
+    }
 }
 __global__ void __launch_bounds__(256) k_add_into(double *__restrict__ dst, const double *__restrict__ src, long long n)
 {
@@ -1644,9 +1713,10 @@ void launch_add_into(double *dst, const double *src, long long n, cudaStream_t s
 {
     if (n > 0) k_add_into<<<(unsigned)((n + 255) / 256 < 148 * 8 ? (n + 255) / 256 : 148 * 8), 256, 0, s>>>(dst, src, n);
 }
-void launch_widen(const double *src_as_float, double *dst, long long n, cudaStream_t s)
+void launch_widen(const GridDesc &gd, const GArr &src32, const GArr &dst64, cudaStream_t s)
 {
-    if (n > 0) k_widen<<<148 * 8, 256, 0, s>>>(reinterpret_cast<const float *>(src_as_float), dst, n);
+    if (gd.Nn > 0)
+        k_widen<<<148 * 8, 256, 0, s>>>(reinterpret_cast<const float4 *>(src32.m), reinterpret_cast<const float4 *>(src32.mv2[0]), dst64, gd.dim, gd.Nn);
 }
 
 void launch_gather_by_id_groups(const double *src, const int *id, double *dst, const SortedMap &map, long long max_groups,

@@ -129,12 +129,13 @@ __device__ __forceinline__ void slow_p2g1(const GridDesc &gd, const GArr &g, con
     for (int ib = 0; ib < (1 << DIM); ++ib) {
         const long long i = corner_node<DIM>(gd, c, ib);
         const double phi = corner_phi<DIM>(xi, ib);
-        if (ACC32) {      // fp32 grid accumulation (TILED family only)
-            atomicAdd(reinterpret_cast<float *>(g.m) + i, (float)(M * phi));
+        if (ACC32) {      // fp32 grid accumulation (TILED family only): node-major float nm[N_n][8] = { m, mv[3], f[3], - }
+            float *nm = reinterpret_cast<float *>(g.m) + 8 * i;
+            atomicAdd(nm, (float)(M * phi));
 #pragma unroll
             for (int a = 0; a < DIM; ++a) {
-                atomicAdd(reinterpret_cast<float *>(g.mv[a]) + i, (float)(M * V[a] * phi));
-                atomicAdd(reinterpret_cast<float *>(g.f[a]) + i, (float)(S * corner_dphi<DIM>(xi, ib, a, gd.inv_h)));
+                atomicAdd(nm + 1 + a, (float)(M * V[a] * phi));
+                atomicAdd(nm + 4 + a, (float)(S * corner_dphi<DIM>(xi, ib, a, gd.inv_h)));
             }
             continue;
         }
